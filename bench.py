@@ -1,0 +1,339 @@
+#!/usr/bin/env python
+"""bench.py -- PI-GAN train-step throughput on B200 (metric of BASELINE.json).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config c5] [--impl pigan|reference] [--all-configs]
+
+A "step" is one pass of the whole hot path: pigan_train_step_grads on one batch of synthetic
+input followed by the three pigan_adam_update calls.  The headline workload is config c5 (the largest; DESIGN.md
+section 6 says why); --all-configs adds a short run of every other config to the same JSON line.  N > 1 runs N
+independent replicas (the path does not shard: north_star says no collectives), one process per GPU under torchrun.
+`--impl reference` times the fp64 oracle (oracle/) on the host cores on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import dataclasses
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+import workloads as wl  # noqa: E402
+
+METRIC = "PI-GAN train-step sample*collocation-points/s"
+UNIT = "sample*collocation-points/s"
+ADAM = dict(lr=1e-4, beta1=0.5, beta2=0.9, adam_eps=1e-8)          # reading G3
+
+
+# ----------------------------------------------------------------------------------------------------------------
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return {"hbm_gbs": d["hbm_gbs"], "tflops_burst": d["bf16_tflops"], "tflops_sustained": d["bf16_tflops_sustained"], "source": "measured"}
+    return {"hbm_gbs": 6650.0, "tflops_burst": 1590.0, "tflops_sustained": 1400.0, "source": "fallback"}
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index=0, period=0.1):
+        super().__init__(daemon=True)
+        self.index, self.period, self.samples, self.reasons, self.max_mhz = index, period, [], set(), None
+        self._stop_evt = threading.Event()
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def run(self):
+        if not self.nv:
+            return
+        nv = self.nv
+        names = {"hw_slowdown": nv.nvmlClocksEventReasonHwSlowdown if hasattr(nv, "nvmlClocksEventReasonHwSlowdown") else nv.nvmlClocksThrottleReasonHwSlowdown,
+                 "hw_thermal_slowdown": getattr(nv, "nvmlClocksEventReasonHwThermalSlowdown", getattr(nv, "nvmlClocksThrottleReasonHwThermalSlowdown", 0)),
+                 "sw_thermal_slowdown": getattr(nv, "nvmlClocksEventReasonSwThermalSlowdown", getattr(nv, "nvmlClocksThrottleReasonSwThermalSlowdown", 0)),
+                 "sw_power_cap": getattr(nv, "nvmlClocksEventReasonSwPowerCap", getattr(nv, "nvmlClocksThrottleReasonSwPowerCap", 0))}
+        while not self._stop_evt.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                try:
+                    r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for k, bit in names.items():
+                    if bit and (r & bit):
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            self._stop_evt.wait(self.period)
+
+    def finish(self):
+        self._stop_evt.set()
+        self.join(timeout=2)
+        return {"sm_mhz": float(np.median(self.samples)) if self.samples else None, "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+# ----------------------------------------------------------------------------------------------------------------
+def cpu_sample_config(cfg, flop_budget=1.5e12):
+    """Bounded sample of cfg for the oracle (about 10-30 s of fp64 numpy work): full generator dimensions, a 32x32
+    grid, N' samples chosen from a flop budget, sensors scaled to keep the config's P:S ratio (so that the cost per
+    (sample x point) is representative of the full workload)."""
+    if wl.step_flops(cfg)["total"] <= flop_budget:
+        return cfg, "whole workload"
+    Gp = min(cfg.G, 32)
+    per_row = 3 * wl.jet_flops_per_point(cfg.L, cfg.H)
+    Np = int(min(cfg.N, max(1, round(flop_budget / per_row / (Gp * Gp)))))
+    Sp = max(2, int(round(cfg.S * (Gp * Gp) / cfg.P)))
+    s = dataclasses.replace(cfg, name=cfg.name + "-cpu-sample", N=Np, G=Gp, S=Sp)
+    return s, f"N={Np} samples x {Gp}x{Gp} grid, S={Sp} sensors (same P:S ratio), full generator dims {cfg.L}x{cfg.H}, m={cfg.m}"
+
+
+def time_oracle(cfg, steps=1, warmup=0):
+    """Times oracle.train_step_grads_ref (+ Adam) as it stands on the host cores.  Returns (units/s, seconds per step, cores, sample)."""
+    from oracle import pigan_oracle as orc
+    scfg, sample = cpu_sample_config(cfg)
+    inp = wl.make_inputs(scfg)
+    Ys = orc.gen_jet_forward_ref(inp["teacher_Y"], *scfg.gen_shape, inp["xy_sensors"], inp["z_real"], 0)[0]
+    Us = orc.gen_jet_forward_ref(inp["teacher_u"], *scfg.gen_shape, inp["xy_sensors"], inp["z_real"], 0)[0]
+    real = np.concatenate([Ys, Us], axis=1)
+    th = [inp["theta_Y"].astype(np.float64), inp["theta_u"].astype(np.float64), inp["theta_D"].astype(np.float64)]
+    mom = [(np.zeros_like(t), np.zeros_like(t)) for t in th]
+    times = []
+    for it in range(warmup + steps):
+        t0 = time.perf_counter()
+        g = orc.train_step_grads_ref(scfg.gen_shape, scfg.disc_shape, th[0], th[1], th[2], inp["xy_colloc"], inp["f"], inp["xy_sensors"],
+                                     inp["z"], real, inp["eps"], 10.0, 1.0)
+        for k in range(3):
+            th[k], m, v = orc.adam_update_ref(th[k], g[k], mom[k][0], mom[k][1], it + 1, ADAM["lr"], ADAM["beta1"], ADAM["beta2"], ADAM["adam_eps"])
+            mom[k] = (m, v)
+        dt = time.perf_counter() - t0
+        if it >= warmup:
+            times.append(dt)
+    sec = float(np.mean(times))
+    try:
+        from threadpoolctl import threadpool_info
+        cores = max([p.get("num_threads", 1) for p in threadpool_info()] + [1])
+    except Exception:
+        cores = os.cpu_count()
+    return scfg.N * scfg.P / sec, sec, cores, sample
+
+
+# ----------------------------------------------------------------------------------------------------------------
+class GpuWorkload:
+    """Device-resident synthetic inputs + state of one config."""
+
+    def __init__(self, cfg, device, seed_shift=0):
+        import torch
+        from paper_1910_13444_b200 import PiGan
+        self.cfg, self.device, self.torch = cfg, device, torch
+        inp = wl.make_inputs(dataclasses.replace(cfg, index=cfg.index + 10 * seed_shift) if seed_shift else cfg)
+        self.pg = PiGan.from_config(cfg, device=device)
+        d = {k: torch.from_numpy(np.ascontiguousarray(v)).to(device) for k, v in inp.items()}
+        # "real" snapshots: the frozen teacher pair evaluated at the sensors by the GPU library, outside any timed region
+        Ys = self.pg.gen_jet_forward(d["teacher_Y"], d["xy_sensors"], d["z_real"], 0)[0]
+        Us = self.pg.gen_jet_forward(d["teacher_u"], d["xy_sensors"], d["z_real"], 0)[0]
+        d["real"] = torch.cat([Ys, Us], dim=1).contiguous()
+        self.d = d
+        self.params = [d["theta_Y"].clone(), d["theta_u"].clone(), d["theta_D"].clone()]
+        self.mom = [(torch.zeros_like(p), torch.zeros_like(p)) for p in self.params]
+        self.out = (torch.empty_like(self.params[0]), torch.empty_like(self.params[1]), torch.empty_like(self.params[2]),
+                    torch.empty(6, device=device), torch.zeros(1, dtype=torch.int32, device=device))
+        self.loss_scale = 1024.0 if cfg.precision == "fp16" else 1.0
+        self.step_no = 0
+        # pinned host copies of the per-step inputs for the end-to-end leg
+        self.host = {k: inp_k.cpu().pin_memory() for k, inp_k in (("z", d["z"]), ("real", d["real"]), ("eps", d["eps"]))}
+        self.host_out = torch.empty(6, dtype=torch.float32).pin_memory()
+        self.flush = torch.empty(256 << 20, dtype=torch.uint8, device=device) if cfg.N * cfg.P < 400000 else None
+
+    def step(self):
+        d, pg = self.d, self.pg
+        self.step_no += 1
+        pg.train_step_grads(self.params[0], self.params[1], self.params[2], d["xy_colloc"], d["f"], d["xy_sensors"], d["z"], d["real"],
+                            d["eps"], self.loss_scale, out=self.out)
+        for k in range(3):
+            pg.adam_update(self.params[k], self.out[k], self.mom[k][0], self.mom[k][1], self.step_no, skip_flag=self.out[4], **ADAM)
+
+    def step_e2e(self):
+        """Same step with the per-step inputs coming from pinned host memory and the losses read back."""
+        d = self.d
+        for k in ("z", "real", "eps"):
+            d[k].copy_(self.host[k], non_blocking=True)
+        self.step()
+        self.host_out.copy_(self.out[3], non_blocking=True)
+
+    def e2e_bytes(self):
+        return sum(int(v.numel() * 4) for v in self.host.values()), 6 * 4
+
+    def timed(self, fn, steps, warmup):
+        """Per-step CUDA-event timing on the launch stream; L2 is flushed between steps for the small configs."""
+        torch = self.torch
+        for _ in range(warmup):
+            fn()
+        torch.cuda.synchronize(self.device)
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        for a, b in ev:
+            if self.flush is not None:
+                self.flush.fill_(1)
+            a.record()
+            fn()
+            b.record()
+        torch.cuda.synchronize(self.device)
+        return [a.elapsed_time(b) for a, b in ev]
+
+
+def run_config(cfg, device, steps, warmup, rank, world, with_roofline=True, seed_shift=0):
+    import torch
+    w = GpuWorkload(cfg, device, seed_shift)
+    peaks = measured_peaks()
+    flops = wl.step_flops(cfg)
+    res = {}
+    sampler = ClockSampler(index=torch.cuda.current_device()); sampler.start()
+    l0 = w.pg.launch_count
+    w.pg.profile_enable(True)
+    # warm-up (untimed), then drop its trace
+    for _ in range(warmup):
+        w.step()
+    torch.cuda.synchronize(device)
+    w.pg.profile_report()
+    l0 = w.pg.launch_count
+    ms = w.timed(w.step, steps, 0)
+    prof = w.pg.profile_report()
+    launches = w.pg.launch_count - l0
+    w.pg.profile_enable(False)
+    res["clocks"] = sampler.finish()
+    res["ms_steps"] = ms
+    res["launches"] = launches
+    res["found_inf"] = int(w.out[4].item())
+    res["losses"] = [float(x) for x in w.out[3].cpu()]
+    # end-to-end leg: host buffers in, losses out, copies inside the timed region
+    ms_e2e = w.timed(w.step_e2e, max(2, steps // 2), 1)
+    res["ms_e2e"] = ms_e2e
+    res["h2d"], res["d2h"] = w.e2e_bytes()
+    # roofline of the dominant kernel class (the tcgen05 jet GEMMs: forward, dgrad+adjoint, wgrad)
+    if with_roofline:
+        tc = {k: v for k, v in prof.items() if k in ("jet_layer_fwd", "jet_layer_bwd", "wgrad")}
+        per_step = {k: [v[0] / steps, v[1] / steps] for k, v in prof.items()}
+        tc_ms = sum(v[1] for v in tc.values()) / steps
+        total_ms = sum(v[1] for v in prof.values()) / steps
+        res["kernel_ms_per_step"] = {k: round(v[1], 4) for k, v in sorted(per_step.items(), key=lambda kv: -kv[1][1])}
+        res["kernel_launches_per_step"] = {k: v[0] for k, v in per_step.items()}
+        if tc_ms > 0:
+            # algorithmic flops of the hidden jet layers of the collocation + sensor rows: 3 GEMMs (fwd, dgrad, wgrad) per layer
+            sens_gemm = cfg.N * 3 * cfg.S * 2 * (cfg.L - 1) * 2 * cfg.H * cfg.H
+            alg = flops["jet_gemm"] + sens_gemm
+            ach = alg / (tc_ms * 1e-3) / 1e12
+            peak = peaks["tflops_sustained"]
+            res["roofline"] = {"bound": "tensor", "achieved": round(ach, 2), "peak": peak, "unit": "TFLOP/s", "frac": round(ach / peak, 4),
+                               "traffic": None, "kernel": "jet_layer_fwd + jet_layer_bwd + wgrad (tcgen05)", "peak_source": peaks["source"] + " sustained bf16",
+                               "frac_of_burst": round(ach / peaks["tflops_burst"], 4), "frac_of_nominal_2250": round(ach / 2250.0, 4),
+                               "share_of_step": round(tc_ms / total_ms, 4) if total_ms > 0 else None,
+                               "per_kernel_tflops": {k: round(alg / 3 / (v[1] / steps * 1e-3) / 1e12, 1) for k, v in tc.items() if v[1] > 0}}
+        else:
+            # fp32 mode (c1): plain FP32 FMA path; report against the fp32 ALU peak (148 SMs x 128 lanes x 2 flop x clock)
+            mhz = res["clocks"]["sm_mhz"] or 1965.0
+            peak = 148 * 128 * 2 * mhz * 1e6 / 1e12
+            ach = flops["total"] / (np.mean(ms) * 1e-3) / 1e12
+            res["roofline"] = {"bound": "alu", "achieved": round(ach, 4), "peak": round(peak, 1), "unit": "TFLOP/s", "frac": round(ach / peak, 5),
+                               "traffic": None, "kernel": "whole fp32 step (launch-latency bound at this size)"}
+    w.pg.close()
+    return res
+
+
+def summarize(cfg, res, n_gpus, steps, warmup, t_max_ms):
+    units = cfg.N * cfg.P
+    value = n_gpus * units / (t_max_ms * 1e-3)
+    e2e_ms = float(np.mean(res["ms_e2e"]))
+    return {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": n_gpus, "steps": steps, "warmup": warmup, "ms_per_step": t_max_ms,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": cfg.precision, "data": "synthetic",
+        "config": {"workload": f"{cfg.name}: {cfg.L}x{cfg.H} tanh generators (m={cfg.m}), {cfg.G}x{cfg.G} grid x {cfg.N} samples, {cfg.S} sensors, "
+                               f"critic {cfg.LD}x{cfg.HD}", "rows_per_step": units, "parallelism": f"replicas x{n_gpus}" if n_gpus > 1 else "single GPU",
+                   "l2": "per-step working set >> L2" if cfg.N * cfg.P >= 400000 else "256 MiB L2 flush between timed steps",
+                   "loss_scale": 1024.0 if cfg.precision == "fp16" else 1.0},
+        "train_steps_per_s": 1e3 / t_max_ms,
+        "step_tflops": wl.step_flops(cfg)["total"] / (t_max_ms * 1e-3) / 1e12,
+        "e2e": {"value": n_gpus * units / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": res["h2d"], "d2h_bytes_per_step": res["d2h"]},
+        "gpu_launches": res["launches"], "clocks": res["clocks"], "roofline": res.get("roofline"),
+        "kernel_ms_per_step": res.get("kernel_ms_per_step"), "losses": res["losses"], "found_inf": res["found_inf"],
+    }
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=None)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="c5", choices=list(wl.CONFIGS))
+    ap.add_argument("--impl", default="pigan", choices=["pigan", "reference"])
+    ap.add_argument("--all-configs", action="store_true", help="also run c1..c4 briefly and attach them as per_config")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    cfg = wl.CONFIGS[args.config]
+    rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    warmup = max(3, args.warmup) if args.impl == "pigan" else args.warmup
+    steps = args.steps if args.steps is not None else (5 if cfg.N * cfg.P > 1000000 else 20)
+
+    if args.impl == "reference":
+        # the oracle, as it stands, on the host cores; rank 0 alone works
+        if rank != 0:
+            return 0
+        val, sec, cores, sample = time_oracle(cfg, steps=max(1, min(steps, 3)), warmup=min(args.warmup, 1))
+        line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": max(1, min(steps, 3)),
+                "warmup": min(args.warmup, 1), "ms_per_step": sec * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "f64", "data": "synthetic", "config": {"workload": f"{cfg.name} (bounded sample: {sample})"},
+                "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+                "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
+        print(json.dumps(line))
+        return 0
+
+    import torch
+    import torch.distributed as dist
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --impl pigan needs a CUDA device: the hot path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    device = torch.device(f"cuda:{local_rank}")
+    if world > 1:
+        dist.init_process_group("nccl", device_id=device)
+        dist.barrier()
+    res = run_config(cfg, device, steps, warmup, rank, world, seed_shift=rank)
+    t_ms = float(np.mean(res["ms_steps"]))
+    if world > 1:
+        t = torch.tensor([t_ms], device=device, dtype=torch.float64)
+        dist.barrier()
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)            # max over ranks; the replicas exchange nothing else
+        t_ms = float(t.item())
+    if rank == 0:
+        line = summarize(cfg, res, world, steps, warmup, t_ms)
+        if args.all_configs:
+            per = {}
+            for name, c in wl.CONFIGS.items():
+                if name == cfg.name:
+                    continue
+                r = run_config(c, device, 5 if c.N * c.P > 1000000 else 20, 3, rank, world)
+                s = summarize(c, r, 1, len(r["ms_steps"]), 3, float(np.mean(r["ms_steps"])))
+                per[name] = {k: s[k] for k in ("value", "ms_per_step", "dtype", "step_tflops", "roofline", "gpu_launches", "e2e", "kernel_ms_per_step")}
+            line["per_config"] = per
+        if not args.no_cpu_baseline:
+            val, sec, cores, sample = time_oracle(cfg)
+            line["cpu_baseline"] = {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample, "seconds": sec}
+        print(json.dumps(line))
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -1,0 +1,211 @@
+"""B200-native PI-GAN hot path (arXiv 1910.13444): thin Python binding over the C-ABI library libpigan.so.
+
+The binding only marshals arguments: every step of the path runs in the library's CUDA kernels (include/pigan.h).
+PyTorch is used for device memory and streams.  There is no CPU fallback: importing works anywhere (so that the
+exported symbols can be checked), but creating a context without a CUDA device raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from ctypes import POINTER, Structure, c_char_p, c_float, c_int, c_size_t, c_ulonglong, c_void_p
+
+from .build import LIB, build
+
+__all__ = ["PiGan", "PiganError", "load_library", "param_count", "EXPORTED_SYMBOLS", "PRECISIONS"]
+
+PRECISIONS = {"fp32": 0, "bf16": 1, "fp16": 2}
+STATUS = {0: "PIGAN_OK", 1: "PIGAN_ERR_INVALID_ARG", 2: "PIGAN_ERR_SHAPE", 3: "PIGAN_ERR_ALLOC", 4: "PIGAN_ERR_CUDA",
+          5: "PIGAN_ERR_UNSUPPORTED"}
+EXPORTED_SYMBOLS = ["pigan_create", "pigan_destroy", "pigan_param_count", "pigan_last_error", "pigan_launch_count",
+                    "pigan_profile_enable", "pigan_profile_report",
+                    "pigan_gen_jet_forward", "pigan_darcy_residual", "pigan_disc_forward", "pigan_gradient_penalty",
+                    "pigan_train_step_grads", "pigan_adam_update"]
+
+
+class PiganError(RuntimeError):
+    def __init__(self, status: int, message: str = ""):
+        super().__init__(f"{STATUS.get(status, status)}: {message}")
+        self.status = status
+
+
+class _MlpShape(Structure):
+    _fields_ = [("in_dim", c_int), ("n_hidden", c_int), ("width", c_int)]
+
+
+class _Config(Structure):
+    _fields_ = [("gen", _MlpShape), ("disc", _MlpShape), ("latent_dim", c_int), ("n_samples", c_int), ("n_colloc", c_int),
+                ("n_sensors", c_int), ("precision", c_int), ("gp_lambda", c_float), ("pde_weight", c_float),
+                ("workspace_bytes", c_size_t)]
+
+
+_lib = None
+
+
+def load_library():
+    """Loads libpigan.so (building it first if it is missing or stale).  Raises if that is impossible."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = LIB
+    if not os.path.exists(path) or os.environ.get("PIGAN_REBUILD"):
+        path = build()
+    lib = ctypes.CDLL(path)
+    fp, ip = POINTER(c_float), POINTER(c_int)
+    lib.pigan_create.argtypes = [POINTER(_Config), c_void_p, POINTER(c_void_p)]
+    lib.pigan_create.restype = c_int
+    lib.pigan_destroy.argtypes = [c_void_p]
+    lib.pigan_destroy.restype = None
+    lib.pigan_param_count.argtypes = [POINTER(_MlpShape)]
+    lib.pigan_param_count.restype = c_size_t
+    lib.pigan_last_error.argtypes = [c_void_p]
+    lib.pigan_last_error.restype = c_char_p
+    lib.pigan_launch_count.argtypes = [c_void_p]
+    lib.pigan_launch_count.restype = c_ulonglong
+    lib.pigan_gen_jet_forward.argtypes = [c_void_p, c_void_p, c_void_p, c_int, c_void_p, c_int, c_int, c_void_p]
+    lib.pigan_darcy_residual.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, c_int, c_int, c_void_p, c_void_p]
+    lib.pigan_disc_forward.argtypes = [c_void_p, c_void_p, c_void_p, c_int, c_void_p]
+    lib.pigan_gradient_penalty.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_int, c_void_p, c_void_p, c_void_p]
+    lib.pigan_train_step_grads.argtypes = [c_void_p] + [c_void_p] * 9 + [c_float] + [c_void_p] * 5
+    lib.pigan_adam_update.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_size_t, c_int, c_float, c_float, c_float,
+                                      c_float, c_void_p]
+    lib.pigan_profile_enable.argtypes = [c_void_p, c_int]
+    lib.pigan_profile_report.argtypes = [c_void_p, c_char_p, c_size_t]
+    for name in EXPORTED_SYMBOLS[5:]:
+        getattr(lib, name).restype = c_int
+    del fp, ip
+    _lib = lib
+    return lib
+
+
+def param_count(in_dim: int, n_hidden: int, width: int) -> int:
+    return int(load_library().pigan_param_count(ctypes.byref(_MlpShape(in_dim, n_hidden, width))))
+
+
+def _ptr(t, name, dtype=None):
+    """Device pointer of a contiguous CUDA tensor (None -> NULL)."""
+    import torch
+    if t is None:
+        return None
+    if not isinstance(t, torch.Tensor) or not t.is_cuda or not t.is_contiguous():
+        raise TypeError(f"{name} must be a contiguous CUDA tensor")
+    if t.dtype != (dtype or torch.float32):
+        raise TypeError(f"{name} must have dtype {dtype or torch.float32}, got {t.dtype}")
+    return c_void_p(t.data_ptr())
+
+
+class PiGan:
+    """One context = one CUDA stream + the workspaces of one PI-GAN configuration (mirrors pigan_ctx)."""
+
+    def __init__(self, *, latent_dim, gen_hidden, gen_width, disc_hidden, disc_width, n_samples, n_colloc, n_sensors,
+                 precision="fp32", gp_lambda=10.0, pde_weight=1.0, workspace_bytes=0, stream=None, device=None):
+        import torch
+        self._lib = load_library()
+        self._ctx = c_void_p()
+        if not torch.cuda.is_available():
+            raise PiganError(4, "no CUDA device: the PI-GAN hot path has no CPU fallback")
+        self.device = torch.device(device if device is not None else f"cuda:{torch.cuda.current_device()}")
+        self.m, self.N, self.P, self.S = latent_dim, n_samples, n_colloc, n_sensors
+        self.gen_shape = (2 + latent_dim, gen_hidden, gen_width)
+        self.disc_shape = (2 * n_sensors, disc_hidden, disc_width)
+        self.precision = precision
+        cfg = _Config(_MlpShape(*self.gen_shape), _MlpShape(*self.disc_shape), latent_dim, n_samples, n_colloc, n_sensors,
+                      PRECISIONS[precision], gp_lambda, pde_weight, workspace_bytes)
+        self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        with torch.cuda.device(self.device):
+            st = self._lib.pigan_create(ctypes.byref(cfg), c_void_p(self._stream.cuda_stream), ctypes.byref(self._ctx))
+        if st != 0:
+            self._ctx = c_void_p()
+            raise PiganError(st, "pigan_create failed")
+        self.n_gen = param_count(*self.gen_shape)
+        self.n_disc = param_count(*self.disc_shape)
+
+    @classmethod
+    def from_config(cls, cfg, **kw):
+        """cfg: a workloads.Config."""
+        return cls(latent_dim=cfg.m, gen_hidden=cfg.L, gen_width=cfg.H, disc_hidden=cfg.LD, disc_width=cfg.HD, n_samples=cfg.N,
+                   n_colloc=cfg.P, n_sensors=cfg.S, precision=cfg.precision, **kw)
+
+    def close(self):
+        if getattr(self, "_ctx", None) and self._ctx.value:
+            self._lib.pigan_destroy(self._ctx)
+            self._ctx = c_void_p()
+
+    __del__ = close
+
+    def _check(self, st):
+        if st != 0:
+            raise PiganError(st, self._lib.pigan_last_error(self._ctx).decode())
+
+    def _new(self, *shape, dtype=None):
+        import torch
+        return torch.empty(*shape, dtype=dtype or torch.float32, device=self.device)
+
+    @property
+    def launch_count(self) -> int:
+        return int(self._lib.pigan_launch_count(self._ctx))
+
+    def profile_enable(self, enable=True):
+        self._check(self._lib.pigan_profile_enable(self._ctx, 1 if enable else 0))
+
+    def profile_report(self) -> dict:
+        """{kernel class: [launches, total_ms]} since profiling was enabled (synchronises the stream)."""
+        import json
+        buf = ctypes.create_string_buffer(1 << 16)
+        self._check(self._lib.pigan_profile_report(self._ctx, buf, len(buf)))
+        return json.loads(buf.value.decode())
+
+    # ---- the six calls of include/pigan.h ---------------------------------------------------------------------
+    def gen_jet_forward(self, gen_params, xy, z, jet_order, out=None):
+        n_pts, n_samples = xy.shape[0], z.shape[0]
+        C = (1, 3, 5)[jet_order]
+        if out is None:
+            out = self._new(C, n_samples, n_pts)
+        self._check(self._lib.pigan_gen_jet_forward(self._ctx, _ptr(gen_params, "gen_params"), _ptr(xy, "xy"), n_pts, _ptr(z, "z"),
+                                                    n_samples, jet_order, _ptr(out, "out")))
+        return out
+
+    def darcy_residual(self, logk_jet, u_jet, f, want_r=True, want_mean=True):
+        if logk_jet.shape[1:] != u_jet.shape[1:] or logk_jet.shape[0] < 3 or u_jet.shape[0] != 5:
+            raise ValueError("logk_jet must be [>=3][N][P] and u_jet [5][N][P]")
+        N, P = u_jet.shape[1], u_jet.shape[2]
+        r = self._new(N, P) if want_r else None
+        msq = self._new(1) if want_mean else None
+        self._check(self._lib.pigan_darcy_residual(self._ctx, _ptr(logk_jet, "logk_jet"), _ptr(u_jet, "u_jet"), _ptr(f, "f"), N, P,
+                                                   _ptr(r, "r"), _ptr(msq, "mean_sq")))
+        return r, msq
+
+    def disc_forward(self, disc_params, snap):
+        B = snap.shape[0]
+        score = self._new(B)
+        self._check(self._lib.pigan_disc_forward(self._ctx, _ptr(disc_params, "disc_params"), _ptr(snap, "snap"), B, _ptr(score, "score")))
+        return score
+
+    def gradient_penalty(self, disc_params, real, fake, eps, want_grad=True):
+        B = real.shape[0]
+        gp, nu = self._new(1), self._new(B)
+        d = self._new(self.n_disc) if want_grad else None
+        self._check(self._lib.pigan_gradient_penalty(self._ctx, _ptr(disc_params, "disc_params"), _ptr(real, "real"), _ptr(fake, "fake"),
+                                                     _ptr(eps, "eps"), B, _ptr(gp, "gp"), _ptr(nu, "grad_norm"), _ptr(d, "d_disc_params")))
+        return gp, nu, d
+
+    def train_step_grads(self, logk_params, u_params, disc_params, xy_colloc, f, xy_sensors, z, real_snap, eps, loss_scale=1.0,
+                         out=None):
+        import torch
+        if out is None:
+            out = (self._new(self.n_gen), self._new(self.n_gen), self._new(self.n_disc), self._new(6), self._new(1, dtype=torch.int32))
+        g_logk, g_u, g_disc, losses, found_inf = out
+        if (xy_colloc.shape[0], xy_sensors.shape[0], tuple(z.shape), tuple(real_snap.shape)) != (self.P, self.S, (self.N, self.m), (self.N, 2 * self.S)):
+            raise ValueError("input sizes disagree with the configuration of this context")
+        self._check(self._lib.pigan_train_step_grads(
+            self._ctx, _ptr(logk_params, "logk_params"), _ptr(u_params, "u_params"), _ptr(disc_params, "disc_params"),
+            _ptr(xy_colloc, "xy_colloc"), _ptr(f, "f"), _ptr(xy_sensors, "xy_sensors"), _ptr(z, "z"), _ptr(real_snap, "real_snap"),
+            _ptr(eps, "eps"), float(loss_scale), _ptr(g_logk, "g_logk"), _ptr(g_u, "g_u"), _ptr(g_disc, "g_disc"), _ptr(losses, "losses"),
+            _ptr(found_inf, "found_inf", torch.int32)))
+        return out
+
+    def adam_update(self, params, grads, m, v, step, lr, beta1, beta2, adam_eps, skip_flag=None):
+        import torch
+        self._check(self._lib.pigan_adam_update(self._ctx, _ptr(params, "params"), _ptr(grads, "grads"), _ptr(m, "m"), _ptr(v, "v"),
+                                                params.numel(), int(step), lr, beta1, beta2, adam_eps,
+                                                _ptr(skip_flag, "skip_flag", torch.int32) if skip_flag is not None else None))

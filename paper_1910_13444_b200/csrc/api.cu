@@ -1,0 +1,452 @@
+// C-ABI entry points (include/pigan.h) and the host-side orchestration of one step: row-chunking of the N*P
+// collocation rows and N*S sensor rows, kernel sequencing on one stream, fp32 accumulation
+// of weight gradients across chunks.  Every step of the path runs in this library's kernels; there is no CPU fallback.
+#include <algorithm>
+#include <cmath>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "common.cuh"
+
+using namespace pigan;
+
+namespace {
+
+struct NetWs {                 // activation workspace of one generator net (planes are [channel][unit][row])
+  int Cmax = 0;
+  char* h = nullptr;           // L x [Cmax][H][R_ld]      post-activations h^1..h^L
+  char* st = nullptr;          // (L-1) x [Cmax-1][H][R_ld] stored a_x, a_y, a_xx, a_yy of layers 2..L
+  char* ah[2] = {nullptr, nullptr};   // adjoint ping-pong, [Cmax][H][R_ld]
+  float* apre = nullptr;       // fp32 mode: [Cmax][H][R_ld] pre-activations / hhat scratch
+  float* o = nullptr;          // [Cmax][R_ld] outputs of the chunk
+  float* oh = nullptr;         // [Cmax][R_ld] output adjoints (seeds)
+  float* Zp = nullptr;         // [N][H]  first-layer z-part
+  float* An = nullptr;         // [N][H]  per-sample sums of the first-layer value adjoint
+  void* w16 = nullptr;         // (L-1) x {W_l, W_l^T} 16-bit copies
+};
+
+}  // namespace
+
+struct pigan_ctx {
+  pigan_config cfg{};
+  NetShape gen{}, disc{};
+  Launcher L;
+  std::string err;
+  int elem = 4;                // bytes per activation element
+  int R_ld = 0;                // rows per chunk (leading dimension of every plane)
+  NetWs net[2];                // 0: G_logk (C <= 3), 1: G_u (C <= 5)
+  CriticWs cw;
+  float* xfake = nullptr;      // [N][2S]
+  float* dX = nullptr;         // [2N][2S]
+  float* seed = nullptr;       // [2N]
+  std::vector<void*> allocs;
+
+  template <typename T> T* alloc(size_t n) {
+    void* p = nullptr;
+    if (n == 0) n = 1;
+    if (cudaMalloc(&p, n * sizeof(T)) != cudaSuccess) { cudaGetLastError(); throw std::bad_alloc(); }
+    allocs.push_back(p);
+    return reinterpret_cast<T*>(p);
+  }
+  size_t plane() const { return (size_t)gen.H * R_ld * elem; }
+  char* h(int n, int l) { return net[n].h + (size_t)(l - 1) * net[n].Cmax * plane(); }              // l = 1..L
+  char* st(int n, int l) { return net[n].st + (size_t)(l - 2) * (net[n].Cmax - 1) * plane(); }      // l = 2..L
+  void* w16(int n, int l, int transposed) { return (char*)net[n].w16 + ((size_t)(l - 2) * 2 + transposed) * gen.H * gen.H * 2; }
+};
+
+namespace {
+
+pigan_status fail(pigan_ctx* c, pigan_status s, const std::string& msg) {
+  if (c) c->err = msg;
+  return s;
+}
+
+pigan_status finish(pigan_ctx* c) {
+  if (c->L.err != cudaSuccess) {
+    c->err = std::string("CUDA error at ") + c->L.where + ": " + cudaGetErrorString(c->L.err);
+    c->L.err = cudaSuccess;
+    return PIGAN_ERR_CUDA;
+  }
+  c->err.clear();
+  return PIGAN_OK;
+}
+
+size_t round_up(size_t a, size_t b) { return (a + b - 1) / b * b; }
+
+// ---- one chunk of generator rows, forward ------------------------------------------------------------------------
+template <typename T>
+void gen_forward_chunk(pigan_ctx* c, int n, const float* theta, int C, const float* xy, const ChunkGeom& g, float* o, long long o_stride,
+                       bool split = false) {
+  const NetShape& s = c->gen;
+  Launcher& L = c->L;
+  const int H = s.H;
+  const long long pl = (long long)H * g.R_ld;
+  // split (16-bit modes, value channel only): activations are carried as two 16-bit planes hi + lo, so that the
+  // snapshot X_fake the critic sees is accurate to ~2^-17 (the loss values are compared at 1e-3 relative)
+  split = split && C == 1 && c->cfg.precision != PIGAN_FP32;
+  first_layer_fwd<T>(L, C, s, theta, c->net[n].Zp, xy, g, (T*)c->h(n, 1), split);
+  for (int l = 2; l <= s.L; ++l) {
+    if (c->cfg.precision == PIGAN_FP32) {
+      // a_c = W_l h_c^{l-1}: M = H, N = rows, K = H, batched over the C channel planes
+      sgemm(L, false, false, H, g.R, H, theta + s.W_off(l), H, 0, (const float*)c->h(n, l - 1), g.R_ld, pl, c->net[n].apre, g.R_ld, pl, C, false);
+      jet_act_fwd_f32(L, C, H, theta + s.b_off(l), g, c->net[n].apre, (float*)c->h(n, l), (float*)c->st(n, l));
+    } else if (split) {
+      tc_layer_fwd_split(L, c->cfg.precision, H, g.R, g.R_ld, c->w16(n, l, 0), theta + s.b_off(l), c->h(n, l - 1), c->h(n, l));
+    } else {
+      tc_layer_fwd(L, c->cfg.precision, C, H, g.R, g.R_ld, c->w16(n, l, 0), theta + s.b_off(l), c->h(n, l - 1), c->h(n, l), c->st(n, l));
+    }
+  }
+  out_fwd<T>(L, C, H, theta + s.W_off(s.L + 1), theta + s.b_off(s.L + 1), g, (const T*)c->h(n, s.L), o, o_stride, split);
+}
+
+// ---- one chunk of generator rows, reverse sweep; output adjoints are in net[n].oh [C][R_ld] ------------------------
+template <typename T>
+void gen_backward_chunk(pigan_ctx* c, int n, const float* theta, float* grads, int C, const float* xy, const ChunkGeom& g) {
+  const NetShape& s = c->gen;
+  Launcher& L = c->L;
+  const int H = s.H;
+  const long long pl = (long long)H * g.R_ld;
+  int cur = 0;
+  jet_act_bwd_launch<T>(L, C, H, g, nullptr, theta + s.W_off(s.L + 1), c->net[n].oh, (const T*)c->h(n, s.L),
+                        s.L >= 2 ? (const T*)c->st(n, s.L) : nullptr, theta, s.in_dim, (T*)c->net[n].ah[cur], grads + s.b_off(s.L),
+                        grads + s.W_off(s.L + 1), grads + s.b_off(s.L + 1));
+  for (int l = s.L; l >= 2; --l) {
+    const T* stash_prev = l - 1 >= 2 ? (const T*)c->st(n, l - 1) : nullptr;
+    if (c->cfg.precision == PIGAN_FP32) {
+      // W_hat_l += sum_c ahat_c h_c^{l-1 T}: M = H, N = H, K = rows
+      sgemm(L, false, true, H, H, g.R, (const float*)c->net[n].ah[cur], g.R_ld, pl, (const float*)c->h(n, l - 1), g.R_ld, pl, grads + s.W_off(l), H, 0, C, true);
+      // hhat_c^{l-1} = W_l^T ahat_c: M = H (in), N = rows, K = H (out); A stored [K][M]
+      sgemm(L, true, false, H, g.R, H, theta + s.W_off(l), H, 0, (const float*)c->net[n].ah[cur], g.R_ld, pl, c->net[n].apre, g.R_ld, pl, C, false);
+      jet_act_bwd_launch<T>(L, C, H, g, c->net[n].apre, nullptr, nullptr, (const T*)c->h(n, l - 1), stash_prev, theta, s.in_dim,
+                            (T*)c->net[n].ah[cur ^ 1], grads + s.b_off(l - 1), nullptr, nullptr);
+    } else {
+      tc_wgrad(L, c->cfg.precision, C, H, g.R, g.R_ld, c->net[n].ah[cur], c->h(n, l - 1), grads + s.W_off(l));
+      tc_layer_bwd(L, c->cfg.precision, C, H, g.R, g.R_ld, c->w16(n, l, 1), c->net[n].ah[cur], c->h(n, l - 1), stash_prev, theta, s.in_dim,
+                   c->net[n].ah[cur ^ 1], grads + s.b_off(l - 1));
+    }
+    cur ^= 1;
+  }
+  first_layer_bwd<T>(L, C, s, xy, g, (const T*)c->net[n].ah[cur], grads, c->net[n].An);
+}
+
+ChunkGeom make_geom(const pigan_ctx* c, long long row0, long long total, int npts) {
+  ChunkGeom g;
+  g.row0 = row0;
+  g.valid = (int)std::min<long long>(c->R_ld, total - row0);
+  g.R = (int)round_up(g.valid, 64);
+  g.R_ld = c->R_ld;
+  g.npts = npts;
+  return g;
+}
+
+void compute_zpart(pigan_ctx* c, int n, const float* theta, const float* z, int n_samples) {
+  const NetShape& s = c->gen;
+  // Zp[n][j] = sum_k W1[j][2+k] z[n][k]   (a1: once per sample; the bias is added with the xy-part)
+  sgemm(c->L, false, true, n_samples, s.H, s.in_dim - 2, z, s.in_dim - 2, 0, theta + 2, s.in_dim, 0, c->net[n].Zp, s.H, 0, 1, false);
+}
+
+template <typename T>
+pigan_status jet_forward_impl(pigan_ctx* c, const float* theta, const float* xy, int n_pts, const float* z, int n_samples, int C, float* out) {
+  const long long total = (long long)n_samples * n_pts;
+  const int n = 1;
+  compute_zpart(c, n, theta, z, n_samples);
+  if (c->cfg.precision != PIGAN_FP32) tc_convert_weights(c->L, c->cfg.precision, c->gen, theta, c->net[n].w16);
+  for (long long row0 = 0; row0 < total; row0 += c->R_ld) {
+    ChunkGeom g = make_geom(c, row0, total, n_pts);
+    gen_forward_chunk<T>(c, n, theta, C, xy, g, out + row0, total, /*split=*/C == 1);
+  }
+  return finish(c);
+}
+
+template <typename T>
+pigan_status train_step_impl(pigan_ctx* c, const float* thY, const float* thU, const float* thD, const float* xy_c, const float* f,
+                             const float* xy_s, const float* z, const float* real, const float* eps, float loss_scale, float* gY,
+                             float* gU, float* gD, float* losses, int* found_inf) {
+  const pigan_config& cfg = c->cfg;
+  Launcher& L = c->L;
+  const NetShape& gs = c->gen; const NetShape& ds = c->disc;
+  const int N = cfg.n_samples, P = cfg.n_colloc, S = cfg.n_sensors, d = 2 * S, HD = ds.H;
+  const float* th[2] = {thY, thU};
+  float* gr[2] = {gY, gU};
+  cudaStream_t st = L.stream;
+  cudaMemsetAsync(gY, 0, gs.count() * 4, st); cudaMemsetAsync(gU, 0, gs.count() * 4, st); cudaMemsetAsync(gD, 0, ds.count() * 4, st);
+  cudaMemsetAsync(c->cw.acc, 0, 8 * sizeof(double), st);
+  if (found_inf) cudaMemsetAsync(found_inf, 0, sizeof(int), st);
+  for (int n = 0; n < 2; ++n) {
+    cudaMemsetAsync(c->net[n].An, 0, (size_t)N * gs.H * 4, st);
+    compute_zpart(c, n, th[n], z, N);
+    if (cfg.precision != PIGAN_FP32) tc_convert_weights(L, cfg.precision, gs, th[n], c->net[n].w16);
+  }
+  // ---- a6: sensor evaluation -> X_fake ----
+  const long long srows = (long long)N * S;
+  for (long long row0 = 0; row0 < srows; row0 += c->R_ld) {
+    ChunkGeom g = make_geom(c, row0, srows, S);
+    for (int n = 0; n < 2; ++n) {
+      gen_forward_chunk<T>(c, n, th[n], 1, xy_s, g, c->net[n].o, c->R_ld, /*split=*/true);
+      scatter_snapshot(L, c->net[n].o, row0, g.valid, S, d, n * S, c->xfake);
+    }
+  }
+  // ---- a7-a9: critic losses and gradient; dX rows [0, N) = (1/N) grad_X D(X_fake) ----
+  build_snapshots(L, c->xfake, real, eps, N, d, c->cw.X);
+  critic_forward(L, ds, thD, c->cw.X, 3 * N, c->cw.g, c->cw.D, nullptr);
+  reduce_scores(L, c->cw.D, N, c->cw.acc);
+  fill_seed(L, c->seed, N);
+  const int gstride = 3 * N * HD;
+  critic_backward(L, ds, thD, c->cw.X, c->cw.g, 2 * N, gstride, c->seed, gD, c->dX, c->cw.t0, c->cw.t1);
+  critic_gp(L, ds, thD, c->cw.X + (size_t)2 * N * d, c->cw.g + (size_t)2 * N * HD, N, gstride, cfg.gp_lambda, c->cw, gD, nullptr);
+  // ---- O7 + a10 on the sensor rows: dL_G/dX_fake = -(1/N) grad_X D(X_fake), value channel only ----
+  for (long long row0 = 0; row0 < srows; row0 += c->R_ld) {
+    ChunkGeom g = make_geom(c, row0, srows, S);
+    for (int n = 0; n < 2; ++n) {
+      gen_forward_chunk<T>(c, n, th[n], 1, xy_s, g, c->net[n].o, c->R_ld);
+      gather_seed(L, c->dX, row0, g.valid, g.R, S, d, n * S, -loss_scale, c->net[n].oh);
+      gen_backward_chunk<T>(c, n, th[n], gr[n], 1, xy_s, g);
+    }
+  }
+  // ---- a1-a5, a10 on the collocation rows ----
+  const long long crows = (long long)N * P;
+  const float seed_scale = (float)(2.0 * cfg.pde_weight / (double)crows * loss_scale);
+  for (long long row0 = 0; row0 < crows; row0 += c->R_ld) {
+    ChunkGeom g = make_geom(c, row0, crows, P);
+    gen_forward_chunk<T>(c, 0, thY, 3, xy_c, g, c->net[0].o, c->R_ld);
+    gen_forward_chunk<T>(c, 1, thU, 5, xy_c, g, c->net[1].o, c->R_ld);
+    residual(L, c->net[0].o, c->R_ld, c->net[1].o, c->R_ld, f, row0, g.valid, g.R, P, nullptr, c->cw.acc + 3, seed_scale, c->net[0].oh,
+             c->net[1].oh, c->R_ld);
+    gen_backward_chunk<T>(c, 0, thY, gY, 3, xy_c, g);
+    gen_backward_chunk<T>(c, 1, thU, gU, 5, xy_c, g);
+  }
+  // ---- finalize: z-part of the first layer, unscale, inf/nan flag, loss scalars ----
+  for (int n = 0; n < 2; ++n) {
+    finalize_first_layer(L, gs, N, c->net[n].An, z, gr[n]);
+    unscale_and_check(L, gr[n], gs.count(), 1.f / loss_scale, found_inf);
+  }
+  unscale_and_check(L, gD, ds.count(), 1.f, found_inf);
+  if (losses) write_losses(L, c->cw.acc, N, crows, cfg.gp_lambda, cfg.pde_weight, losses, nullptr, nullptr, 0);
+  return finish(c);
+}
+
+bool shape_ok(const pigan_mlp_shape& s) { return s.in_dim >= 1 && s.n_hidden >= 1 && s.width >= 1; }
+
+}  // namespace
+
+// =================================================================================================================
+extern "C" {
+
+size_t pigan_param_count(const pigan_mlp_shape* s) {
+  if (!s || !shape_ok(*s)) return 0;
+  NetShape n{s->in_dim, s->n_hidden, s->width};
+  return n.count();
+}
+
+const char* pigan_last_error(const pigan_ctx* c) { return c ? c->err.c_str() : "null context"; }
+unsigned long long pigan_launch_count(const pigan_ctx* c) { return c ? c->L.count : 0; }
+
+pigan_status pigan_profile_enable(pigan_ctx* c, int enable) {
+  if (!c) return PIGAN_ERR_INVALID_ARG;
+  c->L.profiling = enable != 0;
+  if (enable) { c->L.n_rec = 0; c->L.mark("begin"); }
+  return PIGAN_OK;
+}
+
+pigan_status pigan_profile_report(pigan_ctx* c, char* buf, size_t cap) {
+  if (!c || !buf || cap == 0) return PIGAN_ERR_INVALID_ARG;
+  if (c->L.n_rec == 0) return fail(c, PIGAN_ERR_INVALID_ARG, "profiling was not enabled");
+  if (cudaStreamSynchronize(c->L.stream) != cudaSuccess) return fail(c, PIGAN_ERR_CUDA, "stream synchronize failed");
+  std::vector<std::pair<std::string, std::pair<unsigned long long, double>>> acc;
+  for (size_t i = 1; i < c->L.n_rec; ++i) {
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, c->L.events[i - 1], c->L.events[i]);
+    const std::string name = c->L.names[i];
+    size_t k = 0;
+    for (; k < acc.size(); ++k) if (acc[k].first == name) break;
+    if (k == acc.size()) acc.push_back({name, {0ull, 0.0}});
+    acc[k].second.first += 1; acc[k].second.second += ms;
+  }
+  std::string js = "{";
+  for (size_t k = 0; k < acc.size(); ++k) {
+    char tmp[160];
+    snprintf(tmp, sizeof tmp, "%s\"%s\": [%llu, %.6f]", k ? ", " : "", acc[k].first.c_str(), acc[k].second.first, acc[k].second.second);
+    js += tmp;
+  }
+  js += "}";
+  snprintf(buf, cap, "%s", js.c_str());
+  c->L.n_rec = 0;
+  if (c->L.profiling) c->L.mark("begin");
+  return PIGAN_OK;
+}
+
+pigan_status pigan_create(const pigan_config* cfg, void* cuda_stream, pigan_ctx** out) {
+  if (out) *out = nullptr;
+  if (!cfg || !out) return PIGAN_ERR_INVALID_ARG;
+  if (!shape_ok(cfg->gen) || !shape_ok(cfg->disc) || cfg->latent_dim < 1 || cfg->n_samples < 1 || cfg->n_colloc < 1 || cfg->n_sensors < 1)
+    return PIGAN_ERR_INVALID_ARG;
+  if ((int)cfg->precision < 0 || (int)cfg->precision > 2 || !(cfg->gp_lambda >= 0.f)) return PIGAN_ERR_INVALID_ARG;
+  if (cfg->gen.in_dim != 2 + cfg->latent_dim || cfg->disc.in_dim != 2 * cfg->n_sensors) return PIGAN_ERR_SHAPE;
+  if (cfg->precision != PIGAN_FP32) {
+    std::string why;
+    if (!tc_supported(cfg->gen.width, &why)) return PIGAN_ERR_UNSUPPORTED;
+  }
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); return PIGAN_ERR_CUDA; }
+  pigan_ctx* c = new (std::nothrow) pigan_ctx();
+  if (!c) return PIGAN_ERR_ALLOC;
+  c->cfg = *cfg;
+  c->gen = NetShape{cfg->gen.in_dim, cfg->gen.n_hidden, cfg->gen.width};
+  c->disc = NetShape{cfg->disc.in_dim, cfg->disc.n_hidden, cfg->disc.width};
+  c->L.stream = (cudaStream_t)cuda_stream;
+  c->elem = cfg->precision == PIGAN_FP32 ? 4 : 2;
+  const int H = c->gen.H, Lh = c->gen.L, N = cfg->n_samples, S = cfg->n_sensors, d = 2 * S, HD = c->disc.H, LD = c->disc.L;
+  const bool f32 = cfg->precision == PIGAN_FP32;
+  // bytes per chunk row over both nets: h (L*C) + stash ((L-1)(C-1)) + adjoint ping-pong (2C) planes [+ fp32 scratch]
+  size_t per_row = 0;
+  for (int C : {3, 5}) per_row += ((size_t)Lh * C + (size_t)(Lh - 1) * (C - 1) + 2 * C) * H * c->elem + (f32 ? (size_t)C * H * 4 : 0) + 2 * C * 4;
+  const long long max_rows = std::max<long long>((long long)N * cfg->n_colloc, (long long)N * S);
+  size_t free_b = 0, total_b = 0;
+  cudaMemGetInfo(&free_b, &total_b);
+  size_t budget = cfg->workspace_bytes ? cfg->workspace_bytes : std::min<size_t>(free_b / 2, (size_t)24 << 30);
+  long long rows = (long long)(budget / per_row);
+  long long cap = 16384;                                   // default chunk: keeps one layer's planes near the L2 size
+  if (const char* e = getenv("PIGAN_CHUNK_ROWS")) cap = std::max(256LL, atoll(e));
+  if (!cfg->workspace_bytes) rows = std::min(rows, cap);
+  rows = std::min<long long>(rows, (long long)round_up((size_t)max_rows, 256));
+  rows = std::max<long long>(rows / 256 * 256, 256);            // workspace_bytes is a hint: never below one 256-row chunk
+  c->R_ld = (int)rows;
+  try {
+    for (int n = 0; n < 2; ++n) {
+      NetWs& w = c->net[n];
+      w.Cmax = n == 0 ? 3 : 5;
+      const size_t pl = c->plane();
+      w.h = c->alloc<char>((size_t)Lh * w.Cmax * pl);
+      w.st = c->alloc<char>((size_t)std::max(Lh - 1, 1) * (w.Cmax - 1) * pl);
+      w.ah[0] = c->alloc<char>((size_t)w.Cmax * pl);
+      w.ah[1] = c->alloc<char>((size_t)w.Cmax * pl);
+      if (f32) w.apre = c->alloc<float>((size_t)w.Cmax * H * c->R_ld);
+      w.o = c->alloc<float>((size_t)w.Cmax * c->R_ld);
+      w.oh = c->alloc<float>((size_t)w.Cmax * c->R_ld);
+      w.Zp = c->alloc<float>((size_t)N * H);
+      w.An = c->alloc<float>((size_t)N * H);
+      if (!f32) w.w16 = c->alloc<char>((size_t)std::max(Lh - 1, 1) * 2 * H * H * 2);
+    }
+    const size_t wmax = (size_t)std::max(d, HD);
+    CriticWs& cw = c->cw;
+    cw.maxB = N;
+    cw.X = c->alloc<float>((size_t)3 * N * d);
+    cw.g = c->alloc<float>((size_t)LD * 3 * N * HD);
+    cw.D = c->alloc<float>((size_t)3 * N);
+    cw.t0 = c->alloc<float>((size_t)3 * N * wmax);
+    cw.t1 = c->alloc<float>((size_t)3 * N * wmax);
+    cw.t2 = c->alloc<float>((size_t)3 * N * wmax);
+    cw.gbar = c->alloc<float>((size_t)(LD + 1) * N * wmax);
+    cw.abar = c->alloc<float>((size_t)LD * N * HD);
+    cw.adjs = c->alloc<float>((size_t)LD * N * HD);
+    cw.nu = c->alloc<float>((size_t)N);
+    cw.acc = c->alloc<double>(8);
+    c->xfake = c->alloc<float>((size_t)N * d);
+    c->dX = c->alloc<float>((size_t)2 * N * d);
+    c->seed = c->alloc<float>((size_t)2 * N);
+  } catch (const std::bad_alloc&) {
+    pigan_destroy(c);
+    return PIGAN_ERR_ALLOC;
+  }
+  *out = c;
+  return PIGAN_OK;
+}
+
+void pigan_destroy(pigan_ctx* c) {
+  if (!c) return;
+  for (void* p : c->allocs) cudaFree(p);
+  for (cudaEvent_t e : c->L.events) cudaEventDestroy(e);
+  delete c;
+}
+
+pigan_status pigan_gen_jet_forward(pigan_ctx* c, const float* gen_params, const float* xy, int n_pts, const float* z, int n_samples,
+                                   int jet_order, float* out) {
+  if (!c) return PIGAN_ERR_INVALID_ARG;
+  if (jet_order < 0 || jet_order > 2 || n_pts < 0 || n_samples < 0) return fail(c, PIGAN_ERR_INVALID_ARG, "jet_order must be 0..2 and sizes >= 0");
+  if (n_pts == 0 || n_samples == 0) return PIGAN_OK;
+  if (!gen_params || !xy || !z || !out) return fail(c, PIGAN_ERR_INVALID_ARG, "null pointer");
+  if (n_samples > c->cfg.n_samples) return fail(c, PIGAN_ERR_SHAPE, "n_samples exceeds the n_samples of the config");
+  const int C = jet_order == 0 ? 1 : jet_order == 1 ? 3 : 5;
+  switch (c->cfg.precision) {
+    case PIGAN_FP32: return jet_forward_impl<float>(c, gen_params, xy, n_pts, z, n_samples, C, out);
+    case PIGAN_BF16: return jet_forward_impl<__nv_bfloat16>(c, gen_params, xy, n_pts, z, n_samples, C, out);
+    default: return jet_forward_impl<__half>(c, gen_params, xy, n_pts, z, n_samples, C, out);
+  }
+}
+
+pigan_status pigan_darcy_residual(pigan_ctx* c, const float* logk_jet, const float* u_jet, const float* f, int n_samples, int n_pts,
+                                  float* r, float* mean_sq) {
+  if (!c) return PIGAN_ERR_INVALID_ARG;
+  if (n_samples < 0 || n_pts < 0) return fail(c, PIGAN_ERR_INVALID_ARG, "negative size");
+  const long long total = (long long)n_samples * n_pts;
+  if (total > 0 && (!logk_jet || !u_jet || !f)) return fail(c, PIGAN_ERR_INVALID_ARG, "null pointer");
+  cudaMemsetAsync(c->cw.acc, 0, 8 * sizeof(double), c->L.stream);
+  for (long long row0 = 0; row0 < total; row0 += (1 << 30)) {
+    const int rows = (int)std::min<long long>(1 << 30, total - row0);
+    residual(c->L, logk_jet + row0, total, u_jet + row0, total, f, row0, rows, rows, n_pts, r ? r + row0 : nullptr, mean_sq ? c->cw.acc + 3 : nullptr,
+             0.f, nullptr, nullptr, 0);
+  }
+  if (mean_sq) write_losses(c->L, c->cw.acc, 1, 1, 0.f, 0.f, nullptr, nullptr, mean_sq, total);
+  return finish(c);
+}
+
+pigan_status pigan_disc_forward(pigan_ctx* c, const float* disc_params, const float* snap, int B, float* score) {
+  if (!c) return PIGAN_ERR_INVALID_ARG;
+  if (B < 0) return fail(c, PIGAN_ERR_INVALID_ARG, "negative batch");
+  if (B == 0) return PIGAN_OK;
+  if (!disc_params || !snap || !score) return fail(c, PIGAN_ERR_INVALID_ARG, "null pointer");
+  const int d = c->disc.in_dim, cap = 3 * c->cfg.n_samples;
+  for (int b0 = 0; b0 < B; b0 += cap) {
+    const int rows = std::min(cap, B - b0);
+    critic_forward(c->L, c->disc, disc_params, snap + (size_t)b0 * d, rows, c->cw.g, score + b0, nullptr);
+  }
+  return finish(c);
+}
+
+pigan_status pigan_gradient_penalty(pigan_ctx* c, const float* disc_params, const float* real, const float* fake, const float* eps, int B,
+                                    float* gp, float* grad_norm, float* d_disc_params) {
+  if (!c) return PIGAN_ERR_INVALID_ARG;
+  if (B < 1) return fail(c, PIGAN_ERR_INVALID_ARG, "B must be >= 1");
+  if (!disc_params || !real || !fake || !eps) return fail(c, PIGAN_ERR_INVALID_ARG, "null pointer");
+  if (B > c->cfg.n_samples) return fail(c, PIGAN_ERR_SHAPE, "B exceeds the n_samples of the config");
+  const NetShape& ds = c->disc;
+  const int d = ds.in_dim, HD = ds.H;
+  cudaStream_t st = c->L.stream;
+  cudaMemsetAsync(c->cw.acc, 0, 8 * sizeof(double), st);
+  if (d_disc_params) cudaMemsetAsync(d_disc_params, 0, ds.count() * 4, st);
+  build_snapshots(c->L, fake, real, eps, B, d, c->cw.X);
+  float* Xhat = c->cw.X + (size_t)2 * B * d;
+  critic_forward(c->L, ds, disc_params, Xhat, B, c->cw.g, c->cw.D, nullptr);
+  critic_gp(c->L, ds, disc_params, Xhat, c->cw.g, B, B * HD, c->cfg.gp_lambda, c->cw, d_disc_params, grad_norm);
+  if (gp) write_losses(c->L, c->cw.acc, B, 1, c->cfg.gp_lambda, 0.f, nullptr, gp, nullptr, 0);
+  return finish(c);
+}
+
+pigan_status pigan_train_step_grads(pigan_ctx* c, const float* logk_params, const float* u_params, const float* disc_params,
+                                    const float* xy_colloc, const float* f, const float* xy_sensors, const float* z, const float* real_snap,
+                                    const float* eps, float loss_scale, float* g_logk, float* g_u, float* g_disc, float* losses, int* found_inf) {
+  if (!c) return PIGAN_ERR_INVALID_ARG;
+  if (!logk_params || !u_params || !disc_params || !xy_colloc || !f || !xy_sensors || !z || !real_snap || !eps || !g_logk || !g_u || !g_disc)
+    return fail(c, PIGAN_ERR_INVALID_ARG, "null pointer");
+  if (!(loss_scale > 0.f) || !std::isfinite(loss_scale)) return fail(c, PIGAN_ERR_INVALID_ARG, "loss_scale must be positive and finite");
+  switch (c->cfg.precision) {
+    case PIGAN_FP32: return train_step_impl<float>(c, logk_params, u_params, disc_params, xy_colloc, f, xy_sensors, z, real_snap, eps, loss_scale, g_logk, g_u, g_disc, losses, found_inf);
+    case PIGAN_BF16: return train_step_impl<__nv_bfloat16>(c, logk_params, u_params, disc_params, xy_colloc, f, xy_sensors, z, real_snap, eps, loss_scale, g_logk, g_u, g_disc, losses, found_inf);
+    default: return train_step_impl<__half>(c, logk_params, u_params, disc_params, xy_colloc, f, xy_sensors, z, real_snap, eps, loss_scale, g_logk, g_u, g_disc, losses, found_inf);
+  }
+}
+
+pigan_status pigan_adam_update(pigan_ctx* c, float* params, const float* grads, float* m, float* v, size_t n, int step, float lr, float beta1,
+                               float beta2, float adam_eps, const int* skip_flag) {
+  if (!c) return PIGAN_ERR_INVALID_ARG;
+  if (n == 0) return PIGAN_OK;
+  if (!params || !grads || !m || !v) return fail(c, PIGAN_ERR_INVALID_ARG, "null pointer");
+  if (step < 1) return fail(c, PIGAN_ERR_INVALID_ARG, "step is 1-based");
+  const float c1 = (float)(1.0 - std::pow((double)beta1, step)), c2 = (float)(1.0 - std::pow((double)beta2, step));
+  adam(c->L, params, grads, m, v, n, lr, beta1, beta2, adam_eps, c1, c2, skip_flag);
+  return finish(c);
+}
+
+}  // extern "C"

@@ -1,0 +1,189 @@
+// Internal declarations shared by the translation units of libpigan.so (not part of the C-ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <cuda_bf16.h>
+#include <cuda_fp16.h>
+#include <cstdint>
+#include <cstdio>
+#include <string>
+#include <vector>
+
+#include "pigan.h"
+
+namespace pigan {
+
+// ---- flat parameter packing (include/pigan.h): W_l [out][in] then b_l [out], l = 1..L+1 ----------------------
+struct NetShape {
+  int in_dim, L, H;
+  __host__ __device__ size_t first_size() const { return (size_t)H * in_dim + H; }
+  __host__ __device__ size_t W_off(int l) const {              // l is 1-based
+    if (l == 1) return 0;
+    return first_size() + (size_t)(l - 2) * ((size_t)H * H + H);
+  }
+  __host__ __device__ size_t b_off(int l) const {
+    if (l == 1) return (size_t)H * in_dim;
+    if (l <= L) return W_off(l) + (size_t)H * H;
+    return W_off(l) + H;                                       // output layer: w_out [H], then b_out
+  }
+  __host__ __device__ size_t count() const { return first_size() + (size_t)(L - 1) * ((size_t)H * H + H) + H + 1; }
+};
+
+template <typename T> __device__ __forceinline__ float to_f(T v);
+template <> __device__ __forceinline__ float to_f<float>(float v) { return v; }
+template <> __device__ __forceinline__ float to_f<__nv_bfloat16>(__nv_bfloat16 v) { return __bfloat162float(v); }
+template <> __device__ __forceinline__ float to_f<__half>(__half v) { return __half2float(v); }
+template <typename T> __device__ __forceinline__ T from_f(float v);
+template <> __device__ __forceinline__ float from_f<float>(float v) { return v; }
+template <> __device__ __forceinline__ __nv_bfloat16 from_f<__nv_bfloat16>(float v) { return __float2bfloat16_rn(v); }
+template <> __device__ __forceinline__ __half from_f<__half>(float v) { return __float2half_rn(v); }
+
+// ---- the tanh jet chain rule and its adjoint (O4); C = 1, 3 or 5 channels ------------------
+// forward: a[0] already holds the value pre-activation (bias added); a[1..] the derivative pre-activations.
+template <int C>
+__device__ __forceinline__ void jet_act_fwd(float t, const float* a, float* h) {
+  const float s = 1.f - t * t;
+  h[0] = t;
+  if (C >= 3) { h[1] = s * a[1]; h[2] = s * a[2]; }
+  if (C >= 5) {
+    const float q = -2.f * t * s;
+    h[3] = fmaf(s, a[3], q * a[1] * a[1]);
+    h[4] = fmaf(s, a[4], q * a[2] * a[2]);
+  }
+}
+// adjoint: hh = adjoints of h_c; t = tanh(a); ad[0..C-2] = stored a_x, a_y, a_xx, a_yy; aa = adjoints of a_c.
+template <int C>
+__device__ __forceinline__ void jet_act_bwd(float t, const float* ad, const float* hh, float* aa) {
+  const float s = 1.f - t * t;
+  float v = s * hh[0];
+  if (C >= 3) {
+    const float q = -2.f * t * s;
+    v = fmaf(q, fmaf(ad[0], hh[1], ad[1] * hh[2]), v);
+    aa[1] = s * hh[1];
+    aa[2] = s * hh[2];
+    if (C >= 5) {
+      const float qp = -2.f * s * (1.f - 3.f * t * t);
+      v = fmaf(q, fmaf(ad[2], hh[3], ad[3] * hh[4]), v);
+      v = fmaf(qp, fmaf(ad[0] * ad[0], hh[3], ad[1] * ad[1] * hh[4]), v);
+      aa[1] = fmaf(2.f * q * ad[0], hh[3], aa[1]);
+      aa[2] = fmaf(2.f * q * ad[1], hh[4], aa[2]);
+      aa[3] = s * hh[3];
+      aa[4] = s * hh[4];
+    }
+  }
+  aa[0] = v;
+}
+
+// ---- launch bookkeeping -------------------------------------------------------------------------------------
+struct Launcher {
+  cudaStream_t stream = nullptr;
+  unsigned long long count = 0;
+  cudaError_t err = cudaSuccess;
+  const char* where = "";
+  // optional per-launch CUDA-event trace (pigan_profile_*): one event after every launch on the launch stream;
+  // the duration of launch i is event_i - event_{i-1} (the stream is kept busy, so gaps are launch latency only).
+  bool profiling = false;
+  std::vector<cudaEvent_t> events;
+  std::vector<const char*> names;
+  size_t n_rec = 0;
+  void check(const char* w) {
+    ++count;
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess && err == cudaSuccess) { err = e; where = w; }
+    if (profiling) mark(w);
+  }
+  void mark(const char* w) {
+    if (n_rec == events.size()) { cudaEvent_t ev; cudaEventCreate(&ev); events.push_back(ev); names.push_back(w); }
+    names[n_rec] = w;
+    cudaEventRecord(events[n_rec++], stream);
+  }
+};
+
+// ---- SIMT kernels (simt_kernels.cu) ---------------------------------------------------------------------------
+// C[M x N] (ldc) = or += alpha * op(A)[M x K] op(B)[K x N], batched (batch index adds sA/sB/sC), fp32.
+//   TA: A stored [K][M] (lda) else [M][K];  TB: B stored [N][K] (ldb) else [K][N].
+//   accumulate: atomicAdd into C (C must be initialised) -- also used when the K range is split.
+void sgemm(Launcher& L, bool TA, bool TB, int M, int N, int K, const float* A, int lda, long long sA, const float* B,
+           int ldb, long long sB, float* C, int ldc, long long sC, int batch, bool accumulate, float alpha = 1.f);
+
+struct ChunkGeom {          // one chunk of generator rows r = row0 .. row0+valid-1 ; row -> (n, p) = (r / npts, r % npts)
+  long long row0;           // first global row of the chunk
+  int valid;                // rows of the chunk that exist (<= R)
+  int R;                    // rows computed (valid rounded up to the row tile)
+  int R_ld;                 // leading dimension (rows) of every plane
+  int npts;                 // points per latent sample
+};
+
+template <typename T>
+void first_layer_fwd(Launcher& L, int C, const NetShape& s, const float* theta, const float* Zp, const float* xy,
+                     const ChunkGeom& g, T* h1, bool split = false);   // split: C = 1, writes planes (hi, lo)
+void jet_act_fwd_f32(Launcher& L, int C, int H, const float* bias, const ChunkGeom& g, const float* apre, float* h, float* stash);
+template <typename T>
+void out_fwd(Launcher& L, int C, int H, const float* w_out, const float* b_out, const ChunkGeom& g, const T* hL,
+             float* o, long long o_plane_stride, bool split = false);          // split: C = 1, sums planes (hi, lo)
+void residual(Launcher& L, const float* Y, long long y_stride, const float* U, long long u_stride, const float* f,
+              long long row0, int valid, int R, int npts, float* r_out, double* sum_sq, float seed_scale, float* seedY,
+              float* seedU, int seed_ld);
+// adjoint of one tanh layer: hh_c = (hhat planes) or (w_out[j] * ohat_c[r]) ; writes ahat planes, accumulates
+// b_hat_l[j] += sum_r ahat_0 (and for the output layer w_hat_out[j], b_hat_out).
+template <typename T>
+void jet_act_bwd_launch(Launcher& L, int C, int H, const ChunkGeom& g, const float* hhat /*or null*/,
+                        const float* w_out, const float* ohat /*[C][R_ld] when hhat null*/, const T* h /*[C][H][R_ld]*/,
+                        const T* stash /*[C-1][H][R_ld] or null = layer 1*/, const float* W1, int in_dim, T* ahat,
+                        float* g_bias, float* g_wout, float* g_bout);
+template <typename T>
+void first_layer_bwd(Launcher& L, int C, const NetShape& s, const float* xy, const ChunkGeom& g, const T* ahat,
+                     float* gW1 /* flat grads base of this net */, float* An /*[N][H]*/);
+void finalize_first_layer(Launcher& L, const NetShape& s, int N, const float* An, const float* z, float* grads);
+void unscale_and_check(Launcher& L, float* g, size_t n, float inv_scale, int* found_inf);
+void adam(Launcher& L, float* p, const float* g, float* m, float* v, size_t n, float lr, float b1, float b2, float eps,
+          float c1, float c2, const int* skip);
+
+// critic (always fp32; activations are batch-major [rows][width])
+struct CriticWs {
+  float* X = nullptr;       // [3B][d]   fake, real, xhat
+  float* g = nullptr;       // (LD) x [3B][HD]   g^1..g^LD
+  float* D = nullptr;       // [3B]
+  float* t0 = nullptr;      // scratch [3B][max(d,HD)]
+  float* t1 = nullptr;      // scratch [3B][max(d,HD)]
+  float* t2 = nullptr;      // scratch [3B][max(d,HD)]
+  float* gbar = nullptr;    // (LD+1) x [B][max(d,HD)]  gbar^0..gbar^LD  (gp)
+  float* abar = nullptr;    // (LD) x [B][HD]           abar^1..abar^LD
+  float* adjs = nullptr;    // (LD) x [B][HD]           adj(s^l)
+  float* nu = nullptr;      // [B]
+  double* acc = nullptr;    // [8] accumulators: 0 sum D fake, 1 sum D real, 2 sum (nu-1)^2, 3 sum r^2
+  int maxB = 0;
+};
+void critic_forward(Launcher& L, const NetShape& s, const float* theta, const float* X, int rows, float* g, float* D,
+                    float* scratch);
+// plain backprop of sum_b seed[b] D(X_b) over `rows` rows starting at activations g; accumulates into grads if non-null;
+// writes d/dX into dX if non-null.
+void critic_backward(Launcher& L, const NetShape& s, const float* theta, const float* X, const float* g, int rows,
+                     int ld_rows, const float* seed, float* grads, float* dX, float* t0, float* t1);
+void critic_gp(Launcher& L, const NetShape& s, const float* theta, const float* Xhat, const float* g /*of xhat rows*/,
+               int B, int g_layer_stride, float lambda, CriticWs& w, float* grads /*may be null*/, float* grad_norm);
+void build_snapshots(Launcher& L, const float* fake, const float* real, const float* eps, int B, int d, float* X);
+void scale_copy(Launcher& L, const float* src, float* dst, size_t n, float alpha);
+void fill_seed(Launcher& L, float* seed, int B);
+void scatter_snapshot(Launcher& L, const float* o, long long row0, int valid, int S, int d, int col0, float* X);
+void gather_seed(Launcher& L, const float* dX, long long row0, int valid, int R, int S, int d, int col0, float alpha, float* seed);
+void reduce_scores(Launcher& L, const float* D, int B, double* acc);
+void write_losses(Launcher& L, const double* acc, int N, long long NP, float lambda, float w_pde, float* losses, float* gp_out,
+                  float* meansq_out, long long meansq_count);
+
+// ---- tensor-core kernels (tc_kernels.cu), 16-bit modes -------------------------------------------------------
+struct TcPlan;   // opaque: tensor maps + 16-bit weight copies for one (net, chunk buffer set)
+bool tc_supported(int H, std::string* why);
+// Converts W_l (l = 2..L) of one net to 16-bit: w16[(l-2)*2+0] = W_l [out][in], w16[(l-2)*2+1] = W_l^T [in][out].
+void tc_convert_weights(Launcher& L, int precision, const NetShape& s, const float* theta, void* w16);
+// hidden layer l forward: h_in [C][H][R_ld] -> h_out [C][H][R_ld], stash [C-1][H][R_ld]   (fused tanh-jet epilogue)
+void tc_layer_fwd(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* w16_l, const float* bias,
+                  const void* h_in, void* h_out, void* stash);
+void tc_layer_fwd_split(Launcher& L, int precision, int H, int R, int R_ld, const void* w16_l, const float* bias, const void* h_in, void* h_out);
+// dgrad of layer l with the adjoint of layer l-1's tanh fused: ahat_in (layer l) -> ahat_out (layer l-1)
+void tc_layer_bwd(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* w16T_l, const void* ahat_in,
+                  const void* h_prev /*[C][H][R_ld], value plane = t*/, const void* stash_prev /*null = layer 1*/,
+                  const float* W1, int in_dim, void* ahat_out, float* g_bias_prev);
+// wgrad of layer l: gW [H][H] += sum_c ahat_c h_prev_c^T   (fp32 atomics)
+void tc_wgrad(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* ahat, const void* h_prev, float* gW);
+
+}  // namespace pigan

@@ -1,0 +1,332 @@
+// Generator-side SIMT kernels (HBM-bound): first layer (S8a a1/a2), output dot (a4), adjoint of a tanh layer in SIMT form
+// (top layer in every mode, all layers in fp32 mode; O4), first-layer backward.  Planes are [channel][unit][row]; every
+// thread owns 8 consecutive rows of one unit, so all plane accesses are 16-byte (16-bit modes) or 32-byte (fp32) vectors
+// and a warp touches 512 contiguous bytes per plane.
+#include "common.cuh"
+
+namespace pigan {
+
+static inline int cdiv(long long a, long long b) { return (int)((a + b - 1) / b); }
+
+template <typename T> __device__ __forceinline__ void load8(const T* p, float* v);
+template <> __device__ __forceinline__ void load8<float>(const float* p, float* v) {
+  const float4 a = *reinterpret_cast<const float4*>(p), b = *reinterpret_cast<const float4*>(p + 4);
+  v[0] = a.x; v[1] = a.y; v[2] = a.z; v[3] = a.w; v[4] = b.x; v[5] = b.y; v[6] = b.z; v[7] = b.w;
+}
+template <> __device__ __forceinline__ void load8<__nv_bfloat16>(const __nv_bfloat16* p, float* v) {
+  const uint4 u = *reinterpret_cast<const uint4*>(p);
+  const __nv_bfloat162* h = reinterpret_cast<const __nv_bfloat162*>(&u);
+#pragma unroll
+  for (int i = 0; i < 4; ++i) { const float2 f = __bfloat1622float2(h[i]); v[2 * i] = f.x; v[2 * i + 1] = f.y; }
+}
+template <> __device__ __forceinline__ void load8<__half>(const __half* p, float* v) {
+  const uint4 u = *reinterpret_cast<const uint4*>(p);
+  const __half2* h = reinterpret_cast<const __half2*>(&u);
+#pragma unroll
+  for (int i = 0; i < 4; ++i) { const float2 f = __half22float2(h[i]); v[2 * i] = f.x; v[2 * i + 1] = f.y; }
+}
+template <typename T> __device__ __forceinline__ void store8(T* p, const float* v);
+template <> __device__ __forceinline__ void store8<float>(float* p, const float* v) {
+  *reinterpret_cast<float4*>(p) = make_float4(v[0], v[1], v[2], v[3]);
+  *reinterpret_cast<float4*>(p + 4) = make_float4(v[4], v[5], v[6], v[7]);
+}
+template <> __device__ __forceinline__ void store8<__nv_bfloat16>(__nv_bfloat16* p, const float* v) {
+  uint4 u;
+  __nv_bfloat162* h = reinterpret_cast<__nv_bfloat162*>(&u);
+#pragma unroll
+  for (int i = 0; i < 4; ++i) h[i] = __floats2bfloat162_rn(v[2 * i], v[2 * i + 1]);
+  *reinterpret_cast<uint4*>(p) = u;
+}
+template <> __device__ __forceinline__ void store8<__half>(__half* p, const float* v) {
+  uint4 u;
+  __half2* h = reinterpret_cast<__half2*>(&u);
+#pragma unroll
+  for (int i = 0; i < 4; ++i) h[i] = __floats2half2_rn(v[2 * i], v[2 * i + 1]);
+  *reinterpret_cast<uint4*>(p) = u;
+}
+
+__device__ __forceinline__ float warp_sum_f(float v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+// sums `v` over the 256 threads of the block; result valid in thread 0
+__device__ __forceinline__ float block_sum_256(float v, float* red /*[8]*/) {
+  v = warp_sum_f(v);
+  __syncthreads();
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = v;
+  __syncthreads();
+  float s = 0.f;
+  if (threadIdx.x == 0) for (int w = 0; w < 8; ++w) s += red[w];
+  return s;
+}
+
+// =============================================================================================================
+// first layer: a = Zp[n] + b1 + W1[:,0] x + W1[:,1] y ; a_x = W1[:,0], a_y = W1[:,1], a_xx = a_yy = 0 ; tanh jet.  fp32 math.
+// block = 256 rows x 32 units: lane -> 8 rows, warp w -> units w, w+8, w+16, w+24 of the block's group
+// =============================================================================================================
+template <typename T, int C, bool SPLIT>
+__global__ void __launch_bounds__(256) first_layer_fwd_kernel(NetShape s, const float* __restrict__ theta, const float* __restrict__ Zp,
+                                                              const float* __restrict__ xy, ChunkGeom g, T* __restrict__ h1) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int r0 = blockIdx.x * 256 + lane * 8;
+  if (r0 >= g.R) return;
+  float x[8], y[8]; int n[8];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) {
+    const long long rg = g.row0 + min(r0 + i, g.valid - 1);      // padded rows repeat the last valid row (finite values)
+    n[i] = (int)(rg / g.npts);
+    const int p = (int)(rg % g.npts);
+    const float2 q = *reinterpret_cast<const float2*>(xy + 2 * p);
+    x[i] = q.x; y[i] = q.y;
+  }
+  const bool one_sample = n[0] == n[7];
+  const float* W1 = theta; const float* b1 = theta + s.b_off(1);
+  const size_t plane = (size_t)s.H * g.R_ld;
+  for (int j = blockIdx.y * 32 + warp; j < min(s.H, blockIdx.y * 32 + 32); j += 8) {
+    const float wx = W1[(size_t)j * s.in_dim], wy = W1[(size_t)j * s.in_dim + 1], bj = b1[j];
+    const float z0 = Zp[(size_t)n[0] * s.H + j];
+    float o[C][8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+      const float zp = one_sample ? z0 : Zp[(size_t)n[i] * s.H + j];
+      const float a0 = zp + bj + wx * x[i] + wy * y[i];
+      float a[5] = {a0, wx, wy, 0.f, 0.f}, h[5];
+      jet_act_fwd<C>(tanhf(a0), a, h);
+#pragma unroll
+      for (int c = 0; c < C; ++c) o[c][i] = h[c];
+    }
+#pragma unroll
+    for (int c = 0; c < C; ++c) store8<T>(h1 + c * plane + (size_t)j * g.R_ld + r0, o[c]);
+    if (SPLIT) {                                             // second plane: what the 16-bit rounding of t dropped
+      float lo[8];
+#pragma unroll
+      for (int i = 0; i < 8; ++i) lo[i] = o[0][i] - to_f<T>(from_f<T>(o[0][i]));
+      store8<T>(h1 + plane + (size_t)j * g.R_ld + r0, lo);
+    }
+  }
+}
+
+template <typename T>
+void first_layer_fwd(Launcher& L, int C, const NetShape& s, const float* theta, const float* Zp, const float* xy, const ChunkGeom& g, T* h1, bool split) {
+  if (g.R <= 0) return;
+  dim3 grid(cdiv(g.R, 256), cdiv(s.H, 32));
+  if (split) first_layer_fwd_kernel<T, 1, true><<<grid, 256, 0, L.stream>>>(s, theta, Zp, xy, g, h1);
+  else if (C == 1) first_layer_fwd_kernel<T, 1, false><<<grid, 256, 0, L.stream>>>(s, theta, Zp, xy, g, h1);
+  else if (C == 3) first_layer_fwd_kernel<T, 3, false><<<grid, 256, 0, L.stream>>>(s, theta, Zp, xy, g, h1);
+  else first_layer_fwd_kernel<T, 5, false><<<grid, 256, 0, L.stream>>>(s, theta, Zp, xy, g, h1);
+  L.check("first_layer_fwd");
+}
+template void first_layer_fwd<float>(Launcher&, int, const NetShape&, const float*, const float*, const float*, const ChunkGeom&, float*, bool);
+template void first_layer_fwd<__nv_bfloat16>(Launcher&, int, const NetShape&, const float*, const float*, const float*, const ChunkGeom&, __nv_bfloat16*, bool);
+template void first_layer_fwd<__half>(Launcher&, int, const NetShape&, const float*, const float*, const float*, const ChunkGeom&, __half*, bool);
+
+// =============================================================================================================
+// output layer (a4): o_c[r] = w_out . h_c[:, r] (+ b_out on the value channel)
+// block = 256 rows x (H / gridDim.y) units; warp w strides over the block's units; cross-warp sum in smem; one
+// atomicAdd per (channel, row) per block (o is zeroed by the launcher)
+// =============================================================================================================
+template <typename T, int C, bool SPLIT>
+__global__ void __launch_bounds__(256) out_fwd_kernel(int H, const float* __restrict__ w_out, const float* __restrict__ b_out, ChunkGeom g,
+                                                      const T* __restrict__ hL, float* __restrict__ o, long long o_stride) {
+  __shared__ float red[8][C][256];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int seg = blockIdx.x * 256, r0 = seg + lane * 8;
+  const int per = (H + gridDim.y - 1) / gridDim.y, jb = blockIdx.y * per, je = min(H, jb + per);
+  const size_t plane = (size_t)H * g.R_ld;
+  float acc[C][8];
+#pragma unroll
+  for (int c = 0; c < C; ++c)
+#pragma unroll
+    for (int i = 0; i < 8; ++i) acc[c][i] = 0.f;
+  if (r0 < g.R) {
+#pragma unroll 2
+    for (int j = jb + warp; j < je; j += 8) {
+      const float w = __ldg(w_out + j);
+#pragma unroll
+      for (int c = 0; c < C; ++c) {
+        float v[8];
+        load8<T>(hL + c * plane + (size_t)j * g.R_ld + r0, v);
+#pragma unroll
+        for (int i = 0; i < 8; ++i) acc[c][i] = fmaf(w, v[i], acc[c][i]);
+      }
+    }
+  }
+#pragma unroll
+  for (int c = 0; c < C; ++c)
+#pragma unroll
+    for (int i = 0; i < 8; ++i) red[warp][c][lane * 8 + i] = acc[c][i];
+  __syncthreads();
+  const int r = seg + threadIdx.x;
+  if (r < g.valid) {
+    if (SPLIT) {                                             // planes (hi, lo) of one value channel
+      float sum = 0.f;
+#pragma unroll
+      for (int w = 0; w < 8; ++w) sum += red[w][0][threadIdx.x] + red[w][C - 1][threadIdx.x];
+      if (blockIdx.y == 0) sum += b_out[0];
+      atomicAdd(o + r, sum);
+    } else {
+#pragma unroll
+      for (int c = 0; c < C; ++c) {
+        float sum = 0.f;
+#pragma unroll
+        for (int w = 0; w < 8; ++w) sum += red[w][c][threadIdx.x];
+        if (c == 0 && blockIdx.y == 0) sum += b_out[0];
+        atomicAdd(o + c * o_stride + r, sum);
+      }
+    }
+  }
+}
+
+template <typename T>
+void out_fwd(Launcher& L, int C, int H, const float* w_out, const float* b_out, const ChunkGeom& g, const T* hL, float* o, long long o_plane_stride,
+             bool split) {
+  if (g.valid <= 0) return;
+  cudaMemset2DAsync(o, (size_t)o_plane_stride * 4, 0, (size_t)g.valid * 4, split ? 1 : C, L.stream);
+  const int rb = cdiv(g.R, 256);
+  int jsplit = std::max(1, std::min(cdiv(600, rb), H / 8));
+  dim3 grid(rb, jsplit);
+  if (split) out_fwd_kernel<T, 2, true><<<grid, 256, 0, L.stream>>>(H, w_out, b_out, g, hL, o, o_plane_stride);
+  else if (C == 1) out_fwd_kernel<T, 1, false><<<grid, 256, 0, L.stream>>>(H, w_out, b_out, g, hL, o, o_plane_stride);
+  else if (C == 3) out_fwd_kernel<T, 3, false><<<grid, 256, 0, L.stream>>>(H, w_out, b_out, g, hL, o, o_plane_stride);
+  else out_fwd_kernel<T, 5, false><<<grid, 256, 0, L.stream>>>(H, w_out, b_out, g, hL, o, o_plane_stride);
+  L.check("out_fwd");
+}
+template void out_fwd<float>(Launcher&, int, int, const float*, const float*, const ChunkGeom&, const float*, float*, long long, bool);
+template void out_fwd<__nv_bfloat16>(Launcher&, int, int, const float*, const float*, const ChunkGeom&, const __nv_bfloat16*, float*, long long, bool);
+template void out_fwd<__half>(Launcher&, int, int, const float*, const float*, const ChunkGeom&, const __half*, float*, long long, bool);
+
+// =============================================================================================================
+// adjoint of one tanh layer (O4), SIMT form.  block = one unit x 2048 rows (8 rows per thread).
+//   hh_c = hhat_c[j][r] (fp32 planes from sgemm) or w_out[j] * ohat_c[r] (output layer).
+//   writes ahat planes; b_hat_l[j] += sum_r ahat_0 ; output layer also w_hat_out[j] += sum_{c,r} ohat_c h_c, b_hat_out += sum ohat_0
+// =============================================================================================================
+template <typename T, int C>
+__global__ void __launch_bounds__(256) jet_act_bwd_kernel(int H, ChunkGeom g, const float* __restrict__ hhat, const float* __restrict__ w_out,
+                                                          const float* __restrict__ ohat, const T* __restrict__ h, const T* __restrict__ stash,
+                                                          const float* __restrict__ W1, int in_dim, T* __restrict__ ahat,
+                                                          float* __restrict__ g_bias, float* __restrict__ g_wout, float* __restrict__ g_bout) {
+  __shared__ float red[8];
+  const int j = blockIdx.y;
+  const size_t plane = (size_t)H * g.R_ld;
+  const float wj = w_out ? w_out[j] : 0.f;
+  float ad1[4] = {0.f, 0.f, 0.f, 0.f};
+  if (!stash && C >= 3) { ad1[0] = W1[(size_t)j * in_dim]; ad1[1] = W1[(size_t)j * in_dim + 1]; }   // layer 1: a_x = W1[:,0], a_y = W1[:,1], a_xx = a_yy = 0
+  float s_bias = 0.f, s_wout = 0.f, s_bout = 0.f;
+  const int r0 = blockIdx.x * 2048 + threadIdx.x * 8;
+  if (r0 < g.R) {
+    const size_t off = (size_t)j * g.R_ld + r0;
+    float hv[C][8], hh[C][8], ad[C > 1 ? C - 1 : 1][8], o[C][8];
+#pragma unroll
+    for (int c = 0; c < C; ++c) load8<T>(h + c * plane + off, hv[c]);
+    if (hhat) {
+#pragma unroll
+      for (int c = 0; c < C; ++c) load8<float>(hhat + c * plane + off, hh[c]);
+    } else {
+#pragma unroll
+      for (int c = 0; c < C; ++c) {
+        float ov[8];
+        load8<float>(ohat + (size_t)c * g.R_ld + r0, ov);
+#pragma unroll
+        for (int i = 0; i < 8; ++i) { hh[c][i] = wj * ov[i]; s_wout = fmaf(ov[i], hv[c][i], s_wout); if (c == 0) s_bout += ov[i]; }
+      }
+    }
+    if (stash) {
+#pragma unroll
+      for (int c = 0; c < C - 1; ++c) load8<T>(stash + c * plane + off, ad[c]);
+    }
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+      float hx[5], a4[4], aa[5];
+#pragma unroll
+      for (int c = 0; c < C; ++c) hx[c] = hh[c][i];
+#pragma unroll
+      for (int c = 0; c < C - 1; ++c) a4[c] = stash ? ad[c][i] : ad1[c];
+      jet_act_bwd<C>(hv[0][i], a4, hx, aa);
+      s_bias += aa[0];
+#pragma unroll
+      for (int c = 0; c < C; ++c) o[c][i] = aa[c];
+    }
+#pragma unroll
+    for (int c = 0; c < C; ++c) store8<T>(ahat + c * plane + off, o[c]);
+  }
+  float v = block_sum_256(s_bias, red);
+  if (threadIdx.x == 0) atomicAdd(g_bias + j, v);
+  if (g_wout) { v = block_sum_256(s_wout, red); if (threadIdx.x == 0) atomicAdd(g_wout + j, v); }
+  if (g_bout && j == 0) { v = block_sum_256(s_bout, red); if (threadIdx.x == 0) atomicAdd(g_bout, v); }
+}
+
+template <typename T>
+void jet_act_bwd_launch(Launcher& L, int C, int H, const ChunkGeom& g, const float* hhat, const float* w_out, const float* ohat, const T* h,
+                        const T* stash, const float* W1, int in_dim, T* ahat, float* g_bias, float* g_wout, float* g_bout) {
+  if (g.R <= 0) return;
+  dim3 grid(cdiv(g.R, 2048), H);
+#define PIGAN_BWD(c) jet_act_bwd_kernel<T, c><<<grid, 256, 0, L.stream>>>(H, g, hhat, w_out, ohat, h, stash, W1, in_dim, ahat, g_bias, g_wout, g_bout)
+  if (C == 1) PIGAN_BWD(1); else if (C == 3) PIGAN_BWD(3); else PIGAN_BWD(5);
+#undef PIGAN_BWD
+  L.check("jet_act_bwd");
+}
+template void jet_act_bwd_launch<float>(Launcher&, int, int, const ChunkGeom&, const float*, const float*, const float*, const float*, const float*, const float*, int, float*, float*, float*, float*);
+template void jet_act_bwd_launch<__nv_bfloat16>(Launcher&, int, int, const ChunkGeom&, const float*, const float*, const float*, const __nv_bfloat16*, const __nv_bfloat16*, const float*, int, __nv_bfloat16*, float*, float*, float*);
+template void jet_act_bwd_launch<__half>(Launcher&, int, int, const ChunkGeom&, const float*, const float*, const float*, const __half*, const __half*, const float*, int, __half*, float*, float*, float*);
+
+// =============================================================================================================
+// first-layer backward (O4 'First layer'): W_hat_1[:,0] += sum (ahat x + ahat_x), W_hat_1[:,1] += sum (ahat y + ahat_y),
+// An[n][j] += sum_{p in chunk} ahat[j][(n,p)]  (the z-part GEMM and b_hat_1 use An / the layer-1 adjoint reduction).
+// block = one unit x 2048 rows
+// =============================================================================================================
+template <typename T, int C>
+__global__ void __launch_bounds__(256) first_layer_bwd_kernel(NetShape s, const float* __restrict__ xy, ChunkGeom g, const T* __restrict__ ahat,
+                                                              float* __restrict__ gW1, float* __restrict__ An) {
+  __shared__ float red[8];
+  const int j = blockIdx.y;
+  const size_t plane = (size_t)s.H * g.R_ld;
+  const int b0 = blockIdx.x * 2048, r0 = b0 + threadIdx.x * 8;
+  const int n_first = (int)((g.row0 + b0) / g.npts), n_last = (int)((g.row0 + min(b0 + 2047, g.valid - 1)) / g.npts);
+  const bool uniform = n_first == n_last;                   // the whole block lies inside one latent sample
+  float sx = 0.f, sy = 0.f, sa = 0.f;
+  if (r0 < g.valid) {
+    const size_t off = (size_t)j * g.R_ld + r0;
+    float a0[8], ax[8], ay[8];
+    load8<T>(ahat + off, a0);
+    if (C >= 3) { load8<T>(ahat + plane + off, ax); load8<T>(ahat + 2 * plane + off, ay); }
+    int run_n = -1; float run = 0.f;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+      if (r0 + i < g.valid) {
+        const long long rg = g.row0 + r0 + i;
+        const int p = (int)(rg % g.npts);
+        const float2 q = *reinterpret_cast<const float2*>(xy + 2 * p);
+        sx = fmaf(a0[i], q.x, sx); sy = fmaf(a0[i], q.y, sy);
+        if (C >= 3) { sx += ax[i]; sy += ay[i]; }
+        if (uniform) sa += a0[i];
+        else {
+          const int n = (int)(rg / g.npts);
+          if (n != run_n) { if (run_n >= 0) atomicAdd(An + (size_t)run_n * s.H + j, run); run_n = n; run = 0.f; }
+          run += a0[i];
+        }
+      }
+    }
+    if (!uniform && run_n >= 0) atomicAdd(An + (size_t)run_n * s.H + j, run);
+  }
+  float v = block_sum_256(sx, red);
+  if (threadIdx.x == 0) atomicAdd(gW1 + (size_t)j * s.in_dim, v);
+  v = block_sum_256(sy, red);
+  if (threadIdx.x == 0) atomicAdd(gW1 + (size_t)j * s.in_dim + 1, v);
+  if (uniform) { v = block_sum_256(sa, red); if (threadIdx.x == 0) atomicAdd(An + (size_t)n_first * s.H + j, v); }
+}
+
+template <typename T>
+void first_layer_bwd(Launcher& L, int C, const NetShape& s, const float* xy, const ChunkGeom& g, const T* ahat, float* gW1, float* An) {
+  if (g.valid <= 0) return;
+  dim3 grid(cdiv(g.valid, 2048), s.H);
+  if (C == 1) first_layer_bwd_kernel<T, 1><<<grid, 256, 0, L.stream>>>(s, xy, g, ahat, gW1, An);
+  else if (C == 3) first_layer_bwd_kernel<T, 3><<<grid, 256, 0, L.stream>>>(s, xy, g, ahat, gW1, An);
+  else first_layer_bwd_kernel<T, 5><<<grid, 256, 0, L.stream>>>(s, xy, g, ahat, gW1, An);
+  L.check("first_layer_bwd");
+}
+template void first_layer_bwd<float>(Launcher&, int, const NetShape&, const float*, const ChunkGeom&, const float*, float*, float*);
+template void first_layer_bwd<__nv_bfloat16>(Launcher&, int, const NetShape&, const float*, const ChunkGeom&, const __nv_bfloat16*, float*, float*);
+template void first_layer_bwd<__half>(Launcher&, int, const NetShape&, const float*, const ChunkGeom&, const __half*, float*, float*);
+
+}  // namespace pigan

@@ -1,0 +1,719 @@
+// sm_100a tensor-core kernels of the jet MLP: tcgen05.mma with TMEM accumulators, operands
+// staged by TMA, the tanh-jet chain rule (forward) or its adjoint (backward) fused into the epilogue.
+//
+// Orientation ("units as lanes"): D[unit (128 TMEM lanes)][(channel, row) columns] = W_tile[128 x K] . act[K x (C*64)].
+//   A = 16-bit weights, K-major, 128B swizzle (TMA 2D box 64 x 128).
+//   B = activation planes [channel][unit][row] -- rows contiguous, i.e. MN-major -- 128B swizzle (TMA 3D box
+//       64 rows x 64 units x C channels): the C jet channels are stacked as extra GEMM columns of ONE tile pass.
+//   An epilogue thread owns one unit (TMEM lane) and sees all C channels of a (row, unit) pair, so the chain rule
+//   is thread-local; its outputs are contiguous along rows and leave through swizzled smem + TMA stores.
+// wgrad: D[out unit][in unit] += sum_{c,row} ahat_c[out][row] h_c[in][row]; both operands K-major (rows contiguous).
+#include <cuda.h>
+
+#include "common.cuh"
+
+namespace pigan {
+
+// =============================================================================================================
+// PTX wrappers
+// =============================================================================================================
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
+  uint32_t ok;
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+      "selp.u32 %0, 1, 0, p;\n\t}"
+      : "=r"(ok)
+      : "r"(smem_u32(bar)), "r"(parity)
+      : "memory");
+  return ok != 0;
+}
+// Bounded wait: a protocol bug traps (surfacing as a CUDA error) instead of hanging the GPU.
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  uint32_t spins = 0;
+  while (!mbar_try_wait(bar, parity)) {
+    if (++spins > (1u << 26)) { printf("pigan: mbarrier wait timed out (block %d thread %d)\n", (int)blockIdx.x, (int)threadIdx.x); __trap(); }
+  }
+}
+__device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
+__device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* map, uint64_t* bar, int c0, int c1) {
+  asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];" ::"r"(smem_u32(dst)),
+               "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1)
+               : "memory");
+}
+__device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, uint64_t* bar, int c0, int c1, int c2) {
+  asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];" ::"r"(smem_u32(dst)),
+               "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2)
+               : "memory");
+}
+__device__ __forceinline__ void tma_store_3d(const CUtensorMap* map, const void* src, int c0, int c1, int c2) {
+  asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.bulk_group [%0, {%2, %3, %4}], [%1];" ::"l"(map), "r"(smem_u32(src)), "r"(c0),
+               "r"(c1), "r"(c2)
+               : "memory");
+}
+__device__ __forceinline__ void tma_commit_group() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void tma_wait_read_all() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void tma_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+__device__ __forceinline__ void prefetch_tmap(const CUtensorMap* map) { asm volatile("prefetch.tensormap [%0];" ::"l"(map) : "memory"); }
+
+__device__ __forceinline__ void tmem_alloc(uint32_t* dst_smem, uint32_t ncols) {
+  asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(dst_smem)), "r"(ncols) : "memory");
+  asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_dealloc(uint32_t taddr, uint32_t ncols) {
+  asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(ncols) : "memory");
+}
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_commit(uint64_t* bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+// D[tmem] (+)= A[smem] . B[smem], kind::f16 (bf16 / fp16 operands, fp32 accumulate)
+__device__ __forceinline__ void tc_mma(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}" ::"r"(d_tmem),
+      "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
+      : "memory");
+}
+__device__ __forceinline__ void tmem_ld8(uint32_t taddr, float* v) {
+  uint32_t r[8];
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
+               : "r"(taddr));
+#pragma unroll
+  for (int i = 0; i < 8; ++i) v[i] = __uint_as_float(r[i]);
+}
+__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+
+// ---- UMMA descriptors (field layout as documented in CUTLASS cute/arch/mma_sm100_desc.hpp) ---------------------
+// smem matrix descriptor: [0,14) start>>4, [16,30) leading byte offset>>4, [32,46) stride byte offset>>4,
+// [46,48) version = 1, [61,64) layout (2 = SWIZZLE_128B).
+__device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
+  return (uint64_t)((saddr >> 4) & 0x3FFF) | ((uint64_t)((lbo_bytes >> 4) & 0x3FFF) << 16) | ((uint64_t)((sbo_bytes >> 4) & 0x3FFF) << 32) |
+         (1ull << 46) | (2ull << 61);
+}
+// instruction descriptor: [4,6) D fmt (1 = f32), [7,10) A fmt, [10,13) B fmt (0 = f16, 1 = bf16), bit 15 A major,
+// bit 16 B major (0 = K, 1 = MN), [17,23) N>>3, [24,29) M>>4.
+__host__ __device__ constexpr uint32_t umma_idesc(int fmt16, int a_mn, int b_mn, int M, int N) {
+  return (1u << 4) | ((uint32_t)fmt16 << 7) | ((uint32_t)fmt16 << 10) | ((uint32_t)a_mn << 15) | ((uint32_t)b_mn << 16) | ((uint32_t)(N >> 3) << 17) |
+         ((uint32_t)(M >> 4) << 24);
+}
+
+template <typename T> struct Fmt;
+template <> struct Fmt<__nv_bfloat16> { static constexpr int umma = 1; };
+template <> struct Fmt<__half> { static constexpr int umma = 0; };
+
+__device__ __forceinline__ float fast_tanh(float x) {
+  float y;
+  asm("tanh.approx.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+template <typename T> __device__ __forceinline__ uint32_t pack2(float a, float b);
+template <> __device__ __forceinline__ uint32_t pack2<__nv_bfloat16>(float a, float b) {
+  __nv_bfloat162 v = __floats2bfloat162_rn(a, b);
+  return *reinterpret_cast<uint32_t*>(&v);
+}
+template <> __device__ __forceinline__ uint32_t pack2<__half>(float a, float b) {
+  __half2 v = __floats2half2_rn(a, b);
+  return *reinterpret_cast<uint32_t*>(&v);
+}
+template <typename T> __device__ __forceinline__ float2 unpack2(uint32_t u);
+template <> __device__ __forceinline__ float2 unpack2<__nv_bfloat16>(uint32_t u) { return __bfloat1622float2(*reinterpret_cast<__nv_bfloat162*>(&u)); }
+template <> __device__ __forceinline__ float2 unpack2<__half>(uint32_t u) { return __half22float2(*reinterpret_cast<__half2*>(&u)); }
+
+template <typename T> __device__ __forceinline__ uint4 pack8(const float* v) {
+  return make_uint4(pack2<T>(v[0], v[1]), pack2<T>(v[2], v[3]), pack2<T>(v[4], v[5]), pack2<T>(v[6], v[7]));
+}
+template <typename T> __device__ __forceinline__ void unpack8(uint4 u, float* v) {
+  float2 a = unpack2<T>(u.x), b = unpack2<T>(u.y), c = unpack2<T>(u.z), d = unpack2<T>(u.w);
+  v[0] = a.x; v[1] = a.y; v[2] = b.x; v[3] = b.y; v[4] = c.x; v[5] = c.y; v[6] = d.x; v[7] = d.y;
+}
+
+// =============================================================================================================
+// jet layer kernel: forward (MODE 0) and dgrad + adjoint (MODE 1)
+// =============================================================================================================
+constexpr int kBM = 128;          // units per tile (TMEM lanes)
+constexpr int kRT = 64;           // rows per tile
+constexpr int kBK = 64;           // contraction elements per pipeline stage (128 B of K-major A)
+constexpr int kAStage = kBM * kBK * 2;                 // 16 KB
+constexpr int kBPlane = kBK * kRT * 2;                 // 8 KB per channel per stage
+constexpr int kStgPlane = 32 * 64;                     // epilogue staging: 32 units x 32 rows x 2 B per warp per plane
+
+template <int C> struct JetCfg {
+  static constexpr int kNumStages = C == 5 ? 3 : 4;
+  static constexpr int kStageBytes = kAStage + C * kBPlane;
+  static constexpr int kCols = C * kRT;                               // accumulator columns of one tile
+  static constexpr int kNumBuf = (2 * kCols <= 512) ? 2 : 1;          // TMEM double buffering when it fits
+  static constexpr int kTmemCols = kNumBuf * kCols <= 64 ? 64 : kNumBuf * kCols <= 128 ? 128 : kNumBuf * kCols <= 256 ? 256 : 512;
+  static constexpr int kStgBytes = 4 * C * kStgPlane;                 // 4 epilogue warps x C planes
+  static constexpr int kSmemBytes = kNumStages * kStageBytes + kStgBytes + 1024 /*align*/ + 256 /*barriers*/;
+};
+
+struct JetParams {
+  int H;                 // width (K and number of output units)
+  int n_row_tiles;       // R / 64
+  int has_stash;         // MODE 1: 0 = previous layer is layer 1 (analytic a_x, a_y; a_xx = a_yy = 0)
+  int in_dim;            // MODE 1, layer 1: leading dimension of W1
+  const float* bias;     // MODE 0: b_l
+  const float* W1;       // MODE 1, layer 1
+  float* g_bias;         // MODE 1: b_hat_{l-1}
+};
+
+template <typename T, int C, int MODE>
+__global__ void __launch_bounds__(256, 1) jet_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H] 16-bit, box 64 x 128, SW128
+                                                           const __grid_constant__ CUtensorMap tmB,      // input planes, box 64 rows x 64 units x C, SW128
+                                                           const __grid_constant__ CUtensorMap tmO,      // MODE 0: h_out; MODE 1: ahat_out (box 32 x 32 x 1, SW64)
+                                                           const __grid_constant__ CUtensorMap tmS,      // MODE 0: stash out; MODE 1: stash_prev in
+                                                           const __grid_constant__ CUtensorMap tmT,      // MODE 1: h_prev (plane 0 = t) in
+                                                           JetParams p) {
+  using Cfg = JetCfg<C>;
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  uint8_t* stages = smem;
+  uint8_t* staging = smem + Cfg::kNumStages * Cfg::kStageBytes;
+  uint64_t* bars = reinterpret_cast<uint64_t*>(staging + Cfg::kStgBytes);
+  uint64_t* full = bars;                                   // [kNumStages]
+  uint64_t* empty = bars + Cfg::kNumStages;                // [kNumStages]
+  uint64_t* tfull = empty + Cfg::kNumStages;               // [kNumBuf]
+  uint64_t* tempty = tfull + Cfg::kNumBuf;                 // [kNumBuf]
+  uint64_t* sbar = tempty + Cfg::kNumBuf;                  // [4] staging-load barriers (MODE 1), one per epilogue warp
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(sbar + 4);
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int n_ut = p.H / kBM;
+  const int n_tiles = n_ut * p.n_row_tiles;
+  const int n_kb = p.H / kBK;
+
+  if (warp == 0 && lane == 0) {
+    prefetch_tmap(&tmA); prefetch_tmap(&tmB); prefetch_tmap(&tmO);
+    if ((C > 1 && MODE == 0) || MODE == 1) prefetch_tmap(&tmS);
+    if (MODE == 1) prefetch_tmap(&tmT);
+  }
+  if (warp == 1 && lane == 0) {
+    for (int i = 0; i < Cfg::kNumStages; ++i) { mbar_init(full + i, 1); mbar_init(empty + i, 1); }
+    for (int i = 0; i < Cfg::kNumBuf; ++i) { mbar_init(tfull + i, 1); mbar_init(tempty + i, 4); }
+    for (int i = 0; i < 4; ++i) mbar_init(sbar + i, 1);
+    fence_barrier_init();
+  }
+  if (warp == 2) tmem_alloc(tmem_slot, Cfg::kTmemCols);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = *tmem_slot;
+
+  if (warp == 0) {
+    // ===================== TMA producer =====================
+    if (lane == 0) {
+      int stage = 0; uint32_t phase = 0;
+      for (int t = blockIdx.x; t < n_tiles; t += gridDim.x) {
+        const int ut = t % n_ut, rt = t / n_ut;
+        for (int kb = 0; kb < n_kb; ++kb) {
+          mbar_wait(empty + stage, phase ^ 1);
+          uint8_t* sA = stages + stage * Cfg::kStageBytes;
+          mbar_expect_tx(full + stage, Cfg::kStageBytes);
+          tma_load_2d(sA, &tmA, full + stage, kb * kBK, ut * kBM);
+          tma_load_3d(sA + kAStage, &tmB, full + stage, rt * kRT, kb * kBK, 0);
+          if (++stage == Cfg::kNumStages) { stage = 0; phase ^= 1; }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ===================== MMA issuer (one thread) =====================
+    if (lane == 0) {
+      int stage = 0; uint32_t phase = 0; int it = 0;
+      for (int t = blockIdx.x; t < n_tiles; t += gridDim.x, ++it) {
+        const int buf = it % Cfg::kNumBuf;
+        const uint32_t bphase = (it / Cfg::kNumBuf) & 1;
+        mbar_wait(tempty + buf, bphase ^ 1);                 // epilogue has drained this accumulator
+        tc_fence_after();
+        const uint32_t d0 = tmem_base + buf * Cfg::kCols;
+        for (int kb = 0; kb < n_kb; ++kb) {
+          mbar_wait(full + stage, phase);
+          tc_fence_after();
+          const uint32_t sA = smem_u32(stages + stage * Cfg::kStageBytes), sB = sA + kAStage;
+#pragma unroll
+          for (int k = 0; k < kBK / 16; ++k) {
+            const uint64_t ad = umma_desc_sw128(sA + k * 32, 16, 1024);                      // K-major: +32 B per 16 elements
+            const uint32_t acc = (kb | k) ? 1u : 0u;
+            // N is issued in groups of <= 3 channel blocks (N <= 256); channel blocks are 8 KB apart (LBO)
+#pragma unroll
+            for (int c0 = 0; c0 < C; c0 += 3) {
+              const int nc = (C - c0) < 3 ? (C - c0) : 3;
+              const uint64_t bd = umma_desc_sw128(sB + c0 * kBPlane + k * 2048, kBPlane, 1024);   // MN-major: +16 k-rows of 128 B
+              tc_mma(d0 + c0 * kRT, ad, bd, umma_idesc(Fmt<T>::umma, 0, 1, kBM, nc * kRT), acc);
+            }
+          }
+          tc_commit(empty + stage);                          // frees the smem slot when these MMAs retire
+          if (++stage == Cfg::kNumStages) { stage = 0; phase ^= 1; }
+        }
+        tc_commit(tfull + buf);                              // accumulator complete
+      }
+    }
+  } else if (warp >= 4) {
+    // ===================== epilogue: 4 warps, warp q owns TMEM lanes / units [32q, 32q+32) =====================
+    const int q = warp - 4;
+    uint8_t* stg = staging + q * (C * kStgPlane);
+    const uint32_t swz = (uint32_t)((lane >> 1) & 3);       // 64B swizzle of a 64-byte row: chunk ^= (row >> 1) & 3
+    uint8_t* my_row = stg + lane * 64;
+    uint32_t sphase = 0;
+    int it = 0;
+    for (int t = blockIdx.x; t < n_tiles; t += gridDim.x, ++it) {
+      const int ut = t % n_ut, rt = t / n_ut;
+      const int buf = it % Cfg::kNumBuf;
+      const uint32_t bphase = (it / Cfg::kNumBuf) & 1;
+      const int unit0 = ut * kBM + q * 32, unit = unit0 + lane;
+      const uint32_t tbase = tmem_base + ((uint32_t)(q * 32) << 16) + buf * Cfg::kCols;
+      float bias = 0.f, ad1[4] = {0.f, 0.f, 0.f, 0.f}, bias_acc = 0.f;
+      if (MODE == 0 || MODE == 2) bias = p.bias[unit];
+      if (MODE == 1 && !p.has_stash && C >= 3) { ad1[0] = p.W1[(size_t)unit * p.in_dim]; ad1[1] = p.W1[(size_t)unit * p.in_dim + 1]; }
+      const int n_in = p.has_stash ? C : 1;                  // MODE 1: planes to load per half tile (t, then stash)
+
+      auto issue_stage_loads = [&](int hf) {                 // MODE 1: t and stash of the previous layer -> staging
+        if (lane == 0) {
+          tma_wait_read_all();                               // earlier stores have finished reading the staging buffer
+          mbar_expect_tx(sbar + q, n_in * kStgPlane);
+          tma_load_3d(stg, &tmT, sbar + q, rt * kRT + hf * 32, unit0, 0);
+          for (int c = 1; c < n_in; ++c) tma_load_3d(stg + c * kStgPlane, &tmS, sbar + q, rt * kRT + hf * 32, unit0, c - 1);
+        }
+      };
+      if (MODE == 1) issue_stage_loads(0);
+      mbar_wait(tfull + buf, bphase);
+      tc_fence_after();
+
+#pragma unroll 1
+      for (int hf = 0; hf < 2; ++hf) {
+        if (MODE == 0) {
+          // ---- pass A: h_c = tanh-jet(a_c) ----
+          if (lane == 0) tma_wait_read_all();
+          __syncwarp();
+#pragma unroll 1
+          for (int rc = 0; rc < 4; ++rc) {
+            float v[C][8], o[C][8];
+#pragma unroll
+            for (int c = 0; c < C; ++c) tmem_ld8(tbase + c * kRT + hf * 32 + rc * 8, v[c]);
+            tmem_ld_wait();
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+              float a[5], h[5];
+#pragma unroll
+              for (int c = 0; c < C; ++c) a[c] = v[c][i];
+              a[0] += bias;
+              jet_act_fwd<C>(fast_tanh(a[0]), a, h);
+#pragma unroll
+              for (int c = 0; c < C; ++c) o[c][i] = h[c];
+            }
+            const uint32_t off = ((uint32_t)rc ^ swz) << 4;
+#pragma unroll
+            for (int c = 0; c < C; ++c) *reinterpret_cast<uint4*>(my_row + c * kStgPlane + off) = pack8<T>(o[c]);
+          }
+          fence_proxy_async();
+          __syncwarp();
+          if (lane == 0) {
+            for (int c = 0; c < C; ++c) tma_store_3d(&tmO, stg + c * kStgPlane, rt * kRT + hf * 32, unit0, c);
+            tma_commit_group();
+          }
+          // ---- pass B: stash a_x, a_y, a_xx, a_yy (raw accumulators) ----
+          if (C > 1) {
+            if (lane == 0) tma_wait_read_all();
+            __syncwarp();
+#pragma unroll 1
+            for (int rc = 0; rc < 4; ++rc) {
+              float v[C][8];
+#pragma unroll
+              for (int c = 1; c < C; ++c) tmem_ld8(tbase + c * kRT + hf * 32 + rc * 8, v[c]);
+              tmem_ld_wait();
+              const uint32_t off = ((uint32_t)rc ^ swz) << 4;
+#pragma unroll
+              for (int c = 1; c < C; ++c) *reinterpret_cast<uint4*>(my_row + (c - 1) * kStgPlane + off) = pack8<T>(v[c]);
+            }
+            fence_proxy_async();
+            __syncwarp();
+            if (lane == 0) {
+              for (int c = 1; c < C; ++c) tma_store_3d(&tmS, stg + (c - 1) * kStgPlane, rt * kRT + hf * 32, unit0, c - 1);
+              tma_commit_group();
+            }
+          }
+        } else if (MODE == 2) {
+          // ---- value-only layer with split activations: a = W (h_hi + h_lo) + b; t = tanh a; t_hi = rn16(t), t_lo = rn16(t - t_hi) ----
+          if (lane == 0) tma_wait_read_all();
+          __syncwarp();
+#pragma unroll 1
+          for (int rc = 0; rc < 4; ++rc) {
+            float v0[8], v1[8], hi[8], lo[8];
+            tmem_ld8(tbase + hf * 32 + rc * 8, v0);
+            tmem_ld8(tbase + kRT + hf * 32 + rc * 8, v1);
+            tmem_ld_wait();
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+              const float t = tanhf(v0[i] + v1[i] + bias);
+              hi[i] = to_f<T>(from_f<T>(t));
+              lo[i] = t - hi[i];
+            }
+            const uint32_t off = ((uint32_t)rc ^ swz) << 4;
+            *reinterpret_cast<uint4*>(my_row + off) = pack8<T>(hi);
+            *reinterpret_cast<uint4*>(my_row + kStgPlane + off) = pack8<T>(lo);
+          }
+          fence_proxy_async();
+          __syncwarp();
+          if (lane == 0) {
+            tma_store_3d(&tmO, stg, rt * kRT + hf * 32, unit0, 0);
+            tma_store_3d(&tmO, stg + kStgPlane, rt * kRT + hf * 32, unit0, 1);
+            tma_commit_group();
+          }
+        } else {
+          // ---- adjoint of the previous layer's tanh: ahat^{l-1} = J^T hhat^{l-1} ----
+          if (hf == 1) issue_stage_loads(1);
+          __syncwarp();
+          mbar_wait(sbar + q, sphase); sphase ^= 1;
+#pragma unroll 1
+          for (int rc = 0; rc < 4; ++rc) {
+            float hh[C][8], tv[8], sv[4][8], o[C][8];
+#pragma unroll
+            for (int c = 0; c < C; ++c) tmem_ld8(tbase + c * kRT + hf * 32 + rc * 8, hh[c]);
+            const uint32_t off = ((uint32_t)rc ^ swz) << 4;
+            unpack8<T>(*reinterpret_cast<const uint4*>(my_row + off), tv);
+            if (p.has_stash) {
+#pragma unroll
+              for (int c = 1; c < C; ++c) unpack8<T>(*reinterpret_cast<const uint4*>(my_row + c * kStgPlane + off), sv[c - 1]);
+            }
+            tmem_ld_wait();
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+              float hx[5], ad[4], aa[5];
+#pragma unroll
+              for (int c = 0; c < C; ++c) hx[c] = hh[c][i];
+#pragma unroll
+              for (int c = 0; c < C - 1; ++c) ad[c] = p.has_stash ? sv[c][i] : ad1[c];
+              jet_act_bwd<C>(tv[i], ad, hx, aa);
+              bias_acc += aa[0];
+#pragma unroll
+              for (int c = 0; c < C; ++c) o[c][i] = aa[c];
+            }
+#pragma unroll
+            for (int c = 0; c < C; ++c) *reinterpret_cast<uint4*>(my_row + c * kStgPlane + off) = pack8<T>(o[c]);
+          }
+          fence_proxy_async();
+          __syncwarp();
+          if (lane == 0) {
+            for (int c = 0; c < C; ++c) tma_store_3d(&tmO, stg + c * kStgPlane, rt * kRT + hf * 32, unit0, c);
+            tma_commit_group();
+          }
+        }
+      }
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(tempty + buf);
+      if (MODE == 1) atomicAdd(p.g_bias + unit, bias_acc);
+    }
+    if (lane == 0) tma_wait_all();                           // global writes of the last stores are complete before exit
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 2) { tc_fence_after(); tmem_dealloc(tmem_base, Cfg::kTmemCols); }
+}
+
+// =============================================================================================================
+// wgrad kernel: gW[j][k] += sum_{c, r} ahat_c[j][r] h_c[k][r]
+// =============================================================================================================
+constexpr int kWStages = 4;
+struct WgradParams {
+  int H, C;
+  int NW;              // output tile width (min(H, 256))
+  int n_slices;        // row slices
+  int slice_rows;      // rows per slice (multiple of 64)
+  int R;               // rows of the chunk (multiple of 64)
+  float* gW;           // [H][H] fp32
+};
+
+template <typename T>
+__global__ void __launch_bounds__(192, 1) wgrad_kernel(const __grid_constant__ CUtensorMap tmA,    // ahat planes, box 64 rows x 128 units x 1, SW128
+                                                       const __grid_constant__ CUtensorMap tmB,    // h_prev planes, box 64 rows x NW units x 1, SW128
+                                                       WgradParams p) {
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  const int stage_bytes = kAStage + p.NW * 128;
+  uint8_t* stages = smem;
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + kWStages * (kAStage + 256 * 128));
+  uint64_t* full = bars; uint64_t* empty = bars + kWStages; uint64_t* tfull = empty + kWStages; uint64_t* tempty = tfull + 2;
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(tempty + 2);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int n_mt = p.H / kBM, n_nt = p.H / p.NW;
+  const int n_items = n_mt * n_nt * p.n_slices;
+
+  if (warp == 0 && lane == 0) { prefetch_tmap(&tmA); prefetch_tmap(&tmB); }
+  if (warp == 1 && lane == 0) {
+    for (int i = 0; i < kWStages; ++i) { mbar_init(full + i, 1); mbar_init(empty + i, 1); }
+    for (int i = 0; i < 2; ++i) { mbar_init(tfull + i, 1); mbar_init(tempty + i, 4); }
+    fence_barrier_init();
+  }
+  __syncwarp();
+  if (warp == 1) tmem_alloc(tmem_slot, 512);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = *tmem_slot;
+
+  auto decode = [&](int w, int& mt, int& nt, int& r0, int& r1) {
+    const int tile = w % (n_mt * n_nt), sl = w / (n_mt * n_nt);
+    mt = tile % n_mt; nt = tile / n_mt;
+    r0 = sl * p.slice_rows; r1 = min(p.R, r0 + p.slice_rows);
+  };
+
+  if (warp == 0) {
+    if (lane == 0) {
+      int stage = 0; uint32_t phase = 0;
+      for (int w = blockIdx.x; w < n_items; w += gridDim.x) {
+        int mt, nt, r0, r1; decode(w, mt, nt, r0, r1);
+        for (int c = 0; c < p.C; ++c)
+          for (int r = r0; r < r1; r += 64) {
+            mbar_wait(empty + stage, phase ^ 1);
+            uint8_t* sA = stages + stage * stage_bytes;
+            mbar_expect_tx(full + stage, stage_bytes);
+            tma_load_3d(sA, &tmA, full + stage, r, mt * kBM, c);
+            tma_load_3d(sA + kAStage, &tmB, full + stage, r, nt * p.NW, c);
+            if (++stage == kWStages) { stage = 0; phase ^= 1; }
+          }
+      }
+    }
+  } else if (warp == 1) {
+    if (lane == 0) {
+      int stage = 0; uint32_t phase = 0; int it = 0;
+      const uint32_t idesc = umma_idesc(Fmt<T>::umma, 0, 0, kBM, p.NW);
+      for (int w = blockIdx.x; w < n_items; w += gridDim.x, ++it) {
+        int mt, nt, r0, r1; decode(w, mt, nt, r0, r1);
+        const int buf = it & 1; const uint32_t bphase = (it >> 1) & 1;
+        mbar_wait(tempty + buf, bphase ^ 1);
+        tc_fence_after();
+        const uint32_t d0 = tmem_base + buf * 256;
+        uint32_t acc = 0;
+        for (int c = 0; c < p.C; ++c)
+          for (int r = r0; r < r1; r += 64) {
+            mbar_wait(full + stage, phase);
+            tc_fence_after();
+            const uint32_t sA = smem_u32(stages + stage * stage_bytes), sB = sA + kAStage;
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+              tc_mma(d0, umma_desc_sw128(sA + k * 32, 16, 1024), umma_desc_sw128(sB + k * 32, 16, 1024), idesc, acc);
+              acc = 1;
+            }
+            tc_commit(empty + stage);
+            if (++stage == kWStages) { stage = 0; phase ^= 1; }
+          }
+        tc_commit(tfull + buf);
+      }
+    }
+  } else {
+    // epilogue warps 2..5 -> TMEM lane quarter (warp % 4)
+    const int q = warp & 3;
+    int it = 0;
+    for (int w = blockIdx.x; w < n_items; w += gridDim.x, ++it) {
+      int mt, nt, r0, r1; decode(w, mt, nt, r0, r1);
+      const int buf = it & 1; const uint32_t bphase = (it >> 1) & 1;
+      mbar_wait(tfull + buf, bphase);
+      tc_fence_after();
+      const uint32_t tbase = tmem_base + ((uint32_t)(q * 32) << 16) + buf * 256;
+      float* dst = p.gW + (size_t)(mt * kBM + q * 32 + lane) * p.H + nt * p.NW;
+      for (int n = 0; n < p.NW; n += 8) {
+        float v[8];
+        tmem_ld8(tbase + n, v);
+        tmem_ld_wait();
+        asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(dst + n), "f"(v[0]), "f"(v[1]), "f"(v[2]), "f"(v[3]) : "memory");
+        asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(dst + n + 4), "f"(v[4]), "f"(v[5]), "f"(v[6]), "f"(v[7]) : "memory");
+      }
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(tempty + buf);
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) { tc_fence_after(); tmem_dealloc(tmem_base, 512); }
+}
+
+// =============================================================================================================
+// 16-bit weight copies: W_l and W_l^T for l = 2..L
+// =============================================================================================================
+template <typename T>
+__global__ void __launch_bounds__(256) convert_weights_kernel(NetShape s, const float* __restrict__ theta, T* __restrict__ w16) {
+  __shared__ float tile[32][33];
+  const int l = blockIdx.z + 2, H = s.H;
+  const float* W = theta + s.W_off(l);
+  T* out = w16 + (size_t)(l - 2) * 2 * H * H;
+  T* outT = out + (size_t)H * H;
+  const int bx = blockIdx.x * 32, by = blockIdx.y * 32, tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+  for (int i = ty; i < 32; i += 8) {
+    const float v = W[(size_t)(by + i) * H + bx + tx];
+    tile[i][tx] = v;
+    out[(size_t)(by + i) * H + bx + tx] = from_f<T>(v);
+  }
+  __syncthreads();
+  for (int i = ty; i < 32; i += 8) outT[(size_t)(bx + i) * H + by + tx] = from_f<T>(tile[tx][i]);
+}
+
+void tc_convert_weights(Launcher& L, int precision, const NetShape& s, const float* theta, void* w16) {
+  if (s.L < 2) return;
+  dim3 grid(s.H / 32, s.H / 32, s.L - 1);
+  if (precision == PIGAN_BF16) convert_weights_kernel<__nv_bfloat16><<<grid, 256, 0, L.stream>>>(s, theta, (__nv_bfloat16*)w16);
+  else convert_weights_kernel<__half><<<grid, 256, 0, L.stream>>>(s, theta, (__half*)w16);
+  L.check("convert_weights");
+}
+
+// =============================================================================================================
+// host side: tensor maps and launches
+// =============================================================================================================
+bool tc_supported(int H, std::string* why) {
+  if (H % 128 != 0) { if (why) *why = "16-bit precision needs a width that is a multiple of 128"; return false; }
+  return true;
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
+                                  const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static EncodeTiledFn get_encode() {
+  static EncodeTiledFn fn = nullptr;
+  if (!fn) {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) == cudaSuccess && qres == cudaDriverEntryPointSuccess)
+      fn = (EncodeTiledFn)p;
+  }
+  return fn;
+}
+
+static bool make_map(Launcher& L, CUtensorMap* m, int precision, const void* base, int rank, const cuuint64_t* dims, const cuuint64_t* strides_bytes,
+                     const cuuint32_t* box, CUtensorMapSwizzle swz) {
+  EncodeTiledFn fn = get_encode();
+  cuuint32_t estr[3] = {1, 1, 1};
+  const CUtensorMapDataType dt = precision == PIGAN_BF16 ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16 : CU_TENSOR_MAP_DATA_TYPE_FLOAT16;
+  if (!fn || fn(m, dt, rank, const_cast<void*>(base), dims, strides_bytes, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, swz,
+                CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS) {
+    if (L.err == cudaSuccess) { L.err = cudaErrorInvalidValue; L.where = "cuTensorMapEncodeTiled"; }
+    return false;
+  }
+  return true;
+}
+// planes [C][H][R_ld] viewed as a 3D tensor (rows, units, channels)
+static bool plane_map(Launcher& L, CUtensorMap* m, int precision, const void* base, int H, int R_ld, int nch, int box_rows, int box_units, int box_ch,
+                      CUtensorMapSwizzle swz) {
+  cuuint64_t dims[3] = {(cuuint64_t)R_ld, (cuuint64_t)H, (cuuint64_t)nch};
+  cuuint64_t str[2] = {(cuuint64_t)R_ld * 2, (cuuint64_t)R_ld * 2 * H};
+  cuuint32_t box[3] = {(cuuint32_t)box_rows, (cuuint32_t)box_units, (cuuint32_t)box_ch};
+  return make_map(L, m, precision, base, 3, dims, str, box, swz);
+}
+static bool weight_map(Launcher& L, CUtensorMap* m, int precision, const void* base, int H) {
+  cuuint64_t dims[2] = {(cuuint64_t)H, (cuuint64_t)H};
+  cuuint64_t str[1] = {(cuuint64_t)H * 2};
+  cuuint32_t box[2] = {(cuuint32_t)kBK, (cuuint32_t)kBM};
+  return make_map(L, m, precision, base, 2, dims, str, box, CU_TENSOR_MAP_SWIZZLE_128B);
+}
+
+static int num_sms() {
+  static int n = 0;
+  if (!n) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev); if (n <= 0) n = 148; }
+  return n;
+}
+
+template <typename T, int C, int MODE>
+static void launch_jet(Launcher& L, const CUtensorMap& a, const CUtensorMap& b, const CUtensorMap& o, const CUtensorMap& s, const CUtensorMap& t,
+                       const JetParams& p) {
+  using Cfg = JetCfg<C>;
+  static bool attr_set = false;
+  auto kern = jet_layer_kernel<T, C, MODE>;
+  if (!attr_set) { cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::kSmemBytes); attr_set = true; }
+  const int tiles = (p.H / kBM) * p.n_row_tiles;
+  const int grid = std::min(tiles, num_sms());
+  kern<<<grid, 256, Cfg::kSmemBytes, L.stream>>>(a, b, o, s, t, p);
+  L.check(MODE == 0 ? "jet_layer_fwd" : MODE == 1 ? "jet_layer_bwd" : "jet_layer_fwd_split");
+}
+
+template <int MODE>
+static void dispatch_jet(Launcher& L, int precision, int C, const CUtensorMap& a, const CUtensorMap& b, const CUtensorMap& o, const CUtensorMap& s,
+                         const CUtensorMap& t, const JetParams& p) {
+#define PIGAN_JET(TT)                                                  \
+  if (C == 1) launch_jet<TT, 1, MODE>(L, a, b, o, s, t, p);            \
+  else if (C == 3) launch_jet<TT, 3, MODE>(L, a, b, o, s, t, p);       \
+  else launch_jet<TT, 5, MODE>(L, a, b, o, s, t, p)
+  if (precision == PIGAN_BF16) { PIGAN_JET(__nv_bfloat16); } else { PIGAN_JET(__half); }
+#undef PIGAN_JET
+}
+
+void tc_layer_fwd(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* w16_l, const float* bias, const void* h_in, void* h_out,
+                  void* stash) {
+  if (R <= 0) return;
+  CUtensorMap a, b, o, s;
+  bool ok = weight_map(L, &a, precision, w16_l, H) && plane_map(L, &b, precision, h_in, H, R_ld, C, kRT, kBK, C, CU_TENSOR_MAP_SWIZZLE_128B) &&
+            plane_map(L, &o, precision, h_out, H, R_ld, C, 32, 32, 1, CU_TENSOR_MAP_SWIZZLE_64B);
+  if (C > 1) ok = ok && plane_map(L, &s, precision, stash, H, R_ld, C - 1, 32, 32, 1, CU_TENSOR_MAP_SWIZZLE_64B); else s = o;
+  if (!ok) return;
+  JetParams p{};
+  p.H = H; p.n_row_tiles = R / kRT; p.bias = bias;
+  dispatch_jet<0>(L, precision, C, a, b, o, s, o, p);
+}
+
+// value-only layer on split activations (2 planes: hi, lo) -> 2 planes; used where the snapshot X_fake is built
+void tc_layer_fwd_split(Launcher& L, int precision, int H, int R, int R_ld, const void* w16_l, const float* bias, const void* h_in, void* h_out) {
+  if (R <= 0) return;
+  CUtensorMap a, b, o;
+  if (!(weight_map(L, &a, precision, w16_l, H) && plane_map(L, &b, precision, h_in, H, R_ld, 2, kRT, kBK, 2, CU_TENSOR_MAP_SWIZZLE_128B) &&
+        plane_map(L, &o, precision, h_out, H, R_ld, 2, 32, 32, 1, CU_TENSOR_MAP_SWIZZLE_64B)))
+    return;
+  JetParams p{};
+  p.H = H; p.n_row_tiles = R / kRT; p.bias = bias;
+  if (precision == PIGAN_BF16) launch_jet<__nv_bfloat16, 2, 2>(L, a, b, o, o, o, p); else launch_jet<__half, 2, 2>(L, a, b, o, o, o, p);
+}
+
+void tc_layer_bwd(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* w16T_l, const void* ahat_in, const void* h_prev,
+                  const void* stash_prev, const float* W1, int in_dim, void* ahat_out, float* g_bias_prev) {
+  if (R <= 0) return;
+  CUtensorMap a, b, o, s, t;
+  bool ok = weight_map(L, &a, precision, w16T_l, H) && plane_map(L, &b, precision, ahat_in, H, R_ld, C, kRT, kBK, C, CU_TENSOR_MAP_SWIZZLE_128B) &&
+            plane_map(L, &o, precision, ahat_out, H, R_ld, C, 32, 32, 1, CU_TENSOR_MAP_SWIZZLE_64B) &&
+            plane_map(L, &t, precision, h_prev, H, R_ld, 1, 32, 32, 1, CU_TENSOR_MAP_SWIZZLE_64B);
+  if (stash_prev && C > 1) ok = ok && plane_map(L, &s, precision, stash_prev, H, R_ld, C - 1, 32, 32, 1, CU_TENSOR_MAP_SWIZZLE_64B); else s = t;
+  if (!ok) return;
+  JetParams p{};
+  p.H = H; p.n_row_tiles = R / kRT; p.has_stash = (stash_prev && C > 1) ? 1 : 0; p.in_dim = in_dim; p.W1 = W1; p.g_bias = g_bias_prev;
+  dispatch_jet<1>(L, precision, C, a, b, o, s, t, p);
+}
+
+void tc_wgrad(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* ahat, const void* h_prev, float* gW) {
+  if (R <= 0) return;
+  WgradParams p{};
+  p.H = H; p.C = C; p.NW = std::min(H, 256); p.R = R; p.gW = gW;
+  const int n_tiles = (H / kBM) * (H / p.NW);
+  int slices = std::max(1, (2 * num_sms()) / n_tiles);
+  int slice_rows = ((R + slices - 1) / slices + 63) / 64 * 64;
+  if (slice_rows < 64) slice_rows = 64;
+  p.slice_rows = slice_rows; p.n_slices = (R + slice_rows - 1) / slice_rows;
+  CUtensorMap a, b;
+  if (!(plane_map(L, &a, precision, ahat, H, R_ld, C, 64, kBM, 1, CU_TENSOR_MAP_SWIZZLE_128B) &&
+        plane_map(L, &b, precision, h_prev, H, R_ld, C, 64, p.NW, 1, CU_TENSOR_MAP_SWIZZLE_128B)))
+    return;
+  const int smem = kWStages * (kAStage + 256 * 128) + 1024 + 256;
+  static bool attr_set[2] = {false, false};
+  const int grid = std::min(n_tiles * p.n_slices, num_sms());
+  if (precision == PIGAN_BF16) {
+    if (!attr_set[0]) { cudaFuncSetAttribute(wgrad_kernel<__nv_bfloat16>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); attr_set[0] = true; }
+    wgrad_kernel<__nv_bfloat16><<<grid, 192, smem, L.stream>>>(a, b, p);
+  } else {
+    if (!attr_set[1]) { cudaFuncSetAttribute(wgrad_kernel<__half>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); attr_set[1] = true; }
+    wgrad_kernel<__half><<<grid, 192, smem, L.stream>>>(a, b, p);
+  }
+  L.check("wgrad");
+}
+
+}  // namespace pigan

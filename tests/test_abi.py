@@ -1,0 +1,52 @@
+"""CPU-side checks of the boundary: the library builds/loads and exports every symbol include/pigan.h declares;
+argument validation that needs no GPU."""
+import ctypes
+import os
+import re
+
+import paper_1910_13444_b200 as pkg
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_header_and_library_agree():
+    header = open(os.path.join(ROOT, "include", "pigan.h")).read()
+    declared = sorted(set(re.findall(r"\b(pigan_[a-z_]+)\s*\(", header)))
+    lib = pkg.load_library()
+    assert declared, "no declarations found"
+    for name in declared:
+        assert hasattr(lib, name), f"{name} declared in pigan.h but not exported by libpigan.so"
+    assert sorted(pkg.EXPORTED_SYMBOLS) == declared
+
+
+def test_param_count_and_null_handling():
+    assert pkg.param_count(6, 3, 32) == 2369 and pkg.param_count(10000, 6, 1024) == 15490049
+    lib = pkg.load_library()
+    assert lib.pigan_param_count(None) == 0
+    assert lib.pigan_launch_count(None) == 0
+    assert lib.pigan_last_error(None) == b"null context"
+    lib.pigan_destroy(None)
+    ctx = ctypes.c_void_p()
+    assert lib.pigan_create(None, None, ctypes.byref(ctx)) == 1 and not ctx.value           # INVALID_ARG
+    assert lib.pigan_gen_jet_forward(None, None, None, 0, None, 0, 0, None) == 1
+    assert lib.pigan_adam_update(None, None, None, None, None, 0, 1, 0.0, 0.0, 0.0, 0.0, None) == 1
+
+
+def test_create_validates_config_before_touching_cuda():
+    lib = pkg.load_library()
+    ctx = ctypes.c_void_p()
+    bad_shape = pkg._Config(pkg._MlpShape(7, 3, 32), pkg._MlpShape(20, 3, 32), 4, 16, 64, 10, 0, 10.0, 1.0, 0)   # gen.in_dim != 2 + m
+    assert lib.pigan_create(ctypes.byref(bad_shape), None, ctypes.byref(ctx)) == 2                                   # SHAPE
+    unsup = pkg._Config(pkg._MlpShape(6, 3, 32), pkg._MlpShape(20, 3, 32), 4, 16, 64, 10, 1, 10.0, 1.0, 0)         # bf16 with width 32
+    assert lib.pigan_create(ctypes.byref(unsup), None, ctypes.byref(ctx)) == 5                                       # UNSUPPORTED
+    neg = pkg._Config(pkg._MlpShape(6, 0, 32), pkg._MlpShape(20, 3, 32), 4, 16, 64, 10, 0, 10.0, 1.0, 0)
+    assert lib.pigan_create(ctypes.byref(neg), None, ctypes.byref(ctx)) == 1
+
+
+def test_no_cpu_fallback():
+    import pytest
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    with pytest.raises(pkg.PiganError):
+        pkg.PiGan(latent_dim=4, gen_hidden=3, gen_width=32, disc_hidden=3, disc_width=32, n_samples=16, n_colloc=64, n_sensors=10)

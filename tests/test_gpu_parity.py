@@ -1,0 +1,197 @@
+"""GPU parity tests: the CUDA path (through the C-ABI) against the fp64 oracle on the same seeded inputs.
+
+Tolerances (BASELINE.json north_star): per output tensor max|gpu - ref| / max|ref| <= 1e-4 in fp32
+mode and <= 2e-2 in bf16/fp16 mode; loss values within 1e-3 relative.
+"""
+import dataclasses
+
+import numpy as np
+import pytest
+
+import workloads as wl
+from oracle import pigan_oracle as orc
+from parity_util import jets_parity, rel_err, step_parity, to_dev
+
+pytestmark = pytest.mark.gpu
+
+TOL = {"fp32": 1e-4, "bf16": 2e-2, "fp16": 2e-2}
+LOSS_TOL = 1e-3
+
+
+def check_step(cfg, **kw):
+    errs, lg, lr, found_inf = step_parity(cfg, **kw)
+    bad = {k: v for k, v in errs.items() if not v <= TOL[cfg.precision]}
+    assert not bad, f"{cfg.name}: tensors over tolerance {bad}"
+    assert found_inf == 0
+    lrel = np.abs(lg - lr) / np.maximum(np.abs(lr), 1e-12)
+    assert np.all(lrel <= LOSS_TOL), f"{cfg.name}: losses gpu {lg} ref {lr} rel {lrel}"
+    return errs
+
+
+# ---- fp32 (config c1) ------------------------------------------------------------------------------------------
+def test_c1_full_step():
+    check_step(wl.CONFIGS["c1"])
+    check_step(wl.CONFIGS["c1"], bias_std=0.0)              # the BASELINE recipe proper: zero biases
+
+
+def test_c1_ragged_rows_and_many_chunks():
+    cfg = dataclasses.replace(wl.CONFIGS["c1"], name="c1-ragged", G=7, N=5, S=3)      # 245 and 15 rows: ragged tails
+    check_step(cfg)
+    cfg = dataclasses.replace(wl.CONFIGS["c1"], name="c1-chunks", G=13, N=7, S=11)    # 1183 rows in 256-row chunks
+    check_step(cfg, workspace_bytes=1)
+
+
+@pytest.mark.parametrize("order", [0, 1, 2])
+def test_c1_jets(order):
+    errs, _, _ = jets_parity(wl.CONFIGS["c1"], order)
+    assert max(errs.values()) <= 1e-4, errs
+
+
+def test_single_hidden_layer_network():
+    cfg = dataclasses.replace(wl.CONFIGS["c1"], name="c1-L1", L=1, LD=1)               # degenerate depth
+    check_step(cfg)
+
+
+def test_residual_entry_point_manufactured_solution():
+    import torch
+    from paper_1910_13444_b200 import PiGan
+    pg = PiGan.from_config(wl.CONFIGS["c1"])
+    rng = np.random.default_rng(0)
+    N, P = 3, 77
+    x = rng.uniform(-1, 1, size=(N, P)); y = rng.uniform(-1, 1, size=(N, P)); f = rng.normal(size=P)
+    a, b = 0.7, -0.4
+    Yj = np.stack([a * x + b * y, a + 0 * x, b + 0 * x]).astype(np.float32)
+    Uj = np.stack([x * x + y * y, 2 * x, 2 * y, 2 + 0 * x, 2 + 0 * x]).astype(np.float32)
+    r, msq = pg.darcy_residual(torch.from_numpy(Yj).cuda(), torch.from_numpy(Uj).cuda(), torch.from_numpy(f.astype(np.float32)).cuda())
+    ref, ref_msq = orc.darcy_residual_ref(Yj, Uj, f.astype(np.float32))
+    assert rel_err(r.cpu().numpy(), ref) <= 1e-5 and abs(msq.item() - ref_msq) <= 1e-5 * ref_msq
+    # closed form: exp(ax+by)(2ax+2by+4) - f
+    assert rel_err(r.cpu().numpy(), np.exp(a * x + b * y) * (2 * a * x + 2 * b * y + 4) - f[None, :]) <= 1e-5
+    pg.close()
+
+
+def test_critic_entry_points():
+    import torch
+    from paper_1910_13444_b200 import PiGan
+    cfg = wl.CONFIGS["c1"]
+    inp = wl.make_inputs(cfg, bias_std=0.2)
+    rng = np.random.default_rng(1)
+    real = rng.normal(size=(cfg.N, 2 * cfg.S)).astype(np.float32); fake = rng.normal(size=(cfg.N, 2 * cfg.S)).astype(np.float32)
+    pg = PiGan.from_config(cfg)
+    th = torch.from_numpy(inp["theta_D"]).cuda()
+    score = pg.disc_forward(th, torch.from_numpy(real).cuda())
+    assert rel_err(score.cpu().numpy(), orc.disc_forward_ref(inp["theta_D"], *cfg.disc_shape, real)) <= 1e-5
+    gp, nu, d = pg.gradient_penalty(th, torch.from_numpy(real).cuda(), torch.from_numpy(fake).cuda(), torch.from_numpy(inp["eps"]).cuda())
+    rgp, rnu, rd = orc.gradient_penalty_ref(inp["theta_D"], *cfg.disc_shape, real, fake, inp["eps"], 10.0)
+    assert abs(gp.item() - rgp) <= 1e-4 * abs(rgp) and rel_err(nu.cpu().numpy(), rnu) <= 1e-5 and rel_err(d.cpu().numpy(), rd) <= 1e-4
+    # eps = 1 -> xhat = real; eps = 0 -> xhat = fake
+    one = torch.ones(cfg.N, device="cuda")
+    g1, _, _ = pg.gradient_penalty(th, torch.from_numpy(real).cuda(), torch.from_numpy(fake).cuda(), one)
+    g2, _, _ = pg.gradient_penalty(th, torch.from_numpy(real).cuda(), torch.from_numpy(real).cuda(), 0 * one)
+    assert abs(g1.item() - g2.item()) <= 1e-6 * abs(g2.item())
+    pg.close()
+
+
+def test_adam_entry_point():
+    import torch
+    from paper_1910_13444_b200 import PiGan
+    pg = PiGan.from_config(wl.CONFIGS["c1"])
+    rng = np.random.default_rng(2)
+    n = 1003                                               # not a multiple of 4: exercises the scalar tail
+    th = rng.normal(size=n).astype(np.float32); m = np.zeros(n, np.float32); v = np.zeros(n, np.float32)
+    dth, dm, dv = (torch.from_numpy(a.copy()).cuda() for a in (th, m, v))
+    rth, rm, rv = th.astype(np.float64), m.astype(np.float64), v.astype(np.float64)
+    for step in range(1, 4):
+        g = rng.normal(size=n).astype(np.float32)
+        pg.adam_update(dth, torch.from_numpy(g).cuda(), dm, dv, step, 1e-2, 0.5, 0.9, 1e-8)
+        rth, rm, rv = orc.adam_update_ref(rth, g, rm, rv, step, 1e-2, 0.5, 0.9, 1e-8)
+    assert rel_err(dth.cpu().numpy(), rth) <= 1e-6 and rel_err(dm.cpu().numpy(), rm) <= 1e-6 and rel_err(dv.cpu().numpy(), rv) <= 1e-6
+    before = (dth.clone(), dm.clone(), dv.clone())
+    flag = torch.ones(1, dtype=torch.int32, device="cuda")
+    pg.adam_update(dth, torch.from_numpy(g).cuda(), dm, dv, 4, 1e-2, 0.5, 0.9, 1e-8, skip_flag=flag)
+    assert all(torch.equal(a, b) for a, b in zip(before, (dth, dm, dv)))                 # bit-identical when skipped
+    pg.close()
+
+
+def test_edge_cases_and_errors():
+    import torch
+    from paper_1910_13444_b200 import PiGan, PiganError
+    cfg = wl.CONFIGS["c1"]
+    pg = PiGan.from_config(cfg)
+    inp = to_dev(wl.make_inputs(cfg), "cuda:0")
+    empty = pg.gen_jet_forward(inp["theta_u"], inp["xy_colloc"][:0].contiguous(), inp["z"], 2)     # n_pts = 0 is a no-op
+    assert empty.shape == (5, cfg.N, 0)
+    assert pg.disc_forward(inp["theta_D"], torch.empty(0, 2 * cfg.S, device="cuda")).numel() == 0
+    with pytest.raises(PiganError):                                                        # more samples than the context was sized for
+        pg.gen_jet_forward(inp["theta_u"], inp["xy_colloc"], torch.zeros(cfg.N + 1, cfg.m, device="cuda"), 2)
+    with pytest.raises(PiganError):
+        pg.adam_update(inp["theta_u"], inp["theta_u"], inp["theta_u"], inp["theta_u"], 0, 1e-3, 0.9, 0.99, 1e-8)   # step is 1-based
+    with pytest.raises(PiganError):                                                        # 16-bit needs width % 128 == 0
+        PiGan.from_config(dataclasses.replace(cfg, precision="bf16"))
+    pg.close()
+
+
+# ---- 16-bit tensor-core path -------------------------------------------------------------------------------------
+def test_c2_full_step_bf16():
+    check_step(wl.CONFIGS["c2"], bias_std=0.0)
+
+
+def test_c2_jets_all_orders():
+    for order in (0, 1, 2):
+        errs, _, _ = jets_parity(wl.CONFIGS["c2"], order, n_samples=8)
+        assert max(errs.values()) <= 2e-2, (order, errs)
+
+
+def test_c3_reduced_rows_bf16():
+    check_step(wl.CONFIGS["c3"].reduced(16, 32), bias_std=0.0)
+
+
+def test_c4_full_dims_reduced_rows_bf16():
+    check_step(wl.CONFIGS["c4"].reduced(4, 16), bias_std=0.0)
+
+
+def test_c5_full_dims_reduced_rows_fp16_loss_scaled():
+    check_step(wl.CONFIGS["c5"].reduced(4, 16), bias_std=0.0, loss_scale=1024.0)
+
+
+def test_ragged_rows_and_chunking_16bit():
+    cfg = dataclasses.replace(wl.CONFIGS["c2"], name="c2-ragged", N=5, G=13, S=37)          # 845 / 185 rows: not multiples of 64
+    check_step(cfg)
+    check_step(cfg, workspace_bytes=1)                                                      # 256-row chunks, ragged last chunk
+
+
+def test_fp16_overflow_is_flagged_not_an_error():
+    cfg = dataclasses.replace(wl.CONFIGS["c2"], name="c2-fp16", precision="fp16", N=4, G=16, S=16)
+    errs, lg, lr, found_inf = step_parity(cfg, loss_scale=2.0 ** 60)                         # absurd scale -> inf adjoints
+    assert found_inf == 1
+    errs, lg, lr, found_inf = step_parity(cfg, loss_scale=256.0)
+    assert found_inf == 0 and max(errs.values()) <= 2e-2
+
+
+@pytest.mark.parametrize("name", ["c4", "c5"])
+def test_full_size_jets_sampled_against_oracle(name):
+    """BASELINE full sizes, in the chunked launch configuration bench.py times: all N x P rows on the GPU, checked at
+    sampled (n, p) pairs the oracle computes one by one, plus L_pde recomputed in fp64 from the GPU's own jets."""
+    import torch
+    from paper_1910_13444_b200 import PiGan
+    cfg = wl.CONFIGS[name]
+    inp = wl.make_inputs(cfg)
+    pg = PiGan.from_config(cfg)
+    dev = "cuda:0"
+    xy, z = torch.from_numpy(inp["xy_colloc"]).to(dev), torch.from_numpy(inp["z"]).to(dev)
+    U = pg.gen_jet_forward(torch.from_numpy(inp["theta_u"]).to(dev), xy, z, 2)
+    Y = pg.gen_jet_forward(torch.from_numpy(inp["theta_Y"]).to(dev), xy, z, 1)
+    r, msq = pg.darcy_residual(Y, U, torch.from_numpy(inp["f"]).to(dev))
+    torch.cuda.synchronize()
+    rng = np.random.default_rng(7)
+    ns = rng.choice(cfg.N, size=8, replace=False); ps = np.sort(rng.choice(cfg.P, size=512, replace=False))   # 4096 pairs
+    refU = orc.gen_jet_forward_ref(inp["theta_u"], *cfg.gen_shape, inp["xy_colloc"][ps], inp["z"][ns], 2)
+    refY = orc.gen_jet_forward_ref(inp["theta_Y"], *cfg.gen_shape, inp["xy_colloc"][ps], inp["z"][ns], 1)
+    gotU = U[:, ns][:, :, ps].cpu().numpy(); gotY = Y[:, ns][:, :, ps].cpu().numpy()
+    for c in range(5):
+        assert rel_err(gotU[c], refU[c]) <= 2e-2, (name, "u", c, rel_err(gotU[c], refU[c]))
+    for c in range(3):
+        assert rel_err(gotY[c], refY[c]) <= 2e-2, (name, "Y", c)
+    r_ref, _ = orc.darcy_residual_ref(Y.cpu().numpy(), U.cpu().numpy(), inp["f"])
+    assert abs(msq.item() - float(np.mean(r_ref * r_ref))) <= 1e-4 * float(np.mean(r_ref * r_ref))
+    pg.close()
