@@ -41,6 +41,7 @@ struct pigan_ctx {
   float* xfake = nullptr;      // [N][2S]
   float* dX = nullptr;         // [2N][2S]
   float* seed = nullptr;       // [2N]
+  float* amax = nullptr;       // [2] largest output adjoint of the current chunk, per net (block scale of the adjoint planes)
   std::vector<void*> allocs;
 
   template <typename T> T* alloc(size_t n) {
@@ -109,9 +110,10 @@ void gen_backward_chunk(pigan_ctx* c, int n, const float* theta, float* grads, i
   const int H = s.H;
   const long long pl = (long long)H * g.R_ld;
   int cur = 0;
+  const float* amax = c->cfg.precision == PIGAN_FP32 ? nullptr : c->amax + n;
   jet_act_bwd_launch<T>(L, C, H, g, nullptr, theta + s.W_off(s.L + 1), c->net[n].oh, (const T*)c->h(n, s.L),
                         s.L >= 2 ? (const T*)c->st(n, s.L) : nullptr, theta, s.in_dim, (T*)c->net[n].ah[cur], grads + s.b_off(s.L),
-                        grads + s.W_off(s.L + 1), grads + s.b_off(s.L + 1));
+                        grads + s.W_off(s.L + 1), grads + s.b_off(s.L + 1), amax);
   for (int l = s.L; l >= 2; --l) {
     const T* stash_prev = l - 1 >= 2 ? (const T*)c->st(n, l - 1) : nullptr;
     if (c->cfg.precision == PIGAN_FP32) {
@@ -120,15 +122,15 @@ void gen_backward_chunk(pigan_ctx* c, int n, const float* theta, float* grads, i
       // hhat_c^{l-1} = W_l^T ahat_c: M = H (in), N = rows, K = H (out); A stored [K][M]
       sgemm(L, true, false, H, g.R, H, theta + s.W_off(l), H, 0, (const float*)c->net[n].ah[cur], g.R_ld, pl, c->net[n].apre, g.R_ld, pl, C, false);
       jet_act_bwd_launch<T>(L, C, H, g, c->net[n].apre, nullptr, nullptr, (const T*)c->h(n, l - 1), stash_prev, theta, s.in_dim,
-                            (T*)c->net[n].ah[cur ^ 1], grads + s.b_off(l - 1), nullptr, nullptr);
+                            (T*)c->net[n].ah[cur ^ 1], grads + s.b_off(l - 1), nullptr, nullptr, amax);
     } else {
-      tc_wgrad(L, c->cfg.precision, C, H, g.R, g.R_ld, c->net[n].ah[cur], c->h(n, l - 1), grads + s.W_off(l));
+      tc_wgrad(L, c->cfg.precision, C, H, g.R, g.R_ld, c->net[n].ah[cur], c->h(n, l - 1), grads + s.W_off(l), amax);
       tc_layer_bwd(L, c->cfg.precision, C, H, g.R, g.R_ld, c->w16(n, l, 1), c->net[n].ah[cur], c->h(n, l - 1), stash_prev, theta, s.in_dim,
-                   c->net[n].ah[cur ^ 1], grads + s.b_off(l - 1));
+                   c->net[n].ah[cur ^ 1], grads + s.b_off(l - 1), amax);
     }
     cur ^= 1;
   }
-  first_layer_bwd<T>(L, C, s, xy, g, (const T*)c->net[n].ah[cur], grads, c->net[n].An);
+  first_layer_bwd<T>(L, C, s, xy, g, (const T*)c->net[n].ah[cur], grads, c->net[n].An, amax);
 }
 
 ChunkGeom make_geom(const pigan_ctx* c, long long row0, long long total, int npts) {
@@ -201,7 +203,8 @@ pigan_status train_step_impl(pigan_ctx* c, const float* thY, const float* thU, c
     ChunkGeom g = make_geom(c, row0, srows, S);
     for (int n = 0; n < 2; ++n) {
       gen_forward_chunk<T>(c, n, th[n], 1, xy_s, g, c->net[n].o, c->R_ld);
-      gather_seed(L, c->dX, row0, g.valid, g.R, S, d, n * S, -loss_scale, c->net[n].oh);
+      cudaMemsetAsync(c->amax + n, 0, 4, st);
+      gather_seed(L, c->dX, row0, g.valid, g.R, S, d, n * S, -loss_scale, c->net[n].oh, c->amax + n);
       gen_backward_chunk<T>(c, n, th[n], gr[n], 1, xy_s, g);
     }
   }
@@ -212,8 +215,9 @@ pigan_status train_step_impl(pigan_ctx* c, const float* thY, const float* thU, c
     ChunkGeom g = make_geom(c, row0, crows, P);
     gen_forward_chunk<T>(c, 0, thY, 3, xy_c, g, c->net[0].o, c->R_ld);
     gen_forward_chunk<T>(c, 1, thU, 5, xy_c, g, c->net[1].o, c->R_ld);
+    cudaMemsetAsync(c->amax, 0, 8, st);
     residual(L, c->net[0].o, c->R_ld, c->net[1].o, c->R_ld, f, row0, g.valid, g.R, P, nullptr, c->cw.acc + 3, seed_scale, c->net[0].oh,
-             c->net[1].oh, c->R_ld);
+             c->net[1].oh, c->R_ld, c->amax, c->amax + 1);
     gen_backward_chunk<T>(c, 0, thY, gY, 3, xy_c, g);
     gen_backward_chunk<T>(c, 1, thU, gU, 5, xy_c, g);
   }
@@ -346,6 +350,7 @@ pigan_status pigan_create(const pigan_config* cfg, void* cuda_stream, pigan_ctx*
     c->xfake = c->alloc<float>((size_t)N * d);
     c->dX = c->alloc<float>((size_t)2 * N * d);
     c->seed = c->alloc<float>((size_t)2 * N);
+    c->amax = c->alloc<float>(2);
   } catch (const std::bad_alloc&) {
     pigan_destroy(c);
     return PIGAN_ERR_ALLOC;
@@ -371,7 +376,7 @@ pigan_status pigan_gen_jet_forward(pigan_ctx* c, const float* gen_params, const 
   const int C = jet_order == 0 ? 1 : jet_order == 1 ? 3 : 5;
   switch (c->cfg.precision) {
     case PIGAN_FP32: return jet_forward_impl<float>(c, gen_params, xy, n_pts, z, n_samples, C, out);
-    case PIGAN_BF16: return jet_forward_impl<__nv_bfloat16>(c, gen_params, xy, n_pts, z, n_samples, C, out);
+    case PIGAN_BF16: return jet_forward_impl<__half>(c, gen_params, xy, n_pts, z, n_samples, C, out);
     default: return jet_forward_impl<__half>(c, gen_params, xy, n_pts, z, n_samples, C, out);
   }
 }
@@ -433,7 +438,7 @@ pigan_status pigan_train_step_grads(pigan_ctx* c, const float* logk_params, cons
   if (!(loss_scale > 0.f) || !std::isfinite(loss_scale)) return fail(c, PIGAN_ERR_INVALID_ARG, "loss_scale must be positive and finite");
   switch (c->cfg.precision) {
     case PIGAN_FP32: return train_step_impl<float>(c, logk_params, u_params, disc_params, xy_colloc, f, xy_sensors, z, real_snap, eps, loss_scale, g_logk, g_u, g_disc, losses, found_inf);
-    case PIGAN_BF16: return train_step_impl<__nv_bfloat16>(c, logk_params, u_params, disc_params, xy_colloc, f, xy_sensors, z, real_snap, eps, loss_scale, g_logk, g_u, g_disc, losses, found_inf);
+    case PIGAN_BF16: return train_step_impl<__half>(c, logk_params, u_params, disc_params, xy_colloc, f, xy_sensors, z, real_snap, eps, loss_scale, g_logk, g_u, g_disc, losses, found_inf);
     default: return train_step_impl<__half>(c, logk_params, u_params, disc_params, xy_colloc, f, xy_sensors, z, real_snap, eps, loss_scale, g_logk, g_u, g_disc, losses, found_inf);
   }
 }

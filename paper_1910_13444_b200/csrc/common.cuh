@@ -73,6 +73,21 @@ __device__ __forceinline__ void jet_act_bwd(float t, const float* ad, const floa
   aa[0] = v;
 }
 
+// ---- block scaling of the 16-bit adjoint planes -----------------------------------------------------------------
+// The output adjoints of a chunk are multiplied by 2^(8-e), e = exponent of their largest magnitude (amax = m 2^e,
+// m in [0.5, 1)), so that the adjoint planes sit in the middle of the fp16 range whatever 1/(N P) and loss_scale are;
+// every reduction of adjoints into an fp32 gradient multiplies by the exact inverse.  amax == nullptr (fp32 mode): 1.
+__device__ __forceinline__ int adj_exponent(const float* amax) {
+  if (!amax) return 8;
+  const float a = *amax;
+  if (!(a > 0.f) || !isfinite(a)) return 8;
+  int e;
+  frexpf(a, &e);
+  return min(max(e, -100), 100);
+}
+__device__ __forceinline__ float adj_scale(const float* amax) { return ldexpf(1.f, 8 - adj_exponent(amax)); }
+__device__ __forceinline__ float adj_inv_scale(const float* amax) { return ldexpf(1.f, adj_exponent(amax) - 8); }
+
 // ---- launch bookkeeping -------------------------------------------------------------------------------------
 struct Launcher {
   cudaStream_t stream = nullptr;
@@ -122,17 +137,17 @@ void out_fwd(Launcher& L, int C, int H, const float* w_out, const float* b_out, 
              float* o, long long o_plane_stride, bool split = false);          // split: C = 1, sums planes (hi, lo)
 void residual(Launcher& L, const float* Y, long long y_stride, const float* U, long long u_stride, const float* f,
               long long row0, int valid, int R, int npts, float* r_out, double* sum_sq, float seed_scale, float* seedY,
-              float* seedU, int seed_ld);
+              float* seedU, int seed_ld, float* amaxY = nullptr, float* amaxU = nullptr);
 // adjoint of one tanh layer: hh_c = (hhat planes) or (w_out[j] * ohat_c[r]) ; writes ahat planes, accumulates
 // b_hat_l[j] += sum_r ahat_0 (and for the output layer w_hat_out[j], b_hat_out).
 template <typename T>
 void jet_act_bwd_launch(Launcher& L, int C, int H, const ChunkGeom& g, const float* hhat /*or null*/,
                         const float* w_out, const float* ohat /*[C][R_ld] when hhat null*/, const T* h /*[C][H][R_ld]*/,
                         const T* stash /*[C-1][H][R_ld] or null = layer 1*/, const float* W1, int in_dim, T* ahat,
-                        float* g_bias, float* g_wout, float* g_bout);
+                        float* g_bias, float* g_wout, float* g_bout, const float* amax);
 template <typename T>
 void first_layer_bwd(Launcher& L, int C, const NetShape& s, const float* xy, const ChunkGeom& g, const T* ahat,
-                     float* gW1 /* flat grads base of this net */, float* An /*[N][H]*/);
+                     float* gW1 /* flat grads base of this net */, float* An /*[N][H]*/, const float* amax);
 void finalize_first_layer(Launcher& L, const NetShape& s, int N, const float* An, const float* z, float* grads);
 void unscale_and_check(Launcher& L, float* g, size_t n, float inv_scale, int* found_inf);
 void adam(Launcher& L, float* p, const float* g, float* m, float* v, size_t n, float lr, float b1, float b2, float eps,
@@ -165,7 +180,7 @@ void build_snapshots(Launcher& L, const float* fake, const float* real, const fl
 void scale_copy(Launcher& L, const float* src, float* dst, size_t n, float alpha);
 void fill_seed(Launcher& L, float* seed, int B);
 void scatter_snapshot(Launcher& L, const float* o, long long row0, int valid, int S, int d, int col0, float* X);
-void gather_seed(Launcher& L, const float* dX, long long row0, int valid, int R, int S, int d, int col0, float alpha, float* seed);
+void gather_seed(Launcher& L, const float* dX, long long row0, int valid, int R, int S, int d, int col0, float alpha, float* seed, float* amax);
 void reduce_scores(Launcher& L, const float* D, int B, double* acc);
 void write_losses(Launcher& L, const double* acc, int N, long long NP, float lambda, float w_pde, float* losses, float* gp_out,
                   float* meansq_out, long long meansq_count);
@@ -182,8 +197,8 @@ void tc_layer_fwd_split(Launcher& L, int precision, int H, int R, int R_ld, cons
 // dgrad of layer l with the adjoint of layer l-1's tanh fused: ahat_in (layer l) -> ahat_out (layer l-1)
 void tc_layer_bwd(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* w16T_l, const void* ahat_in,
                   const void* h_prev /*[C][H][R_ld], value plane = t*/, const void* stash_prev /*null = layer 1*/,
-                  const float* W1, int in_dim, void* ahat_out, float* g_bias_prev);
+                  const float* W1, int in_dim, void* ahat_out, float* g_bias_prev, const float* amax);
 // wgrad of layer l: gW [H][H] += sum_c ahat_c h_prev_c^T   (fp32 atomics)
-void tc_wgrad(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* ahat, const void* h_prev, float* gW);
+void tc_wgrad(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* ahat, const void* h_prev, float* gW, const float* amax);
 
 }  // namespace pigan

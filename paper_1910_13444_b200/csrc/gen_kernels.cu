@@ -205,11 +205,13 @@ template <typename T, int C>
 __global__ void __launch_bounds__(256) jet_act_bwd_kernel(int H, ChunkGeom g, const float* __restrict__ hhat, const float* __restrict__ w_out,
                                                           const float* __restrict__ ohat, const T* __restrict__ h, const T* __restrict__ stash,
                                                           const float* __restrict__ W1, int in_dim, T* __restrict__ ahat,
-                                                          float* __restrict__ g_bias, float* __restrict__ g_wout, float* __restrict__ g_bout) {
+                                                          float* __restrict__ g_bias, float* __restrict__ g_wout, float* __restrict__ g_bout,
+                                                          const float* __restrict__ amax) {
   __shared__ float red[8];
   const int j = blockIdx.y;
   const size_t plane = (size_t)H * g.R_ld;
-  const float wj = w_out ? w_out[j] : 0.f;
+  const float sc = adj_scale(amax), inv_sc = adj_inv_scale(amax);     // block scale of the adjoint planes (1 in fp32 mode)
+  const float wj = w_out ? w_out[j] * sc : 0.f;
   float ad1[4] = {0.f, 0.f, 0.f, 0.f};
   if (!stash && C >= 3) { ad1[0] = W1[(size_t)j * in_dim]; ad1[1] = W1[(size_t)j * in_dim + 1]; }   // layer 1: a_x = W1[:,0], a_y = W1[:,1], a_xx = a_yy = 0
   float s_bias = 0.f, s_wout = 0.f, s_bout = 0.f;
@@ -251,24 +253,24 @@ __global__ void __launch_bounds__(256) jet_act_bwd_kernel(int H, ChunkGeom g, co
     for (int c = 0; c < C; ++c) store8<T>(ahat + c * plane + off, o[c]);
   }
   float v = block_sum_256(s_bias, red);
-  if (threadIdx.x == 0) atomicAdd(g_bias + j, v);
+  if (threadIdx.x == 0) atomicAdd(g_bias + j, v * inv_sc);
   if (g_wout) { v = block_sum_256(s_wout, red); if (threadIdx.x == 0) atomicAdd(g_wout + j, v); }
   if (g_bout && j == 0) { v = block_sum_256(s_bout, red); if (threadIdx.x == 0) atomicAdd(g_bout, v); }
 }
 
 template <typename T>
 void jet_act_bwd_launch(Launcher& L, int C, int H, const ChunkGeom& g, const float* hhat, const float* w_out, const float* ohat, const T* h,
-                        const T* stash, const float* W1, int in_dim, T* ahat, float* g_bias, float* g_wout, float* g_bout) {
+                        const T* stash, const float* W1, int in_dim, T* ahat, float* g_bias, float* g_wout, float* g_bout, const float* amax) {
   if (g.R <= 0) return;
   dim3 grid(cdiv(g.R, 2048), H);
-#define PIGAN_BWD(c) jet_act_bwd_kernel<T, c><<<grid, 256, 0, L.stream>>>(H, g, hhat, w_out, ohat, h, stash, W1, in_dim, ahat, g_bias, g_wout, g_bout)
+#define PIGAN_BWD(c) jet_act_bwd_kernel<T, c><<<grid, 256, 0, L.stream>>>(H, g, hhat, w_out, ohat, h, stash, W1, in_dim, ahat, g_bias, g_wout, g_bout, amax)
   if (C == 1) PIGAN_BWD(1); else if (C == 3) PIGAN_BWD(3); else PIGAN_BWD(5);
 #undef PIGAN_BWD
   L.check("jet_act_bwd");
 }
-template void jet_act_bwd_launch<float>(Launcher&, int, int, const ChunkGeom&, const float*, const float*, const float*, const float*, const float*, const float*, int, float*, float*, float*, float*);
-template void jet_act_bwd_launch<__nv_bfloat16>(Launcher&, int, int, const ChunkGeom&, const float*, const float*, const float*, const __nv_bfloat16*, const __nv_bfloat16*, const float*, int, __nv_bfloat16*, float*, float*, float*);
-template void jet_act_bwd_launch<__half>(Launcher&, int, int, const ChunkGeom&, const float*, const float*, const float*, const __half*, const __half*, const float*, int, __half*, float*, float*, float*);
+template void jet_act_bwd_launch<float>(Launcher&, int, int, const ChunkGeom&, const float*, const float*, const float*, const float*, const float*, const float*, int, float*, float*, float*, float*, const float*);
+template void jet_act_bwd_launch<__nv_bfloat16>(Launcher&, int, int, const ChunkGeom&, const float*, const float*, const float*, const __nv_bfloat16*, const __nv_bfloat16*, const float*, int, __nv_bfloat16*, float*, float*, float*, const float*);
+template void jet_act_bwd_launch<__half>(Launcher&, int, int, const ChunkGeom&, const float*, const float*, const float*, const __half*, const __half*, const float*, int, __half*, float*, float*, float*, const float*);
 
 // =============================================================================================================
 // first-layer backward (O4 'First layer'): W_hat_1[:,0] += sum (ahat x + ahat_x), W_hat_1[:,1] += sum (ahat y + ahat_y),
@@ -277,10 +279,11 @@ template void jet_act_bwd_launch<__half>(Launcher&, int, int, const ChunkGeom&, 
 // =============================================================================================================
 template <typename T, int C>
 __global__ void __launch_bounds__(256) first_layer_bwd_kernel(NetShape s, const float* __restrict__ xy, ChunkGeom g, const T* __restrict__ ahat,
-                                                              float* __restrict__ gW1, float* __restrict__ An) {
+                                                              float* __restrict__ gW1, float* __restrict__ An, const float* __restrict__ amax) {
   __shared__ float red[8];
   const int j = blockIdx.y;
   const size_t plane = (size_t)s.H * g.R_ld;
+  const float inv_sc = adj_inv_scale(amax);
   const int b0 = blockIdx.x * 2048, r0 = b0 + threadIdx.x * 8;
   const int n_first = (int)((g.row0 + b0) / g.npts), n_last = (int)((g.row0 + min(b0 + 2047, g.valid - 1)) / g.npts);
   const bool uniform = n_first == n_last;                   // the whole block lies inside one latent sample
@@ -302,31 +305,31 @@ __global__ void __launch_bounds__(256) first_layer_bwd_kernel(NetShape s, const 
         if (uniform) sa += a0[i];
         else {
           const int n = (int)(rg / g.npts);
-          if (n != run_n) { if (run_n >= 0) atomicAdd(An + (size_t)run_n * s.H + j, run); run_n = n; run = 0.f; }
+          if (n != run_n) { if (run_n >= 0) atomicAdd(An + (size_t)run_n * s.H + j, run * inv_sc); run_n = n; run = 0.f; }
           run += a0[i];
         }
       }
     }
-    if (!uniform && run_n >= 0) atomicAdd(An + (size_t)run_n * s.H + j, run);
+    if (!uniform && run_n >= 0) atomicAdd(An + (size_t)run_n * s.H + j, run * inv_sc);
   }
   float v = block_sum_256(sx, red);
-  if (threadIdx.x == 0) atomicAdd(gW1 + (size_t)j * s.in_dim, v);
+  if (threadIdx.x == 0) atomicAdd(gW1 + (size_t)j * s.in_dim, v * inv_sc);
   v = block_sum_256(sy, red);
-  if (threadIdx.x == 0) atomicAdd(gW1 + (size_t)j * s.in_dim + 1, v);
-  if (uniform) { v = block_sum_256(sa, red); if (threadIdx.x == 0) atomicAdd(An + (size_t)n_first * s.H + j, v); }
+  if (threadIdx.x == 0) atomicAdd(gW1 + (size_t)j * s.in_dim + 1, v * inv_sc);
+  if (uniform) { v = block_sum_256(sa, red); if (threadIdx.x == 0) atomicAdd(An + (size_t)n_first * s.H + j, v * inv_sc); }
 }
 
 template <typename T>
-void first_layer_bwd(Launcher& L, int C, const NetShape& s, const float* xy, const ChunkGeom& g, const T* ahat, float* gW1, float* An) {
+void first_layer_bwd(Launcher& L, int C, const NetShape& s, const float* xy, const ChunkGeom& g, const T* ahat, float* gW1, float* An, const float* amax) {
   if (g.valid <= 0) return;
   dim3 grid(cdiv(g.valid, 2048), s.H);
-  if (C == 1) first_layer_bwd_kernel<T, 1><<<grid, 256, 0, L.stream>>>(s, xy, g, ahat, gW1, An);
-  else if (C == 3) first_layer_bwd_kernel<T, 3><<<grid, 256, 0, L.stream>>>(s, xy, g, ahat, gW1, An);
-  else first_layer_bwd_kernel<T, 5><<<grid, 256, 0, L.stream>>>(s, xy, g, ahat, gW1, An);
+  if (C == 1) first_layer_bwd_kernel<T, 1><<<grid, 256, 0, L.stream>>>(s, xy, g, ahat, gW1, An, amax);
+  else if (C == 3) first_layer_bwd_kernel<T, 3><<<grid, 256, 0, L.stream>>>(s, xy, g, ahat, gW1, An, amax);
+  else first_layer_bwd_kernel<T, 5><<<grid, 256, 0, L.stream>>>(s, xy, g, ahat, gW1, An, amax);
   L.check("first_layer_bwd");
 }
-template void first_layer_bwd<float>(Launcher&, int, const NetShape&, const float*, const ChunkGeom&, const float*, float*, float*);
-template void first_layer_bwd<__nv_bfloat16>(Launcher&, int, const NetShape&, const float*, const ChunkGeom&, const __nv_bfloat16*, float*, float*);
-template void first_layer_bwd<__half>(Launcher&, int, const NetShape&, const float*, const ChunkGeom&, const __half*, float*, float*);
+template void first_layer_bwd<float>(Launcher&, int, const NetShape&, const float*, const ChunkGeom&, const float*, float*, float*, const float*);
+template void first_layer_bwd<__nv_bfloat16>(Launcher&, int, const NetShape&, const float*, const ChunkGeom&, const __nv_bfloat16*, float*, float*, const float*);
+template void first_layer_bwd<__half>(Launcher&, int, const NetShape&, const float*, const ChunkGeom&, const __half*, float*, float*, const float*);
 
 }  // namespace pigan

@@ -146,8 +146,10 @@ __device__ __forceinline__ double warp_sum_d(double v) {
 __global__ void __launch_bounds__(256) residual_kernel(const float* __restrict__ Y, long long ys, const float* __restrict__ U, long long us,
                                                        const float* __restrict__ f, long long row0, int valid, int R, int npts,
                                                        float* __restrict__ r_out, double* __restrict__ sum_sq, float seed_scale,
-                                                       float* __restrict__ seedY, float* __restrict__ seedU, int seed_ld) {
+                                                       float* __restrict__ seedY, float* __restrict__ seedU, int seed_ld,
+                                                       float* __restrict__ amaxY, float* __restrict__ amaxU) {
   __shared__ double red[8];
+  float my = 0.f, mu = 0.f;
   const int r = blockIdx.x * 256 + threadIdx.x;
   double sq = 0.0;
   if (r < R) {
@@ -164,12 +166,24 @@ __global__ void __launch_bounds__(256) residual_kernel(const float* __restrict__
       const float rk = seed_scale * res * k;                  // r_hat * k  (loss-scaled in 16-bit modes)
       sy[0] = rk * D; sy[1] = rk * ux; sy[2] = rk * uy;
       su[1] = rk * yx; su[2] = rk * yy; su[3] = rk; su[4] = rk;
+      my = fmaxf(fabsf(sy[0]), fmaxf(fabsf(sy[1]), fabsf(sy[2])));
+      mu = fmaxf(fabsf(su[1]), fmaxf(fabsf(su[2]), fabsf(su[3])));
     }
     if (seedY) {
 #pragma unroll
       for (int c = 0; c < 3; ++c) seedY[(size_t)c * seed_ld + r] = sy[c];
 #pragma unroll
       for (int c = 0; c < 5; ++c) seedU[(size_t)c * seed_ld + r] = su[c];
+    }
+  }
+  if (amaxY) {                                               // largest output adjoint of the chunk (positive floats order as ints)
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) { my = fmaxf(my, __shfl_xor_sync(0xffffffffu, my, o)); mu = fmaxf(mu, __shfl_xor_sync(0xffffffffu, mu, o)); }
+    if ((threadIdx.x & 31) == 0) {
+      if (!(my <= 3.0e38f)) my = INFINITY;                   // NaN/inf -> inf (flagged downstream through the gradients)
+      if (!(mu <= 3.0e38f)) mu = INFINITY;
+      atomicMax(reinterpret_cast<int*>(amaxY), __float_as_int(my));
+      atomicMax(reinterpret_cast<int*>(amaxU), __float_as_int(mu));
     }
   }
   if (sum_sq) {
@@ -185,10 +199,11 @@ __global__ void __launch_bounds__(256) residual_kernel(const float* __restrict__
 }
 
 void residual(Launcher& L, const float* Y, long long y_stride, const float* U, long long u_stride, const float* f, long long row0,
-              int valid, int R, int npts, float* r_out, double* sum_sq, float seed_scale, float* seedY, float* seedU, int seed_ld) {
+              int valid, int R, int npts, float* r_out, double* sum_sq, float seed_scale, float* seedY, float* seedU, int seed_ld,
+              float* amaxY, float* amaxU) {
   if (R <= 0) return;
   residual_kernel<<<cdiv(R, 256), 256, 0, L.stream>>>(Y, y_stride, U, u_stride, f, row0, valid, R, npts, r_out, sum_sq, seed_scale,
-                                                      seedY, seedU, seed_ld);
+                                                      seedY, seedU, seed_ld, amaxY, amaxU);
   L.check("residual");
 }
 
@@ -507,15 +522,24 @@ void scatter_snapshot(Launcher& L, const float* o, long long row0, int valid, in
   L.check("scatter_snapshot");
 }
 __global__ void gather_seed_kernel(const float* __restrict__ dX, long long row0, int valid, int R, int S, int d, int col0, float alpha,
-                                   float* __restrict__ seed) {
+                                   float* __restrict__ seed, float* __restrict__ amax) {
   const int r = blockIdx.x * blockDim.x + threadIdx.x;
-  if (r >= R) return;
-  const long long rg = row0 + r;
-  seed[r] = r < valid ? alpha * dX[(rg / S) * d + col0 + (rg % S)] : 0.f;
+  float v = 0.f;
+  if (r < R) {
+    const long long rg = row0 + r;
+    v = r < valid ? alpha * dX[(rg / S) * d + col0 + (rg % S)] : 0.f;
+    seed[r] = v;
+  }
+  if (amax) {
+    float m = fabsf(v);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if ((threadIdx.x & 31) == 0) { if (!(m <= 3.0e38f)) m = INFINITY; atomicMax(reinterpret_cast<int*>(amax), __float_as_int(m)); }
+  }
 }
-void gather_seed(Launcher& L, const float* dX, long long row0, int valid, int R, int S, int d, int col0, float alpha, float* seed) {
+void gather_seed(Launcher& L, const float* dX, long long row0, int valid, int R, int S, int d, int col0, float alpha, float* seed, float* amax) {
   if (R <= 0) return;
-  gather_seed_kernel<<<cdiv(R, 256), 256, 0, L.stream>>>(dX, row0, valid, R, S, d, col0, alpha, seed);
+  gather_seed_kernel<<<cdiv(R, 256), 256, 0, L.stream>>>(dX, row0, valid, R, S, d, col0, alpha, seed, amax);
   L.check("gather_seed");
 }
 

@@ -172,6 +172,7 @@ struct JetParams {
   const float* bias;     // MODE 0: b_l
   const float* W1;       // MODE 1, layer 1
   float* g_bias;         // MODE 1: b_hat_{l-1}
+  const float* amax;     // MODE 1: block-scale source of the adjoint planes (common.cuh adj_inv_scale)
 };
 
 template <typename T, int C, int MODE>
@@ -418,7 +419,7 @@ __global__ void __launch_bounds__(256, 1) jet_layer_kernel(const __grid_constant
       tc_fence_before();
       __syncwarp();
       if (lane == 0) mbar_arrive(tempty + buf);
-      if (MODE == 1) atomicAdd(p.g_bias + unit, bias_acc);
+      if (MODE == 1) atomicAdd(p.g_bias + unit, bias_acc * adj_inv_scale(p.amax));
     }
     if (lane == 0) tma_wait_all();                           // global writes of the last stores are complete before exit
   }
@@ -438,6 +439,7 @@ struct WgradParams {
   int slice_rows;      // rows per slice (multiple of 64)
   int R;               // rows of the chunk (multiple of 64)
   float* gW;           // [H][H] fp32
+  const float* amax;   // block-scale source of the adjoint planes
 };
 
 template <typename T>
@@ -528,10 +530,13 @@ __global__ void __launch_bounds__(192, 1) wgrad_kernel(const __grid_constant__ C
       tc_fence_after();
       const uint32_t tbase = tmem_base + ((uint32_t)(q * 32) << 16) + buf * 256;
       float* dst = p.gW + (size_t)(mt * kBM + q * 32 + lane) * p.H + nt * p.NW;
+      const float inv_sc = adj_inv_scale(p.amax);
       for (int n = 0; n < p.NW; n += 8) {
         float v[8];
         tmem_ld8(tbase + n, v);
         tmem_ld_wait();
+#pragma unroll
+        for (int i = 0; i < 8; ++i) v[i] *= inv_sc;
         asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(dst + n), "f"(v[0]), "f"(v[1]), "f"(v[2]), "f"(v[3]) : "memory");
         asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(dst + n + 4), "f"(v[4]), "f"(v[5]), "f"(v[6]), "f"(v[7]) : "memory");
       }
@@ -568,8 +573,8 @@ __global__ void __launch_bounds__(256) convert_weights_kernel(NetShape s, const 
 void tc_convert_weights(Launcher& L, int precision, const NetShape& s, const float* theta, void* w16) {
   if (s.L < 2) return;
   dim3 grid(s.H / 32, s.H / 32, s.L - 1);
-  if (precision == PIGAN_BF16) convert_weights_kernel<__nv_bfloat16><<<grid, 256, 0, L.stream>>>(s, theta, (__nv_bfloat16*)w16);
-  else convert_weights_kernel<__half><<<grid, 256, 0, L.stream>>>(s, theta, (__half*)w16);
+  (void)precision;   // bf16-representable weights convert to fp16 exactly (|w| >= 2^-14), so both 16-bit modes share the fp16 copies
+  convert_weights_kernel<__half><<<grid, 256, 0, L.stream>>>(s, theta, (__half*)w16);
   L.check("convert_weights");
 }
 
@@ -598,7 +603,8 @@ static bool make_map(Launcher& L, CUtensorMap* m, int precision, const void* bas
                      const cuuint32_t* box, CUtensorMapSwizzle swz) {
   EncodeTiledFn fn = get_encode();
   cuuint32_t estr[3] = {1, 1, 1};
-  const CUtensorMapDataType dt = precision == PIGAN_BF16 ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16 : CU_TENSOR_MAP_DATA_TYPE_FLOAT16;
+  (void)precision;
+  const CUtensorMapDataType dt = CU_TENSOR_MAP_DATA_TYPE_FLOAT16;
   if (!fn || fn(m, dt, rank, const_cast<void*>(base), dims, strides_bytes, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, swz,
                 CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS) {
     if (L.err == cudaSuccess) { L.err = cudaErrorInvalidValue; L.where = "cuTensorMapEncodeTiled"; }
@@ -647,7 +653,8 @@ static void dispatch_jet(Launcher& L, int precision, int C, const CUtensorMap& a
   if (C == 1) launch_jet<TT, 1, MODE>(L, a, b, o, s, t, p);            \
   else if (C == 3) launch_jet<TT, 3, MODE>(L, a, b, o, s, t, p);       \
   else launch_jet<TT, 5, MODE>(L, a, b, o, s, t, p)
-  if (precision == PIGAN_BF16) { PIGAN_JET(__nv_bfloat16); } else { PIGAN_JET(__half); }
+  (void)precision;                                          // both 16-bit modes compute with fp16 operands
+  PIGAN_JET(__half);
 #undef PIGAN_JET
 }
 
@@ -673,11 +680,11 @@ void tc_layer_fwd_split(Launcher& L, int precision, int H, int R, int R_ld, cons
     return;
   JetParams p{};
   p.H = H; p.n_row_tiles = R / kRT; p.bias = bias;
-  if (precision == PIGAN_BF16) launch_jet<__nv_bfloat16, 2, 2>(L, a, b, o, o, o, p); else launch_jet<__half, 2, 2>(L, a, b, o, o, o, p);
+  launch_jet<__half, 2, 2>(L, a, b, o, o, o, p);
 }
 
 void tc_layer_bwd(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* w16T_l, const void* ahat_in, const void* h_prev,
-                  const void* stash_prev, const float* W1, int in_dim, void* ahat_out, float* g_bias_prev) {
+                  const void* stash_prev, const float* W1, int in_dim, void* ahat_out, float* g_bias_prev, const float* amax) {
   if (R <= 0) return;
   CUtensorMap a, b, o, s, t;
   bool ok = weight_map(L, &a, precision, w16T_l, H) && plane_map(L, &b, precision, ahat_in, H, R_ld, C, kRT, kBK, C, CU_TENSOR_MAP_SWIZZLE_128B) &&
@@ -686,14 +693,14 @@ void tc_layer_bwd(Launcher& L, int precision, int C, int H, int R, int R_ld, con
   if (stash_prev && C > 1) ok = ok && plane_map(L, &s, precision, stash_prev, H, R_ld, C - 1, 32, 32, 1, CU_TENSOR_MAP_SWIZZLE_64B); else s = t;
   if (!ok) return;
   JetParams p{};
-  p.H = H; p.n_row_tiles = R / kRT; p.has_stash = (stash_prev && C > 1) ? 1 : 0; p.in_dim = in_dim; p.W1 = W1; p.g_bias = g_bias_prev;
+  p.H = H; p.n_row_tiles = R / kRT; p.has_stash = (stash_prev && C > 1) ? 1 : 0; p.in_dim = in_dim; p.W1 = W1; p.g_bias = g_bias_prev; p.amax = amax;
   dispatch_jet<1>(L, precision, C, a, b, o, s, t, p);
 }
 
-void tc_wgrad(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* ahat, const void* h_prev, float* gW) {
+void tc_wgrad(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* ahat, const void* h_prev, float* gW, const float* amax) {
   if (R <= 0) return;
   WgradParams p{};
-  p.H = H; p.C = C; p.NW = std::min(H, 256); p.R = R; p.gW = gW;
+  p.H = H; p.C = C; p.NW = std::min(H, 256); p.R = R; p.gW = gW; p.amax = amax;
   const int n_tiles = (H / kBM) * (H / p.NW);
   int slices = std::max(1, (2 * num_sms()) / n_tiles);
   int slice_rows = ((R + slices - 1) / slices + 63) / 64 * 64;
@@ -704,15 +711,10 @@ void tc_wgrad(Launcher& L, int precision, int C, int H, int R, int R_ld, const v
         plane_map(L, &b, precision, h_prev, H, R_ld, C, 64, p.NW, 1, CU_TENSOR_MAP_SWIZZLE_128B)))
     return;
   const int smem = kWStages * (kAStage + 256 * 128) + 1024 + 256;
-  static bool attr_set[2] = {false, false};
+  static bool attr_set = false;
   const int grid = std::min(n_tiles * p.n_slices, num_sms());
-  if (precision == PIGAN_BF16) {
-    if (!attr_set[0]) { cudaFuncSetAttribute(wgrad_kernel<__nv_bfloat16>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); attr_set[0] = true; }
-    wgrad_kernel<__nv_bfloat16><<<grid, 192, smem, L.stream>>>(a, b, p);
-  } else {
-    if (!attr_set[1]) { cudaFuncSetAttribute(wgrad_kernel<__half>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); attr_set[1] = true; }
-    wgrad_kernel<__half><<<grid, 192, smem, L.stream>>>(a, b, p);
-  }
+  if (!attr_set) { cudaFuncSetAttribute(wgrad_kernel<__half>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); attr_set = true; }
+  wgrad_kernel<__half><<<grid, 192, smem, L.stream>>>(a, b, p);
   L.check("wgrad");
 }
 
