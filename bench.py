@@ -278,8 +278,12 @@ def main():
     ap.add_argument("--impl", default="pigan", choices=["pigan", "reference"])
     ap.add_argument("--all-configs", action="store_true", help="also run c1..c4 briefly and attach them as per_config")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--samples", type=int, default=None, help="override N (latent samples per step): a smaller job for ncu captures; "
+                    "the line then says so in config.workload and is not a benchmark value")
     args = ap.parse_args()
     cfg = wl.CONFIGS[args.config]
+    if args.samples:
+        cfg = dataclasses.replace(cfg, name=f"{cfg.name}[N={args.samples} profiling subset]", N=args.samples)
     rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     warmup = max(3, args.warmup) if args.impl == "pigan" else args.warmup

@@ -309,9 +309,9 @@ pigan_status pigan_create(const pigan_config* cfg, void* cuda_stream, pigan_ctx*
   const long long max_rows = std::max<long long>((long long)N * cfg->n_colloc, (long long)N * S);
   size_t free_b = 0, total_b = 0;
   cudaMemGetInfo(&free_b, &total_b);
-  size_t budget = cfg->workspace_bytes ? cfg->workspace_bytes : std::min<size_t>(free_b / 2, (size_t)24 << 30);
+  size_t budget = cfg->workspace_bytes ? cfg->workspace_bytes : std::min<size_t>(free_b / 2, (size_t)48 << 30);
   long long rows = (long long)(budget / per_row);
-  long long cap = 16384;                                   // default chunk: keeps one layer's planes near the L2 size
+  long long cap = 65536;                                   // default chunk rows (sweep on B200: larger chunks amortise launch ramps)
   if (const char* e = getenv("PIGAN_CHUNK_ROWS")) cap = std::max(256LL, atoll(e));
   if (!cfg->workspace_bytes) rows = std::min(rows, cap);
   rows = std::min<long long>(rows, (long long)round_up((size_t)max_rows, 256));
