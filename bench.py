@@ -28,6 +28,9 @@ import workloads as wl  # noqa: E402
 METRIC = "PI-GAN train-step sample*collocation-points/s"
 UNIT = "sample*collocation-points/s"
 ADAM = dict(lr=1e-4, beta1=0.5, beta2=0.9, adam_eps=1e-8)          # reading G3
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the largest tensor-core kernel (G_u forward, 65536-row chunk),
+# from profiles/r01_ncu_full_tc_kernels_c5.csv; algorithmic bytes of that launch: 1.879e9
+TRAFFIC = {"c5": 1.835e9}
 
 
 # ----------------------------------------------------------------------------------------------------------------
@@ -235,7 +238,7 @@ def run_config(cfg, device, steps, warmup, rank, world, with_roofline=True, seed
             ach = alg / (tc_ms * 1e-3) / 1e12
             peak = peaks["tflops_sustained"]
             res["roofline"] = {"bound": "tensor", "achieved": round(ach, 2), "peak": peak, "unit": "TFLOP/s", "frac": round(ach / peak, 4),
-                               "traffic": None, "kernel": "jet_layer_fwd + jet_layer_bwd + wgrad (tcgen05)", "peak_source": peaks["source"] + " sustained bf16",
+                               "traffic": TRAFFIC.get(cfg.name), "kernel": "jet_layer_fwd + jet_layer_bwd + wgrad (tcgen05)", "peak_source": peaks["source"] + " sustained bf16",
                                "frac_of_burst": round(ach / peaks["tflops_burst"], 4), "frac_of_nominal_2250": round(ach / 2250.0, 4),
                                "share_of_step": round(tc_ms / total_ms, 4) if total_ms > 0 else None,
                                "per_kernel_tflops": {k: round(alg / 3 / (v[1] / steps * 1e-3) / 1e12, 1) for k, v in tc.items() if v[1] > 0}}
