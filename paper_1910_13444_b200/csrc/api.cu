@@ -17,7 +17,6 @@ namespace {
 struct NetWs {                 // activation workspace of one generator net (planes are [channel][unit][row])
   int Cmax = 0;
   char* h = nullptr;           // L x [Cmax][H][R_ld]      post-activations h^1..h^L
-  char* st = nullptr;          // (L-1) x [Cmax-1][H][R_ld] stored a_x, a_y, a_xx, a_yy of layers 2..L
   char* ah[2] = {nullptr, nullptr};   // adjoint ping-pong, [Cmax][H][R_ld]
   float* apre = nullptr;       // fp32 mode: [Cmax][H][R_ld] pre-activations / hhat scratch
   float* o = nullptr;          // [Cmax][R_ld] outputs of the chunk
@@ -53,7 +52,6 @@ struct pigan_ctx {
   }
   size_t plane() const { return (size_t)gen.H * R_ld * elem; }
   char* h(int n, int l) { return net[n].h + (size_t)(l - 1) * net[n].Cmax * plane(); }              // l = 1..L
-  char* st(int n, int l) { return net[n].st + (size_t)(l - 2) * (net[n].Cmax - 1) * plane(); }      // l = 2..L
   void* w16(int n, int l, int transposed) { return (char*)net[n].w16 + ((size_t)(l - 2) * 2 + transposed) * gen.H * gen.H * 2; }
 };
 
@@ -92,11 +90,11 @@ void gen_forward_chunk(pigan_ctx* c, int n, const float* theta, int C, const flo
     if (c->cfg.precision == PIGAN_FP32) {
       // a_c = W_l h_c^{l-1}: M = H, N = rows, K = H, batched over the C channel planes
       sgemm(L, false, false, H, g.R, H, theta + s.W_off(l), H, 0, (const float*)c->h(n, l - 1), g.R_ld, pl, c->net[n].apre, g.R_ld, pl, C, false);
-      jet_act_fwd_f32(L, C, H, theta + s.b_off(l), g, c->net[n].apre, (float*)c->h(n, l), (float*)c->st(n, l));
+      jet_act_fwd_f32(L, C, H, theta + s.b_off(l), g, c->net[n].apre, (float*)c->h(n, l));
     } else if (split) {
       tc_layer_fwd_split(L, c->cfg.precision, H, g.R, g.R_ld, c->w16(n, l, 0), theta + s.b_off(l), c->h(n, l - 1), c->h(n, l));
     } else {
-      tc_layer_fwd(L, c->cfg.precision, C, H, g.R, g.R_ld, c->w16(n, l, 0), theta + s.b_off(l), c->h(n, l - 1), c->h(n, l), c->st(n, l));
+      tc_layer_fwd(L, c->cfg.precision, C, H, g.R, g.R_ld, c->w16(n, l, 0), theta + s.b_off(l), c->h(n, l - 1), c->h(n, l));
     }
   }
   out_fwd<T>(L, C, H, theta + s.W_off(s.L + 1), theta + s.b_off(s.L + 1), g, (const T*)c->h(n, s.L), o, o_stride, split);
@@ -112,20 +110,19 @@ void gen_backward_chunk(pigan_ctx* c, int n, const float* theta, float* grads, i
   int cur = 0;
   const float* amax = c->cfg.precision == PIGAN_FP32 ? nullptr : c->amax + n;
   jet_act_bwd_launch<T>(L, C, H, g, nullptr, theta + s.W_off(s.L + 1), c->net[n].oh, (const T*)c->h(n, s.L),
-                        s.L >= 2 ? (const T*)c->st(n, s.L) : nullptr, theta, s.in_dim, (T*)c->net[n].ah[cur], grads + s.b_off(s.L),
+                        (T*)c->net[n].ah[cur], grads + s.b_off(s.L),
                         grads + s.W_off(s.L + 1), grads + s.b_off(s.L + 1), amax);
   for (int l = s.L; l >= 2; --l) {
-    const T* stash_prev = l - 1 >= 2 ? (const T*)c->st(n, l - 1) : nullptr;
     if (c->cfg.precision == PIGAN_FP32) {
       // W_hat_l += sum_c ahat_c h_c^{l-1 T}: M = H, N = H, K = rows
       sgemm(L, false, true, H, H, g.R, (const float*)c->net[n].ah[cur], g.R_ld, pl, (const float*)c->h(n, l - 1), g.R_ld, pl, grads + s.W_off(l), H, 0, C, true);
       // hhat_c^{l-1} = W_l^T ahat_c: M = H (in), N = rows, K = H (out); A stored [K][M]
       sgemm(L, true, false, H, g.R, H, theta + s.W_off(l), H, 0, (const float*)c->net[n].ah[cur], g.R_ld, pl, c->net[n].apre, g.R_ld, pl, C, false);
-      jet_act_bwd_launch<T>(L, C, H, g, c->net[n].apre, nullptr, nullptr, (const T*)c->h(n, l - 1), stash_prev, theta, s.in_dim,
+      jet_act_bwd_launch<T>(L, C, H, g, c->net[n].apre, nullptr, nullptr, (const T*)c->h(n, l - 1),
                             (T*)c->net[n].ah[cur ^ 1], grads + s.b_off(l - 1), nullptr, nullptr, amax);
     } else {
       tc_wgrad(L, c->cfg.precision, C, H, g.R, g.R_ld, c->net[n].ah[cur], c->h(n, l - 1), grads + s.W_off(l), amax);
-      tc_layer_bwd(L, c->cfg.precision, C, H, g.R, g.R_ld, c->w16(n, l, 1), c->net[n].ah[cur], c->h(n, l - 1), stash_prev, theta, s.in_dim,
+      tc_layer_bwd(L, c->cfg.precision, C, H, g.R, g.R_ld, c->w16(n, l, 1), c->net[n].ah[cur], c->h(n, l - 1),
                    c->net[n].ah[cur ^ 1], grads + s.b_off(l - 1), amax);
     }
     cur ^= 1;
@@ -303,9 +300,9 @@ pigan_status pigan_create(const pigan_config* cfg, void* cuda_stream, pigan_ctx*
   c->elem = cfg->precision == PIGAN_FP32 ? 4 : 2;
   const int H = c->gen.H, Lh = c->gen.L, N = cfg->n_samples, S = cfg->n_sensors, d = 2 * S, HD = c->disc.H, LD = c->disc.L;
   const bool f32 = cfg->precision == PIGAN_FP32;
-  // bytes per chunk row over both nets: h (L*C) + stash ((L-1)(C-1)) + adjoint ping-pong (2C) planes [+ fp32 scratch]
+  // bytes per chunk row over both nets: h (L*C) + adjoint ping-pong (2C) planes [+ fp32 scratch]
   size_t per_row = 0;
-  for (int C : {3, 5}) per_row += ((size_t)Lh * C + (size_t)(Lh - 1) * (C - 1) + 2 * C) * H * c->elem + (f32 ? (size_t)C * H * 4 : 0) + 2 * C * 4;
+  for (int C : {3, 5}) per_row += ((size_t)Lh * C + 2 * C) * H * c->elem + (f32 ? (size_t)C * H * 4 : 0) + 2 * C * 4;
   const long long max_rows = std::max<long long>((long long)N * cfg->n_colloc, (long long)N * S);
   size_t free_b = 0, total_b = 0;
   cudaMemGetInfo(&free_b, &total_b);
@@ -323,7 +320,6 @@ pigan_status pigan_create(const pigan_config* cfg, void* cuda_stream, pigan_ctx*
       w.Cmax = n == 0 ? 3 : 5;
       const size_t pl = c->plane();
       w.h = c->alloc<char>((size_t)Lh * w.Cmax * pl);
-      w.st = c->alloc<char>((size_t)std::max(Lh - 1, 1) * (w.Cmax - 1) * pl);
       w.ah[0] = c->alloc<char>((size_t)w.Cmax * pl);
       w.ah[1] = c->alloc<char>((size_t)w.Cmax * pl);
       if (f32) w.apre = c->alloc<float>((size_t)w.Cmax * H * c->R_ld);

@@ -50,22 +50,26 @@ __device__ __forceinline__ void jet_act_fwd(float t, const float* a, float* h) {
     h[4] = fmaf(s, a[4], q * a[2] * a[2]);
   }
 }
-// adjoint: hh = adjoints of h_c; t = tanh(a); ad[0..C-2] = stored a_x, a_y, a_xx, a_yy; aa = adjoints of a_c.
+// adjoint, written in the layer's OUTPUT jet h = (t, h_x, h_y, h_xx, h_yy) -- no pre-activation derivatives are kept.
+// With s = 1 - t^2, q = -2ts, q' = -2s(1 - 3t^2) and h_x = s a_x, h_xx = s a_xx + q a_x^2, O4 becomes
+//   q a_x = -2t h_x,   q a_xx + q' a_x^2 = -2t h_xx - 2 h_x^2   (substitute s a_xx = h_xx - q a_x^2), so
+//   ahat_xx = s hhat_xx;  ahat_x = s hhat_x - 4t h_x hhat_xx;
+//   ahat = s hhat - 2t (h_x hhat_x + h_y hhat_y + h_xx hhat_xx + h_yy hhat_yy) - 2 (h_x^2 hhat_xx + h_y^2 hhat_yy).
+// hh = adjoints of h_c; aa = adjoints of a_c.
 template <int C>
-__device__ __forceinline__ void jet_act_bwd(float t, const float* ad, const float* hh, float* aa) {
-  const float s = 1.f - t * t;
+__device__ __forceinline__ void jet_act_bwd(const float* h, const float* hh, float* aa) {
+  const float t = h[0], s = 1.f - t * t;
   float v = s * hh[0];
   if (C >= 3) {
-    const float q = -2.f * t * s;
-    v = fmaf(q, fmaf(ad[0], hh[1], ad[1] * hh[2]), v);
+    const float m2t = -2.f * t;
+    v = fmaf(m2t, fmaf(h[1], hh[1], h[2] * hh[2]), v);
     aa[1] = s * hh[1];
     aa[2] = s * hh[2];
     if (C >= 5) {
-      const float qp = -2.f * s * (1.f - 3.f * t * t);
-      v = fmaf(q, fmaf(ad[2], hh[3], ad[3] * hh[4]), v);
-      v = fmaf(qp, fmaf(ad[0] * ad[0], hh[3], ad[1] * ad[1] * hh[4]), v);
-      aa[1] = fmaf(2.f * q * ad[0], hh[3], aa[1]);
-      aa[2] = fmaf(2.f * q * ad[1], hh[4], aa[2]);
+      v = fmaf(m2t, fmaf(h[3], hh[3], h[4] * hh[4]), v);
+      v = fmaf(-2.f, fmaf(h[1] * h[1], hh[3], h[2] * h[2] * hh[4]), v);
+      aa[1] = fmaf(2.f * m2t * h[1], hh[3], aa[1]);
+      aa[2] = fmaf(2.f * m2t * h[2], hh[4], aa[2]);
       aa[3] = s * hh[3];
       aa[4] = s * hh[4];
     }
@@ -131,7 +135,7 @@ struct ChunkGeom {          // one chunk of generator rows r = row0 .. row0+vali
 template <typename T>
 void first_layer_fwd(Launcher& L, int C, const NetShape& s, const float* theta, const float* Zp, const float* xy,
                      const ChunkGeom& g, T* h1, bool split = false);   // split: C = 1, writes planes (hi, lo)
-void jet_act_fwd_f32(Launcher& L, int C, int H, const float* bias, const ChunkGeom& g, const float* apre, float* h, float* stash);
+void jet_act_fwd_f32(Launcher& L, int C, int H, const float* bias, const ChunkGeom& g, const float* apre, float* h);
 template <typename T>
 void out_fwd(Launcher& L, int C, int H, const float* w_out, const float* b_out, const ChunkGeom& g, const T* hL,
              float* o, long long o_plane_stride, bool split = false);          // split: C = 1, sums planes (hi, lo)
@@ -142,8 +146,7 @@ void residual(Launcher& L, const float* Y, long long y_stride, const float* U, l
 // b_hat_l[j] += sum_r ahat_0 (and for the output layer w_hat_out[j], b_hat_out).
 template <typename T>
 void jet_act_bwd_launch(Launcher& L, int C, int H, const ChunkGeom& g, const float* hhat /*or null*/,
-                        const float* w_out, const float* ohat /*[C][R_ld] when hhat null*/, const T* h /*[C][H][R_ld]*/,
-                        const T* stash /*[C-1][H][R_ld] or null = layer 1*/, const float* W1, int in_dim, T* ahat,
+                        const float* w_out, const float* ohat /*[C][R_ld] when hhat null*/, const T* h /*[C][H][R_ld]*/, T* ahat,
                         float* g_bias, float* g_wout, float* g_bout, const float* amax);
 template <typename T>
 void first_layer_bwd(Launcher& L, int C, const NetShape& s, const float* xy, const ChunkGeom& g, const T* ahat,
@@ -190,15 +193,24 @@ struct TcPlan;   // opaque: tensor maps + 16-bit weight copies for one (net, chu
 bool tc_supported(int H, std::string* why);
 // Converts W_l (l = 2..L) of one net to 16-bit: w16[(l-2)*2+0] = W_l [out][in], w16[(l-2)*2+1] = W_l^T [in][out].
 void tc_convert_weights(Launcher& L, int precision, const NetShape& s, const float* theta, void* w16);
-// hidden layer l forward: h_in [C][H][R_ld] -> h_out [C][H][R_ld], stash [C-1][H][R_ld]   (fused tanh-jet epilogue)
+// hidden layer l forward: h_in [C][H][R_ld] -> h_out [C][H][R_ld]   (fused tanh-jet epilogue)
 void tc_layer_fwd(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* w16_l, const float* bias,
-                  const void* h_in, void* h_out, void* stash);
+                  const void* h_in, void* h_out);
 void tc_layer_fwd_split(Launcher& L, int precision, int H, int R, int R_ld, const void* w16_l, const float* bias, const void* h_in, void* h_out);
 // dgrad of layer l with the adjoint of layer l-1's tanh fused: ahat_in (layer l) -> ahat_out (layer l-1)
 void tc_layer_bwd(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* w16T_l, const void* ahat_in,
-                  const void* h_prev /*[C][H][R_ld], value plane = t*/, const void* stash_prev /*null = layer 1*/,
-                  const float* W1, int in_dim, void* ahat_out, float* g_bias_prev, const float* amax);
+                  const void* h_prev /*[C][H][R_ld]*/, void* ahat_out, float* g_bias_prev, const float* amax);
 // wgrad of layer l: gW [H][H] += sum_c ahat_c h_prev_c^T   (fp32 atomics)
 void tc_wgrad(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* ahat, const void* h_prev, float* gW, const float* amax);
+
+
+// ---- the same four on CTA pairs (tc2_kernels.cu, cta_group::2), taken when tc2_supported(H) ---------------------
+bool tc2_supported(int H);
+void tc2_layer_fwd(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* w16_l, const float* bias,
+                   const void* h_in, void* h_out);
+void tc2_layer_fwd_split(Launcher& L, int precision, int H, int R, int R_ld, const void* w16_l, const float* bias, const void* h_in, void* h_out);
+void tc2_layer_bwd(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* w16T_l, const void* ahat_in,
+                   const void* h_prev, void* ahat_out, float* g_bias_prev, const float* amax);
+void tc2_wgrad(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* ahat, const void* h_prev, float* gW, const float* amax);
 
 }  // namespace pigan

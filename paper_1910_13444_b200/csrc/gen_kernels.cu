@@ -203,8 +203,7 @@ template void out_fwd<__half>(Launcher&, int, int, const float*, const float*, c
 // =============================================================================================================
 template <typename T, int C>
 __global__ void __launch_bounds__(256) jet_act_bwd_kernel(int H, ChunkGeom g, const float* __restrict__ hhat, const float* __restrict__ w_out,
-                                                          const float* __restrict__ ohat, const T* __restrict__ h, const T* __restrict__ stash,
-                                                          const float* __restrict__ W1, int in_dim, T* __restrict__ ahat,
+                                                          const float* __restrict__ ohat, const T* __restrict__ h, T* __restrict__ ahat,
                                                           float* __restrict__ g_bias, float* __restrict__ g_wout, float* __restrict__ g_bout,
                                                           const float* __restrict__ amax) {
   __shared__ float red[8];
@@ -212,13 +211,11 @@ __global__ void __launch_bounds__(256) jet_act_bwd_kernel(int H, ChunkGeom g, co
   const size_t plane = (size_t)H * g.R_ld;
   const float sc = adj_scale(amax), inv_sc = adj_inv_scale(amax);     // block scale of the adjoint planes (1 in fp32 mode)
   const float wj = w_out ? w_out[j] * sc : 0.f;
-  float ad1[4] = {0.f, 0.f, 0.f, 0.f};
-  if (!stash && C >= 3) { ad1[0] = W1[(size_t)j * in_dim]; ad1[1] = W1[(size_t)j * in_dim + 1]; }   // layer 1: a_x = W1[:,0], a_y = W1[:,1], a_xx = a_yy = 0
   float s_bias = 0.f, s_wout = 0.f, s_bout = 0.f;
   const int r0 = blockIdx.x * 2048 + threadIdx.x * 8;
   if (r0 < g.R) {
     const size_t off = (size_t)j * g.R_ld + r0;
-    float hv[C][8], hh[C][8], ad[C > 1 ? C - 1 : 1][8], o[C][8];
+    float hv[C][8], hh[C][8], o[C][8];
 #pragma unroll
     for (int c = 0; c < C; ++c) load8<T>(h + c * plane + off, hv[c]);
     if (hhat) {
@@ -233,18 +230,12 @@ __global__ void __launch_bounds__(256) jet_act_bwd_kernel(int H, ChunkGeom g, co
         for (int i = 0; i < 8; ++i) { hh[c][i] = wj * ov[i]; s_wout = fmaf(ov[i], hv[c][i], s_wout); if (c == 0) s_bout += ov[i]; }
       }
     }
-    if (stash) {
-#pragma unroll
-      for (int c = 0; c < C - 1; ++c) load8<T>(stash + c * plane + off, ad[c]);
-    }
 #pragma unroll
     for (int i = 0; i < 8; ++i) {
-      float hx[5], a4[4], aa[5];
+      float hx[5], hj[5], aa[5];
 #pragma unroll
-      for (int c = 0; c < C; ++c) hx[c] = hh[c][i];
-#pragma unroll
-      for (int c = 0; c < C - 1; ++c) a4[c] = stash ? ad[c][i] : ad1[c];
-      jet_act_bwd<C>(hv[0][i], a4, hx, aa);
+      for (int c = 0; c < C; ++c) { hx[c] = hh[c][i]; hj[c] = hv[c][i]; }
+      jet_act_bwd<C>(hj, hx, aa);
       s_bias += aa[0];
 #pragma unroll
       for (int c = 0; c < C; ++c) o[c][i] = aa[c];
@@ -260,17 +251,17 @@ __global__ void __launch_bounds__(256) jet_act_bwd_kernel(int H, ChunkGeom g, co
 
 template <typename T>
 void jet_act_bwd_launch(Launcher& L, int C, int H, const ChunkGeom& g, const float* hhat, const float* w_out, const float* ohat, const T* h,
-                        const T* stash, const float* W1, int in_dim, T* ahat, float* g_bias, float* g_wout, float* g_bout, const float* amax) {
+                        T* ahat, float* g_bias, float* g_wout, float* g_bout, const float* amax) {
   if (g.R <= 0) return;
   dim3 grid(cdiv(g.R, 2048), H);
-#define PIGAN_BWD(c) jet_act_bwd_kernel<T, c><<<grid, 256, 0, L.stream>>>(H, g, hhat, w_out, ohat, h, stash, W1, in_dim, ahat, g_bias, g_wout, g_bout, amax)
+#define PIGAN_BWD(c) jet_act_bwd_kernel<T, c><<<grid, 256, 0, L.stream>>>(H, g, hhat, w_out, ohat, h, ahat, g_bias, g_wout, g_bout, amax)
   if (C == 1) PIGAN_BWD(1); else if (C == 3) PIGAN_BWD(3); else PIGAN_BWD(5);
 #undef PIGAN_BWD
   L.check("jet_act_bwd");
 }
-template void jet_act_bwd_launch<float>(Launcher&, int, int, const ChunkGeom&, const float*, const float*, const float*, const float*, const float*, const float*, int, float*, float*, float*, float*, const float*);
-template void jet_act_bwd_launch<__nv_bfloat16>(Launcher&, int, int, const ChunkGeom&, const float*, const float*, const float*, const __nv_bfloat16*, const __nv_bfloat16*, const float*, int, __nv_bfloat16*, float*, float*, float*, const float*);
-template void jet_act_bwd_launch<__half>(Launcher&, int, int, const ChunkGeom&, const float*, const float*, const float*, const __half*, const __half*, const float*, int, __half*, float*, float*, float*, const float*);
+template void jet_act_bwd_launch<float>(Launcher&, int, int, const ChunkGeom&, const float*, const float*, const float*, const float*, float*, float*, float*, float*, const float*);
+template void jet_act_bwd_launch<__nv_bfloat16>(Launcher&, int, int, const ChunkGeom&, const float*, const float*, const float*, const __nv_bfloat16*, __nv_bfloat16*, float*, float*, float*, const float*);
+template void jet_act_bwd_launch<__half>(Launcher&, int, int, const ChunkGeom&, const float*, const float*, const float*, const __half*, __half*, float*, float*, float*, const float*);
 
 // =============================================================================================================
 // first-layer backward (O4 'First layer'): W_hat_1[:,0] += sum (ahat x + ahat_x), W_hat_1[:,1] += sum (ahat y + ahat_y),

@@ -106,7 +106,7 @@ void sgemm(Launcher& L, bool TA, bool TB, int M, int N, int K, const float* A, i
 // fp32 mode: tanh-jet chain rule applied to the pre-activations written by sgemm
 template <int C>
 __global__ void __launch_bounds__(128) jet_act_fwd_kernel(int H, const float* __restrict__ bias, ChunkGeom g,
-                                                          const float* __restrict__ apre, float* __restrict__ h, float* __restrict__ stash) {
+                                                          const float* __restrict__ apre, float* __restrict__ h) {
   const int r = blockIdx.x * 128 + threadIdx.x, j = blockIdx.y;
   if (r >= g.R) return;
   const size_t plane = (size_t)H * g.R_ld, off = (size_t)j * g.R_ld + r;
@@ -117,15 +117,13 @@ __global__ void __launch_bounds__(128) jet_act_fwd_kernel(int H, const float* __
   jet_act_fwd<C>(tanhf(a[0]), a, o);
 #pragma unroll
   for (int c = 0; c < C; ++c) h[c * plane + off] = o[c];
-#pragma unroll
-  for (int c = 1; c < C; ++c) stash[(c - 1) * plane + off] = a[c];
 }
 
-void jet_act_fwd_f32(Launcher& L, int C, int H, const float* bias, const ChunkGeom& g, const float* apre, float* h, float* stash) {
+void jet_act_fwd_f32(Launcher& L, int C, int H, const float* bias, const ChunkGeom& g, const float* apre, float* h) {
   dim3 grid(cdiv(g.R, 128), H);
-  if (C == 1) jet_act_fwd_kernel<1><<<grid, 128, 0, L.stream>>>(H, bias, g, apre, h, stash);
-  else if (C == 3) jet_act_fwd_kernel<3><<<grid, 128, 0, L.stream>>>(H, bias, g, apre, h, stash);
-  else jet_act_fwd_kernel<5><<<grid, 128, 0, L.stream>>>(H, bias, g, apre, h, stash);
+  if (C == 1) jet_act_fwd_kernel<1><<<grid, 128, 0, L.stream>>>(H, bias, g, apre, h);
+  else if (C == 3) jet_act_fwd_kernel<3><<<grid, 128, 0, L.stream>>>(H, bias, g, apre, h);
+  else jet_act_fwd_kernel<5><<<grid, 128, 0, L.stream>>>(H, bias, g, apre, h);
   L.check("jet_act_fwd");
 }
 

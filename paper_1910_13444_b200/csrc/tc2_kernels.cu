@@ -1,0 +1,596 @@
+// sm_100a tensor-core kernels of the jet MLP on CTA PAIRS (tcgen05 cta_group::2), used when the width is a multiple
+// of 256.  Same math and plane layout as tc_kernels.cu; what changes is
+// how much every SM must pull in per flop: the SM's inbound path (~64 B/clk) bounds the one-CTA kernels, and a pair
+// shares the activation operand, so each CTA loads its own 128 x K weight rows but only HALF of the activation tile.
+//
+// jet layer:  D[256 units][(channel, row) columns] = W_tile[256 x K] . act[K x (C * 64 rows)]
+//   A = weights, K-major, SW128: CTA r of the pair loads units [128 r, 128 r + 128) of the tile.
+//   B = activation planes [channel][unit][row], MN-major, SW64: CTA r loads rows [32 r, 32 r + 32) of the 64-row tile
+//       for all C channels (one 3D TMA box 32 rows x 64 units x C).  One MMA covers a group of nc channels,
+//       N = 64 nc; its accumulator columns are [CTA half h][channel][32 rows].
+//   C = 5 needs 320 of the 512 TMEM columns, so tiles alternate between columns [0, 320) and [192, 512) with the
+//       (xx, yy) group always at [192, 320): the epilogue pulls that group into registers first and releases it, so
+//       the next tile's MMAs start while the rest of the epilogue runs.  C <= 3 double-buffers.
+//   Epilogue: 8 warps per CTA; warp (q, h) owns units [32 q, 32 q + 32) (TMEM lanes) x rows [32 h, 32 h + 32).
+// wgrad:  D[256 out units][256 in units] += sum_{c, row} ahat_c[out][row] h_c[in][row], both operands K-major SW128.
+#include "tc_ptx.cuh"
+
+namespace pigan {
+
+constexpr int k2AStage = 128 * 64 * 2;      // 16 KB: 128 units x 64 contraction elements
+constexpr int k2BPlane = 64 * 32 * 2;       // 4 KB: 64 contraction units x 32 rows of one channel
+constexpr int k2StgPlane = 32 * 64;         // epilogue staging plane: 32 units x 32 rows x 2 B
+constexpr int k2EpiWarps = 8;
+constexpr int k2Threads = (4 + k2EpiWarps) * 32;
+
+#ifdef PIGAN_PROBE_FREERUN
+#define LOOKAHEAD(b, p) false
+#else
+#define LOOKAHEAD(b, p) mbar_try_wait(b, p)
+#endif
+
+template <int C, int MODE> struct Jet2Cfg {
+  static constexpr int kStageBytes = k2AStage + C * k2BPlane;
+  static constexpr int kCols = C * 64;                                 // accumulator columns of one tile
+  static constexpr int kNumBuf = C == 5 ? 1 : 2;                       // C = 5: alternating placement, early release
+  static constexpr int kTmemCols = C == 5 ? 512 : 2 * kCols <= 128 ? 128 : 2 * kCols <= 256 ? 256 : 512;
+  static constexpr int kSlots = C;                                     // staging planes per epilogue warp
+  static constexpr int kStgBytes = k2EpiWarps * kSlots * k2StgPlane;
+  static constexpr int kBudget = 232448 - 1024 - 512 - kStgBytes;
+  static constexpr int kNumStages = kBudget / kStageBytes > 6 ? 6 : kBudget / kStageBytes;
+  static constexpr int kSmemBytes = kNumStages * kStageBytes + kStgBytes + 1024 /*align*/ + 512 /*barriers*/;
+};
+
+struct Jet2Params {
+  int H;                 // width (K and number of output units), multiple of 256
+  int n_row_tiles;       // R / 64
+  const float* bias;     // MODE 0, 2: b_l
+  float* g_bias;         // MODE 1: b_hat_{l-1}
+  const float* amax;     // MODE 1: block-scale source of the adjoint planes
+};
+
+// MODE 0: forward; MODE 1: dgrad + adjoint of the previous tanh; MODE 2: value-only forward on split (hi, lo) planes
+template <typename T, int C, int MODE>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(k2Threads, 1)
+jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H] 16-bit, box 64 x 128, SW128
+                  const __grid_constant__ CUtensorMap tmB,      // input planes, box 32 rows x 64 units x C, SW64
+                  const __grid_constant__ CUtensorMap tmO,      // MODE 0, 2: h_out; MODE 1: ahat_out (box 32 x 32 x 1, SW64)
+                  const __grid_constant__ CUtensorMap tmT,      // MODE 1: h_prev planes in (box 32 x 32 x 1, SW64)
+                  Jet2Params p) {
+  using Cfg = Jet2Cfg<C, MODE>;
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  uint8_t* stages = smem;
+  uint8_t* staging = smem + Cfg::kNumStages * Cfg::kStageBytes;
+  uint64_t* bars = reinterpret_cast<uint64_t*>(staging + Cfg::kStgBytes);
+  uint64_t* full = bars;                                   // [kNumStages]  leader's is used
+  uint64_t* empty = bars + Cfg::kNumStages;                // [kNumStages]  per CTA
+  uint64_t* tfull = empty + Cfg::kNumStages;               // [kNumBuf]     per CTA
+  uint64_t* tempty = tfull + Cfg::kNumBuf;                 // [kNumBuf]     leader's is used, 16 arrivals
+  uint64_t* sbar = tempty + Cfg::kNumBuf;                  // [8]           staging loads (MODE 1), one per epilogue warp
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(sbar + k2EpiWarps);
+
+#ifdef PIGAN_PROBE_TRACE
+  __shared__ long long tr_wait[16], tr_issue[16], tr_prod[16], tr_prod0[16];
+#endif
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const uint32_t rank = cluster_ctarank();
+  const int cluster_id = blockIdx.x >> 1, n_clusters = gridDim.x >> 1;
+  const int n_ut = p.H / 256;
+  const int n_tiles = n_ut * p.n_row_tiles;
+  const int n_kb = p.H / 64;
+
+  if (warp == 0 && lane == 0) {
+    prefetch_tmap(&tmA); prefetch_tmap(&tmB); prefetch_tmap(&tmO);
+    if (MODE == 1) prefetch_tmap(&tmT);
+  }
+  if (warp == 1 && lane == 0) {
+    for (int i = 0; i < Cfg::kNumStages; ++i) { mbar_init(full + i, 1); mbar_init(empty + i, 1); }
+    for (int i = 0; i < Cfg::kNumBuf; ++i) { mbar_init(tfull + i, 1); mbar_init(tempty + i, 2 * k2EpiWarps); }
+    for (int i = 0; i < k2EpiWarps; ++i) mbar_init(sbar + i, 1);
+    fence_barrier_init();
+  }
+  if (warp == 2) tmem2_alloc(tmem_slot, Cfg::kTmemCols);
+  tc_fence_before();
+  __syncthreads();
+  cluster_sync_all();                                      // the peer's barriers are initialised before anything signals them
+  tc_fence_after();
+  const uint32_t tmem_base = *tmem_slot;
+
+  // accumulator columns: tile `it` of this cluster; channel group 0 = channels [0, min(C, 3)), group 1 = (xx, yy)
+  auto g0_col = [&](int it) -> uint32_t { return C == 5 ? ((it & 1) ? 320u : 0u) : (uint32_t)((it % Cfg::kNumBuf) * Cfg::kCols); };
+  constexpr uint32_t g1_col = 192;
+  constexpr int nc0 = C == 5 ? 3 : C;                      // channels in group 0
+
+  if (warp == 0) {
+    // ===================== TMA producer (both CTAs) =====================
+    if (lane == 0) {
+      int stage = 0; uint32_t phase = 0;
+      for (int t = cluster_id; t < n_tiles; t += n_clusters) {
+        const int ut = t % n_ut, rt = t / n_ut;
+        for (int kb = 0; kb < n_kb; ++kb) {
+#ifdef PIGAN_PROBE_FREERUN
+          continue;
+#endif
+#ifdef PIGAN_PROBE_TRACE
+          if (rank == 0 && cluster_id == 0 && t == cluster_id + 10 * n_clusters) tr_prod0[kb] = clock64();
+#endif
+          mbar_wait(empty + stage, phase ^ 1);
+#ifdef PIGAN_PROBE_TRACE
+          if (rank == 0 && cluster_id == 0 && t == cluster_id + 10 * n_clusters) tr_prod[kb] = clock64();
+#endif
+          uint8_t* sA = stages + stage * Cfg::kStageBytes;
+          const uint32_t lbar = mapa_u32(full + stage, 0);
+#ifdef PIGAN_PROBE_NOLOAD
+          if (rank == 0) mbar_arrive(full + stage);
+          (void)sA; (void)lbar;
+#else
+          if (rank == 0) mbar_expect_tx(full + stage, 2 * Cfg::kStageBytes);
+          tma2_load_2d(sA, &tmA, lbar, kb * 64, ut * 256 + (int)rank * 128);
+          tma2_load_3d(sA + k2AStage, &tmB, lbar, rt * 64 + (int)rank * 32, kb * 64, 0);
+#endif
+          if (++stage == Cfg::kNumStages) { stage = 0; phase ^= 1; }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ===================== MMA issuer (one thread of the leader CTA) =====================
+    if (rank == 0 && lane == 0) {
+      // tcgen05.mma issue returns when the MMA starts executing (the queue is about one deep), so a barrier wait
+      // issued after the last MMA of a stage idles the tensor pipe for its whole latency.  The wait for the NEXT
+      // stage is therefore polled behind the longest MMA of the last k-step, and only repeated (blocking) on a miss.
+      int stage = 0; uint32_t phase = 0; int it = 0;
+      bool ready = false;                                    // full[stage] of the upcoming k-block already seen complete
+#ifdef PIGAN_PROBE_TIMING
+      long long tm_start = clock64(), tm_te = 0, tm_full = 0, tm0;
+#endif
+      constexpr uint32_t idesc0 = umma_idesc(Fmt<T>::umma, 0, 1, 256, nc0 * 64);
+      constexpr uint32_t idesc1 = umma_idesc(Fmt<T>::umma, 0, 1, 256, 128);
+      for (int t = cluster_id; t < n_tiles; t += n_clusters, ++it) {
+        const int buf = it % Cfg::kNumBuf;
+        const uint32_t bphase = (it / Cfg::kNumBuf) & 1;
+        const bool last_tile = t + n_clusters >= n_tiles;
+#ifdef PIGAN_PROBE_TIMING
+        tm0 = clock64();
+#endif
+        mbar_wait_cluster(tempty + buf, bphase ^ 1);         // both CTAs' epilogues have released what this tile overwrites
+        tc_fence_after();
+#ifdef PIGAN_PROBE_TIMING
+        tm_te += clock64() - tm0;
+#endif
+        const uint32_t d0 = tmem_base + g0_col(it), d1 = tmem_base + g1_col;
+        for (int kb = 0; kb < n_kb; ++kb) {
+#ifdef PIGAN_PROBE_TIMING
+          tm0 = clock64();
+#endif
+#ifndef PIGAN_PROBE_FREERUN
+          if (!ready) mbar_wait(full + stage, phase);
+#endif
+          tc_fence_after();
+#ifdef PIGAN_PROBE_TIMING
+          tm_full += clock64() - tm0;
+#endif
+#ifdef PIGAN_PROBE_TRACE
+          if (cluster_id == 0 && it == 10) tr_wait[kb] = clock64();
+#endif
+          const uint32_t sA = smem_u32(stages + stage * Cfg::kStageBytes), sB = sA + k2AStage;
+          int nstage = stage + 1; uint32_t nphase = phase;
+          if (nstage == Cfg::kNumStages) { nstage = 0; nphase ^= 1; }
+#pragma unroll
+          for (int k = 0; k < 4; ++k) {
+            const uint64_t ad = umma_desc_sw128(sA + k * 32, 16, 1024);                       // K-major: +32 B per 16 elements
+            const uint32_t acc = (kb | k) ? 1u : 0u;
+            // MN-major SW64: channel planes are 4 KB apart (LBO), 8-unit groups 512 B apart (SBO), 16 units = +1 KB
+#ifndef PIGAN_PROBE_NOMMA
+            if (C == 5 && k < 3) tc2_mma(d1, ad, umma_desc_sw64(sB + 3 * k2BPlane + k * 1024, k2BPlane, 512), idesc1, acc);
+            if (C != 5 && k == 3) ready = !(last_tile && kb == n_kb - 1) && LOOKAHEAD(full + nstage, nphase);
+            tc2_mma(d0, ad, umma_desc_sw64(sB + k * 1024, k2BPlane, 512), idesc0, acc);
+            if (C == 5 && k == 3) {
+              ready = !(last_tile && kb == n_kb - 1) && LOOKAHEAD(full + nstage, nphase);
+              tc2_mma(d1, ad, umma_desc_sw64(sB + 3 * k2BPlane + k * 1024, k2BPlane, 512), idesc1, acc);
+            }
+#endif
+          }
+#ifdef PIGAN_PROBE_COMMIT1
+          tc_commit(empty + stage);
+#elif !defined(PIGAN_PROBE_NOCOMMIT)
+          tc2_commit(empty + stage);                         // frees the smem slot in both CTAs when these MMAs retire
+#endif
+#ifdef PIGAN_PROBE_TRACE
+          if (cluster_id == 0 && it == 10) tr_issue[kb] = clock64();
+#endif
+          stage = nstage; phase = nphase;
+        }
+        tc2_commit(tfull + buf);                             // accumulator complete (both CTAs)
+      }
+#ifdef PIGAN_PROBE_TRACE
+      if (cluster_id == 0 && C == 5 && MODE == 0 && n_tiles > 11 * n_clusters) {
+        for (int kb = 0; kb < 16; ++kb)
+          printf("TRACE kb=%d wait_done=%lld issue_done=%lld prod_wait_begin=%lld prod_empty_seen=%lld\n", kb, tr_wait[kb] - tr_wait[0], tr_issue[kb] - tr_wait[0],
+                 tr_prod0[kb] - tr_wait[0], tr_prod[kb] - tr_wait[0]);
+      }
+#endif
+#ifdef PIGAN_PROBE_TIMING
+      if (cluster_id == 0) printf("TIMING mma C=%d MODE=%d tiles=%d total=%lld wait_tempty=%lld wait_full=%lld\n", C, MODE, it, clock64() - tm_start, tm_te, tm_full);
+#endif
+    }
+  } else if (warp >= 4) {
+    // ===================== epilogue: warp (q, hs) owns TMEM lanes / units [32q, 32q+32) x rows [32hs, 32hs+32) ==========
+    const int e = warp - 4, q = e & 3, hs = e >> 2;
+    uint8_t* stg = staging + e * (Cfg::kSlots * k2StgPlane);
+    const uint32_t swz = (uint32_t)((lane >> 1) & 3);       // 64B swizzle of a 64-byte row: chunk ^= (row >> 1) & 3
+    uint8_t* my_row = stg + lane * 64;
+    const uint32_t lane_base = tmem_base + ((uint32_t)(q * 32) << 16);
+    uint32_t sphase = 0;
+    int it = 0;
+#ifdef PIGAN_PROBE_TIMING
+    long long te_start = clock64(), te_tf = 0, te_rel = 0, te0;
+#endif
+    for (int t = cluster_id; t < n_tiles; t += n_clusters, ++it) {
+      const int ut = t % n_ut, rt = t / n_ut;
+      const int buf = it % Cfg::kNumBuf;
+      const uint32_t bphase = (it / Cfg::kNumBuf) & 1;
+      const int unit0 = ut * 256 + (int)rank * 128 + q * 32, unit = unit0 + lane;
+      const int row0 = rt * 64 + hs * 32;
+      // TMEM address of (channel c, row 0 of this warp's half)
+      const uint32_t tb0 = lane_base + g0_col(it) + hs * (nc0 * 32), tb1 = lane_base + g1_col + hs * 64;
+      auto tcol = [&](int c) -> uint32_t { return (C == 5 && c >= 3) ? tb1 + (c - 3) * 32 : tb0 + c * 32; };
+      float bias = 0.f, bias_acc = 0.f;
+      if (MODE == 0 || MODE == 2) bias = p.bias[unit];
+      auto release = [&]() {                                 // this warp no longer reads what the next MMAs overwrite
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive_cluster(mapa_u32(tempty + buf, 0));
+      };
+
+      if (MODE == 1 && lane == 0) {                          // the previous layer's output jet h^{l-1} -> staging
+        tma_wait_read_all();                                 // earlier stores have finished reading the staging buffer
+        mbar_expect_tx(sbar + e, C * k2StgPlane);
+        for (int c = 0; c < C; ++c) tma_load_3d(stg + c * k2StgPlane, &tmT, sbar + e, row0, unit0, c);
+      }
+#ifdef PIGAN_PROBE_TIMING
+      te0 = clock64();
+#endif
+      mbar_wait(tfull + buf, bphase);
+      tc_fence_after();
+#ifdef PIGAN_PROBE_TIMING
+      te_tf += clock64() - te0; te0 = clock64();
+#endif
+#ifdef PIGAN_PROBE_NOEPI
+      if (MODE == 1) { mbar_wait(sbar + e, sphase); sphase ^= 1; }
+      release();
+      continue;
+#endif
+
+      // C = 5: the (xx, yy) group leaves TMEM first
+      float kxx[C == 5 ? 32 : 1], kyy[C == 5 ? 32 : 1];
+      if (C == 5) {
+#pragma unroll
+        for (int rc = 0; rc < 4; ++rc) { tmem_ld8(tcol(3) + rc * 8, kxx + rc * 8); tmem_ld8(tcol(4) + rc * 8, kyy + rc * 8); }
+        tmem_ld_wait();
+        release();
+#ifdef PIGAN_PROBE_TIMING
+        te_rel += clock64() - te0;
+#endif
+      }
+
+      if (MODE == 0) {
+        // ---- h_c = tanh-jet(a_c) ----
+        if (lane == 0) tma_wait_read_all();
+        __syncwarp();
+#pragma unroll
+        for (int rc = 0; rc < 4; ++rc) {
+          float v[C][8], o[C][8];
+#pragma unroll
+          for (int c = 0; c < nc0; ++c) tmem_ld8(tcol(c) + rc * 8, v[c]);
+          tmem_ld_wait();
+#pragma unroll
+          for (int i = 0; i < 8; ++i) {
+            float a[5], h[5];
+#pragma unroll
+            for (int c = 0; c < nc0; ++c) a[c] = v[c][i];
+            if (C == 5) { a[3] = kxx[rc * 8 + i]; a[4] = kyy[rc * 8 + i]; }
+            a[0] += bias;
+            jet_act_fwd<C>(fast_tanh(a[0]), a, h);
+#pragma unroll
+            for (int c = 0; c < C; ++c) o[c][i] = h[c];
+          }
+          const uint32_t off = ((uint32_t)rc ^ swz) << 4;
+#pragma unroll
+          for (int c = 0; c < C; ++c) *reinterpret_cast<uint4*>(my_row + c * k2StgPlane + off) = pack8<T>(o[c]);
+        }
+        if (C != 5) release();
+        fence_proxy_async();
+        __syncwarp();
+        if (lane == 0) {
+          for (int c = 0; c < C; ++c) tma_store_3d(&tmO, stg + c * k2StgPlane, row0, unit0, c);
+          tma_commit_group();
+        }
+      } else if (MODE == 2) {
+        // ---- value-only layer with split activations: a = W (h_hi + h_lo) + b; t = tanh a; t_hi = rn16(t), t_lo = rn16(t - t_hi) ----
+        if (lane == 0) tma_wait_read_all();
+        __syncwarp();
+#pragma unroll 1
+        for (int rc = 0; rc < 4; ++rc) {
+          float v0[8], v1[8], hi[8], lo[8];
+          tmem_ld8(tcol(0) + rc * 8, v0);
+          tmem_ld8(tcol(1) + rc * 8, v1);
+          tmem_ld_wait();
+#pragma unroll
+          for (int i = 0; i < 8; ++i) {
+            const float tt = tanhf(v0[i] + v1[i] + bias);
+            hi[i] = to_f<T>(from_f<T>(tt));
+            lo[i] = tt - hi[i];
+          }
+          const uint32_t off = ((uint32_t)rc ^ swz) << 4;
+          *reinterpret_cast<uint4*>(my_row + off) = pack8<T>(hi);
+          *reinterpret_cast<uint4*>(my_row + k2StgPlane + off) = pack8<T>(lo);
+        }
+        release();
+        fence_proxy_async();
+        __syncwarp();
+        if (lane == 0) {
+          tma_store_3d(&tmO, stg, row0, unit0, 0);
+          tma_store_3d(&tmO, stg + k2StgPlane, row0, unit0, 1);
+          tma_commit_group();
+        }
+      } else {
+        // ---- adjoint of the previous layer's tanh: ahat^{l-1} = J^T hhat^{l-1} ----
+        mbar_wait(sbar + e, sphase); sphase ^= 1;
+#pragma unroll
+        for (int rc = 0; rc < 4; ++rc) {
+          float hh[C][8], hp[C][8], o[C][8];
+#pragma unroll
+          for (int c = 0; c < nc0; ++c) tmem_ld8(tcol(c) + rc * 8, hh[c]);
+          const uint32_t off = ((uint32_t)rc ^ swz) << 4;
+#pragma unroll
+          for (int c = 0; c < C; ++c) unpack8<T>(*reinterpret_cast<const uint4*>(my_row + c * k2StgPlane + off), hp[c]);
+          tmem_ld_wait();
+#pragma unroll
+          for (int i = 0; i < 8; ++i) {
+            float hx[5], hj[5], aa[5];
+#pragma unroll
+            for (int c = 0; c < nc0; ++c) hx[c] = hh[c][i];
+            if (C == 5) { hx[3] = kxx[rc * 8 + i]; hx[4] = kyy[rc * 8 + i]; }
+#pragma unroll
+            for (int c = 0; c < C; ++c) hj[c] = hp[c][i];
+            jet_act_bwd<C>(hj, hx, aa);
+            bias_acc += aa[0];
+#pragma unroll
+            for (int c = 0; c < C; ++c) o[c][i] = aa[c];
+          }
+#pragma unroll
+          for (int c = 0; c < C; ++c) *reinterpret_cast<uint4*>(my_row + c * k2StgPlane + off) = pack8<T>(o[c]);
+        }
+        if (C != 5) release();
+        fence_proxy_async();
+        __syncwarp();
+        if (lane == 0) {
+          for (int c = 0; c < C; ++c) tma_store_3d(&tmO, stg + c * k2StgPlane, row0, unit0, c);
+          tma_commit_group();
+        }
+        atomicAdd(p.g_bias + unit, bias_acc * adj_inv_scale(p.amax));
+      }
+    }
+#ifdef PIGAN_PROBE_TIMING
+    if (blockIdx.x == 0 && e == 0 && lane == 0) printf("TIMING epi C=%d MODE=%d tiles=%d total=%lld wait_tfull=%lld early_release=%lld\n", C, MODE, it, clock64() - te_start, te_tf, te_rel);
+#endif
+    if (lane == 0) tma_wait_all();                           // global writes of the last stores are complete before exit
+  }
+  tc_fence_before();
+  __syncthreads();
+  cluster_sync_all();                                        // neither CTA leaves while the pair still uses its smem / TMEM
+  if (warp == 2) { tc_fence_after(); tmem2_dealloc(tmem_base, Cfg::kTmemCols); }
+}
+
+// =============================================================================================================
+// wgrad on CTA pairs: gW[j][k] += sum_{c, r} ahat_c[j][r] h_c[k][r], 256 x 256 output tiles, rows split into slices
+// =============================================================================================================
+constexpr int kW2Stages = 6;
+constexpr int kW2StageBytes = 2 * k2AStage;     // A: 128 out units x 64 rows, B: 128 in units x 64 rows (this CTA's halves)
+struct Wgrad2Params {
+  int H, C;
+  int n_slices;        // row slices
+  int slice_rows;      // rows per slice (multiple of 64)
+  int R;               // rows of the chunk (multiple of 64)
+  float* gW;           // [H][H] fp32
+  const float* amax;   // block-scale source of the adjoint planes
+};
+
+template <typename T>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(192, 1)
+wgrad2_kernel(const __grid_constant__ CUtensorMap tmA,    // ahat planes, box 64 rows x 128 units x 1, SW128
+              const __grid_constant__ CUtensorMap tmB,    // h_prev planes, box 64 rows x 128 units x 1, SW128
+              Wgrad2Params p) {
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  uint8_t* stages = smem;
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + kW2Stages * kW2StageBytes);
+  uint64_t* full = bars; uint64_t* empty = bars + kW2Stages; uint64_t* tfull = empty + kW2Stages; uint64_t* tempty = tfull + 2;
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(tempty + 2);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const uint32_t rank = cluster_ctarank();
+  const int cluster_id = blockIdx.x >> 1, n_clusters = gridDim.x >> 1;
+  const int n_t = p.H / 256;
+  const int n_items = n_t * n_t * p.n_slices;
+
+  if (warp == 0 && lane == 0) { prefetch_tmap(&tmA); prefetch_tmap(&tmB); }
+  if (warp == 1 && lane == 0) {
+    for (int i = 0; i < kW2Stages; ++i) { mbar_init(full + i, 1); mbar_init(empty + i, 1); }
+    for (int i = 0; i < 2; ++i) { mbar_init(tfull + i, 1); mbar_init(tempty + i, 8); }
+    fence_barrier_init();
+  }
+  __syncwarp();
+  if (warp == 1) tmem2_alloc(tmem_slot, 512);
+  tc_fence_before();
+  __syncthreads();
+  cluster_sync_all();
+  tc_fence_after();
+  const uint32_t tmem_base = *tmem_slot;
+
+  auto decode = [&](int w, int& mt, int& nt, int& r0, int& r1) {
+    const int tile = w % (n_t * n_t), sl = w / (n_t * n_t);
+    mt = tile % n_t; nt = tile / n_t;
+    r0 = sl * p.slice_rows; r1 = min(p.R, r0 + p.slice_rows);
+  };
+
+  if (warp == 0) {
+    if (lane == 0) {
+      int stage = 0; uint32_t phase = 0;
+      for (int w = cluster_id; w < n_items; w += n_clusters) {
+        int mt, nt, r0, r1; decode(w, mt, nt, r0, r1);
+        for (int c = 0; c < p.C; ++c)
+          for (int r = r0; r < r1; r += 64) {
+            mbar_wait(empty + stage, phase ^ 1);
+            uint8_t* sA = stages + stage * kW2StageBytes;
+            const uint32_t lbar = mapa_u32(full + stage, 0);
+            if (rank == 0) mbar_expect_tx(full + stage, 2 * kW2StageBytes);
+            tma2_load_3d(sA, &tmA, lbar, r, mt * 256 + (int)rank * 128, c);
+            tma2_load_3d(sA + k2AStage, &tmB, lbar, r, nt * 256 + (int)rank * 128, c);
+            if (++stage == kW2Stages) { stage = 0; phase ^= 1; }
+          }
+      }
+    }
+  } else if (warp == 1) {
+    if (rank == 0 && lane == 0) {
+      int stage = 0; uint32_t phase = 0; int it = 0;
+      constexpr uint32_t idesc = umma_idesc(Fmt<T>::umma, 0, 0, 256, 256);
+      for (int w = cluster_id; w < n_items; w += n_clusters, ++it) {
+        int mt, nt, r0, r1; decode(w, mt, nt, r0, r1);
+        const int buf = it & 1; const uint32_t bphase = (it >> 1) & 1;
+        mbar_wait_cluster(tempty + buf, bphase ^ 1);
+        tc_fence_after();
+        const uint32_t d0 = tmem_base + buf * 256;
+        uint32_t acc = 0;
+        for (int c = 0; c < p.C; ++c)
+          for (int r = r0; r < r1; r += 64) {
+            mbar_wait_cluster(full + stage, phase);
+            tc_fence_after();
+            const uint32_t sA = smem_u32(stages + stage * kW2StageBytes), sB = sA + k2AStage;
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+              tc2_mma(d0, umma_desc_sw128(sA + k * 32, 16, 1024), umma_desc_sw128(sB + k * 32, 16, 1024), idesc, acc);
+              acc = 1;
+            }
+            tc2_commit(empty + stage);
+            if (++stage == kW2Stages) { stage = 0; phase ^= 1; }
+          }
+        tc2_commit(tfull + buf);
+      }
+    }
+  } else {
+    // epilogue warps 2..5 -> TMEM lane quarter (warp % 4); this CTA holds out units [128 rank, 128 rank + 128) of the tile
+    const int q = warp & 3;
+    int it = 0;
+    for (int w = cluster_id; w < n_items; w += n_clusters, ++it) {
+      int mt, nt, r0, r1; decode(w, mt, nt, r0, r1);
+      const int buf = it & 1; const uint32_t bphase = (it >> 1) & 1;
+      mbar_wait(tfull + buf, bphase);
+      tc_fence_after();
+      const uint32_t tbase = tmem_base + ((uint32_t)(q * 32) << 16) + buf * 256;
+      float* dst = p.gW + (size_t)(mt * 256 + (int)rank * 128 + q * 32 + lane) * p.H + nt * 256;
+      const float inv_sc = adj_inv_scale(p.amax);
+      for (int n = 0; n < 256; n += 8) {
+        float v[8];
+        tmem_ld8(tbase + n, v);
+        tmem_ld_wait();
+#pragma unroll
+        for (int i = 0; i < 8; ++i) v[i] *= inv_sc;
+        asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(dst + n), "f"(v[0]), "f"(v[1]), "f"(v[2]), "f"(v[3]) : "memory");
+        asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(dst + n + 4), "f"(v[4]), "f"(v[5]), "f"(v[6]), "f"(v[7]) : "memory");
+      }
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive_cluster(mapa_u32(tempty + buf, 0));
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  cluster_sync_all();
+  if (warp == 1) { tc_fence_after(); tmem2_dealloc(tmem_base, 512); }
+}
+
+// =============================================================================================================
+// host side
+// =============================================================================================================
+bool tc2_supported(int H) {
+  static int disabled = -1;
+  if (disabled < 0) { const char* e = getenv("PIGAN_NO_CTA_PAIRS"); disabled = (e && e[0] == '1') ? 1 : 0; }
+  return !disabled && H % 256 == 0;
+}
+
+template <typename T, int C, int MODE>
+static void launch_jet2(Launcher& L, const CUtensorMap& a, const CUtensorMap& b, const CUtensorMap& o, const CUtensorMap& t,
+                        const Jet2Params& p) {
+  using Cfg = Jet2Cfg<C, MODE>;
+  static bool attr_set = false;
+  auto kern = jet2_layer_kernel<T, C, MODE>;
+  if (!attr_set) { cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::kSmemBytes); attr_set = true; }
+  const int tiles = (p.H / 256) * p.n_row_tiles;
+  const int clusters = std::min(tiles, num_sms() / 2);
+  kern<<<2 * clusters, k2Threads, Cfg::kSmemBytes, L.stream>>>(a, b, o, t, p);
+  L.check(MODE == 0 ? "jet_layer_fwd" : MODE == 1 ? "jet_layer_bwd" : "jet_layer_fwd_split");
+}
+
+template <int MODE>
+static void dispatch_jet2(Launcher& L, int C, const CUtensorMap& a, const CUtensorMap& b, const CUtensorMap& o, const CUtensorMap& t,
+                          const Jet2Params& p) {
+  if (C == 1) launch_jet2<__half, 1, MODE>(L, a, b, o, t, p);
+  else if (C == 3) launch_jet2<__half, 3, MODE>(L, a, b, o, t, p);
+  else launch_jet2<__half, 5, MODE>(L, a, b, o, t, p);
+}
+
+void tc2_layer_fwd(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* w16_l, const float* bias, const void* h_in, void* h_out) {
+  CUtensorMap a, b, o;
+  bool ok = weight_map(L, &a, precision, w16_l, H) && plane_map(L, &b, precision, h_in, H, R_ld, C, 32, 64, C, CU_TENSOR_MAP_SWIZZLE_64B) &&
+            plane_map(L, &o, precision, h_out, H, R_ld, C, 32, 32, 1, CU_TENSOR_MAP_SWIZZLE_64B);
+  if (!ok) return;
+  Jet2Params p{};
+  p.H = H; p.n_row_tiles = R / 64; p.bias = bias;
+  dispatch_jet2<0>(L, C, a, b, o, o, p);
+}
+
+void tc2_layer_fwd_split(Launcher& L, int precision, int H, int R, int R_ld, const void* w16_l, const float* bias, const void* h_in, void* h_out) {
+  CUtensorMap a, b, o;
+  if (!(weight_map(L, &a, precision, w16_l, H) && plane_map(L, &b, precision, h_in, H, R_ld, 2, 32, 64, 2, CU_TENSOR_MAP_SWIZZLE_64B) &&
+        plane_map(L, &o, precision, h_out, H, R_ld, 2, 32, 32, 1, CU_TENSOR_MAP_SWIZZLE_64B)))
+    return;
+  Jet2Params p{};
+  p.H = H; p.n_row_tiles = R / 64; p.bias = bias;
+  launch_jet2<__half, 2, 2>(L, a, b, o, o, p);
+}
+
+void tc2_layer_bwd(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* w16T_l, const void* ahat_in, const void* h_prev,
+                   void* ahat_out, float* g_bias_prev, const float* amax) {
+  CUtensorMap a, b, o, t;
+  bool ok = weight_map(L, &a, precision, w16T_l, H) && plane_map(L, &b, precision, ahat_in, H, R_ld, C, 32, 64, C, CU_TENSOR_MAP_SWIZZLE_64B) &&
+            plane_map(L, &o, precision, ahat_out, H, R_ld, C, 32, 32, 1, CU_TENSOR_MAP_SWIZZLE_64B) &&
+            plane_map(L, &t, precision, h_prev, H, R_ld, C, 32, 32, 1, CU_TENSOR_MAP_SWIZZLE_64B);
+  if (!ok) return;
+  Jet2Params p{};
+  p.H = H; p.n_row_tiles = R / 64; p.g_bias = g_bias_prev; p.amax = amax;
+  dispatch_jet2<1>(L, C, a, b, o, t, p);
+}
+
+void tc2_wgrad(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* ahat, const void* h_prev, float* gW, const float* amax) {
+  Wgrad2Params p{};
+  p.H = H; p.C = C; p.R = R; p.gW = gW; p.amax = amax;
+  const int n_tiles = (H / 256) * (H / 256);
+  const int n_cl = num_sms() / 2;
+  int slices = std::max(1, (2 * n_cl) / n_tiles);
+  int slice_rows = ((R + slices - 1) / slices + 63) / 64 * 64;
+  if (slice_rows < 64) slice_rows = 64;
+  p.slice_rows = slice_rows; p.n_slices = (R + slice_rows - 1) / slice_rows;
+  CUtensorMap a, b;
+  if (!(plane_map(L, &a, precision, ahat, H, R_ld, C, 64, 128, 1, CU_TENSOR_MAP_SWIZZLE_128B) &&
+        plane_map(L, &b, precision, h_prev, H, R_ld, C, 64, 128, 1, CU_TENSOR_MAP_SWIZZLE_128B)))
+    return;
+  const int smem = kW2Stages * kW2StageBytes + 1024 + 256;
+  static bool attr_set = false;
+  const int clusters = std::min(n_tiles * p.n_slices, n_cl);
+  if (!attr_set) { cudaFuncSetAttribute(wgrad2_kernel<__half>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); attr_set = true; }
+  wgrad2_kernel<__half><<<2 * clusters, 192, smem, L.stream>>>(a, b, p);
+  L.check("wgrad");
+}
+
+}  // namespace pigan

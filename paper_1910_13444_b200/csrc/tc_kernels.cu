@@ -8,141 +8,9 @@
 //   An epilogue thread owns one unit (TMEM lane) and sees all C channels of a (row, unit) pair, so the chain rule
 //   is thread-local; its outputs are contiguous along rows and leave through swizzled smem + TMA stores.
 // wgrad: D[out unit][in unit] += sum_{c,row} ahat_c[out][row] h_c[in][row]; both operands K-major (rows contiguous).
-#include <cuda.h>
-
-#include "common.cuh"
+#include "tc_ptx.cuh"
 
 namespace pigan {
-
-// =============================================================================================================
-// PTX wrappers
-// =============================================================================================================
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-
-__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
-  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
-  uint32_t ok;
-  asm volatile(
-      "{\n\t.reg .pred p;\n\t"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
-      "selp.u32 %0, 1, 0, p;\n\t}"
-      : "=r"(ok)
-      : "r"(smem_u32(bar)), "r"(parity)
-      : "memory");
-  return ok != 0;
-}
-// Bounded wait: a protocol bug traps (surfacing as a CUDA error) instead of hanging the GPU.
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
-  uint32_t spins = 0;
-  while (!mbar_try_wait(bar, parity)) {
-    if (++spins > (1u << 26)) { printf("pigan: mbarrier wait timed out (block %d thread %d)\n", (int)blockIdx.x, (int)threadIdx.x); __trap(); }
-  }
-}
-__device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
-__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
-
-__device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* map, uint64_t* bar, int c0, int c1) {
-  asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];" ::"r"(smem_u32(dst)),
-               "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1)
-               : "memory");
-}
-__device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, uint64_t* bar, int c0, int c1, int c2) {
-  asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];" ::"r"(smem_u32(dst)),
-               "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2)
-               : "memory");
-}
-__device__ __forceinline__ void tma_store_3d(const CUtensorMap* map, const void* src, int c0, int c1, int c2) {
-  asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.bulk_group [%0, {%2, %3, %4}], [%1];" ::"l"(map), "r"(smem_u32(src)), "r"(c0),
-               "r"(c1), "r"(c2)
-               : "memory");
-}
-__device__ __forceinline__ void tma_commit_group() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
-__device__ __forceinline__ void tma_wait_read_all() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
-__device__ __forceinline__ void tma_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
-__device__ __forceinline__ void prefetch_tmap(const CUtensorMap* map) { asm volatile("prefetch.tensormap [%0];" ::"l"(map) : "memory"); }
-
-__device__ __forceinline__ void tmem_alloc(uint32_t* dst_smem, uint32_t ncols) {
-  asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(dst_smem)), "r"(ncols) : "memory");
-  asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
-}
-__device__ __forceinline__ void tmem_dealloc(uint32_t taddr, uint32_t ncols) {
-  asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(ncols) : "memory");
-}
-__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
-__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
-__device__ __forceinline__ void tc_commit(uint64_t* bar) {
-  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-// D[tmem] (+)= A[smem] . B[smem], kind::f16 (bf16 / fp16 operands, fp32 accumulate)
-__device__ __forceinline__ void tc_mma(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
-  asm volatile(
-      "{\n\t.reg .pred p;\n\t"
-      "setp.ne.b32 p, %4, 0;\n\t"
-      "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}" ::"r"(d_tmem),
-      "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
-      : "memory");
-}
-__device__ __forceinline__ void tmem_ld8(uint32_t taddr, float* v) {
-  uint32_t r[8];
-  asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
-               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
-               : "r"(taddr));
-#pragma unroll
-  for (int i = 0; i < 8; ++i) v[i] = __uint_as_float(r[i]);
-}
-__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
-
-// ---- UMMA descriptors (field layout as documented in CUTLASS cute/arch/mma_sm100_desc.hpp) ---------------------
-// smem matrix descriptor: [0,14) start>>4, [16,30) leading byte offset>>4, [32,46) stride byte offset>>4,
-// [46,48) version = 1, [61,64) layout (2 = SWIZZLE_128B).
-__device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
-  return (uint64_t)((saddr >> 4) & 0x3FFF) | ((uint64_t)((lbo_bytes >> 4) & 0x3FFF) << 16) | ((uint64_t)((sbo_bytes >> 4) & 0x3FFF) << 32) |
-         (1ull << 46) | (2ull << 61);
-}
-// instruction descriptor: [4,6) D fmt (1 = f32), [7,10) A fmt, [10,13) B fmt (0 = f16, 1 = bf16), bit 15 A major,
-// bit 16 B major (0 = K, 1 = MN), [17,23) N>>3, [24,29) M>>4.
-__host__ __device__ constexpr uint32_t umma_idesc(int fmt16, int a_mn, int b_mn, int M, int N) {
-  return (1u << 4) | ((uint32_t)fmt16 << 7) | ((uint32_t)fmt16 << 10) | ((uint32_t)a_mn << 15) | ((uint32_t)b_mn << 16) | ((uint32_t)(N >> 3) << 17) |
-         ((uint32_t)(M >> 4) << 24);
-}
-
-template <typename T> struct Fmt;
-template <> struct Fmt<__nv_bfloat16> { static constexpr int umma = 1; };
-template <> struct Fmt<__half> { static constexpr int umma = 0; };
-
-__device__ __forceinline__ float fast_tanh(float x) {
-  float y;
-  asm("tanh.approx.f32 %0, %1;" : "=f"(y) : "f"(x));
-  return y;
-}
-template <typename T> __device__ __forceinline__ uint32_t pack2(float a, float b);
-template <> __device__ __forceinline__ uint32_t pack2<__nv_bfloat16>(float a, float b) {
-  __nv_bfloat162 v = __floats2bfloat162_rn(a, b);
-  return *reinterpret_cast<uint32_t*>(&v);
-}
-template <> __device__ __forceinline__ uint32_t pack2<__half>(float a, float b) {
-  __half2 v = __floats2half2_rn(a, b);
-  return *reinterpret_cast<uint32_t*>(&v);
-}
-template <typename T> __device__ __forceinline__ float2 unpack2(uint32_t u);
-template <> __device__ __forceinline__ float2 unpack2<__nv_bfloat16>(uint32_t u) { return __bfloat1622float2(*reinterpret_cast<__nv_bfloat162*>(&u)); }
-template <> __device__ __forceinline__ float2 unpack2<__half>(uint32_t u) { return __half22float2(*reinterpret_cast<__half2*>(&u)); }
-
-template <typename T> __device__ __forceinline__ uint4 pack8(const float* v) {
-  return make_uint4(pack2<T>(v[0], v[1]), pack2<T>(v[2], v[3]), pack2<T>(v[4], v[5]), pack2<T>(v[6], v[7]));
-}
-template <typename T> __device__ __forceinline__ void unpack8(uint4 u, float* v) {
-  float2 a = unpack2<T>(u.x), b = unpack2<T>(u.y), c = unpack2<T>(u.z), d = unpack2<T>(u.w);
-  v[0] = a.x; v[1] = a.y; v[2] = b.x; v[3] = b.y; v[4] = c.x; v[5] = c.y; v[6] = d.x; v[7] = d.y;
-}
 
 // =============================================================================================================
 // jet layer kernel: forward (MODE 0) and dgrad + adjoint (MODE 1)
@@ -167,10 +35,7 @@ template <int C> struct JetCfg {
 struct JetParams {
   int H;                 // width (K and number of output units)
   int n_row_tiles;       // R / 64
-  int has_stash;         // MODE 1: 0 = previous layer is layer 1 (analytic a_x, a_y; a_xx = a_yy = 0)
-  int in_dim;            // MODE 1, layer 1: leading dimension of W1
   const float* bias;     // MODE 0: b_l
-  const float* W1;       // MODE 1, layer 1
   float* g_bias;         // MODE 1: b_hat_{l-1}
   const float* amax;     // MODE 1: block-scale source of the adjoint planes (common.cuh adj_inv_scale)
 };
@@ -179,8 +44,7 @@ template <typename T, int C, int MODE>
 __global__ void __launch_bounds__(256, 1) jet_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H] 16-bit, box 64 x 128, SW128
                                                            const __grid_constant__ CUtensorMap tmB,      // input planes, box 64 rows x 64 units x C, SW128
                                                            const __grid_constant__ CUtensorMap tmO,      // MODE 0: h_out; MODE 1: ahat_out (box 32 x 32 x 1, SW64)
-                                                           const __grid_constant__ CUtensorMap tmS,      // MODE 0: stash out; MODE 1: stash_prev in
-                                                           const __grid_constant__ CUtensorMap tmT,      // MODE 1: h_prev (plane 0 = t) in
+                                                           const __grid_constant__ CUtensorMap tmT,      // MODE 1: h_prev planes in
                                                            JetParams p) {
   using Cfg = JetCfg<C>;
   extern __shared__ uint8_t smem_raw[];
@@ -202,7 +66,6 @@ __global__ void __launch_bounds__(256, 1) jet_layer_kernel(const __grid_constant
 
   if (warp == 0 && lane == 0) {
     prefetch_tmap(&tmA); prefetch_tmap(&tmB); prefetch_tmap(&tmO);
-    if ((C > 1 && MODE == 0) || MODE == 1) prefetch_tmap(&tmS);
     if (MODE == 1) prefetch_tmap(&tmT);
   }
   if (warp == 1 && lane == 0) {
@@ -279,17 +142,14 @@ __global__ void __launch_bounds__(256, 1) jet_layer_kernel(const __grid_constant
       const uint32_t bphase = (it / Cfg::kNumBuf) & 1;
       const int unit0 = ut * kBM + q * 32, unit = unit0 + lane;
       const uint32_t tbase = tmem_base + ((uint32_t)(q * 32) << 16) + buf * Cfg::kCols;
-      float bias = 0.f, ad1[4] = {0.f, 0.f, 0.f, 0.f}, bias_acc = 0.f;
+      float bias = 0.f, bias_acc = 0.f;
       if (MODE == 0 || MODE == 2) bias = p.bias[unit];
-      if (MODE == 1 && !p.has_stash && C >= 3) { ad1[0] = p.W1[(size_t)unit * p.in_dim]; ad1[1] = p.W1[(size_t)unit * p.in_dim + 1]; }
-      const int n_in = p.has_stash ? C : 1;                  // MODE 1: planes to load per half tile (t, then stash)
 
-      auto issue_stage_loads = [&](int hf) {                 // MODE 1: t and stash of the previous layer -> staging
+      auto issue_stage_loads = [&](int hf) {                 // MODE 1: the previous layer's output jet h^{l-1} -> staging
         if (lane == 0) {
           tma_wait_read_all();                               // earlier stores have finished reading the staging buffer
-          mbar_expect_tx(sbar + q, n_in * kStgPlane);
-          tma_load_3d(stg, &tmT, sbar + q, rt * kRT + hf * 32, unit0, 0);
-          for (int c = 1; c < n_in; ++c) tma_load_3d(stg + c * kStgPlane, &tmS, sbar + q, rt * kRT + hf * 32, unit0, c - 1);
+          mbar_expect_tx(sbar + q, C * kStgPlane);
+          for (int c = 0; c < C; ++c) tma_load_3d(stg + c * kStgPlane, &tmT, sbar + q, rt * kRT + hf * 32, unit0, c);
         }
       };
       if (MODE == 1) issue_stage_loads(0);
@@ -299,7 +159,7 @@ __global__ void __launch_bounds__(256, 1) jet_layer_kernel(const __grid_constant
 #pragma unroll 1
       for (int hf = 0; hf < 2; ++hf) {
         if (MODE == 0) {
-          // ---- pass A: h_c = tanh-jet(a_c) ----
+          // ---- h_c = tanh-jet(a_c) ----
           if (lane == 0) tma_wait_read_all();
           __syncwarp();
 #pragma unroll 1
@@ -327,27 +187,6 @@ __global__ void __launch_bounds__(256, 1) jet_layer_kernel(const __grid_constant
           if (lane == 0) {
             for (int c = 0; c < C; ++c) tma_store_3d(&tmO, stg + c * kStgPlane, rt * kRT + hf * 32, unit0, c);
             tma_commit_group();
-          }
-          // ---- pass B: stash a_x, a_y, a_xx, a_yy (raw accumulators) ----
-          if (C > 1) {
-            if (lane == 0) tma_wait_read_all();
-            __syncwarp();
-#pragma unroll 1
-            for (int rc = 0; rc < 4; ++rc) {
-              float v[C][8];
-#pragma unroll
-              for (int c = 1; c < C; ++c) tmem_ld8(tbase + c * kRT + hf * 32 + rc * 8, v[c]);
-              tmem_ld_wait();
-              const uint32_t off = ((uint32_t)rc ^ swz) << 4;
-#pragma unroll
-              for (int c = 1; c < C; ++c) *reinterpret_cast<uint4*>(my_row + (c - 1) * kStgPlane + off) = pack8<T>(v[c]);
-            }
-            fence_proxy_async();
-            __syncwarp();
-            if (lane == 0) {
-              for (int c = 1; c < C; ++c) tma_store_3d(&tmS, stg + (c - 1) * kStgPlane, rt * kRT + hf * 32, unit0, c - 1);
-              tma_commit_group();
-            }
           }
         } else if (MODE == 2) {
           // ---- value-only layer with split activations: a = W (h_hi + h_lo) + b; t = tanh a; t_hi = rn16(t), t_lo = rn16(t - t_hi) ----
@@ -383,24 +222,19 @@ __global__ void __launch_bounds__(256, 1) jet_layer_kernel(const __grid_constant
           mbar_wait(sbar + q, sphase); sphase ^= 1;
 #pragma unroll 1
           for (int rc = 0; rc < 4; ++rc) {
-            float hh[C][8], tv[8], sv[4][8], o[C][8];
+            float hh[C][8], hp[C][8], o[C][8];
 #pragma unroll
             for (int c = 0; c < C; ++c) tmem_ld8(tbase + c * kRT + hf * 32 + rc * 8, hh[c]);
             const uint32_t off = ((uint32_t)rc ^ swz) << 4;
-            unpack8<T>(*reinterpret_cast<const uint4*>(my_row + off), tv);
-            if (p.has_stash) {
 #pragma unroll
-              for (int c = 1; c < C; ++c) unpack8<T>(*reinterpret_cast<const uint4*>(my_row + c * kStgPlane + off), sv[c - 1]);
-            }
+            for (int c = 0; c < C; ++c) unpack8<T>(*reinterpret_cast<const uint4*>(my_row + c * kStgPlane + off), hp[c]);
             tmem_ld_wait();
 #pragma unroll
             for (int i = 0; i < 8; ++i) {
-              float hx[5], ad[4], aa[5];
+              float hx[5], hj[5], aa[5];
 #pragma unroll
-              for (int c = 0; c < C; ++c) hx[c] = hh[c][i];
-#pragma unroll
-              for (int c = 0; c < C - 1; ++c) ad[c] = p.has_stash ? sv[c][i] : ad1[c];
-              jet_act_bwd<C>(tv[i], ad, hx, aa);
+              for (int c = 0; c < C; ++c) { hx[c] = hh[c][i]; hj[c] = hp[c][i]; }
+              jet_act_bwd<C>(hj, hx, aa);
               bias_acc += aa[0];
 #pragma unroll
               for (int c = 0; c < C; ++c) o[c][i] = aa[c];
@@ -586,55 +420,8 @@ bool tc_supported(int H, std::string* why) {
   return true;
 }
 
-typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
-                                  const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-static EncodeTiledFn get_encode() {
-  static EncodeTiledFn fn = nullptr;
-  if (!fn) {
-    void* p = nullptr;
-    cudaDriverEntryPointQueryResult qres;
-    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) == cudaSuccess && qres == cudaDriverEntryPointSuccess)
-      fn = (EncodeTiledFn)p;
-  }
-  return fn;
-}
-
-static bool make_map(Launcher& L, CUtensorMap* m, int precision, const void* base, int rank, const cuuint64_t* dims, const cuuint64_t* strides_bytes,
-                     const cuuint32_t* box, CUtensorMapSwizzle swz) {
-  EncodeTiledFn fn = get_encode();
-  cuuint32_t estr[3] = {1, 1, 1};
-  (void)precision;
-  const CUtensorMapDataType dt = CU_TENSOR_MAP_DATA_TYPE_FLOAT16;
-  if (!fn || fn(m, dt, rank, const_cast<void*>(base), dims, strides_bytes, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, swz,
-                CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS) {
-    if (L.err == cudaSuccess) { L.err = cudaErrorInvalidValue; L.where = "cuTensorMapEncodeTiled"; }
-    return false;
-  }
-  return true;
-}
-// planes [C][H][R_ld] viewed as a 3D tensor (rows, units, channels)
-static bool plane_map(Launcher& L, CUtensorMap* m, int precision, const void* base, int H, int R_ld, int nch, int box_rows, int box_units, int box_ch,
-                      CUtensorMapSwizzle swz) {
-  cuuint64_t dims[3] = {(cuuint64_t)R_ld, (cuuint64_t)H, (cuuint64_t)nch};
-  cuuint64_t str[2] = {(cuuint64_t)R_ld * 2, (cuuint64_t)R_ld * 2 * H};
-  cuuint32_t box[3] = {(cuuint32_t)box_rows, (cuuint32_t)box_units, (cuuint32_t)box_ch};
-  return make_map(L, m, precision, base, 3, dims, str, box, swz);
-}
-static bool weight_map(Launcher& L, CUtensorMap* m, int precision, const void* base, int H) {
-  cuuint64_t dims[2] = {(cuuint64_t)H, (cuuint64_t)H};
-  cuuint64_t str[1] = {(cuuint64_t)H * 2};
-  cuuint32_t box[2] = {(cuuint32_t)kBK, (cuuint32_t)kBM};
-  return make_map(L, m, precision, base, 2, dims, str, box, CU_TENSOR_MAP_SWIZZLE_128B);
-}
-
-static int num_sms() {
-  static int n = 0;
-  if (!n) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev); if (n <= 0) n = 148; }
-  return n;
-}
-
 template <typename T, int C, int MODE>
-static void launch_jet(Launcher& L, const CUtensorMap& a, const CUtensorMap& b, const CUtensorMap& o, const CUtensorMap& s, const CUtensorMap& t,
+static void launch_jet(Launcher& L, const CUtensorMap& a, const CUtensorMap& b, const CUtensorMap& o, const CUtensorMap& t,
                        const JetParams& p) {
   using Cfg = JetCfg<C>;
   static bool attr_set = false;
@@ -642,63 +429,64 @@ static void launch_jet(Launcher& L, const CUtensorMap& a, const CUtensorMap& b, 
   if (!attr_set) { cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::kSmemBytes); attr_set = true; }
   const int tiles = (p.H / kBM) * p.n_row_tiles;
   const int grid = std::min(tiles, num_sms());
-  kern<<<grid, 256, Cfg::kSmemBytes, L.stream>>>(a, b, o, s, t, p);
+  kern<<<grid, 256, Cfg::kSmemBytes, L.stream>>>(a, b, o, t, p);
   L.check(MODE == 0 ? "jet_layer_fwd" : MODE == 1 ? "jet_layer_bwd" : "jet_layer_fwd_split");
 }
 
 template <int MODE>
-static void dispatch_jet(Launcher& L, int precision, int C, const CUtensorMap& a, const CUtensorMap& b, const CUtensorMap& o, const CUtensorMap& s,
+static void dispatch_jet(Launcher& L, int precision, int C, const CUtensorMap& a, const CUtensorMap& b, const CUtensorMap& o,
                          const CUtensorMap& t, const JetParams& p) {
 #define PIGAN_JET(TT)                                                  \
-  if (C == 1) launch_jet<TT, 1, MODE>(L, a, b, o, s, t, p);            \
-  else if (C == 3) launch_jet<TT, 3, MODE>(L, a, b, o, s, t, p);       \
-  else launch_jet<TT, 5, MODE>(L, a, b, o, s, t, p)
+  if (C == 1) launch_jet<TT, 1, MODE>(L, a, b, o, t, p);            \
+  else if (C == 3) launch_jet<TT, 3, MODE>(L, a, b, o, t, p);       \
+  else launch_jet<TT, 5, MODE>(L, a, b, o, t, p)
   (void)precision;                                          // both 16-bit modes compute with fp16 operands
   PIGAN_JET(__half);
 #undef PIGAN_JET
 }
 
-void tc_layer_fwd(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* w16_l, const float* bias, const void* h_in, void* h_out,
-                  void* stash) {
+void tc_layer_fwd(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* w16_l, const float* bias, const void* h_in, void* h_out) {
   if (R <= 0) return;
-  CUtensorMap a, b, o, s;
+  if (tc2_supported(H)) { tc2_layer_fwd(L, precision, C, H, R, R_ld, w16_l, bias, h_in, h_out); return; }
+  CUtensorMap a, b, o;
   bool ok = weight_map(L, &a, precision, w16_l, H) && plane_map(L, &b, precision, h_in, H, R_ld, C, kRT, kBK, C, CU_TENSOR_MAP_SWIZZLE_128B) &&
             plane_map(L, &o, precision, h_out, H, R_ld, C, 32, 32, 1, CU_TENSOR_MAP_SWIZZLE_64B);
-  if (C > 1) ok = ok && plane_map(L, &s, precision, stash, H, R_ld, C - 1, 32, 32, 1, CU_TENSOR_MAP_SWIZZLE_64B); else s = o;
   if (!ok) return;
   JetParams p{};
   p.H = H; p.n_row_tiles = R / kRT; p.bias = bias;
-  dispatch_jet<0>(L, precision, C, a, b, o, s, o, p);
+  dispatch_jet<0>(L, precision, C, a, b, o, o, p);
 }
 
 // value-only layer on split activations (2 planes: hi, lo) -> 2 planes; used where the snapshot X_fake is built
 void tc_layer_fwd_split(Launcher& L, int precision, int H, int R, int R_ld, const void* w16_l, const float* bias, const void* h_in, void* h_out) {
   if (R <= 0) return;
+  if (tc2_supported(H)) { tc2_layer_fwd_split(L, precision, H, R, R_ld, w16_l, bias, h_in, h_out); return; }
   CUtensorMap a, b, o;
   if (!(weight_map(L, &a, precision, w16_l, H) && plane_map(L, &b, precision, h_in, H, R_ld, 2, kRT, kBK, 2, CU_TENSOR_MAP_SWIZZLE_128B) &&
         plane_map(L, &o, precision, h_out, H, R_ld, 2, 32, 32, 1, CU_TENSOR_MAP_SWIZZLE_64B)))
     return;
   JetParams p{};
   p.H = H; p.n_row_tiles = R / kRT; p.bias = bias;
-  launch_jet<__half, 2, 2>(L, a, b, o, o, o, p);
+  launch_jet<__half, 2, 2>(L, a, b, o, o, p);
 }
 
 void tc_layer_bwd(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* w16T_l, const void* ahat_in, const void* h_prev,
-                  const void* stash_prev, const float* W1, int in_dim, void* ahat_out, float* g_bias_prev, const float* amax) {
+                  void* ahat_out, float* g_bias_prev, const float* amax) {
   if (R <= 0) return;
-  CUtensorMap a, b, o, s, t;
+  if (tc2_supported(H)) { tc2_layer_bwd(L, precision, C, H, R, R_ld, w16T_l, ahat_in, h_prev, ahat_out, g_bias_prev, amax); return; }
+  CUtensorMap a, b, o, t;
   bool ok = weight_map(L, &a, precision, w16T_l, H) && plane_map(L, &b, precision, ahat_in, H, R_ld, C, kRT, kBK, C, CU_TENSOR_MAP_SWIZZLE_128B) &&
             plane_map(L, &o, precision, ahat_out, H, R_ld, C, 32, 32, 1, CU_TENSOR_MAP_SWIZZLE_64B) &&
-            plane_map(L, &t, precision, h_prev, H, R_ld, 1, 32, 32, 1, CU_TENSOR_MAP_SWIZZLE_64B);
-  if (stash_prev && C > 1) ok = ok && plane_map(L, &s, precision, stash_prev, H, R_ld, C - 1, 32, 32, 1, CU_TENSOR_MAP_SWIZZLE_64B); else s = t;
+            plane_map(L, &t, precision, h_prev, H, R_ld, C, 32, 32, 1, CU_TENSOR_MAP_SWIZZLE_64B);
   if (!ok) return;
   JetParams p{};
-  p.H = H; p.n_row_tiles = R / kRT; p.has_stash = (stash_prev && C > 1) ? 1 : 0; p.in_dim = in_dim; p.W1 = W1; p.g_bias = g_bias_prev; p.amax = amax;
-  dispatch_jet<1>(L, precision, C, a, b, o, s, t, p);
+  p.H = H; p.n_row_tiles = R / kRT; p.g_bias = g_bias_prev; p.amax = amax;
+  dispatch_jet<1>(L, precision, C, a, b, o, t, p);
 }
 
 void tc_wgrad(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* ahat, const void* h_prev, float* gW, const float* amax) {
   if (R <= 0) return;
+  if (tc2_supported(H)) { tc2_wgrad(L, precision, C, H, R, R_ld, ahat, h_prev, gW, amax); return; }
   WgradParams p{};
   p.H = H; p.C = C; p.NW = std::min(H, 256); p.R = R; p.gW = gW; p.amax = amax;
   const int n_tiles = (H / kBM) * (H / p.NW);
