@@ -73,7 +73,7 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
 #ifdef PIGAN_PROBE_TRACE
   __shared__ long long tr_wait[16], tr_issue[16], tr_prod[16], tr_prod0[16];
 #endif
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int warp = uniform_warp_idx(), lane = threadIdx.x & 31;
   const uint32_t rank = cluster_ctarank();
   const int cluster_id = blockIdx.x >> 1, n_clusters = gridDim.x >> 1;
   const int n_ut = p.H / 256;
@@ -95,7 +95,7 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
   __syncthreads();
   cluster_sync_all();                                      // the peer's barriers are initialised before anything signals them
   tc_fence_after();
-  const uint32_t tmem_base = *tmem_slot;
+  const uint32_t tmem_base = __shfl_sync(0xffffffffu, *tmem_slot, 0);       // uniform: TMEM addresses live in uniform registers
 
   // accumulator columns: tile `it` of this cluster; channel group 0 = channels [0, min(C, 3)), group 1 = (xx, yy)
   auto g0_col = [&](int it) -> uint32_t { return C == 5 ? ((it & 1) ? 320u : 0u) : (uint32_t)((it % Cfg::kNumBuf) * Cfg::kCols); };
@@ -103,8 +103,8 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
   constexpr int nc0 = C == 5 ? 3 : C;                      // channels in group 0
 
   if (warp == 0) {
-    // ===================== TMA producer (both CTAs) =====================
-    if (lane == 0) {
+    // ===================== TMA producer (both CTAs; the warp stays converged, one elected lane issues) =====================
+    {
       int stage = 0; uint32_t phase = 0;
       for (int t = cluster_id; t < n_tiles; t += n_clusters) {
         const int ut = t % n_ut, rt = t / n_ut;
@@ -122,20 +122,23 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
           uint8_t* sA = stages + stage * Cfg::kStageBytes;
           const uint32_t lbar = mapa_u32(full + stage, 0);
 #ifdef PIGAN_PROBE_NOLOAD
-          if (rank == 0) mbar_arrive(full + stage);
+          if (rank == 0 && elect_one()) mbar_arrive(full + stage);
           (void)sA; (void)lbar;
 #else
-          if (rank == 0) mbar_expect_tx(full + stage, 2 * Cfg::kStageBytes);
-          tma2_load_2d(sA, &tmA, lbar, kb * 64, ut * 256 + (int)rank * 128);
-          tma2_load_3d(sA + k2AStage, &tmB, lbar, rt * 64 + (int)rank * 32, kb * 64, 0);
+          if (elect_one()) {
+            if (rank == 0) mbar_expect_tx(full + stage, 2 * Cfg::kStageBytes);
+            tma2_load_2d(sA, &tmA, lbar, kb * 64, ut * 256 + (int)rank * 128);
+            tma2_load_3d(sA + k2AStage, &tmB, lbar, rt * 64 + (int)rank * 32, kb * 64, 0);
+          }
+          __syncwarp();
 #endif
           if (++stage == Cfg::kNumStages) { stage = 0; phase ^= 1; }
         }
       }
     }
   } else if (warp == 1) {
-    // ===================== MMA issuer (one thread of the leader CTA) =====================
-    if (rank == 0 && lane == 0) {
+    // ===================== MMA issuer (leader CTA; converged warp, one elected lane issues) =====================
+    if (rank == 0) {
       // tcgen05.mma issue returns when the MMA starts executing (the queue is about one deep), so a barrier wait
       // issued after the last MMA of a stage idles the tensor pipe for its whole latency.  The wait for the NEXT
       // stage is therefore polled behind the longest MMA of the last k-step, and only repeated (blocking) on a miss.
@@ -182,26 +185,24 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
             const uint32_t acc = (kb | k) ? 1u : 0u;
             // MN-major SW64: channel planes are 4 KB apart (LBO), 8-unit groups 512 B apart (SBO), 16 units = +1 KB
 #ifndef PIGAN_PROBE_NOMMA
-            if (C == 5 && k < 3) tc2_mma(d1, ad, umma_desc_sw64(sB + 3 * k2BPlane + k * 1024, k2BPlane, 512), idesc1, acc);
-            if (C != 5 && k == 3) ready = !(last_tile && kb == n_kb - 1) && LOOKAHEAD(full + nstage, nphase);
-            tc2_mma(d0, ad, umma_desc_sw64(sB + k * 1024, k2BPlane, 512), idesc0, acc);
+            if (C == 5 && k < 3 && elect_one()) tc2_mma(d1, ad, umma_desc_sw64(sB + 3 * k2BPlane + k * 1024, k2BPlane, 512), idesc1, acc);
+            if (C != 5 && k == 3) ready = !(last_tile && kb == n_kb - 1) && __all_sync(0xffffffffu, LOOKAHEAD(full + nstage, nphase));
+            if (elect_one()) tc2_mma(d0, ad, umma_desc_sw64(sB + k * 1024, k2BPlane, 512), idesc0, acc);
             if (C == 5 && k == 3) {
-              ready = !(last_tile && kb == n_kb - 1) && LOOKAHEAD(full + nstage, nphase);
-              tc2_mma(d1, ad, umma_desc_sw64(sB + 3 * k2BPlane + k * 1024, k2BPlane, 512), idesc1, acc);
+              ready = !(last_tile && kb == n_kb - 1) && __all_sync(0xffffffffu, LOOKAHEAD(full + nstage, nphase));
+              if (elect_one()) tc2_mma(d1, ad, umma_desc_sw64(sB + 3 * k2BPlane + k * 1024, k2BPlane, 512), idesc1, acc);
             }
 #endif
           }
-#ifdef PIGAN_PROBE_COMMIT1
-          tc_commit(empty + stage);
-#elif !defined(PIGAN_PROBE_NOCOMMIT)
-          tc2_commit(empty + stage);                         // frees the smem slot in both CTAs when these MMAs retire
-#endif
+          if (elect_one()) tc2_commit(empty + stage);        // frees the smem slot in both CTAs when these MMAs retire
+          __syncwarp();
 #ifdef PIGAN_PROBE_TRACE
           if (cluster_id == 0 && it == 10) tr_issue[kb] = clock64();
 #endif
           stage = nstage; phase = nphase;
         }
-        tc2_commit(tfull + buf);                             // accumulator complete (both CTAs)
+        if (elect_one()) tc2_commit(tfull + buf);            // accumulator complete (both CTAs)
+        __syncwarp();
       }
 #ifdef PIGAN_PROBE_TRACE
       if (cluster_id == 0 && C == 5 && MODE == 0 && n_tiles > 11 * n_clusters) {
@@ -211,7 +212,7 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
       }
 #endif
 #ifdef PIGAN_PROBE_TIMING
-      if (cluster_id == 0) printf("TIMING mma C=%d MODE=%d tiles=%d total=%lld wait_tempty=%lld wait_full=%lld\n", C, MODE, it, clock64() - tm_start, tm_te, tm_full);
+      if (cluster_id == 0 && lane == 0) printf("TIMING mma C=%d MODE=%d tiles=%d total=%lld wait_tempty=%lld wait_full=%lld\n", C, MODE, it, clock64() - tm_start, tm_te, tm_full);
 #endif
     }
   } else if (warp >= 4) {
@@ -243,7 +244,7 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
         if (lane == 0) mbar_arrive_cluster(mapa_u32(tempty + buf, 0));
       };
 
-      if (MODE == 1 && lane == 0) {                          // the previous layer's output jet h^{l-1} -> staging
+      if (MODE == 1 && elect_one()) {                        // the previous layer's output jet h^{l-1} -> staging
         tma_wait_read_all();                                 // earlier stores have finished reading the staging buffer
         mbar_expect_tx(sbar + e, C * k2StgPlane);
         for (int c = 0; c < C; ++c) tma_load_3d(stg + c * k2StgPlane, &tmT, sbar + e, row0, unit0, c);
@@ -276,7 +277,7 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
 
       if (MODE == 0) {
         // ---- h_c = tanh-jet(a_c) ----
-        if (lane == 0) tma_wait_read_all();
+        if (elect_one()) tma_wait_read_all();
         __syncwarp();
 #pragma unroll
         for (int rc = 0; rc < 4; ++rc) {
@@ -302,13 +303,13 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
         if (C != 5) release();
         fence_proxy_async();
         __syncwarp();
-        if (lane == 0) {
+        if (elect_one()) {
           for (int c = 0; c < C; ++c) tma_store_3d(&tmO, stg + c * k2StgPlane, row0, unit0, c);
           tma_commit_group();
         }
       } else if (MODE == 2) {
         // ---- value-only layer with split activations: a = W (h_hi + h_lo) + b; t = tanh a; t_hi = rn16(t), t_lo = rn16(t - t_hi) ----
-        if (lane == 0) tma_wait_read_all();
+        if (elect_one()) tma_wait_read_all();
         __syncwarp();
 #pragma unroll 1
         for (int rc = 0; rc < 4; ++rc) {
@@ -329,7 +330,7 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
         release();
         fence_proxy_async();
         __syncwarp();
-        if (lane == 0) {
+        if (elect_one()) {
           tma_store_3d(&tmO, stg, row0, unit0, 0);
           tma_store_3d(&tmO, stg + k2StgPlane, row0, unit0, 1);
           tma_commit_group();
@@ -365,7 +366,7 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
         if (C != 5) release();
         fence_proxy_async();
         __syncwarp();
-        if (lane == 0) {
+        if (elect_one()) {
           for (int c = 0; c < C; ++c) tma_store_3d(&tmO, stg + c * k2StgPlane, row0, unit0, c);
           tma_commit_group();
         }
@@ -375,7 +376,8 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
 #ifdef PIGAN_PROBE_TIMING
     if (blockIdx.x == 0 && e == 0 && lane == 0) printf("TIMING epi C=%d MODE=%d tiles=%d total=%lld wait_tfull=%lld early_release=%lld\n", C, MODE, it, clock64() - te_start, te_tf, te_rel);
 #endif
-    if (lane == 0) tma_wait_all();                           // global writes of the last stores are complete before exit
+    __syncwarp();
+    if (elect_one()) tma_wait_all();                         // global writes of the last stores are complete before exit
   }
   tc_fence_before();
   __syncthreads();
@@ -408,7 +410,7 @@ wgrad2_kernel(const __grid_constant__ CUtensorMap tmA,    // ahat planes, box 64
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem + kW2Stages * kW2StageBytes);
   uint64_t* full = bars; uint64_t* empty = bars + kW2Stages; uint64_t* tfull = empty + kW2Stages; uint64_t* tempty = tfull + 2;
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(tempty + 2);
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int warp = uniform_warp_idx(), lane = threadIdx.x & 31;
   const uint32_t rank = cluster_ctarank();
   const int cluster_id = blockIdx.x >> 1, n_clusters = gridDim.x >> 1;
   const int n_t = p.H / 256;
@@ -426,7 +428,7 @@ wgrad2_kernel(const __grid_constant__ CUtensorMap tmA,    // ahat planes, box 64
   __syncthreads();
   cluster_sync_all();
   tc_fence_after();
-  const uint32_t tmem_base = *tmem_slot;
+  const uint32_t tmem_base = __shfl_sync(0xffffffffu, *tmem_slot, 0);       // uniform: TMEM addresses live in uniform registers
 
   auto decode = [&](int w, int& mt, int& nt, int& r0, int& r1) {
     const int tile = w % (n_t * n_t), sl = w / (n_t * n_t);
@@ -435,7 +437,7 @@ wgrad2_kernel(const __grid_constant__ CUtensorMap tmA,    // ahat planes, box 64
   };
 
   if (warp == 0) {
-    if (lane == 0) {
+    {
       int stage = 0; uint32_t phase = 0;
       for (int w = cluster_id; w < n_items; w += n_clusters) {
         int mt, nt, r0, r1; decode(w, mt, nt, r0, r1);
@@ -444,15 +446,18 @@ wgrad2_kernel(const __grid_constant__ CUtensorMap tmA,    // ahat planes, box 64
             mbar_wait(empty + stage, phase ^ 1);
             uint8_t* sA = stages + stage * kW2StageBytes;
             const uint32_t lbar = mapa_u32(full + stage, 0);
-            if (rank == 0) mbar_expect_tx(full + stage, 2 * kW2StageBytes);
-            tma2_load_3d(sA, &tmA, lbar, r, mt * 256 + (int)rank * 128, c);
-            tma2_load_3d(sA + k2AStage, &tmB, lbar, r, nt * 256 + (int)rank * 128, c);
+            if (elect_one()) {
+              if (rank == 0) mbar_expect_tx(full + stage, 2 * kW2StageBytes);
+              tma2_load_3d(sA, &tmA, lbar, r, mt * 256 + (int)rank * 128, c);
+              tma2_load_3d(sA + k2AStage, &tmB, lbar, r, nt * 256 + (int)rank * 128, c);
+            }
+            __syncwarp();
             if (++stage == kW2Stages) { stage = 0; phase ^= 1; }
           }
       }
     }
   } else if (warp == 1) {
-    if (rank == 0 && lane == 0) {
+    if (rank == 0) {
       int stage = 0; uint32_t phase = 0; int it = 0;
       constexpr uint32_t idesc = umma_idesc(Fmt<T>::umma, 0, 0, 256, 256);
       for (int w = cluster_id; w < n_items; w += n_clusters, ++it) {
@@ -467,15 +472,18 @@ wgrad2_kernel(const __grid_constant__ CUtensorMap tmA,    // ahat planes, box 64
             mbar_wait_cluster(full + stage, phase);
             tc_fence_after();
             const uint32_t sA = smem_u32(stages + stage * kW2StageBytes), sB = sA + k2AStage;
+            if (elect_one()) {
 #pragma unroll
-            for (int k = 0; k < 4; ++k) {
-              tc2_mma(d0, umma_desc_sw128(sA + k * 32, 16, 1024), umma_desc_sw128(sB + k * 32, 16, 1024), idesc, acc);
-              acc = 1;
+              for (int k = 0; k < 4; ++k)
+                tc2_mma(d0, umma_desc_sw128(sA + k * 32, 16, 1024), umma_desc_sw128(sB + k * 32, 16, 1024), idesc, (acc | k) ? 1u : 0u);
+              tc2_commit(empty + stage);
             }
-            tc2_commit(empty + stage);
+            __syncwarp();
+            acc = 1;
             if (++stage == kW2Stages) { stage = 0; phase ^= 1; }
           }
-        tc2_commit(tfull + buf);
+        if (elect_one()) tc2_commit(tfull + buf);
+        __syncwarp();
       }
     }
   } else {

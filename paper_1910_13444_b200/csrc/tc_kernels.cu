@@ -59,7 +59,7 @@ __global__ void __launch_bounds__(256, 1) jet_layer_kernel(const __grid_constant
   uint64_t* sbar = tempty + Cfg::kNumBuf;                  // [4] staging-load barriers (MODE 1), one per epilogue warp
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(sbar + 4);
 
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int warp = uniform_warp_idx(), lane = threadIdx.x & 31;
   const int n_ut = p.H / kBM;
   const int n_tiles = n_ut * p.n_row_tiles;
   const int n_kb = p.H / kBK;
@@ -78,27 +78,30 @@ __global__ void __launch_bounds__(256, 1) jet_layer_kernel(const __grid_constant
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
-  const uint32_t tmem_base = *tmem_slot;
+  const uint32_t tmem_base = __shfl_sync(0xffffffffu, *tmem_slot, 0);       // uniform: TMEM addresses live in uniform registers
 
   if (warp == 0) {
-    // ===================== TMA producer =====================
-    if (lane == 0) {
+    // ===================== TMA producer (converged warp, one elected lane issues; see tc_ptx.cuh) =====================
+    {
       int stage = 0; uint32_t phase = 0;
       for (int t = blockIdx.x; t < n_tiles; t += gridDim.x) {
         const int ut = t % n_ut, rt = t / n_ut;
         for (int kb = 0; kb < n_kb; ++kb) {
           mbar_wait(empty + stage, phase ^ 1);
           uint8_t* sA = stages + stage * Cfg::kStageBytes;
-          mbar_expect_tx(full + stage, Cfg::kStageBytes);
-          tma_load_2d(sA, &tmA, full + stage, kb * kBK, ut * kBM);
-          tma_load_3d(sA + kAStage, &tmB, full + stage, rt * kRT, kb * kBK, 0);
+          if (elect_one()) {
+            mbar_expect_tx(full + stage, Cfg::kStageBytes);
+            tma_load_2d(sA, &tmA, full + stage, kb * kBK, ut * kBM);
+            tma_load_3d(sA + kAStage, &tmB, full + stage, rt * kRT, kb * kBK, 0);
+          }
+          __syncwarp();
           if (++stage == Cfg::kNumStages) { stage = 0; phase ^= 1; }
         }
       }
     }
   } else if (warp == 1) {
-    // ===================== MMA issuer (one thread) =====================
-    if (lane == 0) {
+    // ===================== MMA issuer (converged warp, one elected lane issues) =====================
+    {
       int stage = 0; uint32_t phase = 0; int it = 0;
       for (int t = blockIdx.x; t < n_tiles; t += gridDim.x, ++it) {
         const int buf = it % Cfg::kNumBuf;
@@ -119,13 +122,15 @@ __global__ void __launch_bounds__(256, 1) jet_layer_kernel(const __grid_constant
             for (int c0 = 0; c0 < C; c0 += 3) {
               const int nc = (C - c0) < 3 ? (C - c0) : 3;
               const uint64_t bd = umma_desc_sw128(sB + c0 * kBPlane + k * 2048, kBPlane, 1024);   // MN-major: +16 k-rows of 128 B
-              tc_mma(d0 + c0 * kRT, ad, bd, umma_idesc(Fmt<T>::umma, 0, 1, kBM, nc * kRT), acc);
+              if (elect_one()) tc_mma(d0 + c0 * kRT, ad, bd, umma_idesc(Fmt<T>::umma, 0, 1, kBM, nc * kRT), acc);
             }
           }
-          tc_commit(empty + stage);                          // frees the smem slot when these MMAs retire
+          if (elect_one()) tc_commit(empty + stage);         // frees the smem slot when these MMAs retire
+          __syncwarp();
           if (++stage == Cfg::kNumStages) { stage = 0; phase ^= 1; }
         }
-        tc_commit(tfull + buf);                              // accumulator complete
+        if (elect_one()) tc_commit(tfull + buf);             // accumulator complete
+        __syncwarp();
       }
     }
   } else if (warp >= 4) {
@@ -146,7 +151,7 @@ __global__ void __launch_bounds__(256, 1) jet_layer_kernel(const __grid_constant
       if (MODE == 0 || MODE == 2) bias = p.bias[unit];
 
       auto issue_stage_loads = [&](int hf) {                 // MODE 1: the previous layer's output jet h^{l-1} -> staging
-        if (lane == 0) {
+        if (elect_one()) {
           tma_wait_read_all();                               // earlier stores have finished reading the staging buffer
           mbar_expect_tx(sbar + q, C * kStgPlane);
           for (int c = 0; c < C; ++c) tma_load_3d(stg + c * kStgPlane, &tmT, sbar + q, rt * kRT + hf * 32, unit0, c);
@@ -160,7 +165,7 @@ __global__ void __launch_bounds__(256, 1) jet_layer_kernel(const __grid_constant
       for (int hf = 0; hf < 2; ++hf) {
         if (MODE == 0) {
           // ---- h_c = tanh-jet(a_c) ----
-          if (lane == 0) tma_wait_read_all();
+          if (elect_one()) tma_wait_read_all();
           __syncwarp();
 #pragma unroll 1
           for (int rc = 0; rc < 4; ++rc) {
@@ -184,13 +189,13 @@ __global__ void __launch_bounds__(256, 1) jet_layer_kernel(const __grid_constant
           }
           fence_proxy_async();
           __syncwarp();
-          if (lane == 0) {
+          if (elect_one()) {
             for (int c = 0; c < C; ++c) tma_store_3d(&tmO, stg + c * kStgPlane, rt * kRT + hf * 32, unit0, c);
             tma_commit_group();
           }
         } else if (MODE == 2) {
           // ---- value-only layer with split activations: a = W (h_hi + h_lo) + b; t = tanh a; t_hi = rn16(t), t_lo = rn16(t - t_hi) ----
-          if (lane == 0) tma_wait_read_all();
+          if (elect_one()) tma_wait_read_all();
           __syncwarp();
 #pragma unroll 1
           for (int rc = 0; rc < 4; ++rc) {
@@ -210,7 +215,7 @@ __global__ void __launch_bounds__(256, 1) jet_layer_kernel(const __grid_constant
           }
           fence_proxy_async();
           __syncwarp();
-          if (lane == 0) {
+          if (elect_one()) {
             tma_store_3d(&tmO, stg, rt * kRT + hf * 32, unit0, 0);
             tma_store_3d(&tmO, stg + kStgPlane, rt * kRT + hf * 32, unit0, 1);
             tma_commit_group();
@@ -244,7 +249,7 @@ __global__ void __launch_bounds__(256, 1) jet_layer_kernel(const __grid_constant
           }
           fence_proxy_async();
           __syncwarp();
-          if (lane == 0) {
+          if (elect_one()) {
             for (int c = 0; c < C; ++c) tma_store_3d(&tmO, stg + c * kStgPlane, rt * kRT + hf * 32, unit0, c);
             tma_commit_group();
           }
@@ -255,7 +260,8 @@ __global__ void __launch_bounds__(256, 1) jet_layer_kernel(const __grid_constant
       if (lane == 0) mbar_arrive(tempty + buf);
       if (MODE == 1) atomicAdd(p.g_bias + unit, bias_acc * adj_inv_scale(p.amax));
     }
-    if (lane == 0) tma_wait_all();                           // global writes of the last stores are complete before exit
+    __syncwarp();
+    if (elect_one()) tma_wait_all();                         // global writes of the last stores are complete before exit
   }
   tc_fence_before();
   __syncthreads();
@@ -287,7 +293,7 @@ __global__ void __launch_bounds__(192, 1) wgrad_kernel(const __grid_constant__ C
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem + kWStages * (kAStage + 256 * 128));
   uint64_t* full = bars; uint64_t* empty = bars + kWStages; uint64_t* tfull = empty + kWStages; uint64_t* tempty = tfull + 2;
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(tempty + 2);
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int warp = uniform_warp_idx(), lane = threadIdx.x & 31;
   const int n_mt = p.H / kBM, n_nt = p.H / p.NW;
   const int n_items = n_mt * n_nt * p.n_slices;
 
@@ -302,7 +308,7 @@ __global__ void __launch_bounds__(192, 1) wgrad_kernel(const __grid_constant__ C
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
-  const uint32_t tmem_base = *tmem_slot;
+  const uint32_t tmem_base = __shfl_sync(0xffffffffu, *tmem_slot, 0);       // uniform: TMEM addresses live in uniform registers
 
   auto decode = [&](int w, int& mt, int& nt, int& r0, int& r1) {
     const int tile = w % (n_mt * n_nt), sl = w / (n_mt * n_nt);
@@ -311,7 +317,7 @@ __global__ void __launch_bounds__(192, 1) wgrad_kernel(const __grid_constant__ C
   };
 
   if (warp == 0) {
-    if (lane == 0) {
+    {
       int stage = 0; uint32_t phase = 0;
       for (int w = blockIdx.x; w < n_items; w += gridDim.x) {
         int mt, nt, r0, r1; decode(w, mt, nt, r0, r1);
@@ -319,15 +325,18 @@ __global__ void __launch_bounds__(192, 1) wgrad_kernel(const __grid_constant__ C
           for (int r = r0; r < r1; r += 64) {
             mbar_wait(empty + stage, phase ^ 1);
             uint8_t* sA = stages + stage * stage_bytes;
-            mbar_expect_tx(full + stage, stage_bytes);
-            tma_load_3d(sA, &tmA, full + stage, r, mt * kBM, c);
-            tma_load_3d(sA + kAStage, &tmB, full + stage, r, nt * p.NW, c);
+            if (elect_one()) {
+              mbar_expect_tx(full + stage, stage_bytes);
+              tma_load_3d(sA, &tmA, full + stage, r, mt * kBM, c);
+              tma_load_3d(sA + kAStage, &tmB, full + stage, r, nt * p.NW, c);
+            }
+            __syncwarp();
             if (++stage == kWStages) { stage = 0; phase ^= 1; }
           }
       }
     }
   } else if (warp == 1) {
-    if (lane == 0) {
+    {
       int stage = 0; uint32_t phase = 0; int it = 0;
       const uint32_t idesc = umma_idesc(Fmt<T>::umma, 0, 0, kBM, p.NW);
       for (int w = blockIdx.x; w < n_items; w += gridDim.x, ++it) {
@@ -342,15 +351,18 @@ __global__ void __launch_bounds__(192, 1) wgrad_kernel(const __grid_constant__ C
             mbar_wait(full + stage, phase);
             tc_fence_after();
             const uint32_t sA = smem_u32(stages + stage * stage_bytes), sB = sA + kAStage;
+            if (elect_one()) {
 #pragma unroll
-            for (int k = 0; k < 4; ++k) {
-              tc_mma(d0, umma_desc_sw128(sA + k * 32, 16, 1024), umma_desc_sw128(sB + k * 32, 16, 1024), idesc, acc);
-              acc = 1;
+              for (int k = 0; k < 4; ++k)
+                tc_mma(d0, umma_desc_sw128(sA + k * 32, 16, 1024), umma_desc_sw128(sB + k * 32, 16, 1024), idesc, (acc | k) ? 1u : 0u);
+              tc_commit(empty + stage);
             }
-            tc_commit(empty + stage);
+            __syncwarp();
+            acc = 1;
             if (++stage == kWStages) { stage = 0; phase ^= 1; }
           }
-        tc_commit(tfull + buf);
+        if (elect_one()) tc_commit(tfull + buf);
+        __syncwarp();
       }
     }
   } else {

@@ -12,6 +12,21 @@ namespace pigan {
 // =============================================================================================================
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
+// Warp-uniform role code: tcgen05.mma / commit / TMA take their descriptors in UNIFORM registers.  Issued from inside
+// `if (lane == 0)` ptxas cannot prove the operands uniform and wraps every instruction in an ELECT + 5 x R2UR.BROADCAST
+// + BRA.U.ANY "waterfall" (~100 clk per MMA, measured: it was the floor of the issue loop).  So role warps run their
+// loops converged, derive everything from uniform values, and only the instruction itself sits under elect_one().
+__device__ __forceinline__ int uniform_warp_idx() { return __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0); }
+__device__ __forceinline__ bool elect_one() {
+  uint32_t pred;
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "elect.sync _|p, 0xffffffff;\n\t"
+      "selp.u32 %0, 1, 0, p;\n\t}"
+      : "=r"(pred));
+  return pred != 0;
+}
+
 __device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
   asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
 }
