@@ -122,6 +122,13 @@ void gen_backward_chunk(pigan_ctx* c, int n, const float* theta, float* grads, i
                             (T*)c->net[n].ah[cur ^ 1], grads + s.b_off(l - 1), nullptr, nullptr, amax);
     } else {
       tc_wgrad(L, c->cfg.precision, C, H, g.R, g.R_ld, c->net[n].ah[cur], c->h(n, l - 1), grads + s.W_off(l), amax);
+      if (l == 2 && tc_first_layer_fusable(H, g)) {
+        // the adjoint of the first tanh layer is reduced inside the dgrad epilogue (ahat^1 is never written)
+        FirstLayerFuse fl{xy, g.row0, g.npts, s.in_dim, grads, c->net[n].An};
+        tc_layer_bwd(L, c->cfg.precision, C, H, g.R, g.R_ld, c->w16(n, l, 1), c->net[n].ah[cur], c->h(n, l - 1),
+                     c->net[n].ah[cur ^ 1], grads + s.b_off(l - 1), amax, &fl);
+        return;
+      }
       tc_layer_bwd(L, c->cfg.precision, C, H, g.R, g.R_ld, c->w16(n, l, 1), c->net[n].ah[cur], c->h(n, l - 1),
                    c->net[n].ah[cur ^ 1], grads + s.b_off(l - 1), amax);
     }
@@ -308,7 +315,7 @@ pigan_status pigan_create(const pigan_config* cfg, void* cuda_stream, pigan_ctx*
   cudaMemGetInfo(&free_b, &total_b);
   size_t budget = cfg->workspace_bytes ? cfg->workspace_bytes : std::min<size_t>(free_b / 2, (size_t)48 << 30);
   long long rows = (long long)(budget / per_row);
-  long long cap = 65536;                                   // default chunk rows (sweep on B200: larger chunks amortise launch ramps)
+  long long cap = 131072;                                  // default chunk rows (sweep on B200: larger chunks amortise launch ramps)
   if (const char* e = getenv("PIGAN_CHUNK_ROWS")) cap = std::max(256LL, atoll(e));
   if (!cfg->workspace_bytes) rows = std::min(rows, cap);
   rows = std::min<long long>(rows, (long long)round_up((size_t)max_rows, 256));

@@ -198,11 +198,20 @@ void tc_layer_fwd(Launcher& L, int precision, int C, int H, int R, int R_ld, con
                   const void* h_in, void* h_out);
 void tc_layer_fwd_split(Launcher& L, int precision, int H, int R, int R_ld, const void* w16_l, const float* bias, const void* h_in, void* h_out);
 // dgrad of layer l with the adjoint of layer l-1's tanh fused: ahat_in (layer l) -> ahat_out (layer l-1)
+struct FirstLayerFuse;
 void tc_layer_bwd(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* w16T_l, const void* ahat_in,
-                  const void* h_prev /*[C][H][R_ld]*/, void* ahat_out, float* g_bias_prev, const float* amax);
+                  const void* h_prev /*[C][H][R_ld]*/, void* ahat_out, float* g_bias_prev, const float* amax,
+                  const FirstLayerFuse* fl = nullptr);
 // wgrad of layer l: gW [H][H] += sum_c ahat_c h_prev_c^T   (fp32 atomics)
 void tc_wgrad(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* ahat, const void* h_prev, float* gW, const float* amax);
 
+
+// first-layer backward fused into the dgrad of layer 2 (CTA-pair kernels only): the adjoint planes ahat^1 are reduced
+// in the epilogue into W_hat_1[:, 0:2], An and b_hat_1 and never written.  Valid when npts % 64 == 0 and R == valid.
+struct FirstLayerFuse {
+  const float* xy; long long row0; int npts; int in_dim; float* gW1; float* An;
+};
+bool tc_first_layer_fusable(int H, const ChunkGeom& g);
 
 // ---- the same four on CTA pairs (tc2_kernels.cu, cta_group::2), taken when tc2_supported(H) ---------------------
 bool tc2_supported(int H);
@@ -210,7 +219,7 @@ void tc2_layer_fwd(Launcher& L, int precision, int C, int H, int R, int R_ld, co
                    const void* h_in, void* h_out);
 void tc2_layer_fwd_split(Launcher& L, int precision, int H, int R, int R_ld, const void* w16_l, const float* bias, const void* h_in, void* h_out);
 void tc2_layer_bwd(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* w16T_l, const void* ahat_in,
-                   const void* h_prev, void* ahat_out, float* g_bias_prev, const float* amax);
+                   const void* h_prev, void* ahat_out, float* g_bias_prev, const float* amax, const FirstLayerFuse* fl);
 void tc2_wgrad(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* ahat, const void* h_prev, float* gW, const float* amax);
 
 }  // namespace pigan

@@ -46,10 +46,18 @@ struct Jet2Params {
   int n_row_tiles;       // R / 64
   const float* bias;     // MODE 0, 2: b_l
   float* g_bias;         // MODE 1: b_hat_{l-1}
-  const float* amax;     // MODE 1: block-scale source of the adjoint planes
+  const float* amax;     // MODE 1, 3: block-scale source of the adjoint planes
+  // MODE 3 (dgrad of layer 2 + adjoint of the FIRST tanh layer + first-layer reduction, O4 'First layer'): ahat^1 is
+  // consumed in registers and never written.  Requires npts % 64 == 0 (a row tile lies inside one latent sample).
+  const float* xy;       // [npts][2]
+  long long row0;        // first global row of the chunk
+  int npts, in_dim;
+  float* gW1;            // W_hat_1 [H][in_dim]: columns 0, 1 += sum_r (ahat x_r + ahat_x), (ahat y_r + ahat_y)
+  float* An;             // [N][H] += sum_{r in sample n} ahat
 };
 
-// MODE 0: forward; MODE 1: dgrad + adjoint of the previous tanh; MODE 2: value-only forward on split (hi, lo) planes
+// MODE 0: forward; MODE 1: dgrad + adjoint of the previous tanh; MODE 2: value-only forward on split (hi, lo) planes;
+// MODE 3: MODE 1 with the first-layer backward reduction fused (no adjoint planes written)
 template <typename T, int C, int MODE>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(k2Threads, 1)
 jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H] 16-bit, box 64 x 128, SW128
@@ -82,7 +90,7 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
 
   if (warp == 0 && lane == 0) {
     prefetch_tmap(&tmA); prefetch_tmap(&tmB); prefetch_tmap(&tmO);
-    if (MODE == 1) prefetch_tmap(&tmT);
+    if (MODE == 1 || MODE == 3) prefetch_tmap(&tmT);
   }
   if (warp == 1 && lane == 0) {
     for (int i = 0; i < Cfg::kNumStages; ++i) { mbar_init(full + i, 1); mbar_init(empty + i, 1); }
@@ -244,7 +252,7 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
         if (lane == 0) mbar_arrive_cluster(mapa_u32(tempty + buf, 0));
       };
 
-      if (MODE == 1 && elect_one()) {                        // the previous layer's output jet h^{l-1} -> staging
+      if ((MODE == 1 || MODE == 3) && elect_one()) {         // the previous layer's output jet h^{l-1} -> staging
         tma_wait_read_all();                                 // earlier stores have finished reading the staging buffer
         mbar_expect_tx(sbar + e, C * k2StgPlane);
         for (int c = 0; c < C; ++c) tma_load_3d(stg + c * k2StgPlane, &tmT, sbar + e, row0, unit0, c);
@@ -258,7 +266,7 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
       te_tf += clock64() - te0; te0 = clock64();
 #endif
 #ifdef PIGAN_PROBE_NOEPI
-      if (MODE == 1) { mbar_wait(sbar + e, sphase); sphase ^= 1; }
+      if (MODE == 1 || MODE == 3) { mbar_wait(sbar + e, sphase); sphase ^= 1; }
       release();
       continue;
 #endif
@@ -338,6 +346,9 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
       } else {
         // ---- adjoint of the previous layer's tanh: ahat^{l-1} = J^T hhat^{l-1} ----
         mbar_wait(sbar + e, sphase); sphase ^= 1;
+        float sx = 0.f, sy = 0.f;                            // MODE 3
+        const long long grow = p.row0 + row0;                // MODE 3: global row of this warp's first row
+        const float2* xyp = MODE == 3 ? reinterpret_cast<const float2*>(p.xy) + (int)(grow % p.npts) : nullptr;
 #pragma unroll
         for (int rc = 0; rc < 4; ++rc) {
           float hh[C][8], hp[C][8], o[C][8];
@@ -357,18 +368,33 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
             for (int c = 0; c < C; ++c) hj[c] = hp[c][i];
             jet_act_bwd<C>(hj, hx, aa);
             bias_acc += aa[0];
+            if (MODE == 3) {
+              const float2 q = __ldg(xyp + rc * 8 + i);      // same address in every lane: one broadcast load
+              sx = fmaf(aa[0], q.x, sx); sy = fmaf(aa[0], q.y, sy);
+              if (C >= 3) { sx += aa[1]; sy += aa[2]; }
+            }
 #pragma unroll
             for (int c = 0; c < C; ++c) o[c][i] = aa[c];
           }
+          if (MODE == 1) {
 #pragma unroll
-          for (int c = 0; c < C; ++c) *reinterpret_cast<uint4*>(my_row + c * k2StgPlane + off) = pack8<T>(o[c]);
+            for (int c = 0; c < C; ++c) *reinterpret_cast<uint4*>(my_row + c * k2StgPlane + off) = pack8<T>(o[c]);
+          }
         }
         if (C != 5) release();
-        fence_proxy_async();
-        __syncwarp();
-        if (elect_one()) {
-          for (int c = 0; c < C; ++c) tma_store_3d(&tmO, stg + c * k2StgPlane, row0, unit0, c);
-          tma_commit_group();
+        if (MODE == 1) {
+          fence_proxy_async();
+          __syncwarp();
+          if (elect_one()) {
+            for (int c = 0; c < C; ++c) tma_store_3d(&tmO, stg + c * k2StgPlane, row0, unit0, c);
+            tma_commit_group();
+          }
+        } else {
+          __syncwarp();                                      // every lane is done reading the staging planes before the next loads land
+          const float inv = adj_inv_scale(p.amax);
+          atomicAdd(p.An + (size_t)(grow / p.npts) * p.H + unit, bias_acc * inv);
+          atomicAdd(p.gW1 + (size_t)unit * p.in_dim, sx * inv);
+          atomicAdd(p.gW1 + (size_t)unit * p.in_dim + 1, sy * inv);
         }
         atomicAdd(p.g_bias + unit, bias_acc * adj_inv_scale(p.amax));
       }
@@ -537,7 +563,7 @@ static void launch_jet2(Launcher& L, const CUtensorMap& a, const CUtensorMap& b,
   const int tiles = (p.H / 256) * p.n_row_tiles;
   const int clusters = std::min(tiles, num_sms() / 2);
   kern<<<2 * clusters, k2Threads, Cfg::kSmemBytes, L.stream>>>(a, b, o, t, p);
-  L.check(MODE == 0 ? "jet_layer_fwd" : MODE == 1 ? "jet_layer_bwd" : "jet_layer_fwd_split");
+  L.check(MODE == 0 ? "jet_layer_fwd" : MODE == 2 ? "jet_layer_fwd_split" : "jet_layer_bwd");
 }
 
 template <int MODE>
@@ -569,7 +595,7 @@ void tc2_layer_fwd_split(Launcher& L, int precision, int H, int R, int R_ld, con
 }
 
 void tc2_layer_bwd(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* w16T_l, const void* ahat_in, const void* h_prev,
-                   void* ahat_out, float* g_bias_prev, const float* amax) {
+                   void* ahat_out, float* g_bias_prev, const float* amax, const FirstLayerFuse* fl) {
   CUtensorMap a, b, o, t;
   bool ok = weight_map(L, &a, precision, w16T_l, H) && plane_map(L, &b, precision, ahat_in, H, R_ld, C, 32, 64, C, CU_TENSOR_MAP_SWIZZLE_64B) &&
             plane_map(L, &o, precision, ahat_out, H, R_ld, C, 32, 32, 1, CU_TENSOR_MAP_SWIZZLE_64B) &&
@@ -577,6 +603,11 @@ void tc2_layer_bwd(Launcher& L, int precision, int C, int H, int R, int R_ld, co
   if (!ok) return;
   Jet2Params p{};
   p.H = H; p.n_row_tiles = R / 64; p.g_bias = g_bias_prev; p.amax = amax;
+  if (fl) {
+    p.xy = fl->xy; p.row0 = fl->row0; p.npts = fl->npts; p.in_dim = fl->in_dim; p.gW1 = fl->gW1; p.An = fl->An;
+    dispatch_jet2<3>(L, C, a, b, o, t, p);
+    return;
+  }
   dispatch_jet2<1>(L, C, a, b, o, t, p);
 }
 

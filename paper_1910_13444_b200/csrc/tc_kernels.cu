@@ -482,10 +482,12 @@ void tc_layer_fwd_split(Launcher& L, int precision, int H, int R, int R_ld, cons
   launch_jet<__half, 2, 2>(L, a, b, o, o, p);
 }
 
+bool tc_first_layer_fusable(int H, const ChunkGeom& g) { return tc2_supported(H) && g.npts % 64 == 0 && g.R == g.valid && g.R > 0; }
+
 void tc_layer_bwd(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* w16T_l, const void* ahat_in, const void* h_prev,
-                  void* ahat_out, float* g_bias_prev, const float* amax) {
+                  void* ahat_out, float* g_bias_prev, const float* amax, const FirstLayerFuse* fl) {
   if (R <= 0) return;
-  if (tc2_supported(H)) { tc2_layer_bwd(L, precision, C, H, R, R_ld, w16T_l, ahat_in, h_prev, ahat_out, g_bias_prev, amax); return; }
+  if (tc2_supported(H)) { tc2_layer_bwd(L, precision, C, H, R, R_ld, w16T_l, ahat_in, h_prev, ahat_out, g_bias_prev, amax, fl); return; }
   CUtensorMap a, b, o, t;
   bool ok = weight_map(L, &a, precision, w16T_l, H) && plane_map(L, &b, precision, ahat_in, H, R_ld, C, kRT, kBK, C, CU_TENSOR_MAP_SWIZZLE_128B) &&
             plane_map(L, &o, precision, ahat_out, H, R_ld, C, 32, 32, 1, CU_TENSOR_MAP_SWIZZLE_64B) &&
