@@ -45,6 +45,11 @@ template <> __device__ __forceinline__ void store8<__half>(__half* p, const floa
   *reinterpret_cast<uint4*>(p) = u;
 }
 
+__device__ __forceinline__ float tanh_approx(float x) {
+  float y;
+  asm("tanh.approx.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
 __device__ __forceinline__ float warp_sum_f(float v) {
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
@@ -72,13 +77,18 @@ __global__ void __launch_bounds__(256) first_layer_fwd_kernel(NetShape s, const 
   const int r0 = blockIdx.x * 256 + lane * 8;
   if (r0 >= g.R) return;
   float x[8], y[8]; int n[8];
+  {
+    // one 64-bit division per thread; the 8 rows then step through (n, p) incrementally.  Padded rows repeat the
+    // last valid row (finite values).
+    const long long rg0 = g.row0 + min(r0, g.valid - 1);
+    int nn = (int)(rg0 / g.npts), p = (int)(rg0 - (long long)nn * g.npts);
 #pragma unroll
-  for (int i = 0; i < 8; ++i) {
-    const long long rg = g.row0 + min(r0 + i, g.valid - 1);      // padded rows repeat the last valid row (finite values)
-    n[i] = (int)(rg / g.npts);
-    const int p = (int)(rg % g.npts);
-    const float2 q = *reinterpret_cast<const float2*>(xy + 2 * p);
-    x[i] = q.x; y[i] = q.y;
+    for (int i = 0; i < 8; ++i) {
+      n[i] = nn;
+      const float2 q = *reinterpret_cast<const float2*>(xy + 2 * p);
+      x[i] = q.x; y[i] = q.y;
+      if (r0 + i + 1 < g.valid) { if (++p == g.npts) { p = 0; ++nn; } }
+    }
   }
   const bool one_sample = n[0] == n[7];
   const float* W1 = theta; const float* b1 = theta + s.b_off(1);
@@ -92,7 +102,8 @@ __global__ void __launch_bounds__(256) first_layer_fwd_kernel(NetShape s, const 
       const float zp = one_sample ? z0 : Zp[(size_t)n[i] * s.H + j];
       const float a0 = zp + bj + wx * x[i] + wy * y[i];
       float a[5] = {a0, wx, wy, 0.f, 0.f}, h[5];
-      jet_act_fwd<C>(tanhf(a0), a, h);
+      // 16-bit planes round t to 2^-11 anyway: tanh.approx there (R4); fp32 mode and the split snapshot path stay exact
+      jet_act_fwd<C>((sizeof(T) == 2 && !SPLIT) ? tanh_approx(a0) : tanhf(a0), a, h);
 #pragma unroll
       for (int c = 0; c < C; ++c) o[c][i] = h[c];
     }
@@ -249,10 +260,81 @@ __global__ void __launch_bounds__(256) jet_act_bwd_kernel(int H, ChunkGeom g, co
   if (g_bout && j == 0) { v = block_sum_256(s_bout, red); if (threadIdx.x == 0) atomicAdd(g_bout, v); }
 }
 
+
+// Output-layer form of the same adjoint (hh_c = w_out[j] * ohat_c[r]): a block owns 2048 rows x kTopUnits units and keeps
+// the C x 8 output adjoints of its rows in registers across the unit loop, so per unit it only streams the h planes in
+// and the ahat planes out (the generic kernel above re-read ohat for every unit: 3x the bytes through L2).
+constexpr int kTopUnits = 16;
+template <typename T, int C>
+__global__ void __launch_bounds__(256) top_act_bwd_kernel(int H, ChunkGeom g, const float* __restrict__ w_out, const float* __restrict__ ohat,
+                                                          const T* __restrict__ h, T* __restrict__ ahat, float* __restrict__ g_bias,
+                                                          float* __restrict__ g_wout, float* __restrict__ g_bout, const float* __restrict__ amax) {
+  __shared__ float red[kTopUnits][2];
+  __shared__ float red8[8];
+  const int lane = threadIdx.x & 31;
+  const int jb = blockIdx.y * kTopUnits, je = min(H, jb + kTopUnits);
+  const size_t plane = (size_t)H * g.R_ld;
+  const float sc = adj_scale(amax), inv_sc = adj_inv_scale(amax);
+  if (threadIdx.x < kTopUnits * 2) (&red[0][0])[threadIdx.x] = 0.f;
+  __syncthreads();
+  const int r0 = blockIdx.x * 2048 + threadIdx.x * 8;
+  const bool active = r0 < g.R;
+  float ov[C][8];
+  float s_bout = 0.f;
+#pragma unroll
+  for (int c = 0; c < C; ++c) {
+    if (active) load8<float>(ohat + (size_t)c * g.R_ld + r0, ov[c]);
+    else {
+#pragma unroll
+      for (int i = 0; i < 8; ++i) ov[c][i] = 0.f;
+    }
+  }
+#pragma unroll
+  for (int i = 0; i < 8; ++i) s_bout += ov[0][i];
+  for (int j = jb; j < je; ++j) {
+    float s_bias = 0.f, s_wout = 0.f;
+    if (active) {
+      const float wj = w_out[j] * sc;
+      const size_t off = (size_t)j * g.R_ld + r0;
+      float hv[C][8], o[C][8];
+#pragma unroll
+      for (int c = 0; c < C; ++c) load8<T>(h + c * plane + off, hv[c]);
+#pragma unroll
+      for (int i = 0; i < 8; ++i) {
+        float hx[5], hj[5], aa[5];
+#pragma unroll
+        for (int c = 0; c < C; ++c) { hx[c] = wj * ov[c][i]; hj[c] = hv[c][i]; s_wout = fmaf(ov[c][i], hv[c][i], s_wout); }
+        jet_act_bwd<C>(hj, hx, aa);
+        s_bias += aa[0];
+#pragma unroll
+        for (int c = 0; c < C; ++c) o[c][i] = aa[c];
+      }
+#pragma unroll
+      for (int c = 0; c < C; ++c) store8<T>(ahat + c * plane + off, o[c]);
+    }
+    s_bias = warp_sum_f(s_bias); s_wout = warp_sum_f(s_wout);
+    if (lane == 0) { atomicAdd(&red[j - jb][0], s_bias); atomicAdd(&red[j - jb][1], s_wout); }
+  }
+  __syncthreads();
+  if (threadIdx.x < je - jb) {
+    atomicAdd(g_bias + jb + threadIdx.x, red[threadIdx.x][0] * inv_sc);
+    atomicAdd(g_wout + jb + threadIdx.x, red[threadIdx.x][1]);
+  }
+  if (blockIdx.y == 0) { const float v = block_sum_256(s_bout, red8); if (threadIdx.x == 0) atomicAdd(g_bout, v); }
+}
+
 template <typename T>
 void jet_act_bwd_launch(Launcher& L, int C, int H, const ChunkGeom& g, const float* hhat, const float* w_out, const float* ohat, const T* h,
                         T* ahat, float* g_bias, float* g_wout, float* g_bout, const float* amax) {
   if (g.R <= 0) return;
+  if (!hhat) {
+    dim3 tgrid(cdiv(g.R, 2048), cdiv(H, kTopUnits));
+#define PIGAN_TOP(c) top_act_bwd_kernel<T, c><<<tgrid, 256, 0, L.stream>>>(H, g, w_out, ohat, h, ahat, g_bias, g_wout, g_bout, amax)
+    if (C == 1) PIGAN_TOP(1); else if (C == 3) PIGAN_TOP(3); else PIGAN_TOP(5);
+#undef PIGAN_TOP
+    L.check("jet_act_bwd");
+    return;
+  }
   dim3 grid(cdiv(g.R, 2048), H);
 #define PIGAN_BWD(c) jet_act_bwd_kernel<T, c><<<grid, 256, 0, L.stream>>>(H, g, hhat, w_out, ohat, h, ahat, g_bias, g_wout, g_bout, amax)
   if (C == 1) PIGAN_BWD(1); else if (C == 3) PIGAN_BWD(3); else PIGAN_BWD(5);
