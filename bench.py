@@ -28,9 +28,9 @@ import workloads as wl  # noqa: E402
 METRIC = "PI-GAN train-step sample*collocation-points/s"
 UNIT = "sample*collocation-points/s"
 ADAM = dict(lr=1e-4, beta1=0.5, beta2=0.9, adam_eps=1e-8)          # reading G3
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the largest tensor-core kernel (G_u forward, 65536-row chunk),
-# from profiles/r01_ncu_full_tc_kernels_c5.csv; algorithmic bytes of that launch: 1.879e9
-TRAFFIC = {"c5": 1.835e9}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the largest tensor-core kernel (G_u forward, 131072-row chunk),
+# from profiles/r01b_ncu_full_tc_kernels_c5.csv (1.345e9 read + 1.306e9 written); algorithmic bytes of that launch: 2.684e9
+TRAFFIC = {"c5": 2.651e9}
 
 
 # ----------------------------------------------------------------------------------------------------------------

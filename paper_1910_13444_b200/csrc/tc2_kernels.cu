@@ -23,11 +23,6 @@ constexpr int k2StgPlane = 32 * 64;         // epilogue staging plane: 32 units 
 constexpr int k2EpiWarps = 8;
 constexpr int k2Threads = (4 + k2EpiWarps) * 32;
 
-#ifdef PIGAN_PROBE_FREERUN
-#define LOOKAHEAD(b, p) false
-#else
-#define LOOKAHEAD(b, p) mbar_try_wait(b, p)
-#endif
 
 template <int C, int MODE> struct Jet2Cfg {
   static constexpr int kStageBytes = k2AStage + C * k2BPlane;
@@ -78,9 +73,6 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
   uint64_t* sbar = tempty + Cfg::kNumBuf;                  // [8]           staging loads (MODE 1), one per epilogue warp
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(sbar + k2EpiWarps);
 
-#ifdef PIGAN_PROBE_TRACE
-  __shared__ long long tr_wait[16], tr_issue[16], tr_prod[16], tr_prod0[16];
-#endif
   const int warp = uniform_warp_idx(), lane = threadIdx.x & 31;
   const uint32_t rank = cluster_ctarank();
   const int cluster_id = blockIdx.x >> 1, n_clusters = gridDim.x >> 1;
@@ -117,16 +109,7 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
       for (int t = cluster_id; t < n_tiles; t += n_clusters) {
         const int ut = t % n_ut, rt = t / n_ut;
         for (int kb = 0; kb < n_kb; ++kb) {
-#ifdef PIGAN_PROBE_FREERUN
-          continue;
-#endif
-#ifdef PIGAN_PROBE_TRACE
-          if (rank == 0 && cluster_id == 0 && t == cluster_id + 10 * n_clusters) tr_prod0[kb] = clock64();
-#endif
           mbar_wait(empty + stage, phase ^ 1);
-#ifdef PIGAN_PROBE_TRACE
-          if (rank == 0 && cluster_id == 0 && t == cluster_id + 10 * n_clusters) tr_prod[kb] = clock64();
-#endif
           uint8_t* sA = stages + stage * Cfg::kStageBytes;
           const uint32_t lbar = mapa_u32(full + stage, 0);
 #ifdef PIGAN_PROBE_NOLOAD
@@ -174,15 +157,10 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
 #ifdef PIGAN_PROBE_TIMING
           tm0 = clock64();
 #endif
-#ifndef PIGAN_PROBE_FREERUN
           if (!ready) mbar_wait(full + stage, phase);
-#endif
           tc_fence_after();
 #ifdef PIGAN_PROBE_TIMING
           tm_full += clock64() - tm0;
-#endif
-#ifdef PIGAN_PROBE_TRACE
-          if (cluster_id == 0 && it == 10) tr_wait[kb] = clock64();
 #endif
           const uint32_t sA = smem_u32(stages + stage * Cfg::kStageBytes), sB = sA + k2AStage;
           int nstage = stage + 1; uint32_t nphase = phase;
@@ -194,31 +172,21 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
             // MN-major SW64: channel planes are 4 KB apart (LBO), 8-unit groups 512 B apart (SBO), 16 units = +1 KB
 #ifndef PIGAN_PROBE_NOMMA
             if (C == 5 && k < 3 && elect_one()) tc2_mma(d1, ad, umma_desc_sw64(sB + 3 * k2BPlane + k * 1024, k2BPlane, 512), idesc1, acc);
-            if (C != 5 && k == 3) ready = !(last_tile && kb == n_kb - 1) && __all_sync(0xffffffffu, LOOKAHEAD(full + nstage, nphase));
+            if (C != 5 && k == 3) ready = !(last_tile && kb == n_kb - 1) && __all_sync(0xffffffffu, mbar_try_wait(full + nstage, nphase));
             if (elect_one()) tc2_mma(d0, ad, umma_desc_sw64(sB + k * 1024, k2BPlane, 512), idesc0, acc);
             if (C == 5 && k == 3) {
-              ready = !(last_tile && kb == n_kb - 1) && __all_sync(0xffffffffu, LOOKAHEAD(full + nstage, nphase));
+              ready = !(last_tile && kb == n_kb - 1) && __all_sync(0xffffffffu, mbar_try_wait(full + nstage, nphase));
               if (elect_one()) tc2_mma(d1, ad, umma_desc_sw64(sB + 3 * k2BPlane + k * 1024, k2BPlane, 512), idesc1, acc);
             }
 #endif
           }
           if (elect_one()) tc2_commit(empty + stage);        // frees the smem slot in both CTAs when these MMAs retire
           __syncwarp();
-#ifdef PIGAN_PROBE_TRACE
-          if (cluster_id == 0 && it == 10) tr_issue[kb] = clock64();
-#endif
           stage = nstage; phase = nphase;
         }
         if (elect_one()) tc2_commit(tfull + buf);            // accumulator complete (both CTAs)
         __syncwarp();
       }
-#ifdef PIGAN_PROBE_TRACE
-      if (cluster_id == 0 && C == 5 && MODE == 0 && n_tiles > 11 * n_clusters) {
-        for (int kb = 0; kb < 16; ++kb)
-          printf("TRACE kb=%d wait_done=%lld issue_done=%lld prod_wait_begin=%lld prod_empty_seen=%lld\n", kb, tr_wait[kb] - tr_wait[0], tr_issue[kb] - tr_wait[0],
-                 tr_prod0[kb] - tr_wait[0], tr_prod[kb] - tr_wait[0]);
-      }
-#endif
 #ifdef PIGAN_PROBE_TIMING
       if (cluster_id == 0 && lane == 0) printf("TIMING mma C=%d MODE=%d tiles=%d total=%lld wait_tempty=%lld wait_full=%lld\n", C, MODE, it, clock64() - tm_start, tm_te, tm_full);
 #endif
