@@ -42,6 +42,23 @@ def measured_peaks():
     return {"hbm_gbs": 6650.0, "tflops_burst": 1590.0, "tflops_sustained": 1400.0, "source": "fallback"}
 
 
+def max_over_ranks(t_ms: float, dist=None, device=None) -> float:
+    """Max of a per-rank time over all ranks (the only exchange of the replicas-only multi-GPU mode).  Works on any
+    torch.distributed backend: NCCL with a CUDA device in bench runs, gloo with CPU tensors in the CPU tests."""
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return float(t_ms)
+    import torch
+    t = torch.tensor([t_ms], dtype=torch.float64, device=device if device is not None else "cpu")
+    dist.barrier()
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(units_per_rank: int, world: int, t_max_ms: float) -> float:
+    """Whole-job throughput of `world` independent replicas: all ranks' units over the slowest rank's time (weak scaling)."""
+    return world * units_per_rank / (t_max_ms * 1e-3)
+
+
 class ClockSampler(threading.Thread):
     """Samples SM clock and throttle reasons through NVML while the timed region runs."""
 
@@ -175,6 +192,15 @@ class GpuWorkload:
         self.step()
         self.host_out.copy_(self.out[3], non_blocking=True)
 
+    def jet_pass(self):
+        """The jet evaluation alone (a1-a4 forward): G_u at order 2 and G_logk at order 1 on every (sample, point)."""
+        d, pg = self.d, self.pg
+        if not hasattr(self, "jet_out"):
+            n = self.cfg.N * self.cfg.P
+            self.jet_out = (self.torch.empty(5 * n, device=self.device), self.torch.empty(3 * n, device=self.device))
+        pg.gen_jet_forward(self.params[1], d["xy_colloc"], d["z"], 2, out=self.jet_out[0].view(5, self.cfg.N, self.cfg.P))
+        pg.gen_jet_forward(self.params[0], d["xy_colloc"], d["z"], 1, out=self.jet_out[1].view(3, self.cfg.N, self.cfg.P))
+
     def e2e_bytes(self):
         return sum(int(v.numel() * 4) for v in self.host.values()), 6 * 4
 
@@ -223,6 +249,9 @@ def run_config(cfg, device, steps, warmup, rank, world, with_roofline=True, seed
     ms_e2e = w.timed(w.step_e2e, max(2, steps // 2), 1)
     res["ms_e2e"] = ms_e2e
     res["h2d"], res["d2h"] = w.e2e_bytes()
+    # jet evaluations/s (north_star's second throughput figure): forward jets of both nets, no residual, no backward
+    res["ms_jet"] = w.timed(w.jet_pass, max(2, steps // 2), 1)
+    del w.jet_out
     # roofline of the dominant kernel class (the tcgen05 jet GEMMs: forward, dgrad+adjoint, wgrad)
     if with_roofline:
         tc = {k: v for k, v in prof.items() if k in ("jet_layer_fwd", "jet_layer_bwd", "wgrad")}
@@ -255,7 +284,7 @@ def run_config(cfg, device, steps, warmup, rank, world, with_roofline=True, seed
 
 def summarize(cfg, res, n_gpus, steps, warmup, t_max_ms):
     units = cfg.N * cfg.P
-    value = n_gpus * units / (t_max_ms * 1e-3)
+    value = whole_job_value(units, n_gpus, t_max_ms)
     e2e_ms = float(np.mean(res["ms_e2e"]))
     return {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": n_gpus, "steps": steps, "warmup": warmup, "ms_per_step": t_max_ms,
@@ -265,6 +294,7 @@ def summarize(cfg, res, n_gpus, steps, warmup, t_max_ms):
                    "l2": "per-step working set >> L2" if cfg.N * cfg.P >= 400000 else "256 MiB L2 flush between timed steps",
                    "loss_scale": 1024.0 if cfg.precision == "fp16" else 1.0},
         "train_steps_per_s": 1e3 / t_max_ms,
+        "jet_evals_per_s": n_gpus * units / (float(np.mean(res["ms_jet"])) * 1e-3),
         "step_tflops": wl.step_flops(cfg)["total"] / (t_max_ms * 1e-3) / 1e12,
         "e2e": {"value": n_gpus * units / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": res["h2d"], "d2h_bytes_per_step": res["d2h"]},
         "gpu_launches": res["launches"], "clocks": res["clocks"], "roofline": res.get("roofline"),
@@ -317,10 +347,7 @@ def main():
     res = run_config(cfg, device, steps, warmup, rank, world, seed_shift=rank)
     t_ms = float(np.mean(res["ms_steps"]))
     if world > 1:
-        t = torch.tensor([t_ms], device=device, dtype=torch.float64)
-        dist.barrier()
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)            # max over ranks; the replicas exchange nothing else
-        t_ms = float(t.item())
+        t_ms = max_over_ranks(t_ms, dist, device)           # max over ranks; the replicas exchange nothing else
     if rank == 0:
         line = summarize(cfg, res, world, steps, warmup, t_ms)
         if args.all_configs:
@@ -330,7 +357,7 @@ def main():
                     continue
                 r = run_config(c, device, 5 if c.N * c.P > 1000000 else 20, 3, rank, world)
                 s = summarize(c, r, 1, len(r["ms_steps"]), 3, float(np.mean(r["ms_steps"])))
-                per[name] = {k: s[k] for k in ("value", "ms_per_step", "dtype", "step_tflops", "roofline", "gpu_launches", "e2e", "kernel_ms_per_step")}
+                per[name] = {k: s[k] for k in ("value", "ms_per_step", "dtype", "step_tflops", "jet_evals_per_s", "roofline", "gpu_launches", "e2e", "kernel_ms_per_step")}
             line["per_config"] = per
         if not args.no_cpu_baseline:
             val, sec, cores, sample = time_oracle(cfg)

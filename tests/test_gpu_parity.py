@@ -10,7 +10,7 @@ import pytest
 
 import workloads as wl
 from oracle import pigan_oracle as orc
-from parity_util import jets_parity, rel_err, step_parity, to_dev
+from parity_util import jets_parity, per_layer, rel_err, step_parity, to_dev
 
 pytestmark = pytest.mark.gpu
 
@@ -206,3 +206,41 @@ def test_full_size_jets_sampled_against_oracle(name):
     r_ref, _ = orc.darcy_residual_ref(Y.cpu().numpy(), U.cpu().numpy(), inp["f"])
     assert abs(msq.item() - float(np.mean(r_ref * r_ref))) <= 1e-4 * float(np.mean(r_ref * r_ref))
     pg.close()
+
+
+@pytest.mark.parametrize("name", ["c4", "c5"])
+def test_full_size_step_is_the_mean_of_its_half_batches(name):
+    """BASELINE full sizes in the launch configuration bench.py times (default chunking).  Every loss is a mean over
+    samples and the critic is held fixed in L_G, so the six losses and all three gradient sets of the full batch equal
+    the average of those of its two half batches (exactly, in the mathematics; here up to summation order).  Together
+    with the reduced-row parity tests against the oracle this pins the row-chunked accumulation at full scale."""
+    import torch
+    from paper_1910_13444_b200 import PiGan
+    cfg = wl.CONFIGS[name]
+    inp = wl.make_inputs(cfg)
+    rng = np.random.default_rng(11)
+    inp["real"] = rng.normal(size=(cfg.N, 2 * cfg.S)).astype(np.float32)
+    d = to_dev(inp, "cuda:0")
+    ls = 1024.0 if cfg.precision == "fp16" else 1.0
+
+    def run(c, sl):
+        pg = PiGan.from_config(c)
+        out = pg.train_step_grads(d["theta_Y"], d["theta_u"], d["theta_D"], d["xy_colloc"], d["f"], d["xy_sensors"], d["z"][sl].contiguous(),
+                                  d["real"][sl].contiguous(), d["eps"][sl].contiguous(), ls)
+        torch.cuda.synchronize()
+        res = [o.double().cpu().numpy() for o in out[:4]] + [int(out[4].item())]
+        pg.close()
+        return res
+
+    h = cfg.N // 2
+    full = run(cfg, slice(0, cfg.N))
+    half = dataclasses.replace(cfg, name=cfg.name + "-half", N=h)
+    a, b = run(half, slice(0, h)), run(half, slice(h, cfg.N))
+    assert full[4] == 0 and a[4] == 0 and b[4] == 0
+    for k, nm in enumerate(("gY", "gu", "gD")):
+        shape = cfg.disc_shape if nm == "gD" else cfg.gen_shape
+        fa = per_layer(full[k], shape); av = per_layer(0.5 * (a[k] + b[k]), shape)
+        for key in fa:
+            assert rel_err(fa[key], av[key]) <= 1e-3, (name, nm, key, rel_err(fa[key], av[key]))
+    mean = 0.5 * (a[3] + b[3])
+    assert np.all(np.abs(full[3] - mean) <= 1e-3 * np.maximum(np.abs(mean), 1e-6)), (full[3], mean)
