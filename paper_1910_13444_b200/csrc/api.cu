@@ -42,6 +42,16 @@ struct pigan_ctx {
   float* seed = nullptr;       // [2N]
   float* amax = nullptr;       // [2] largest output adjoint of the current chunk, per net (block scale of the adjoint planes)
   std::vector<void*> allocs;
+  // CUDA-graph replay of pigan_train_step_grads: the step is hundreds to thousands of launches, launch-latency bound
+  // for the small configs.  A call whose arguments repeat the previous call's is captured once (on a private stream,
+  // so the caller's stream may be the legacy default stream) and replayed from then on.  PIGAN_NO_GRAPH=1 disables it.
+  struct StepGraph {
+    cudaStream_t cap_stream = nullptr;
+    cudaGraphExec_t exec = nullptr;
+    std::vector<unsigned long long> key, last_key;
+    unsigned long long launches = 0;
+    bool disabled = false;
+  } sg;
 
   template <typename T> T* alloc(size_t n) {
     void* p = nullptr;
@@ -304,6 +314,7 @@ pigan_status pigan_create(const pigan_config* cfg, void* cuda_stream, pigan_ctx*
   c->gen = NetShape{cfg->gen.in_dim, cfg->gen.n_hidden, cfg->gen.width};
   c->disc = NetShape{cfg->disc.in_dim, cfg->disc.n_hidden, cfg->disc.width};
   c->L.stream = (cudaStream_t)cuda_stream;
+  if (const char* e = getenv("PIGAN_NO_GRAPH")) c->sg.disabled = e[0] == '1';
   c->elem = cfg->precision == PIGAN_FP32 ? 4 : 2;
   const int H = c->gen.H, Lh = c->gen.L, N = cfg->n_samples, S = cfg->n_sensors, d = 2 * S, HD = c->disc.H, LD = c->disc.L;
   const bool f32 = cfg->precision == PIGAN_FP32;
@@ -364,6 +375,8 @@ pigan_status pigan_create(const pigan_config* cfg, void* cuda_stream, pigan_ctx*
 
 void pigan_destroy(pigan_ctx* c) {
   if (!c) return;
+  if (c->sg.exec) cudaGraphExecDestroy(c->sg.exec);
+  if (c->sg.cap_stream) cudaStreamDestroy(c->sg.cap_stream);
   for (void* p : c->allocs) cudaFree(p);
   for (cudaEvent_t e : c->L.events) cudaEventDestroy(e);
   delete c;
@@ -439,11 +452,52 @@ pigan_status pigan_train_step_grads(pigan_ctx* c, const float* logk_params, cons
   if (!logk_params || !u_params || !disc_params || !xy_colloc || !f || !xy_sensors || !z || !real_snap || !eps || !g_logk || !g_u || !g_disc)
     return fail(c, PIGAN_ERR_INVALID_ARG, "null pointer");
   if (!(loss_scale > 0.f) || !std::isfinite(loss_scale)) return fail(c, PIGAN_ERR_INVALID_ARG, "loss_scale must be positive and finite");
-  switch (c->cfg.precision) {
-    case PIGAN_FP32: return train_step_impl<float>(c, logk_params, u_params, disc_params, xy_colloc, f, xy_sensors, z, real_snap, eps, loss_scale, g_logk, g_u, g_disc, losses, found_inf);
-    case PIGAN_BF16: return train_step_impl<__half>(c, logk_params, u_params, disc_params, xy_colloc, f, xy_sensors, z, real_snap, eps, loss_scale, g_logk, g_u, g_disc, losses, found_inf);
-    default: return train_step_impl<__half>(c, logk_params, u_params, disc_params, xy_colloc, f, xy_sensors, z, real_snap, eps, loss_scale, g_logk, g_u, g_disc, losses, found_inf);
+  auto run = [&]() -> pigan_status {
+    switch (c->cfg.precision) {
+      case PIGAN_FP32: return train_step_impl<float>(c, logk_params, u_params, disc_params, xy_colloc, f, xy_sensors, z, real_snap, eps, loss_scale, g_logk, g_u, g_disc, losses, found_inf);
+      default: return train_step_impl<__half>(c, logk_params, u_params, disc_params, xy_colloc, f, xy_sensors, z, real_snap, eps, loss_scale, g_logk, g_u, g_disc, losses, found_inf);
+    }
+  };
+  auto& sg = c->sg;
+  if (sg.disabled || c->L.profiling) return run();
+  unsigned int ls_bits; memcpy(&ls_bits, &loss_scale, 4);
+  const void* ptrs[] = {logk_params, u_params, disc_params, xy_colloc, f, xy_sensors, z, real_snap, eps, g_logk, g_u, g_disc, losses, found_inf};
+  std::vector<unsigned long long> key;
+  for (const void* q : ptrs) key.push_back((unsigned long long)(uintptr_t)q);
+  key.push_back(ls_bits);
+  if (sg.exec && key == sg.key) {                            // replay
+    if (cudaGraphLaunch(sg.exec, c->L.stream) != cudaSuccess) { cudaGetLastError(); return fail(c, PIGAN_ERR_CUDA, "cudaGraphLaunch failed"); }
+    c->L.count += sg.launches;
+    return PIGAN_OK;
   }
+  if (key != sg.last_key) {                                  // first sight of these arguments: run eagerly (also sets kernel attributes)
+    sg.last_key = key;
+    return run();
+  }
+  // second consecutive call with the same arguments: capture on the private stream, then replay on the caller's
+  if (sg.exec) { cudaGraphExecDestroy(sg.exec); sg.exec = nullptr; sg.key.clear(); }
+  if (!sg.cap_stream && cudaStreamCreateWithFlags(&sg.cap_stream, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); sg.disabled = true; return run(); }
+  cudaStream_t user = c->L.stream;
+  const unsigned long long count0 = c->L.count;
+  if (cudaStreamBeginCapture(sg.cap_stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { cudaGetLastError(); sg.disabled = true; return run(); }
+  c->L.stream = sg.cap_stream;
+  const pigan_status st = run();
+  c->L.stream = user;
+  cudaGraph_t graph = nullptr;
+  const cudaError_t e = cudaStreamEndCapture(sg.cap_stream, &graph);
+  const unsigned long long n_launch = c->L.count - count0;
+  c->L.count = count0;
+  if (st != PIGAN_OK || e != cudaSuccess || !graph || cudaGraphInstantiate(&sg.exec, graph, 0) != cudaSuccess) {
+    cudaGetLastError();
+    if (graph) cudaGraphDestroy(graph);
+    sg.exec = nullptr; sg.disabled = true;                   // capture is not possible here: stay eager for the life of the context
+    return run();
+  }
+  cudaGraphDestroy(graph);
+  sg.key = key; sg.launches = n_launch;
+  if (cudaGraphLaunch(sg.exec, user) != cudaSuccess) { cudaGetLastError(); return fail(c, PIGAN_ERR_CUDA, "cudaGraphLaunch failed"); }
+  c->L.count += sg.launches;
+  return PIGAN_OK;
 }
 
 pigan_status pigan_adam_update(pigan_ctx* c, float* params, const float* grads, float* m, float* v, size_t n, int step, float lr, float beta1,
