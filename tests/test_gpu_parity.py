@@ -244,3 +244,39 @@ def test_full_size_step_is_the_mean_of_its_half_batches(name):
             assert rel_err(fa[key], av[key]) <= 1e-3, (name, nm, key, rel_err(fa[key], av[key]))
     mean = 0.5 * (a[3] + b[3])
     assert np.all(np.abs(full[3] - mean) <= 1e-3 * np.maximum(np.abs(mean), 1e-6)), (full[3], mean)
+
+
+@pytest.mark.parametrize("name", ["c1", "c2"])
+def test_graph_replay_matches_eager_and_sees_in_place_updates(name):
+    """Calls 1 (eager), 2 (capture + launch) and 3 (replay) of pigan_train_step_grads with the same arguments agree, and a
+    replay after the inputs were modified IN PLACE (what an optimiser step does) equals an eager run on those values."""
+    import torch
+    from paper_1910_13444_b200 import PiGan
+    cfg = wl.CONFIGS[name] if name == "c1" else dataclasses.replace(wl.CONFIGS["c2"], name="c2-graph", N=8, G=16, S=32)
+    inp = wl.make_inputs(cfg, bias_std=0.1)
+    inp["real"] = np.random.default_rng(5).normal(size=(cfg.N, 2 * cfg.S)).astype(np.float32)
+    d = to_dev(inp, "cuda:0")
+    tol = 1e-5 if cfg.precision == "fp32" else 2e-3       # summation order only (atomics)
+
+    def call(pg, out=None):
+        o = pg.train_step_grads(d["theta_Y"], d["theta_u"], d["theta_D"], d["xy_colloc"], d["f"], d["xy_sensors"], d["z"], d["real"], d["eps"], 1.0, out=out)
+        torch.cuda.synchronize()
+        return o
+
+    pg = PiGan.from_config(cfg)
+    out = call(pg)
+    first = [t.clone() for t in out]
+    n1 = pg.launch_count
+    for _ in range(2):
+        call(pg, out)                                      # same argument pointers: capture, then replay
+    assert pg.launch_count == 3 * n1                       # replays are counted as the launches they contain
+    for a, b in zip(first[:4], out[:4]):
+        assert rel_err(b.cpu().numpy(), a.cpu().numpy()) <= tol
+    d["z"].mul_(0.5); d["theta_u"].mul_(1.01)
+    call(pg, out)                                          # replay on the updated values
+    pg2 = PiGan.from_config(cfg)
+    ref = call(pg2)                                        # eager, fresh context
+    for a, b in zip(ref[:4], out[:4]):
+        assert rel_err(b.cpu().numpy(), a.cpu().numpy()) <= tol
+    assert rel_err(out[0].cpu().numpy(), first[0].cpu().numpy()) > 10 * tol      # and the update did change the result
+    pg.close(); pg2.close()
