@@ -41,6 +41,8 @@ struct Jet2Params {
   int n_row_tiles;       // R / 64
   const float* bias;     // MODE 0, 2: b_l
   float* g_bias;         // MODE 1: b_hat_{l-1}
+  void* out;             // MODE 0, 2: h_out planes; MODE 1: ahat_out planes  [C][H][R_ld] 16-bit
+  int R_ld;              // leading dimension (rows) of the output planes
   const float* amax;     // MODE 1, 3: block-scale source of the adjoint planes
   // MODE 3 (dgrad of layer 2 + adjoint of the FIRST tanh layer + first-layer reduction, O4 'First layer'): ahat^1 is
   // consumed in registers and never written.  Requires npts % 64 == 0 (a row tile lies inside one latent sample).
@@ -71,7 +73,8 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
   uint64_t* tfull = empty + Cfg::kNumStages;               // [kNumBuf]     per CTA
   uint64_t* tempty = tfull + Cfg::kNumBuf;                 // [kNumBuf]     leader's is used, 16 arrivals
   uint64_t* sbar = tempty + Cfg::kNumBuf;                  // [8]           staging loads (MODE 1), one per epilogue warp
-  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(sbar + k2EpiWarps);
+  uint64_t* tempty0 = sbar + k2EpiWarps;                   // [2]  C = 5: group-0 columns of tile it (parity it & 1) fully read, 16 arrivals
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(tempty0 + 2);
 
   const int warp = uniform_warp_idx(), lane = threadIdx.x & 31;
   const uint32_t rank = cluster_ctarank();
@@ -88,6 +91,7 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
     for (int i = 0; i < Cfg::kNumStages; ++i) { mbar_init(full + i, 1); mbar_init(empty + i, 1); }
     for (int i = 0; i < Cfg::kNumBuf; ++i) { mbar_init(tfull + i, 1); mbar_init(tempty + i, 2 * k2EpiWarps); }
     for (int i = 0; i < k2EpiWarps; ++i) mbar_init(sbar + i, 1);
+    for (int i = 0; i < 2; ++i) mbar_init(tempty0 + i, 2 * k2EpiWarps);
     fence_barrier_init();
   }
   if (warp == 2) tmem2_alloc(tmem_slot, Cfg::kTmemCols);
@@ -147,13 +151,67 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
 #ifdef PIGAN_PROBE_TIMING
         tm0 = clock64();
 #endif
-        mbar_wait_cluster(tempty + buf, bphase ^ 1);         // both CTAs' epilogues have released what this tile overwrites
+        // C <= 3: the accumulator is double-buffered.  C = 5 (320 of 512 columns): group 0 (value, x, y) alternates between
+        // two placements and group 1 (xx, yy) has one, which the epilogue of the previous tile releases as soon as it has
+        // pulled it into registers.  That release arrives ~700 clk after the previous tile's last MMA, so the first kDefer
+        // k-blocks of a tile issue only their group-0 MMAs (whose columns the epilogue of tile it-2 freed long ago,
+        // tempty0), and their group-1 MMAs follow once the release is in; their smem stages are freed after that.
+        constexpr int kDefer = C == 5 ? 2 : 0;
+        if (C == 5) mbar_wait_cluster(tempty0 + (it & 1), (uint32_t)(((it >> 1) & 1) ^ 1));
+        else mbar_wait_cluster(tempty + buf, bphase ^ 1);    // both CTAs' epilogues have released what this tile overwrites
         tc_fence_after();
 #ifdef PIGAN_PROBE_TIMING
         tm_te += clock64() - tm0;
 #endif
         const uint32_t d0 = tmem_base + g0_col(it), d1 = tmem_base + g1_col;
-        for (int kb = 0; kb < n_kb; ++kb) {
+        if (C == 5) {
+          int dstage[kDefer > 0 ? kDefer : 1];
+#pragma unroll
+          for (int kb = 0; kb < kDefer; ++kb) {
+#ifdef PIGAN_PROBE_TIMING
+            tm0 = clock64();
+#endif
+            if (!ready) mbar_wait(full + stage, phase);
+            ready = false;
+            tc_fence_after();
+#ifdef PIGAN_PROBE_TIMING
+            tm_full += clock64() - tm0;
+#endif
+            const uint32_t sA = smem_u32(stages + stage * Cfg::kStageBytes), sB = sA + k2AStage;
+#ifndef PIGAN_PROBE_NOMMA
+            if (elect_one()) {
+#pragma unroll
+              for (int k = 0; k < 4; ++k)
+                tc2_mma(d0, umma_desc_sw128(sA + k * 32, 16, 1024), umma_desc_sw64(sB + k * 1024, k2BPlane, 512), idesc0, (kb | k) ? 1u : 0u);
+            }
+            __syncwarp();
+#endif
+            dstage[kb] = stage;
+            if (++stage == Cfg::kNumStages) { stage = 0; phase ^= 1; }
+          }
+#ifdef PIGAN_PROBE_TIMING
+          tm0 = clock64();
+#endif
+          mbar_wait_cluster(tempty + buf, bphase ^ 1);       // group 1 of the previous tile is in the epilogue's registers
+          tc_fence_after();
+#ifdef PIGAN_PROBE_TIMING
+          tm_te += clock64() - tm0;
+#endif
+#pragma unroll
+          for (int kb = 0; kb < kDefer; ++kb) {
+            const uint32_t sA = smem_u32(stages + dstage[kb] * Cfg::kStageBytes), sB = sA + k2AStage;
+            if (elect_one()) {
+#ifndef PIGAN_PROBE_NOMMA
+#pragma unroll
+              for (int k = 0; k < 4; ++k)
+                tc2_mma(d1, umma_desc_sw128(sA + k * 32, 16, 1024), umma_desc_sw64(sB + 3 * k2BPlane + k * 1024, k2BPlane, 512), idesc1, (kb | k) ? 1u : 0u);
+#endif
+              tc2_commit(empty + dstage[kb]);
+            }
+            __syncwarp();
+          }
+        }
+        for (int kb = kDefer; kb < n_kb; ++kb) {
 #ifdef PIGAN_PROBE_TIMING
           tm0 = clock64();
 #endif
@@ -214,6 +272,32 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
       auto tcol = [&](int c) -> uint32_t { return (C == 5 && c >= 3) ? tb1 + (c - 3) * 32 : tb0 + c * 32; };
       float bias = 0.f, bias_acc = 0.f;
       if (MODE == 0 || MODE == 2) bias = p.bias[unit];
+      // Staged planes -> global with the epilogue warp's own 16-byte stores (4 lanes cover the 64 contiguous bytes of one
+      // unit's 32 rows).  Measured: a TMA store drains shared memory at ~26 B/clk per SM whatever the box shape, and the
+      // TMA unit serves loads and stores one after the other, so storing a C = 5 tile through it cost the operand
+      // pipeline ~2.6 k of the tile's ~14 k clk.
+      auto copy_out = [&](int nplanes) {
+        __syncwarp();
+        T* gout = reinterpret_cast<T*>(p.out);
+        const int ch = lane & 3, ul = lane >> 2;
+#pragma unroll
+        for (int c = 0; c < 5; ++c) {
+          if (c < nplanes) {
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+              const int u = j * 8 + ul;
+              const uint4 v = *reinterpret_cast<const uint4*>(stg + c * k2StgPlane + u * 64 + ((ch ^ ((u >> 1) & 3)) << 4));
+              *reinterpret_cast<uint4*>(gout + ((size_t)c * p.H + unit0 + u) * p.R_ld + row0 + ch * 8) = v;
+            }
+          }
+        }
+        __syncwarp();                                        // the staging rows are rewritten by other lanes in the next tile
+      };
+      auto release0 = [&]() {                                // C = 5: this warp has read all of group 0 of this tile
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive_cluster(mapa_u32(tempty0 + (it & 1), 0));
+      };
       auto release = [&]() {                                 // this warp no longer reads what the next MMAs overwrite
         tc_fence_before();
         __syncwarp();
@@ -221,7 +305,7 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
       };
 
       if ((MODE == 1 || MODE == 3) && elect_one()) {         // the previous layer's output jet h^{l-1} -> staging
-        tma_wait_read_all();                                 // earlier stores have finished reading the staging buffer
+        fence_proxy_async();                                 // the lanes' reads / writes of the staging planes (ordered by __syncwarp) precede the TMA fill
         mbar_expect_tx(sbar + e, C * k2StgPlane);
         for (int c = 0; c < C; ++c) tma_load_3d(stg + c * k2StgPlane, &tmT, sbar + e, row0, unit0, c);
       }
@@ -236,6 +320,7 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
 #ifdef PIGAN_PROBE_NOEPI
       if (MODE == 1 || MODE == 3) { mbar_wait(sbar + e, sphase); sphase ^= 1; }
       release();
+      if (C == 5) release0();
       continue;
 #endif
 
@@ -253,8 +338,6 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
 
       if (MODE == 0) {
         // ---- h_c = tanh-jet(a_c) ----
-        if (elect_one()) tma_wait_read_all();
-        __syncwarp();
 #pragma unroll
         for (int rc = 0; rc < 4; ++rc) {
           float v[C][8], o[C][8];
@@ -276,17 +359,10 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
 #pragma unroll
           for (int c = 0; c < C; ++c) *reinterpret_cast<uint4*>(my_row + c * k2StgPlane + off) = pack8<T>(o[c]);
         }
-        if (C != 5) release();
-        fence_proxy_async();
-        __syncwarp();
-        if (elect_one()) {
-          for (int c = 0; c < C; ++c) tma_store_3d(&tmO, stg + c * k2StgPlane, row0, unit0, c);
-          tma_commit_group();
-        }
+        if (C != 5) release(); else release0();
+        copy_out(C);
       } else if (MODE == 2) {
         // ---- value-only layer with split activations: a = W (h_hi + h_lo) + b; t = tanh a; t_hi = rn16(t), t_lo = rn16(t - t_hi) ----
-        if (elect_one()) tma_wait_read_all();
-        __syncwarp();
 #pragma unroll 1
         for (int rc = 0; rc < 4; ++rc) {
           float v0[8], v1[8], hi[8], lo[8];
@@ -304,13 +380,7 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
           *reinterpret_cast<uint4*>(my_row + k2StgPlane + off) = pack8<T>(lo);
         }
         release();
-        fence_proxy_async();
-        __syncwarp();
-        if (elect_one()) {
-          tma_store_3d(&tmO, stg, row0, unit0, 0);
-          tma_store_3d(&tmO, stg + k2StgPlane, row0, unit0, 1);
-          tma_commit_group();
-        }
+        copy_out(2);
       } else {
         // ---- adjoint of the previous layer's tanh: ahat^{l-1} = J^T hhat^{l-1} ----
         mbar_wait(sbar + e, sphase); sphase ^= 1;
@@ -349,14 +419,11 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
             for (int c = 0; c < C; ++c) *reinterpret_cast<uint4*>(my_row + c * k2StgPlane + off) = pack8<T>(o[c]);
           }
         }
-        if (C != 5) release();
+        if (C != 5) release(); else release0();
         if (MODE == 1) {
-          fence_proxy_async();
+          copy_out(C);
+          fence_proxy_async();                               // generic-proxy accesses of the staging planes before the next tile's TMA fill
           __syncwarp();
-          if (elect_one()) {
-            for (int c = 0; c < C; ++c) tma_store_3d(&tmO, stg + c * k2StgPlane, row0, unit0, c);
-            tma_commit_group();
-          }
         } else {
           __syncwarp();                                      // every lane is done reading the staging planes before the next loads land
           const float inv = adj_inv_scale(p.amax);
@@ -370,8 +437,6 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
 #ifdef PIGAN_PROBE_TIMING
     if (blockIdx.x == 0 && e == 0 && lane == 0) printf("TIMING epi C=%d MODE=%d tiles=%d total=%lld wait_tfull=%lld early_release=%lld\n", C, MODE, it, clock64() - te_start, te_tf, te_rel);
 #endif
-    __syncwarp();
-    if (elect_one()) tma_wait_all();                         // global writes of the last stores are complete before exit
   }
   tc_fence_before();
   __syncthreads();
@@ -548,7 +613,7 @@ void tc2_layer_fwd(Launcher& L, int precision, int C, int H, int R, int R_ld, co
             plane_map(L, &o, precision, h_out, H, R_ld, C, 32, 32, 1, CU_TENSOR_MAP_SWIZZLE_64B);
   if (!ok) return;
   Jet2Params p{};
-  p.H = H; p.n_row_tiles = R / 64; p.bias = bias;
+  p.H = H; p.n_row_tiles = R / 64; p.bias = bias; p.out = h_out; p.R_ld = R_ld;
   dispatch_jet2<0>(L, C, a, b, o, o, p);
 }
 
@@ -558,7 +623,7 @@ void tc2_layer_fwd_split(Launcher& L, int precision, int H, int R, int R_ld, con
         plane_map(L, &o, precision, h_out, H, R_ld, 2, 32, 32, 1, CU_TENSOR_MAP_SWIZZLE_64B)))
     return;
   Jet2Params p{};
-  p.H = H; p.n_row_tiles = R / 64; p.bias = bias;
+  p.H = H; p.n_row_tiles = R / 64; p.bias = bias; p.out = h_out; p.R_ld = R_ld;
   launch_jet2<__half, 2, 2>(L, a, b, o, o, p);
 }
 
@@ -570,7 +635,7 @@ void tc2_layer_bwd(Launcher& L, int precision, int C, int H, int R, int R_ld, co
             plane_map(L, &t, precision, h_prev, H, R_ld, C, 32, 32, 1, CU_TENSOR_MAP_SWIZZLE_64B);
   if (!ok) return;
   Jet2Params p{};
-  p.H = H; p.n_row_tiles = R / 64; p.g_bias = g_bias_prev; p.amax = amax;
+  p.H = H; p.n_row_tiles = R / 64; p.g_bias = g_bias_prev; p.amax = amax; p.out = ahat_out; p.R_ld = R_ld;
   if (fl) {
     p.xy = fl->xy; p.row0 = fl->row0; p.npts = fl->npts; p.in_dim = fl->in_dim; p.gW1 = fl->gW1; p.An = fl->An;
     dispatch_jet2<3>(L, C, a, b, o, t, p);
