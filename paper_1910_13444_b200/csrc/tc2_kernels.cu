@@ -286,7 +286,7 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
               const int u = j * 8 + ul;
-              const uint4 v = *reinterpret_cast<const uint4*>(stg + c * k2StgPlane + u * 64 + ((ch ^ ((u >> 1) & 3)) << 4));
+              const uint4 v = lds128(stg + c * k2StgPlane + u * 64 + ((ch ^ ((u >> 1) & 3)) << 4));
               *reinterpret_cast<uint4*>(gout + ((size_t)c * p.H + unit0 + u) * p.R_ld + row0 + ch * 8) = v;
             }
           }
@@ -357,7 +357,7 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
           }
           const uint32_t off = ((uint32_t)rc ^ swz) << 4;
 #pragma unroll
-          for (int c = 0; c < C; ++c) *reinterpret_cast<uint4*>(my_row + c * k2StgPlane + off) = pack8<T>(o[c]);
+          for (int c = 0; c < C; ++c) sts128(my_row + c * k2StgPlane + off, pack8<T>(o[c]));
         }
         if (C != 5) release(); else release0();
         copy_out(C);
@@ -376,8 +376,8 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
             lo[i] = tt - hi[i];
           }
           const uint32_t off = ((uint32_t)rc ^ swz) << 4;
-          *reinterpret_cast<uint4*>(my_row + off) = pack8<T>(hi);
-          *reinterpret_cast<uint4*>(my_row + k2StgPlane + off) = pack8<T>(lo);
+          sts128(my_row + off, pack8<T>(hi));
+          sts128(my_row + k2StgPlane + off, pack8<T>(lo));
         }
         release();
         copy_out(2);
@@ -394,7 +394,7 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
           for (int c = 0; c < nc0; ++c) tmem_ld8(tcol(c) + rc * 8, hh[c]);
           const uint32_t off = ((uint32_t)rc ^ swz) << 4;
 #pragma unroll
-          for (int c = 0; c < C; ++c) unpack8<T>(*reinterpret_cast<const uint4*>(my_row + c * k2StgPlane + off), hp[c]);
+          for (int c = 0; c < C; ++c) unpack8<T>(lds128(my_row + c * k2StgPlane + off), hp[c]);
           tmem_ld_wait();
 #pragma unroll
           for (int i = 0; i < 8; ++i) {
@@ -416,7 +416,7 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
           }
           if (MODE == 1) {
 #pragma unroll
-            for (int c = 0; c < C; ++c) *reinterpret_cast<uint4*>(my_row + c * k2StgPlane + off) = pack8<T>(o[c]);
+            for (int c = 0; c < C; ++c) sts128(my_row + c * k2StgPlane + off, pack8<T>(o[c]));
           }
         }
         if (C != 5) release(); else release0();
