@@ -29,7 +29,7 @@ METRIC = "PI-GAN train-step sample*collocation-points/s"
 UNIT = "sample*collocation-points/s"
 ADAM = dict(lr=1e-4, beta1=0.5, beta2=0.9, adam_eps=1e-8)          # reading G3
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the largest tensor-core kernel (G_u forward, 131072-row chunk),
-# from profiles/r01b_ncu_full_tc_kernels_c5.csv (1.345e9 read + 1.306e9 written); algorithmic bytes of that launch: 2.684e9
+# from profiles/r01c_ncu_full_tc_kernels_c5.csv (1.345e9 read + 1.306e9 written); algorithmic bytes of that launch: 2.684e9
 TRAFFIC = {"c5": 2.651e9}
 
 
