@@ -258,6 +258,7 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
     const uint32_t lane_base = tmem_base + ((uint32_t)(q * 32) << 16);
     uint32_t sphase = 0;
     int it = 0;
+    const float inv_amax = (MODE == 1 || MODE == 3) ? adj_inv_scale(p.amax) : 1.f;   // constant over the launch: one global load, not one per tile
 #ifdef PIGAN_PROBE_TIMING
     long long te_start = clock64(), te_tf = 0, te_rel = 0, te0;
 #endif
@@ -305,7 +306,9 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
       };
 
       if ((MODE == 1 || MODE == 3) && elect_one()) {         // the previous layer's output jet h^{l-1} -> staging
-        fence_proxy_async();                                 // the lanes' reads / writes of the staging planes (ordered by __syncwarp) precede the TMA fill
+        // No fence.proxy.async: every generic-proxy access of the staging planes was a read, or a write that the copy-out
+        // of this warp has read back, all ordered before this point by __syncwarp; the fence would also wait for the
+        // copy-out's global stores to be acknowledged (measured as long-scoreboard stalls on it).
         mbar_expect_tx(sbar + e, C * k2StgPlane);
         for (int c = 0; c < C; ++c) tma_load_3d(stg + c * k2StgPlane, &tmT, sbar + e, row0, unit0, c);
       }
@@ -422,16 +425,14 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
         if (C != 5) release(); else release0();
         if (MODE == 1) {
           copy_out(C);
-          fence_proxy_async();                               // generic-proxy accesses of the staging planes before the next tile's TMA fill
-          __syncwarp();
         } else {
           __syncwarp();                                      // every lane is done reading the staging planes before the next loads land
-          const float inv = adj_inv_scale(p.amax);
+          const float inv = inv_amax;
           atomicAdd(p.An + (size_t)(grow / p.npts) * p.H + unit, bias_acc * inv);
           atomicAdd(p.gW1 + (size_t)unit * p.in_dim, sx * inv);
           atomicAdd(p.gW1 + (size_t)unit * p.in_dim + 1, sy * inv);
         }
-        atomicAdd(p.g_bias + unit, bias_acc * adj_inv_scale(p.amax));
+        atomicAdd(p.g_bias + unit, bias_acc * inv_amax);
       }
     }
 #ifdef PIGAN_PROBE_TIMING
