@@ -296,7 +296,9 @@ def summarize(cfg, res, n_gpus, steps, warmup, t_max_ms):
     e2e_ms = float(np.mean(res["ms_e2e"]))
     return {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": n_gpus, "steps": steps, "warmup": warmup, "ms_per_step": t_max_ms,
-        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": cfg.precision, "data": "synthetic",
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        # the arithmetic type of the tensor-core operands: both 16-bit modes compute with fp16 operands and fp32 accumulation (R1)
+        "dtype": "fp32" if cfg.precision == "fp32" else "fp16", "precision_mode": cfg.precision, "data": "synthetic",
         "config": {"workload": f"{cfg.name}: {cfg.L}x{cfg.H} tanh generators (m={cfg.m}), {cfg.G}x{cfg.G} grid x {cfg.N} samples, {cfg.S} sensors, "
                                f"critic {cfg.LD}x{cfg.HD}", "rows_per_step": units, "parallelism": f"replicas x{n_gpus}" if n_gpus > 1 else "single GPU",
                    "l2": "per-step working set >> L2" if cfg.N * cfg.P >= 400000 else "256 MiB L2 flush between timed steps",
@@ -317,13 +319,15 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", default="c5", choices=list(wl.CONFIGS))
     ap.add_argument("--impl", default="pigan", choices=["pigan", "reference"])
-    ap.add_argument("--all-configs", action="store_true", help="also run c1..c4 briefly and attach them as per_config")
+    ap.add_argument("--all-configs", action="store_true", default=True, help="also run the other configs briefly and attach them as per_config (default)")
+    ap.add_argument("--headline-only", dest="all_configs", action="store_false", help="time only --config")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--samples", type=int, default=None, help="override N (latent samples per step): a smaller job for ncu captures; "
                     "the line then says so in config.workload and is not a benchmark value")
     args = ap.parse_args()
     cfg = wl.CONFIGS[args.config]
     if args.samples:
+        args.all_configs = False
         cfg = dataclasses.replace(cfg, name=f"{cfg.name}[N={args.samples} profiling subset]", N=args.samples)
     rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))

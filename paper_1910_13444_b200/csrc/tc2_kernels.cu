@@ -59,7 +59,6 @@ template <typename T, int C, int MODE>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(k2Threads, 1)
 jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H] 16-bit, box 64 x 128, SW128
                   const __grid_constant__ CUtensorMap tmB,      // input planes, box 32 rows x 64 units x C, SW64
-                  const __grid_constant__ CUtensorMap tmO,      // MODE 0, 2: h_out; MODE 1: ahat_out (box 32 x 32 x 1, SW64)
                   const __grid_constant__ CUtensorMap tmT,      // MODE 1: h_prev planes in (box 32 x 32 x 1, SW64)
                   Jet2Params p) {
   using Cfg = Jet2Cfg<C, MODE>;
@@ -84,7 +83,7 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
   const int n_kb = p.H / 64;
 
   if (warp == 0 && lane == 0) {
-    prefetch_tmap(&tmA); prefetch_tmap(&tmB); prefetch_tmap(&tmO);
+    prefetch_tmap(&tmA); prefetch_tmap(&tmB);
     if (MODE == 1 || MODE == 3) prefetch_tmap(&tmT);
   }
   if (warp == 1 && lane == 0) {
@@ -588,7 +587,7 @@ bool tc2_supported(int H) {
 }
 
 template <typename T, int C, int MODE>
-static void launch_jet2(Launcher& L, const CUtensorMap& a, const CUtensorMap& b, const CUtensorMap& o, const CUtensorMap& t,
+static void launch_jet2(Launcher& L, const CUtensorMap& a, const CUtensorMap& b, const CUtensorMap& t,
                         const Jet2Params& p) {
   using Cfg = Jet2Cfg<C, MODE>;
   static bool attr_set = false;
@@ -596,53 +595,49 @@ static void launch_jet2(Launcher& L, const CUtensorMap& a, const CUtensorMap& b,
   if (!attr_set) { cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::kSmemBytes); attr_set = true; }
   const int tiles = (p.H / 256) * p.n_row_tiles;
   const int clusters = std::min(tiles, num_sms() / 2);
-  kern<<<2 * clusters, k2Threads, Cfg::kSmemBytes, L.stream>>>(a, b, o, t, p);
+  kern<<<2 * clusters, k2Threads, Cfg::kSmemBytes, L.stream>>>(a, b, t, p);
   L.check(MODE == 0 ? "jet_layer_fwd" : MODE == 2 ? "jet_layer_fwd_split" : "jet_layer_bwd");
 }
 
 template <int MODE>
-static void dispatch_jet2(Launcher& L, int C, const CUtensorMap& a, const CUtensorMap& b, const CUtensorMap& o, const CUtensorMap& t,
+static void dispatch_jet2(Launcher& L, int C, const CUtensorMap& a, const CUtensorMap& b, const CUtensorMap& t,
                           const Jet2Params& p) {
-  if (C == 1) launch_jet2<__half, 1, MODE>(L, a, b, o, t, p);
-  else if (C == 3) launch_jet2<__half, 3, MODE>(L, a, b, o, t, p);
-  else launch_jet2<__half, 5, MODE>(L, a, b, o, t, p);
+  if (C == 1) launch_jet2<__half, 1, MODE>(L, a, b, t, p);
+  else if (C == 3) launch_jet2<__half, 3, MODE>(L, a, b, t, p);
+  else launch_jet2<__half, 5, MODE>(L, a, b, t, p);
 }
 
 void tc2_layer_fwd(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* w16_l, const float* bias, const void* h_in, void* h_out) {
-  CUtensorMap a, b, o;
-  bool ok = weight_map(L, &a, precision, w16_l, H) && plane_map(L, &b, precision, h_in, H, R_ld, C, 32, 64, C, CU_TENSOR_MAP_SWIZZLE_64B) &&
-            plane_map(L, &o, precision, h_out, H, R_ld, C, 32, 32, 1, CU_TENSOR_MAP_SWIZZLE_64B);
+  CUtensorMap a, b;
+  bool ok = weight_map(L, &a, precision, w16_l, H) && plane_map(L, &b, precision, h_in, H, R_ld, C, 32, 64, C, CU_TENSOR_MAP_SWIZZLE_64B);
   if (!ok) return;
   Jet2Params p{};
   p.H = H; p.n_row_tiles = R / 64; p.bias = bias; p.out = h_out; p.R_ld = R_ld;
-  dispatch_jet2<0>(L, C, a, b, o, o, p);
+  dispatch_jet2<0>(L, C, a, b, b, p);
 }
 
 void tc2_layer_fwd_split(Launcher& L, int precision, int H, int R, int R_ld, const void* w16_l, const float* bias, const void* h_in, void* h_out) {
-  CUtensorMap a, b, o;
-  if (!(weight_map(L, &a, precision, w16_l, H) && plane_map(L, &b, precision, h_in, H, R_ld, 2, 32, 64, 2, CU_TENSOR_MAP_SWIZZLE_64B) &&
-        plane_map(L, &o, precision, h_out, H, R_ld, 2, 32, 32, 1, CU_TENSOR_MAP_SWIZZLE_64B)))
-    return;
+  CUtensorMap a, b;
+  if (!(weight_map(L, &a, precision, w16_l, H) && plane_map(L, &b, precision, h_in, H, R_ld, 2, 32, 64, 2, CU_TENSOR_MAP_SWIZZLE_64B))) return;
   Jet2Params p{};
   p.H = H; p.n_row_tiles = R / 64; p.bias = bias; p.out = h_out; p.R_ld = R_ld;
-  launch_jet2<__half, 2, 2>(L, a, b, o, o, p);
+  launch_jet2<__half, 2, 2>(L, a, b, b, p);
 }
 
 void tc2_layer_bwd(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* w16T_l, const void* ahat_in, const void* h_prev,
                    void* ahat_out, float* g_bias_prev, const float* amax, const FirstLayerFuse* fl) {
-  CUtensorMap a, b, o, t;
+  CUtensorMap a, b, t;
   bool ok = weight_map(L, &a, precision, w16T_l, H) && plane_map(L, &b, precision, ahat_in, H, R_ld, C, 32, 64, C, CU_TENSOR_MAP_SWIZZLE_64B) &&
-            plane_map(L, &o, precision, ahat_out, H, R_ld, C, 32, 32, 1, CU_TENSOR_MAP_SWIZZLE_64B) &&
             plane_map(L, &t, precision, h_prev, H, R_ld, C, 32, 32, 1, CU_TENSOR_MAP_SWIZZLE_64B);
   if (!ok) return;
   Jet2Params p{};
   p.H = H; p.n_row_tiles = R / 64; p.g_bias = g_bias_prev; p.amax = amax; p.out = ahat_out; p.R_ld = R_ld;
   if (fl) {
     p.xy = fl->xy; p.row0 = fl->row0; p.npts = fl->npts; p.in_dim = fl->in_dim; p.gW1 = fl->gW1; p.An = fl->An;
-    dispatch_jet2<3>(L, C, a, b, o, t, p);
+    dispatch_jet2<3>(L, C, a, b, t, p);
     return;
   }
-  dispatch_jet2<1>(L, C, a, b, o, t, p);
+  dispatch_jet2<1>(L, C, a, b, t, p);
 }
 
 void tc2_wgrad(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* ahat, const void* h_prev, float* gW, const float* amax) {
@@ -650,7 +645,11 @@ void tc2_wgrad(Launcher& L, int precision, int C, int H, int R, int R_ld, const 
   p.H = H; p.C = C; p.R = R; p.gW = gW; p.amax = amax;
   const int n_tiles = (H / 256) * (H / 256);
   const int n_cl = num_sms() / 2;
-  int slices = std::max(1, (2 * n_cl) / n_tiles);
+  // row slices: one work item per CTA (pair) when that fills >= 90 % of the machine, else two; every extra slice costs one
+  // more fp32 red.add pass over the H x H gradient (measured on c2 / c3: 1 slice per CTA is 10 % faster than 2)
+  const int units = n_cl;
+  int slices = std::max(1, units / n_tiles);
+  if (n_tiles * slices * 10 < units * 9) slices = std::max(1, (2 * units) / n_tiles);
   int slice_rows = ((R + slices - 1) / slices + 63) / 64 * 64;
   if (slice_rows < 64) slice_rows = 64;
   p.slice_rows = slice_rows; p.n_slices = (R + slice_rows - 1) / slice_rows;

@@ -504,7 +504,11 @@ void tc_wgrad(Launcher& L, int precision, int C, int H, int R, int R_ld, const v
   WgradParams p{};
   p.H = H; p.C = C; p.NW = std::min(H, 256); p.R = R; p.gW = gW; p.amax = amax;
   const int n_tiles = (H / kBM) * (H / p.NW);
-  int slices = std::max(1, (2 * num_sms()) / n_tiles);
+  // row slices: one work item per CTA (pair) when that fills >= 90 % of the machine, else two; every extra slice costs one
+  // more fp32 red.add pass over the H x H gradient (measured on c2 / c3: 1 slice per CTA is 10 % faster than 2)
+  const int units = num_sms();
+  int slices = std::max(1, units / n_tiles);
+  if (n_tiles * slices * 10 < units * 9) slices = std::max(1, (2 * units) / n_tiles);
   int slice_rows = ((R + slices - 1) / slices + 63) / 64 * 64;
   if (slice_rows < 64) slice_rows = 64;
   p.slice_rows = slice_rows; p.n_slices = (R + slice_rows - 1) / slice_rows;
