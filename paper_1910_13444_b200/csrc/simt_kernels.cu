@@ -9,17 +9,21 @@ namespace pigan {
 static inline int cdiv(long long a, long long b) { return (int)((a + b - 1) / b); }
 
 // =============================================================================================================
-// generic batched SGEMM (64x64x16 tiles, 4x4 micro-tiles); used by fp32 mode and by the critic
+// generic batched SGEMM (64x64x32 tiles, 4x4 micro-tiles, register prefetch); used by fp32 mode and by the critic
 // =============================================================================================================
 template <bool TA, bool TB>
 __global__ void __launch_bounds__(256) sgemm_kernel(int M, int N, int K, const float* __restrict__ A, int lda, long long sA,
                                                     const float* __restrict__ B, int ldb, long long sB, float* __restrict__ C,
                                                     int ldc, long long sC, int ksplit, int atomic, float alpha) {
-  __shared__ float As[16][68];
-  __shared__ float Bs[16][68];
+  // 64 x 64 output tile, 32-deep k-steps; the global loads of step k+1 are issued into registers before step k is
+  // multiplied, so their latency overlaps the FMAs (the critic's GEMMs are a handful of CTAs with 4-13 k-steps each:
+  // latency, not throughput, is what they cost).
+  constexpr int BK = 32;
+  __shared__ float As[BK][68];
+  __shared__ float Bs[BK][68];
   const int batch = blockIdx.z / ksplit, ks = blockIdx.z % ksplit;
   A += (long long)batch * sA; B += (long long)batch * sB; C += (long long)batch * sC;
-  int kchunk = (K + ksplit - 1) / ksplit; kchunk = (kchunk + 15) / 16 * 16;
+  int kchunk = (K + ksplit - 1) / ksplit; kchunk = (kchunk + BK - 1) / BK * BK;
   const int k0 = ks * kchunk, k1 = min(K, k0 + kchunk);
   const int m0 = blockIdx.y * 64, n0 = blockIdx.x * 64;
   const int tid = threadIdx.x, tx = tid % 16, ty = tid / 16;
@@ -28,24 +32,38 @@ __global__ void __launch_bounds__(256) sgemm_kernel(int M, int N, int K, const f
   for (int i = 0; i < 4; ++i)
 #pragma unroll
     for (int j = 0; j < 4; ++j) acc[i][j] = 0.f;
-  for (int k = k0; k < k1; k += 16) {
+  float ra[8], rb[8];
+  auto fetch = [&](int k) {                                  // this thread's 8 + 8 elements of the (64 x BK) A and (BK x 64) B tiles
 #pragma unroll
-    for (int i = 0; i < 4; ++i) {
+    for (int i = 0; i < 8; ++i) {
       const int idx = tid + i * 256;
       int m, kk;
-      if (!TA) { m = idx / 16; kk = idx % 16; } else { kk = idx / 64; m = idx % 64; }
+      if (!TA) { m = idx / BK; kk = idx % BK; } else { kk = idx / 64; m = idx % 64; }
       float v = 0.f;
       if (m0 + m < M && k + kk < k1) v = TA ? A[(long long)(k + kk) * lda + m0 + m] : A[(long long)(m0 + m) * lda + k + kk];
-      As[kk][m] = v;
+      ra[i] = v;
       int n;
-      if (!TB) { kk = idx / 64; n = idx % 64; } else { n = idx / 16; kk = idx % 16; }
+      if (!TB) { kk = idx / 64; n = idx % 64; } else { n = idx / BK; kk = idx % BK; }
       v = 0.f;
       if (n0 + n < N && k + kk < k1) v = TB ? B[(long long)(n0 + n) * ldb + k + kk] : B[(long long)(k + kk) * ldb + n0 + n];
-      Bs[kk][n] = v;
+      rb[i] = v;
     }
-    __syncthreads();
+  };
+  auto stash = [&]() {
 #pragma unroll
-    for (int kk = 0; kk < 16; ++kk) {
+    for (int i = 0; i < 8; ++i) {
+      const int idx = tid + i * 256;
+      if (!TA) As[idx % BK][idx / BK] = ra[i]; else As[idx / 64][idx % 64] = ra[i];
+      if (!TB) Bs[idx / 64][idx % 64] = rb[i]; else Bs[idx % BK][idx / BK] = rb[i];
+    }
+  };
+  if (k0 < k1) fetch(k0);
+  for (int k = k0; k < k1; k += BK) {
+    stash();
+    __syncthreads();
+    if (k + BK < k1) fetch(k + BK);
+#pragma unroll
+    for (int kk = 0; kk < BK; ++kk) {
       float a[4], b[4];
 #pragma unroll
       for (int i = 0; i < 4; ++i) a[i] = As[kk][ty * 4 + i];
