@@ -228,12 +228,17 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
             const uint32_t acc = (kb | k) ? 1u : 0u;
             // MN-major SW64: channel planes are 4 KB apart (LBO), 8-unit groups 512 B apart (SBO), 16 units = +1 KB
 #ifndef PIGAN_PROBE_NOMMA
-            if (C == 5 && k < 3 && elect_one()) tc2_mma(d1, ad, umma_desc_sw64(sB + 3 * k2BPlane + k * 1024, k2BPlane, 512), idesc1, acc);
+            // C = 5: the two MMAs of a k-step read the same A slice: the first fills the A collector, the second reuses it
+            if (C == 5 && k < 3 && elect_one()) tc2_mma_a_fill(d1, ad, umma_desc_sw64(sB + 3 * k2BPlane + k * 1024, k2BPlane, 512), idesc1, acc);
             if (C != 5 && k == 3) ready = !(last_tile && kb == n_kb - 1) && __all_sync(0xffffffffu, mbar_try_wait(full + nstage, nphase));
-            if (elect_one()) tc2_mma(d0, ad, umma_desc_sw64(sB + k * 1024, k2BPlane, 512), idesc0, acc);
+            if (elect_one()) {
+              if (C != 5) tc2_mma(d0, ad, umma_desc_sw64(sB + k * 1024, k2BPlane, 512), idesc0, acc);
+              else if (k < 3) tc2_mma_a_lastuse(d0, ad, umma_desc_sw64(sB + k * 1024, k2BPlane, 512), idesc0, acc);
+              else tc2_mma_a_fill(d0, ad, umma_desc_sw64(sB + k * 1024, k2BPlane, 512), idesc0, acc);
+            }
             if (C == 5 && k == 3) {
               ready = !(last_tile && kb == n_kb - 1) && __all_sync(0xffffffffu, mbar_try_wait(full + nstage, nphase));
-              if (elect_one()) tc2_mma(d1, ad, umma_desc_sw64(sB + 3 * k2BPlane + k * 1024, k2BPlane, 512), idesc1, acc);
+              if (elect_one()) tc2_mma_a_lastuse(d1, ad, umma_desc_sw64(sB + 3 * k2BPlane + k * 1024, k2BPlane, 512), idesc1, acc);
             }
 #endif
           }
