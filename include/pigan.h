@@ -114,7 +114,12 @@ pigan_status pigan_gradient_penalty(pigan_ctx* ctx, const float* disc_params, co
  *   xy_colloc [P][2], f [P], xy_sensors [S][2], z [N][m], real_snap [N][2S], eps [N]; sizes from the config.
  *   loss_scale (host value, > 0) multiplies the adjoints of the 16-bit backward pass; gradients are returned
  *   UNSCALED in fp32 (overwritten).  losses[6] = {L_D, mean D(fake), mean D(real), GP, L_G, L_pde}.
- *   *found_inf (device int, overwritten) = 1 if any gradient is inf/nan, else 0.  losses, found_inf may be NULL. */
+ *   *found_inf (device int, overwritten) = 1 if any gradient is inf/nan, else 0.  losses, found_inf may be NULL.
+ *   Execution: asynchronous on the context's stream.  A call whose arguments (all pointers and loss_scale) repeat the
+ *   previous call's is captured into a CUDA graph and replayed on later identical calls; the arrays are read when the
+ *   step RUNS, so updating them in place between calls (an optimiser step, new z / eps copied into the same buffers)
+ *   behaves exactly as an eager call.  Environment: PIGAN_NO_GRAPH=1 disables the replay, PIGAN_CHUNK_ROWS=<n> sets the
+ *   row-chunk size (default 131072 rows; workspace_bytes of the config bounds it as well). */
 pigan_status pigan_train_step_grads(pigan_ctx* ctx, const float* logk_params, const float* u_params,
                                     const float* disc_params, const float* xy_colloc, const float* f,
                                     const float* xy_sensors, const float* z, const float* real_snap,
