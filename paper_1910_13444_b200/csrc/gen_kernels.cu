@@ -367,20 +367,21 @@ __global__ void __launch_bounds__(256) first_layer_bwd_kernel(NetShape s, const 
     load8<T>(ahat + off, a0);
     if (C >= 3) { load8<T>(ahat + plane + off, ax); load8<T>(ahat + 2 * plane + off, ay); }
     int run_n = -1; float run = 0.f;
+    // one 64-bit division per thread; the 8 rows then step through (n, p) incrementally
+    const long long rg0 = g.row0 + r0;
+    int n = (int)(rg0 / g.npts), p = (int)(rg0 - (long long)n * g.npts);
 #pragma unroll
     for (int i = 0; i < 8; ++i) {
       if (r0 + i < g.valid) {
-        const long long rg = g.row0 + r0 + i;
-        const int p = (int)(rg % g.npts);
         const float2 q = *reinterpret_cast<const float2*>(xy + 2 * p);
         sx = fmaf(a0[i], q.x, sx); sy = fmaf(a0[i], q.y, sy);
         if (C >= 3) { sx += ax[i]; sy += ay[i]; }
         if (uniform) sa += a0[i];
         else {
-          const int n = (int)(rg / g.npts);
           if (n != run_n) { if (run_n >= 0) atomicAdd(An + (size_t)run_n * s.H + j, run * inv_sc); run_n = n; run = 0.f; }
           run += a0[i];
         }
+        if (++p == g.npts) { p = 0; ++n; }
       }
     }
     if (!uniform && run_n >= 0) atomicAdd(An + (size_t)run_n * s.H + j, run * inv_sc);

@@ -326,12 +326,22 @@ __global__ void mul_s_kernel(const float* __restrict__ a, const float* __restric
   const size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x;
   if (i < n) { const float gg = g[i]; out[i] = a[i] * (1.f - gg * gg); }
 }
-__global__ void colsum_acc_kernel(const float* __restrict__ A, int rows, int cols, float* __restrict__ out) {
-  const int j = blockIdx.x * blockDim.x + threadIdx.x;
-  if (j >= cols) return;
+// out[j] += sum_n A[n][j]; block = 32 columns x 8 row groups (the batch is a few hundred rows: a serial loop per column was
+// 8 us of dependent-latency per call)
+__global__ void __launch_bounds__(256) colsum_acc_kernel(const float* __restrict__ A, int rows, int cols, float* __restrict__ out) {
+  __shared__ float red[8][33];
+  const int c = threadIdx.x & 31, rg = threadIdx.x >> 5, j = blockIdx.x * 32 + c;
   float s = 0.f;
-  for (int n = 0; n < rows; ++n) s += A[(size_t)n * cols + j];
-  out[j] += s;
+  if (j < cols)
+    for (int n = rg; n < rows; n += 8) s += A[(size_t)n * cols + j];
+  red[rg][c] = s;
+  __syncthreads();
+  if (rg == 0 && j < cols) {
+    float t = 0.f;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) t += red[k][c];
+    out[j] += t;
+  }
 }
 // out[b][j] = seed[b] * w[j]
 __global__ void outer_kernel(const float* __restrict__ seed, const float* __restrict__ w, int rows, int cols, float* __restrict__ out) {
@@ -348,7 +358,7 @@ void critic_backward(Launcher& L, const NetShape& s, const float* theta, const f
   if (grads) {
     // v_hat_out += seed^T g^LD ; c_hat_out += sum seed
     sgemm(L, true, false, 1, HD, rows, seed, 1, 0, gL, HD, 0, grads + s.W_off(LD + 1), HD, 0, 1, true);
-    colsum_acc_kernel<<<1, 32, 0, L.stream>>>(seed, rows, 1, grads + s.b_off(LD + 1));
+    colsum_acc_kernel<<<1, 256, 0, L.stream>>>(seed, rows, 1, grads + s.b_off(LD + 1));
     L.check("colsum_acc");
   }
   float* ghat = t0; float* ahat = t1;
@@ -362,7 +372,7 @@ void critic_backward(Launcher& L, const NetShape& s, const float* theta, const f
     L.check("mul_s");
     if (grads) {
       sgemm(L, true, false, HD, in_dim, rows, ahat, HD, 0, gprev, in_dim, 0, grads + s.W_off(l), in_dim, 0, 1, true);
-      colsum_acc_kernel<<<cdiv(HD, 128), 128, 0, L.stream>>>(ahat, rows, HD, grads + s.b_off(l));
+      colsum_acc_kernel<<<cdiv(HD, 32), 256, 0, L.stream>>>(ahat, rows, HD, grads + s.b_off(l));
       L.check("colsum_acc");
     }
     if (l > 1 || dX) {
@@ -448,7 +458,7 @@ void critic_gp(Launcher& L, const NetShape& s, const float* theta, const float* 
     std::swap(adj_gbar, spare);                               // adj(gbar^l) now lives in adj_gbar
   }
   // v_hat_out += sum_b adj(gbar^LD)
-  colsum_acc_kernel<<<cdiv(HD, 128), 128, 0, L.stream>>>(adj_gbar, B, HD, grads + s.W_off(LD + 1));
+  colsum_acc_kernel<<<cdiv(HD, 32), 256, 0, L.stream>>>(adj_gbar, B, HD, grads + s.W_off(LD + 1));
   L.check("colsum_acc");
   // O6 descending sweep (adj_g in adj_gbar's buffer is free now: reuse t-buffers)
   float* adj_g = adj_gbar; float* adj_a = adj_abar;
@@ -458,7 +468,7 @@ void critic_gp(Launcher& L, const NetShape& s, const float* theta, const float* 
     gp_descend_kernel<<<nb, 256, 0, L.stream>>>(adj_g, gl(l), adjs(l), adj_a, (size_t)B * HD, l == LD ? 1 : 0);
     L.check("gp_descend");
     sgemm(L, true, false, HD, in_dim, B, adj_a, HD, 0, gprev, in_dim, 0, grads + s.W_off(l), in_dim, 0, 1, true);
-    colsum_acc_kernel<<<cdiv(HD, 128), 128, 0, L.stream>>>(adj_a, B, HD, grads + s.b_off(l));
+    colsum_acc_kernel<<<cdiv(HD, 32), 256, 0, L.stream>>>(adj_a, B, HD, grads + s.b_off(l));
     L.check("colsum_acc");
     if (l > 1) sgemm(L, false, false, B, HD, HD, adj_a, HD, 0, theta + s.W_off(l), HD, 0, adj_g, HD, 0, 1, false);
   }
