@@ -59,6 +59,23 @@ def whole_job_value(units_per_rank: int, world: int, t_max_ms: float) -> float:
     return world * units_per_rank / (t_max_ms * 1e-3)
 
 
+def hbm_class_bytes(cfg) -> dict:
+    """Algorithmic bytes per step of the HBM-bound kernel classes: one pass over the C planes they
+    read / write for the collocation rows of both nets (C = 3 + 5) and the sensor rows (C = 1 per net; the snapshot
+    forward carries 2 planes), 28 B per parameter for Adam, 16 floats per row for the residual."""
+    e = 4 if cfg.precision == "fp32" else 2
+    rows, srows, H = cfg.N * cfg.P, cfg.N * cfg.S, cfg.H
+    plane = H * e
+    col = (3 + 5) * rows * plane                            # one pass over the C planes of both nets, collocation rows
+    sen = 2 * srows * plane                                 # one pass over the value plane of both nets, sensor rows
+    n_par = 2 * wl.param_count(*cfg.gen_shape) + wl.param_count(*cfg.disc_shape)
+    return {"first_layer_fwd": col + sen * (1 + (2 if e == 2 else 1)),   # writes h^1: collocation, sensor pass with stash, snapshot pass (hi, lo)
+            "out_fwd": col + sen * (1 + (2 if e == 2 else 1)),           # reads h^L
+            "jet_act_bwd": 2 * (col + sen),                               # top layer: reads h^L, writes ahat^L
+            "first_layer_bwd": sen + (0 if (e == 2 and cfg.H % 256 == 0 and cfg.P % 64 == 0) else col),   # collocation part fused into the layer-2 dgrad when it can be
+            "adam": 28 * n_par, "residual": 16 * 4 * rows}
+
+
 class ClockSampler(threading.Thread):
     """Samples SM clock and throttle reasons through NVML while the timed region runs."""
 
@@ -286,6 +303,22 @@ def run_config(cfg, device, steps, warmup, rank, world, with_roofline=True, seed
             ach = flops["total"] / (np.mean(ms) * 1e-3) / 1e12
             res["roofline"] = {"bound": "alu", "achieved": round(ach, 4), "peak": round(peak, 1), "unit": "TFLOP/s", "frac": round(ach / peak, 5),
                                "traffic": None, "kernel": "whole fp32 step (launch-latency bound at this size)"}
+    # whole step against its roofline: t_roof = sum over kernel classes of max(flops / tensor peak, bytes / HBM peak)
+    if with_roofline and prof:
+        hb = hbm_class_bytes(cfg)
+        t_roof = 0.0
+        if cfg.precision != "fp32":
+            sens_gemm = cfg.N * 3 * cfg.S * 2 * (cfg.L - 1) * 2 * cfg.H * cfg.H
+            t_roof += (flops["jet_gemm"] + sens_gemm) / (peaks["tflops_sustained"] * 1e12) * 1e3
+        hk = {}
+        for k, b in hb.items():
+            if k in prof and prof[k][1] > 0:
+                ms_k = prof[k][1] / steps
+                t_roof += b / (peaks["hbm_gbs"] * 1e9) * 1e3
+                hk[k] = {"gbs": round(b / (ms_k * 1e-3) / 1e9, 1), "frac": round(b / (ms_k * 1e-3) / 1e9 / peaks["hbm_gbs"], 3), "ms": round(ms_k, 4)}
+        res["step_roofline"] = {"t_roof_ms": round(t_roof, 4), "frac": round(t_roof / float(np.mean(ms)), 4), "hbm_peak_gbs": peaks["hbm_gbs"],
+                                "hbm_kernels": hk, "note": "tensor classes at the measured sustained bf16 rate + HBM-bound classes at the measured copy bandwidth; "
+                                "critic, z-part and launch latency count as zero in t_roof"}
     w.pg.close()
     return res
 
@@ -307,7 +340,7 @@ def summarize(cfg, res, n_gpus, steps, warmup, t_max_ms):
         "jet_evals_per_s": n_gpus * units / (float(np.mean(res["ms_jet"])) * 1e-3),
         "step_tflops": wl.step_flops(cfg)["total"] / (t_max_ms * 1e-3) / 1e12,
         "e2e": {"value": n_gpus * units / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": res["h2d"], "d2h_bytes_per_step": res["d2h"]},
-        "gpu_launches": res["launches"], "clocks": res["clocks"], "roofline": res.get("roofline"),
+        "gpu_launches": res["launches"], "clocks": res["clocks"], "roofline": res.get("roofline"), "step_roofline": res.get("step_roofline"),
         "kernel_ms_per_step": res.get("kernel_ms_per_step"), "losses": res["losses"], "found_inf": res["found_inf"],
     }
 
@@ -369,7 +402,7 @@ def main():
                     continue
                 r = run_config(c, device, 5 if c.N * c.P > 1000000 else 20, 3, rank, world)
                 s = summarize(c, r, 1, len(r["ms_steps"]), 3, float(np.mean(r["ms_steps"])))
-                per[name] = {k: s[k] for k in ("value", "ms_per_step", "dtype", "step_tflops", "jet_evals_per_s", "roofline", "gpu_launches", "e2e", "kernel_ms_per_step")}
+                per[name] = {k: s[k] for k in ("value", "ms_per_step", "dtype", "step_tflops", "jet_evals_per_s", "roofline", "step_roofline", "gpu_launches", "e2e", "kernel_ms_per_step")}
             line["per_config"] = per
         if not args.no_cpu_baseline:
             val, sec, cores, sample = time_oracle(cfg)
