@@ -37,7 +37,9 @@ struct JetParams {
   int n_row_tiles;       // R / 64
   const float* bias;     // MODE 0: b_l
   float* g_bias;         // MODE 1: b_hat_{l-1}
-  const float* amax;     // MODE 1: block-scale source of the adjoint planes (common.cuh adj_inv_scale)
+  const float* amax;     // MODE 1, 3: block-scale source of the adjoint planes (common.cuh adj_inv_scale)
+  // MODE 3 (MODE 1 + first-layer reduction, O4 'First layer'; see tc2_kernels.cu): ahat^1 is consumed in registers
+  const float* xy; long long row0; int npts, in_dim; float* gW1; float* An;
 };
 
 template <typename T, int C, int MODE>
@@ -66,7 +68,7 @@ __global__ void __launch_bounds__(256, 1) jet_layer_kernel(const __grid_constant
 
   if (warp == 0 && lane == 0) {
     prefetch_tmap(&tmA); prefetch_tmap(&tmB); prefetch_tmap(&tmO);
-    if (MODE == 1) prefetch_tmap(&tmT);
+    if (MODE == 1 || MODE == 3) prefetch_tmap(&tmT);
   }
   if (warp == 1 && lane == 0) {
     for (int i = 0; i < Cfg::kNumStages; ++i) { mbar_init(full + i, 1); mbar_init(empty + i, 1); }
@@ -157,7 +159,8 @@ __global__ void __launch_bounds__(256, 1) jet_layer_kernel(const __grid_constant
           for (int c = 0; c < C; ++c) tma_load_3d(stg + c * kStgPlane, &tmT, sbar + q, rt * kRT + hf * 32, unit0, c);
         }
       };
-      if (MODE == 1) issue_stage_loads(0);
+      if (MODE == 1 || MODE == 3) issue_stage_loads(0);
+      float sx = 0.f, sy = 0.f;                              // MODE 3
       mbar_wait(tfull + buf, bphase);
       tc_fence_after();
 
@@ -225,6 +228,7 @@ __global__ void __launch_bounds__(256, 1) jet_layer_kernel(const __grid_constant
           if (hf == 1) issue_stage_loads(1);
           __syncwarp();
           mbar_wait(sbar + q, sphase); sphase ^= 1;
+          const float2* xyp = MODE == 3 ? reinterpret_cast<const float2*>(p.xy) + (int)((p.row0 + rt * kRT + hf * 32) % p.npts) : nullptr;
 #pragma unroll 1
           for (int rc = 0; rc < 4; ++rc) {
             float hh[C][8], hp[C][8], o[C][8];
@@ -241,24 +245,41 @@ __global__ void __launch_bounds__(256, 1) jet_layer_kernel(const __grid_constant
               for (int c = 0; c < C; ++c) { hx[c] = hh[c][i]; hj[c] = hp[c][i]; }
               jet_act_bwd<C>(hj, hx, aa);
               bias_acc += aa[0];
+              if (MODE == 3) {
+                const float2 q2 = __ldg(xyp + rc * 8 + i);   // same address in every lane: one broadcast load
+                sx = fmaf(aa[0], q2.x, sx); sy = fmaf(aa[0], q2.y, sy);
+                if (C >= 3) { sx += aa[1]; sy += aa[2]; }
+              }
 #pragma unroll
               for (int c = 0; c < C; ++c) o[c][i] = aa[c];
             }
+            if (MODE == 1) {
 #pragma unroll
-            for (int c = 0; c < C; ++c) *reinterpret_cast<uint4*>(my_row + c * kStgPlane + off) = pack8<T>(o[c]);
+              for (int c = 0; c < C; ++c) *reinterpret_cast<uint4*>(my_row + c * kStgPlane + off) = pack8<T>(o[c]);
+            }
           }
-          fence_proxy_async();
-          __syncwarp();
-          if (elect_one()) {
-            for (int c = 0; c < C; ++c) tma_store_3d(&tmO, stg + c * kStgPlane, rt * kRT + hf * 32, unit0, c);
-            tma_commit_group();
+          if (MODE == 1) {
+            fence_proxy_async();
+            __syncwarp();
+            if (elect_one()) {
+              for (int c = 0; c < C; ++c) tma_store_3d(&tmO, stg + c * kStgPlane, rt * kRT + hf * 32, unit0, c);
+              tma_commit_group();
+            }
+          } else {
+            __syncwarp();                                    // every lane is done reading the staging planes before they are refilled
           }
         }
       }
       tc_fence_before();
       __syncwarp();
       if (lane == 0) mbar_arrive(tempty + buf);
-      if (MODE == 1) atomicAdd(p.g_bias + unit, bias_acc * adj_inv_scale(p.amax));
+      if (MODE == 1 || MODE == 3) atomicAdd(p.g_bias + unit, bias_acc * adj_inv_scale(p.amax));
+      if (MODE == 3) {
+        const float inv = adj_inv_scale(p.amax);
+        atomicAdd(p.An + (size_t)((p.row0 + rt * kRT) / p.npts) * p.H + unit, bias_acc * inv);
+        atomicAdd(p.gW1 + (size_t)unit * p.in_dim, sx * inv);
+        atomicAdd(p.gW1 + (size_t)unit * p.in_dim + 1, sy * inv);
+      }
     }
     __syncwarp();
     if (elect_one()) tma_wait_all();                         // global writes of the last stores are complete before exit
@@ -442,7 +463,7 @@ static void launch_jet(Launcher& L, const CUtensorMap& a, const CUtensorMap& b, 
   const int tiles = (p.H / kBM) * p.n_row_tiles;
   const int grid = std::min(tiles, num_sms());
   kern<<<grid, 256, Cfg::kSmemBytes, L.stream>>>(a, b, o, t, p);
-  L.check(MODE == 0 ? "jet_layer_fwd" : MODE == 1 ? "jet_layer_bwd" : "jet_layer_fwd_split");
+  L.check(MODE == 0 ? "jet_layer_fwd" : MODE == 2 ? "jet_layer_fwd_split" : "jet_layer_bwd");
 }
 
 template <int MODE>
@@ -482,7 +503,7 @@ void tc_layer_fwd_split(Launcher& L, int precision, int H, int R, int R_ld, cons
   launch_jet<__half, 2, 2>(L, a, b, o, o, p);
 }
 
-bool tc_first_layer_fusable(int H, const ChunkGeom& g) { return tc2_supported(H) && g.npts % 64 == 0 && g.R == g.valid && g.R > 0; }
+bool tc_first_layer_fusable(int H, const ChunkGeom& g) { return H % 128 == 0 && g.npts % 64 == 0 && g.R == g.valid && g.R > 0; }
 
 void tc_layer_bwd(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* w16T_l, const void* ahat_in, const void* h_prev,
                   void* ahat_out, float* g_bias_prev, const float* amax, const FirstLayerFuse* fl) {
@@ -495,6 +516,11 @@ void tc_layer_bwd(Launcher& L, int precision, int C, int H, int R, int R_ld, con
   if (!ok) return;
   JetParams p{};
   p.H = H; p.n_row_tiles = R / kRT; p.g_bias = g_bias_prev; p.amax = amax;
+  if (fl) {
+    p.xy = fl->xy; p.row0 = fl->row0; p.npts = fl->npts; p.in_dim = fl->in_dim; p.gW1 = fl->gW1; p.An = fl->An;
+    dispatch_jet<3>(L, precision, C, a, b, o, t, p);
+    return;
+  }
   dispatch_jet<1>(L, precision, C, a, b, o, t, p);
 }
 
