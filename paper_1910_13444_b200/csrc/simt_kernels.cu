@@ -102,6 +102,11 @@ void sgemm(Launcher& L, bool TA, bool TB, int M, int N, int K, const float* A, i
   if (tiles < 296 && K >= 256) {                // too few tiles to fill 148 SMs: split the contraction
     ksplit = min(cdiv(592, tiles), K / 128);
     if (ksplit < 1) ksplit = 1;
+  } else if (accumulate && tiles < 74 && K >= 64) {
+    // the critic's weight-gradient GEMMs (a handful of tiles, K = batch rows): they accumulate with atomics anyway, so
+    // splitting the contraction costs nothing and turns 6 serial k-steps per CTA into 1-2
+    ksplit = min(cdiv(148, tiles), K / 32);
+    if (ksplit < 1) ksplit = 1;
   }
   bool atomic = accumulate;
   if (ksplit > 1 && !accumulate) {
