@@ -48,10 +48,19 @@ typedef enum {
   PIGAN_ERR_UNSUPPORTED = 5    /* e.g. 16-bit precision with a width that is not a multiple of 128 */
 } pigan_status;
 
-/* Arithmetic of the hidden jet layers (S8a a3, a10).  FP32: plain FP32 FMA.  BF16 / FP16: tcgen05 tensor cores,
- * 16-bit operands, fp32 accumulation in TMEM, fp32 epilogue; first layer, output dot, residual, critic, norms,
- * reductions and weight-gradient accumulation stay fp32 (reading G18). */
+/* Arithmetic of the hidden jet layers (S8a a3, a10).  FP32: plain FP32 FMA.  FP16: tcgen05 tensor cores, fp16
+ * operands (the paper's arithmetic), fp32 accumulation in TMEM, fp32 epilogue; first layer, output dot, residual,
+ * critic, norms, reductions and weight-gradient accumulation stay fp32 (reading G18).
+ * PIGAN_BF16 is an ALIAS of PIGAN_FP16: it selects exactly the same fp16-operand path (reading R1: bf16
+ * activation planes measure 1-2e-2 against the 2e-2 tolerance, and kind::f16 rejects mixed operands).  Weights that
+ * were rounded to bf16 convert to fp16 exactly for |w| >= 2^-14.  Consequence: in both 16-bit modes activation and jet
+ * planes have fp16 RANGE (65504); the derivative channels grow with products of layer gains, and a forward overflow
+ * surfaces as inf/nan gradients with *found_inf = 1 (never as silently wrong finite values). */
 typedef enum { PIGAN_FP32 = 0, PIGAN_BF16 = 1, PIGAN_FP16 = 2 } pigan_precision;
+
+/* pigan_config.flags (debug / measurement switches; 0 is the product path) */
+#define PIGAN_FLAG_NO_GRAPH   1u   /* never capture / replay pigan_train_step_grads as a CUDA graph: every call runs eagerly */
+#define PIGAN_FLAG_ONE_CTA    2u   /* use the one-CTA tcgen05 kernels even where the CTA-pair (cta_group::2) kernels apply */
 
 typedef struct { int in_dim, n_hidden, width; } pigan_mlp_shape;   /* scalar linear output implied (G10) */
 
@@ -66,10 +75,13 @@ typedef struct {
   float gp_lambda;           /* WGAN-GP weight, 10 (G2) */
   float pde_weight;          /* w_pde in L_G = -mean D(fake) + w_pde mean r^2 (G8), default 1 */
   size_t workspace_bytes;    /* 0 = library default; bounds the row-chunk size of the step (S7 H1) */
+  int chunk_rows;            /* 0 = library default (131072); rows per chunk of the generator passes, rounded to 256 */
+  unsigned flags;            /* PIGAN_FLAG_* */
 } pigan_config;
 
-/* Creates a context: validates cfg, allocates the workspace on the current CUDA device.  *out is NULL on failure
- * (the status says why).  cuda_stream is a cudaStream_t. */
+/* Creates a context: validates cfg, allocates the workspace on the CURRENT CUDA device and binds the context to it
+ * (every later call on the context switches to that device for its duration and restores the caller's).  *out is NULL
+ * on failure (the status says why).  cuda_stream is a cudaStream_t of that device. */
 pigan_status pigan_create(const pigan_config* cfg, void* cuda_stream, pigan_ctx** out);
 void         pigan_destroy(pigan_ctx* ctx);                       /* NULL is allowed */
 size_t       pigan_param_count(const pigan_mlp_shape* shape);     /* H*in + H + (L-1)(H*H + H) + H + 1; 0 if shape is NULL/invalid */
@@ -118,8 +130,9 @@ pigan_status pigan_gradient_penalty(pigan_ctx* ctx, const float* disc_params, co
  *   Execution: asynchronous on the context's stream.  A call whose arguments (all pointers and loss_scale) repeat the
  *   previous call's is captured into a CUDA graph and replayed on later identical calls; the arrays are read when the
  *   step RUNS, so updating them in place between calls (an optimiser step, new z / eps copied into the same buffers)
- *   behaves exactly as an eager call.  Environment: PIGAN_NO_GRAPH=1 disables the replay, PIGAN_CHUNK_ROWS=<n> sets the
- *   row-chunk size (default 131072 rows; workspace_bytes of the config bounds it as well). */
+ *   behaves exactly as an eager call.  cfg.flags & PIGAN_FLAG_NO_GRAPH disables the replay; cfg.chunk_rows sets the
+ *   row-chunk size (default 131072 rows; workspace_bytes of the config bounds it as well).  No environment variable
+ *   changes the behaviour of the library. */
 pigan_status pigan_train_step_grads(pigan_ctx* ctx, const float* logk_params, const float* u_params,
                                     const float* disc_params, const float* xy_colloc, const float* f,
                                     const float* xy_sensors, const float* z, const float* real_snap,

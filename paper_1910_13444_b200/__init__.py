@@ -10,9 +10,11 @@ import ctypes
 import os
 from ctypes import POINTER, Structure, c_char_p, c_float, c_int, c_size_t, c_ulonglong, c_void_p
 
-from .build import LIB, build
+from .build import LIB, build, is_stale
 
-__all__ = ["PiGan", "PiganError", "load_library", "param_count", "EXPORTED_SYMBOLS", "PRECISIONS"]
+__all__ = ["PiGan", "PiganError", "load_library", "param_count", "EXPORTED_SYMBOLS", "PRECISIONS", "FLAG_NO_GRAPH", "FLAG_ONE_CTA"]
+
+FLAG_NO_GRAPH, FLAG_ONE_CTA = 1, 2                     # pigan_config.flags (include/pigan.h)
 
 PRECISIONS = {"fp32": 0, "bf16": 1, "fp16": 2}
 STATUS = {0: "PIGAN_OK", 1: "PIGAN_ERR_INVALID_ARG", 2: "PIGAN_ERR_SHAPE", 3: "PIGAN_ERR_ALLOC", 4: "PIGAN_ERR_CUDA",
@@ -36,19 +38,20 @@ class _MlpShape(Structure):
 class _Config(Structure):
     _fields_ = [("gen", _MlpShape), ("disc", _MlpShape), ("latent_dim", c_int), ("n_samples", c_int), ("n_colloc", c_int),
                 ("n_sensors", c_int), ("precision", c_int), ("gp_lambda", c_float), ("pde_weight", c_float),
-                ("workspace_bytes", c_size_t)]
+                ("workspace_bytes", c_size_t), ("chunk_rows", c_int), ("flags", ctypes.c_uint)]
 
 
 _lib = None
 
 
 def load_library():
-    """Loads libpigan.so (building it first if it is missing or stale).  Raises if that is impossible."""
+    """Loads libpigan.so, building it first if it is missing or older than any source under csrc/ or include/pigan.h
+    (nvcc is needed for that; a GPU box receives the built library with the snapshot).  Raises if that is impossible."""
     global _lib
     if _lib is not None:
         return _lib
     path = LIB
-    if not os.path.exists(path) or os.environ.get("PIGAN_REBUILD"):
+    if not os.path.exists(path) or is_stale():
         path = build()
     lib = ctypes.CDLL(path)
     fp, ip = POINTER(c_float), POINTER(c_int)
@@ -98,7 +101,7 @@ class PiGan:
     """One context = one CUDA stream + the workspaces of one PI-GAN configuration (mirrors pigan_ctx)."""
 
     def __init__(self, *, latent_dim, gen_hidden, gen_width, disc_hidden, disc_width, n_samples, n_colloc, n_sensors,
-                 precision="fp32", gp_lambda=10.0, pde_weight=1.0, workspace_bytes=0, stream=None, device=None):
+                 precision="fp32", gp_lambda=10.0, pde_weight=1.0, workspace_bytes=0, chunk_rows=0, flags=0, stream=None, device=None):
         import torch
         self._lib = load_library()
         self._ctx = c_void_p()
@@ -110,7 +113,7 @@ class PiGan:
         self.disc_shape = (2 * n_sensors, disc_hidden, disc_width)
         self.precision = precision
         cfg = _Config(_MlpShape(*self.gen_shape), _MlpShape(*self.disc_shape), latent_dim, n_samples, n_colloc, n_sensors,
-                      PRECISIONS[precision], gp_lambda, pde_weight, workspace_bytes)
+                      PRECISIONS[precision], gp_lambda, pde_weight, workspace_bytes, chunk_rows, flags)
         self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
         with torch.cuda.device(self.device):
             st = self._lib.pigan_create(ctypes.byref(cfg), c_void_p(self._stream.cuda_stream), ctypes.byref(self._ctx))

@@ -12,14 +12,27 @@ SOURCES = sorted(glob.glob(os.path.join(PKG, "csrc", "*.cu")))
 HEADERS = sorted(glob.glob(os.path.join(PKG, "csrc", "*.cuh"))) + [os.path.join(ROOT, "include", "pigan.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC",
-         "--expt-relaxed-constexpr", "-I", os.path.join(ROOT, "include")] + os.environ.get("PIGAN_NVCC_EXTRA", "").split()
+         "--expt-relaxed-constexpr", "-I", os.path.join(ROOT, "include")]
+
+
+STAMP = LIB + ".srchash"      # content hash of the sources the library was built from (mtimes do not survive a copy to a GPU box)
+
+
+def source_hash() -> str:
+    import hashlib
+    h = hashlib.sha256()
+    for f in SOURCES + HEADERS:
+        h.update(os.path.basename(f).encode())
+        h.update(open(f, "rb").read())
+    h.update(" ".join(FLAGS[:-1]).encode())
+    return h.hexdigest()
 
 
 def is_stale() -> bool:
-    if not os.path.exists(LIB):
+    """True when libpigan.so is missing or was built from other sources than the ones in the tree."""
+    if not os.path.exists(LIB) or not os.path.exists(STAMP):
         return True
-    t = os.path.getmtime(LIB)
-    return any(os.path.getmtime(f) > t for f in SOURCES + HEADERS + [os.path.abspath(__file__)])
+    return open(STAMP).read().strip() != source_hash()
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
@@ -40,6 +53,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
         if verbose:
             print(out)
     subprocess.check_call([NVCC, "-shared", "-o", LIB] + objs + ["-gencode", "arch=compute_100a,code=sm_100a"])
+    with open(STAMP, "w") as f:
+        f.write(source_hash() + "\n")
     return LIB
 
 

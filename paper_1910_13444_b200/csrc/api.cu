@@ -44,7 +44,7 @@ struct pigan_ctx {
   std::vector<void*> allocs;
   // CUDA-graph replay of pigan_train_step_grads: the step is hundreds to thousands of launches, launch-latency bound
   // for the small configs.  A call whose arguments repeat the previous call's is captured once (on a private stream,
-  // so the caller's stream may be the legacy default stream) and replayed from then on.  PIGAN_NO_GRAPH=1 disables it.
+  // so the caller's stream may be the legacy default stream) and replayed from then on.  PIGAN_FLAG_NO_GRAPH disables it.
   struct StepGraph {
     cudaStream_t cap_stream = nullptr;
     cudaGraphExec_t exec = nullptr;
@@ -66,6 +66,16 @@ struct pigan_ctx {
 };
 
 namespace {
+
+// Every entry point runs on the device the context was created on, whatever the caller's current device is.
+struct DeviceGuard {
+  int prev = -1; bool switched = false;
+  explicit DeviceGuard(const pigan_ctx* c) {
+    if (!c) return;
+    if (cudaGetDevice(&prev) == cudaSuccess && prev != c->L.device) switched = cudaSetDevice(c->L.device) == cudaSuccess;
+  }
+  ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
+};
 
 pigan_status fail(pigan_ctx* c, pigan_status s, const std::string& msg) {
   if (c) c->err = msg;
@@ -206,7 +216,7 @@ pigan_status train_step_impl(pigan_ctx* c, const float* thY, const float* thU, c
   }
   // ---- a7-a9: critic losses and gradient; dX rows [0, N) = (1/N) grad_X D(X_fake) ----
   build_snapshots(L, c->xfake, real, eps, N, d, c->cw.X);
-  critic_forward(L, ds, thD, c->cw.X, 3 * N, c->cw.g, c->cw.D, nullptr);
+  critic_forward(L, ds, thD, c->cw.X, 3 * N, c->cw.g, c->cw.D);
   reduce_scores(L, c->cw.D, N, c->cw.acc);
   fill_seed(L, c->seed, N);
   const int gstride = 3 * N * HD;
@@ -263,6 +273,7 @@ unsigned long long pigan_launch_count(const pigan_ctx* c) { return c ? c->L.coun
 
 pigan_status pigan_profile_enable(pigan_ctx* c, int enable) {
   if (!c) return PIGAN_ERR_INVALID_ARG;
+  DeviceGuard dg(c);
   c->L.profiling = enable != 0;
   if (enable) { c->L.n_rec = 0; c->L.mark("begin"); }
   return PIGAN_OK;
@@ -270,6 +281,7 @@ pigan_status pigan_profile_enable(pigan_ctx* c, int enable) {
 
 pigan_status pigan_profile_report(pigan_ctx* c, char* buf, size_t cap) {
   if (!c || !buf || cap == 0) return PIGAN_ERR_INVALID_ARG;
+  DeviceGuard dg(c);
   if (c->L.n_rec == 0) return fail(c, PIGAN_ERR_INVALID_ARG, "profiling was not enabled");
   if (cudaStreamSynchronize(c->L.stream) != cudaSuccess) return fail(c, PIGAN_ERR_CUDA, "stream synchronize failed");
   std::vector<std::pair<std::string, std::pair<unsigned long long, double>>> acc;
@@ -300,7 +312,7 @@ pigan_status pigan_create(const pigan_config* cfg, void* cuda_stream, pigan_ctx*
   if (!cfg || !out) return PIGAN_ERR_INVALID_ARG;
   if (!shape_ok(cfg->gen) || !shape_ok(cfg->disc) || cfg->latent_dim < 1 || cfg->n_samples < 1 || cfg->n_colloc < 1 || cfg->n_sensors < 1)
     return PIGAN_ERR_INVALID_ARG;
-  if ((int)cfg->precision < 0 || (int)cfg->precision > 2 || !(cfg->gp_lambda >= 0.f)) return PIGAN_ERR_INVALID_ARG;
+  if ((int)cfg->precision < 0 || (int)cfg->precision > 2 || !(cfg->gp_lambda >= 0.f) || cfg->chunk_rows < 0) return PIGAN_ERR_INVALID_ARG;
   if (cfg->gen.in_dim != 2 + cfg->latent_dim || cfg->disc.in_dim != 2 * cfg->n_sensors) return PIGAN_ERR_SHAPE;
   if (cfg->precision != PIGAN_FP32) {
     std::string why;
@@ -314,7 +326,10 @@ pigan_status pigan_create(const pigan_config* cfg, void* cuda_stream, pigan_ctx*
   c->gen = NetShape{cfg->gen.in_dim, cfg->gen.n_hidden, cfg->gen.width};
   c->disc = NetShape{cfg->disc.in_dim, cfg->disc.n_hidden, cfg->disc.width};
   c->L.stream = (cudaStream_t)cuda_stream;
-  if (const char* e = getenv("PIGAN_NO_GRAPH")) c->sg.disabled = e[0] == '1';
+  cudaGetDevice(&c->L.device);
+  if (cudaDeviceGetAttribute(&c->L.num_sms, cudaDevAttrMultiProcessorCount, c->L.device) != cudaSuccess || c->L.num_sms <= 0) c->L.num_sms = 148;
+  c->L.one_cta = (cfg->flags & PIGAN_FLAG_ONE_CTA) != 0;
+  c->sg.disabled = (cfg->flags & PIGAN_FLAG_NO_GRAPH) != 0;
   c->elem = cfg->precision == PIGAN_FP32 ? 4 : 2;
   const int H = c->gen.H, Lh = c->gen.L, N = cfg->n_samples, S = cfg->n_sensors, d = 2 * S, HD = c->disc.H, LD = c->disc.L;
   const bool f32 = cfg->precision == PIGAN_FP32;
@@ -327,7 +342,7 @@ pigan_status pigan_create(const pigan_config* cfg, void* cuda_stream, pigan_ctx*
   size_t budget = cfg->workspace_bytes ? cfg->workspace_bytes : std::min<size_t>(free_b / 2, (size_t)48 << 30);
   long long rows = (long long)(budget / per_row);
   long long cap = 131072;                                  // default chunk rows (sweep on B200: larger chunks amortise launch ramps)
-  if (const char* e = getenv("PIGAN_CHUNK_ROWS")) cap = std::max(256LL, atoll(e));
+  if (cfg->chunk_rows > 0) cap = std::max(256, cfg->chunk_rows);
   if (!cfg->workspace_bytes) rows = std::min(rows, cap);
   rows = std::min<long long>(rows, (long long)round_up((size_t)max_rows, 256));
   rows = std::max<long long>(rows / 256 * 256, 256);            // workspace_bytes is a hint: never below one 256-row chunk
@@ -375,6 +390,7 @@ pigan_status pigan_create(const pigan_config* cfg, void* cuda_stream, pigan_ctx*
 
 void pigan_destroy(pigan_ctx* c) {
   if (!c) return;
+  DeviceGuard dg(c);
   if (c->sg.exec) cudaGraphExecDestroy(c->sg.exec);
   if (c->sg.cap_stream) cudaStreamDestroy(c->sg.cap_stream);
   for (void* p : c->allocs) cudaFree(p);
@@ -385,6 +401,7 @@ void pigan_destroy(pigan_ctx* c) {
 pigan_status pigan_gen_jet_forward(pigan_ctx* c, const float* gen_params, const float* xy, int n_pts, const float* z, int n_samples,
                                    int jet_order, float* out) {
   if (!c) return PIGAN_ERR_INVALID_ARG;
+  DeviceGuard dg(c);
   if (jet_order < 0 || jet_order > 2 || n_pts < 0 || n_samples < 0) return fail(c, PIGAN_ERR_INVALID_ARG, "jet_order must be 0..2 and sizes >= 0");
   if (n_pts == 0 || n_samples == 0) return PIGAN_OK;
   if (!gen_params || !xy || !z || !out) return fail(c, PIGAN_ERR_INVALID_ARG, "null pointer");
@@ -400,6 +417,7 @@ pigan_status pigan_gen_jet_forward(pigan_ctx* c, const float* gen_params, const 
 pigan_status pigan_darcy_residual(pigan_ctx* c, const float* logk_jet, const float* u_jet, const float* f, int n_samples, int n_pts,
                                   float* r, float* mean_sq) {
   if (!c) return PIGAN_ERR_INVALID_ARG;
+  DeviceGuard dg(c);
   if (n_samples < 0 || n_pts < 0) return fail(c, PIGAN_ERR_INVALID_ARG, "negative size");
   const long long total = (long long)n_samples * n_pts;
   if (total > 0 && (!logk_jet || !u_jet || !f)) return fail(c, PIGAN_ERR_INVALID_ARG, "null pointer");
@@ -415,13 +433,14 @@ pigan_status pigan_darcy_residual(pigan_ctx* c, const float* logk_jet, const flo
 
 pigan_status pigan_disc_forward(pigan_ctx* c, const float* disc_params, const float* snap, int B, float* score) {
   if (!c) return PIGAN_ERR_INVALID_ARG;
+  DeviceGuard dg(c);
   if (B < 0) return fail(c, PIGAN_ERR_INVALID_ARG, "negative batch");
   if (B == 0) return PIGAN_OK;
   if (!disc_params || !snap || !score) return fail(c, PIGAN_ERR_INVALID_ARG, "null pointer");
   const int d = c->disc.in_dim, cap = 3 * c->cfg.n_samples;
   for (int b0 = 0; b0 < B; b0 += cap) {
     const int rows = std::min(cap, B - b0);
-    critic_forward(c->L, c->disc, disc_params, snap + (size_t)b0 * d, rows, c->cw.g, score + b0, nullptr);
+    critic_forward(c->L, c->disc, disc_params, snap + (size_t)b0 * d, rows, c->cw.g, score + b0);
   }
   return finish(c);
 }
@@ -429,6 +448,7 @@ pigan_status pigan_disc_forward(pigan_ctx* c, const float* disc_params, const fl
 pigan_status pigan_gradient_penalty(pigan_ctx* c, const float* disc_params, const float* real, const float* fake, const float* eps, int B,
                                     float* gp, float* grad_norm, float* d_disc_params) {
   if (!c) return PIGAN_ERR_INVALID_ARG;
+  DeviceGuard dg(c);
   if (B < 1) return fail(c, PIGAN_ERR_INVALID_ARG, "B must be >= 1");
   if (!disc_params || !real || !fake || !eps) return fail(c, PIGAN_ERR_INVALID_ARG, "null pointer");
   if (B > c->cfg.n_samples) return fail(c, PIGAN_ERR_SHAPE, "B exceeds the n_samples of the config");
@@ -439,7 +459,7 @@ pigan_status pigan_gradient_penalty(pigan_ctx* c, const float* disc_params, cons
   if (d_disc_params) cudaMemsetAsync(d_disc_params, 0, ds.count() * 4, st);
   build_snapshots(c->L, fake, real, eps, B, d, c->cw.X);
   float* Xhat = c->cw.X + (size_t)2 * B * d;
-  critic_forward(c->L, ds, disc_params, Xhat, B, c->cw.g, c->cw.D, nullptr);
+  critic_forward(c->L, ds, disc_params, Xhat, B, c->cw.g, c->cw.D);
   critic_gp(c->L, ds, disc_params, Xhat, c->cw.g, B, B * HD, c->cfg.gp_lambda, c->cw, d_disc_params, grad_norm);
   if (gp) write_losses(c->L, c->cw.acc, B, 1, c->cfg.gp_lambda, 0.f, nullptr, gp, nullptr, 0);
   return finish(c);
@@ -449,6 +469,7 @@ pigan_status pigan_train_step_grads(pigan_ctx* c, const float* logk_params, cons
                                     const float* xy_colloc, const float* f, const float* xy_sensors, const float* z, const float* real_snap,
                                     const float* eps, float loss_scale, float* g_logk, float* g_u, float* g_disc, float* losses, int* found_inf) {
   if (!c) return PIGAN_ERR_INVALID_ARG;
+  DeviceGuard dg(c);
   if (!logk_params || !u_params || !disc_params || !xy_colloc || !f || !xy_sensors || !z || !real_snap || !eps || !g_logk || !g_u || !g_disc)
     return fail(c, PIGAN_ERR_INVALID_ARG, "null pointer");
   if (!(loss_scale > 0.f) || !std::isfinite(loss_scale)) return fail(c, PIGAN_ERR_INVALID_ARG, "loss_scale must be positive and finite");
@@ -503,6 +524,7 @@ pigan_status pigan_train_step_grads(pigan_ctx* c, const float* logk_params, cons
 pigan_status pigan_adam_update(pigan_ctx* c, float* params, const float* grads, float* m, float* v, size_t n, int step, float lr, float beta1,
                                float beta2, float adam_eps, const int* skip_flag) {
   if (!c) return PIGAN_ERR_INVALID_ARG;
+  DeviceGuard dg(c);
   if (n == 0) return PIGAN_OK;
   if (!params || !grads || !m || !v) return fail(c, PIGAN_ERR_INVALID_ARG, "null pointer");
   if (step < 1) return fail(c, PIGAN_ERR_INVALID_ARG, "step is 1-based");

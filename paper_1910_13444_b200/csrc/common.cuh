@@ -1,7 +1,6 @@
 // Internal declarations shared by the translation units of libpigan.so (not part of the C-ABI).
 #pragma once
 #include <cuda_runtime.h>
-#include <cuda_bf16.h>
 #include <cuda_fp16.h>
 #include <cstdint>
 #include <cstdio>
@@ -30,11 +29,9 @@ struct NetShape {
 
 template <typename T> __device__ __forceinline__ float to_f(T v);
 template <> __device__ __forceinline__ float to_f<float>(float v) { return v; }
-template <> __device__ __forceinline__ float to_f<__nv_bfloat16>(__nv_bfloat16 v) { return __bfloat162float(v); }
 template <> __device__ __forceinline__ float to_f<__half>(__half v) { return __half2float(v); }
 template <typename T> __device__ __forceinline__ T from_f(float v);
 template <> __device__ __forceinline__ float from_f<float>(float v) { return v; }
-template <> __device__ __forceinline__ __nv_bfloat16 from_f<__nv_bfloat16>(float v) { return __float2bfloat16_rn(v); }
 template <> __device__ __forceinline__ __half from_f<__half>(float v) { return __float2half_rn(v); }
 
 // ---- the tanh jet chain rule and its adjoint (O4); C = 1, 3 or 5 channels ------------------
@@ -95,6 +92,9 @@ __device__ __forceinline__ float adj_inv_scale(const float* amax) { return ldexp
 // ---- launch bookkeeping -------------------------------------------------------------------------------------
 struct Launcher {
   cudaStream_t stream = nullptr;
+  int device = 0;              // the CUDA device the owning context was created on
+  int num_sms = 148;           // multiprocessors of that device
+  bool one_cta = false;        // PIGAN_FLAG_ONE_CTA: never take the CTA-pair kernels
   unsigned long long count = 0;
   cudaError_t err = cudaSuccess;
   const char* where = "";
@@ -116,6 +116,13 @@ struct Launcher {
     cudaEventRecord(events[n_rec++], stream);
   }
 };
+
+// cudaFuncAttributeMaxDynamicSharedMemorySize is per (function, device): remember which devices were opted in
+template <typename K>
+inline void ensure_smem_attr(const Launcher& L, K kern, int bytes, unsigned long long& done_mask) {
+  const unsigned long long bit = 1ull << (L.device & 63);
+  if (!(done_mask & bit)) { cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes); done_mask |= bit; }
+}
 
 // ---- SIMT kernels (simt_kernels.cu) ---------------------------------------------------------------------------
 // C[M x N] (ldc) = or += alpha * op(A)[M x K] op(B)[K x N], batched (batch index adds sA/sB/sC), fp32.
@@ -171,8 +178,7 @@ struct CriticWs {
   double* acc = nullptr;    // [8] accumulators: 0 sum D fake, 1 sum D real, 2 sum (nu-1)^2, 3 sum r^2
   int maxB = 0;
 };
-void critic_forward(Launcher& L, const NetShape& s, const float* theta, const float* X, int rows, float* g, float* D,
-                    float* scratch);
+void critic_forward(Launcher& L, const NetShape& s, const float* theta, const float* X, int rows, float* g, float* D);
 // plain backprop of sum_b seed[b] D(X_b) over `rows` rows starting at activations g; accumulates into grads if non-null;
 // writes d/dX into dX if non-null.
 void critic_backward(Launcher& L, const NetShape& s, const float* theta, const float* X, const float* g, int rows,
@@ -180,7 +186,6 @@ void critic_backward(Launcher& L, const NetShape& s, const float* theta, const f
 void critic_gp(Launcher& L, const NetShape& s, const float* theta, const float* Xhat, const float* g /*of xhat rows*/,
                int B, int g_layer_stride, float lambda, CriticWs& w, float* grads /*may be null*/, float* grad_norm);
 void build_snapshots(Launcher& L, const float* fake, const float* real, const float* eps, int B, int d, float* X);
-void scale_copy(Launcher& L, const float* src, float* dst, size_t n, float alpha);
 void fill_seed(Launcher& L, float* seed, int B);
 void scatter_snapshot(Launcher& L, const float* o, long long row0, int valid, int S, int d, int col0, float* X);
 void gather_seed(Launcher& L, const float* dX, long long row0, int valid, int R, int S, int d, int col0, float alpha, float* seed, float* amax);
@@ -214,7 +219,7 @@ struct FirstLayerFuse {
 bool tc_first_layer_fusable(int H, const ChunkGeom& g);
 
 // ---- the same four on CTA pairs (tc2_kernels.cu, cta_group::2), taken when tc2_supported(H) ---------------------
-bool tc2_supported(int H);
+bool tc2_supported(const Launcher& L, int H);
 void tc2_layer_fwd(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* w16_l, const float* bias,
                    const void* h_in, void* h_out);
 void tc2_layer_fwd_split(Launcher& L, int precision, int H, int R, int R_ld, const void* w16_l, const float* bias, const void* h_in, void* h_out);

@@ -13,12 +13,6 @@ template <> __device__ __forceinline__ void load8<float>(const float* p, float* 
   const float4 a = *reinterpret_cast<const float4*>(p), b = *reinterpret_cast<const float4*>(p + 4);
   v[0] = a.x; v[1] = a.y; v[2] = a.z; v[3] = a.w; v[4] = b.x; v[5] = b.y; v[6] = b.z; v[7] = b.w;
 }
-template <> __device__ __forceinline__ void load8<__nv_bfloat16>(const __nv_bfloat16* p, float* v) {
-  const uint4 u = *reinterpret_cast<const uint4*>(p);
-  const __nv_bfloat162* h = reinterpret_cast<const __nv_bfloat162*>(&u);
-#pragma unroll
-  for (int i = 0; i < 4; ++i) { const float2 f = __bfloat1622float2(h[i]); v[2 * i] = f.x; v[2 * i + 1] = f.y; }
-}
 template <> __device__ __forceinline__ void load8<__half>(const __half* p, float* v) {
   const uint4 u = *reinterpret_cast<const uint4*>(p);
   const __half2* h = reinterpret_cast<const __half2*>(&u);
@@ -29,13 +23,6 @@ template <typename T> __device__ __forceinline__ void store8(T* p, const float* 
 template <> __device__ __forceinline__ void store8<float>(float* p, const float* v) {
   *reinterpret_cast<float4*>(p) = make_float4(v[0], v[1], v[2], v[3]);
   *reinterpret_cast<float4*>(p + 4) = make_float4(v[4], v[5], v[6], v[7]);
-}
-template <> __device__ __forceinline__ void store8<__nv_bfloat16>(__nv_bfloat16* p, const float* v) {
-  uint4 u;
-  __nv_bfloat162* h = reinterpret_cast<__nv_bfloat162*>(&u);
-#pragma unroll
-  for (int i = 0; i < 4; ++i) h[i] = __floats2bfloat162_rn(v[2 * i], v[2 * i + 1]);
-  *reinterpret_cast<uint4*>(p) = u;
 }
 template <> __device__ __forceinline__ void store8<__half>(__half* p, const float* v) {
   uint4 u;
@@ -129,7 +116,6 @@ void first_layer_fwd(Launcher& L, int C, const NetShape& s, const float* theta, 
   L.check("first_layer_fwd");
 }
 template void first_layer_fwd<float>(Launcher&, int, const NetShape&, const float*, const float*, const float*, const ChunkGeom&, float*, bool);
-template void first_layer_fwd<__nv_bfloat16>(Launcher&, int, const NetShape&, const float*, const float*, const float*, const ChunkGeom&, __nv_bfloat16*, bool);
 template void first_layer_fwd<__half>(Launcher&, int, const NetShape&, const float*, const float*, const float*, const ChunkGeom&, __half*, bool);
 
 // =============================================================================================================
@@ -204,7 +190,6 @@ void out_fwd(Launcher& L, int C, int H, const float* w_out, const float* b_out, 
   L.check("out_fwd");
 }
 template void out_fwd<float>(Launcher&, int, int, const float*, const float*, const ChunkGeom&, const float*, float*, long long, bool);
-template void out_fwd<__nv_bfloat16>(Launcher&, int, int, const float*, const float*, const ChunkGeom&, const __nv_bfloat16*, float*, long long, bool);
 template void out_fwd<__half>(Launcher&, int, int, const float*, const float*, const ChunkGeom&, const __half*, float*, long long, bool);
 
 // =============================================================================================================
@@ -342,7 +327,6 @@ void jet_act_bwd_launch(Launcher& L, int C, int H, const ChunkGeom& g, const flo
   L.check("jet_act_bwd");
 }
 template void jet_act_bwd_launch<float>(Launcher&, int, int, const ChunkGeom&, const float*, const float*, const float*, const float*, float*, float*, float*, float*, const float*);
-template void jet_act_bwd_launch<__nv_bfloat16>(Launcher&, int, int, const ChunkGeom&, const float*, const float*, const float*, const __nv_bfloat16*, __nv_bfloat16*, float*, float*, float*, const float*);
 template void jet_act_bwd_launch<__half>(Launcher&, int, int, const ChunkGeom&, const float*, const float*, const float*, const __half*, __half*, float*, float*, float*, const float*);
 
 // =============================================================================================================
@@ -403,7 +387,6 @@ void first_layer_bwd(Launcher& L, int C, const NetShape& s, const float* xy, con
   L.check("first_layer_bwd");
 }
 template void first_layer_bwd<float>(Launcher&, int, const NetShape&, const float*, const ChunkGeom&, const float*, float*, float*, const float*);
-template void first_layer_bwd<__nv_bfloat16>(Launcher&, int, const NetShape&, const float*, const ChunkGeom&, const __nv_bfloat16*, float*, float*, const float*);
 template void first_layer_bwd<__half>(Launcher&, int, const NetShape&, const float*, const ChunkGeom&, const __half*, float*, float*, const float*);
 
 }  // namespace pigan

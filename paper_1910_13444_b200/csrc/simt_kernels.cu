@@ -310,8 +310,7 @@ __global__ void bias_add_kernel(float* __restrict__ a, const float* __restrict__
 }
 
 // g: LD arrays [ld_rows][HD] (layer stride ld_rows*HD); D [rows]
-void critic_forward(Launcher& L, const NetShape& s, const float* theta, const float* X, int rows, float* g, float* D, float* scratch) {
-  (void)scratch;
+void critic_forward(Launcher& L, const NetShape& s, const float* theta, const float* X, int rows, float* g, float* D) {
   if (rows <= 0) return;
   const float* in = X; int in_dim = s.in_dim;
   for (int l = 1; l <= s.L; ++l) {
@@ -490,15 +489,6 @@ __global__ void build_snapshots_kernel(const float* __restrict__ fake, const flo
 void build_snapshots(Launcher& L, const float* fake, const float* real, const float* eps, int B, int d, float* X) {
   build_snapshots_kernel<<<cdiv((size_t)B * d, 256), 256, 0, L.stream>>>(fake, real, eps, B, d, X);
   L.check("build_snapshots");
-}
-__global__ void scale_copy_kernel(const float* __restrict__ src, float* __restrict__ dst, size_t n, float alpha) {
-  const size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x;
-  if (i < n) dst[i] = alpha * src[i];
-}
-void scale_copy(Launcher& L, const float* src, float* dst, size_t n, float alpha) {
-  if (n == 0) return;
-  scale_copy_kernel<<<cdiv(n, 256), 256, 0, L.stream>>>(src, dst, n, alpha);
-  L.check("scale_copy");
 }
 // seed[0..B) = +1/B (fake rows), seed[B..2B) = -1/B (real rows)
 __global__ void fill_seed_kernel(float* seed, int B) {

@@ -115,17 +115,12 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
           mbar_wait(empty + stage, phase ^ 1);
           uint8_t* sA = stages + stage * Cfg::kStageBytes;
           const uint32_t lbar = mapa_u32(full + stage, 0);
-#ifdef PIGAN_PROBE_NOLOAD
-          if (rank == 0 && elect_one()) mbar_arrive(full + stage);
-          (void)sA; (void)lbar;
-#else
           if (elect_one()) {
             if (rank == 0) mbar_expect_tx(full + stage, 2 * Cfg::kStageBytes);
             tma2_load_2d(sA, &tmA, lbar, kb * 64, ut * 256 + (int)rank * 128);
             tma2_load_3d(sA + k2AStage, &tmB, lbar, rt * 64 + (int)rank * 32, kb * 64, 0);
           }
           __syncwarp();
-#endif
           if (++stage == Cfg::kNumStages) { stage = 0; phase ^= 1; }
         }
       }
@@ -138,18 +133,12 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
       // stage is therefore polled behind the longest MMA of the last k-step, and only repeated (blocking) on a miss.
       int stage = 0; uint32_t phase = 0; int it = 0;
       bool ready = false;                                    // full[stage] of the upcoming k-block already seen complete
-#ifdef PIGAN_PROBE_TIMING
-      long long tm_start = clock64(), tm_te = 0, tm_full = 0, tm0;
-#endif
       constexpr uint32_t idesc0 = umma_idesc(Fmt<T>::umma, 0, 1, 256, nc0 * 64);
       constexpr uint32_t idesc1 = umma_idesc(Fmt<T>::umma, 0, 1, 256, 128);
       for (int t = cluster_id; t < n_tiles; t += n_clusters, ++it) {
         const int buf = it % Cfg::kNumBuf;
         const uint32_t bphase = (it / Cfg::kNumBuf) & 1;
         const bool last_tile = t + n_clusters >= n_tiles;
-#ifdef PIGAN_PROBE_TIMING
-        tm0 = clock64();
-#endif
         // C <= 3: the accumulator is double-buffered.  C = 5 (320 of 512 columns): group 0 (value, x, y) alternates between
         // two placements and group 1 (xx, yy) has one, which the epilogue of the previous tile releases as soon as it has
         // pulled it into registers.  That release arrives ~700 clk after the previous tile's last MMA, so the first kDefer
@@ -159,66 +148,41 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
         if (C == 5) mbar_wait_cluster(tempty0 + (it & 1), (uint32_t)(((it >> 1) & 1) ^ 1));
         else mbar_wait_cluster(tempty + buf, bphase ^ 1);    // both CTAs' epilogues have released what this tile overwrites
         tc_fence_after();
-#ifdef PIGAN_PROBE_TIMING
-        tm_te += clock64() - tm0;
-#endif
         const uint32_t d0 = tmem_base + g0_col(it), d1 = tmem_base + g1_col;
         if (C == 5) {
           int dstage[kDefer > 0 ? kDefer : 1];
 #pragma unroll
           for (int kb = 0; kb < kDefer; ++kb) {
-#ifdef PIGAN_PROBE_TIMING
-            tm0 = clock64();
-#endif
             if (!ready) mbar_wait(full + stage, phase);
             ready = false;
             tc_fence_after();
-#ifdef PIGAN_PROBE_TIMING
-            tm_full += clock64() - tm0;
-#endif
             const uint32_t sA = smem_u32(stages + stage * Cfg::kStageBytes), sB = sA + k2AStage;
-#ifndef PIGAN_PROBE_NOMMA
             if (elect_one()) {
 #pragma unroll
               for (int k = 0; k < 4; ++k)
                 tc2_mma(d0, umma_desc_sw128(sA + k * 32, 16, 1024), umma_desc_sw64(sB + k * 1024, k2BPlane, 512), idesc0, (kb | k) ? 1u : 0u);
             }
             __syncwarp();
-#endif
             dstage[kb] = stage;
             if (++stage == Cfg::kNumStages) { stage = 0; phase ^= 1; }
           }
-#ifdef PIGAN_PROBE_TIMING
-          tm0 = clock64();
-#endif
           mbar_wait_cluster(tempty + buf, bphase ^ 1);       // group 1 of the previous tile is in the epilogue's registers
           tc_fence_after();
-#ifdef PIGAN_PROBE_TIMING
-          tm_te += clock64() - tm0;
-#endif
 #pragma unroll
           for (int kb = 0; kb < kDefer; ++kb) {
             const uint32_t sA = smem_u32(stages + dstage[kb] * Cfg::kStageBytes), sB = sA + k2AStage;
             if (elect_one()) {
-#ifndef PIGAN_PROBE_NOMMA
 #pragma unroll
               for (int k = 0; k < 4; ++k)
                 tc2_mma(d1, umma_desc_sw128(sA + k * 32, 16, 1024), umma_desc_sw64(sB + 3 * k2BPlane + k * 1024, k2BPlane, 512), idesc1, (kb | k) ? 1u : 0u);
-#endif
               tc2_commit(empty + dstage[kb]);
             }
             __syncwarp();
           }
         }
         for (int kb = kDefer; kb < n_kb; ++kb) {
-#ifdef PIGAN_PROBE_TIMING
-          tm0 = clock64();
-#endif
           if (!ready) mbar_wait(full + stage, phase);
           tc_fence_after();
-#ifdef PIGAN_PROBE_TIMING
-          tm_full += clock64() - tm0;
-#endif
           const uint32_t sA = smem_u32(stages + stage * Cfg::kStageBytes), sB = sA + k2AStage;
           int nstage = stage + 1; uint32_t nphase = phase;
           if (nstage == Cfg::kNumStages) { nstage = 0; nphase ^= 1; }
@@ -227,7 +191,6 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
             const uint64_t ad = umma_desc_sw128(sA + k * 32, 16, 1024);                       // K-major: +32 B per 16 elements
             const uint32_t acc = (kb | k) ? 1u : 0u;
             // MN-major SW64: channel planes are 4 KB apart (LBO), 8-unit groups 512 B apart (SBO), 16 units = +1 KB
-#ifndef PIGAN_PROBE_NOMMA
             // C = 5: the two MMAs of a k-step read the same A slice: the first fills the A collector, the second reuses it
             if (C == 5 && k < 3 && elect_one()) tc2_mma_a_fill(d1, ad, umma_desc_sw64(sB + 3 * k2BPlane + k * 1024, k2BPlane, 512), idesc1, acc);
             if (C != 5 && k == 3) ready = !(last_tile && kb == n_kb - 1) && __all_sync(0xffffffffu, mbar_try_wait(full + nstage, nphase));
@@ -240,7 +203,6 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
               ready = !(last_tile && kb == n_kb - 1) && __all_sync(0xffffffffu, mbar_try_wait(full + nstage, nphase));
               if (elect_one()) tc2_mma_a_lastuse(d1, ad, umma_desc_sw64(sB + 3 * k2BPlane + k * 1024, k2BPlane, 512), idesc1, acc);
             }
-#endif
           }
           if (elect_one()) tc2_commit(empty + stage);        // frees the smem slot in both CTAs when these MMAs retire
           __syncwarp();
@@ -249,9 +211,6 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
         if (elect_one()) tc2_commit(tfull + buf);            // accumulator complete (both CTAs)
         __syncwarp();
       }
-#ifdef PIGAN_PROBE_TIMING
-      if (cluster_id == 0 && lane == 0) printf("TIMING mma C=%d MODE=%d tiles=%d total=%lld wait_tempty=%lld wait_full=%lld\n", C, MODE, it, clock64() - tm_start, tm_te, tm_full);
-#endif
     }
   } else if (warp >= 4) {
     // ===================== epilogue: warp (q, hs) owns TMEM lanes / units [32q, 32q+32) x rows [32hs, 32hs+32) ==========
@@ -263,9 +222,6 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
     uint32_t sphase = 0;
     int it = 0;
     const float inv_amax = (MODE == 1 || MODE == 3) ? adj_inv_scale(p.amax) : 1.f;   // constant over the launch: one global load, not one per tile
-#ifdef PIGAN_PROBE_TIMING
-    long long te_start = clock64(), te_tf = 0, te_rel = 0, te0;
-#endif
     for (int t = cluster_id; t < n_tiles; t += n_clusters, ++it) {
       const int ut = t % n_ut, rt = t / n_ut;
       const int buf = it % Cfg::kNumBuf;
@@ -285,14 +241,34 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
         __syncwarp();
         T* gout = reinterpret_cast<T*>(p.out);
         const int ch = lane & 3, ul = lane >> 2;
+        if (MODE == 1) {
+          // The next tile's TMA load (async proxy) overwrites these staging planes: every lane pulls its share into
+          // registers, then orders its generic-proxy accesses before later async-proxy ones (fence.proxy.async), and only
+          // then issues the global stores -- so the fence waits for shared-memory reads, not for store acknowledgements.
+          uint4 v[C][4];
 #pragma unroll
-        for (int c = 0; c < 5; ++c) {
-          if (c < nplanes) {
+          for (int c = 0; c < C; ++c)
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
               const int u = j * 8 + ul;
-              const uint4 v = lds128(stg + c * k2StgPlane + u * 64 + ((ch ^ ((u >> 1) & 3)) << 4));
-              *reinterpret_cast<uint4*>(gout + ((size_t)c * p.H + unit0 + u) * p.R_ld + row0 + ch * 8) = v;
+              v[c][j] = lds128(stg + c * k2StgPlane + u * 64 + ((ch ^ ((u >> 1) & 3)) << 4));
+            }
+          fence_proxy_async();
+#pragma unroll
+          for (int c = 0; c < C; ++c)
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+              *reinterpret_cast<uint4*>(gout + ((size_t)c * p.H + unit0 + j * 8 + ul) * p.R_ld + row0 + ch * 8) = v[c][j];
+        } else {
+#pragma unroll
+          for (int c = 0; c < 5; ++c) {
+            if (c < nplanes) {
+#pragma unroll
+              for (int j = 0; j < 4; ++j) {
+                const int u = j * 8 + ul;
+                const uint4 v = lds128(stg + c * k2StgPlane + u * 64 + ((ch ^ ((u >> 1) & 3)) << 4));
+                *reinterpret_cast<uint4*>(gout + ((size_t)c * p.H + unit0 + u) * p.R_ld + row0 + ch * 8) = v;
+              }
             }
           }
         }
@@ -310,26 +286,13 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
       };
 
       if ((MODE == 1 || MODE == 3) && elect_one()) {         // the previous layer's output jet h^{l-1} -> staging
-        // No fence.proxy.async: every generic-proxy access of the staging planes was a read, or a write that the copy-out
-        // of this warp has read back, all ordered before this point by __syncwarp; the fence would also wait for the
-        // copy-out's global stores to be acknowledged (measured as long-scoreboard stalls on it).
+        // Generic-proxy accesses of the staging planes by the previous tile were fenced (fence.proxy.async) by every lane
+        // inside copy_out (MODE 1) before its trailing __syncwarp; MODE 3 only reads them (see the fence after its loop).
         mbar_expect_tx(sbar + e, C * k2StgPlane);
         for (int c = 0; c < C; ++c) tma_load_3d(stg + c * k2StgPlane, &tmT, sbar + e, row0, unit0, c);
       }
-#ifdef PIGAN_PROBE_TIMING
-      te0 = clock64();
-#endif
       mbar_wait(tfull + buf, bphase);
       tc_fence_after();
-#ifdef PIGAN_PROBE_TIMING
-      te_tf += clock64() - te0; te0 = clock64();
-#endif
-#ifdef PIGAN_PROBE_NOEPI
-      if (MODE == 1 || MODE == 3) { mbar_wait(sbar + e, sphase); sphase ^= 1; }
-      release();
-      if (C == 5) release0();
-      continue;
-#endif
 
       // C = 5: the (xx, yy) group leaves TMEM first
       float kxx[C == 5 ? 32 : 1], kyy[C == 5 ? 32 : 1];
@@ -338,9 +301,6 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
         for (int rc = 0; rc < 4; ++rc) { tmem_ld8(tcol(3) + rc * 8, kxx + rc * 8); tmem_ld8(tcol(4) + rc * 8, kyy + rc * 8); }
         tmem_ld_wait();
         release();
-#ifdef PIGAN_PROBE_TIMING
-        te_rel += clock64() - te0;
-#endif
       }
 
       if (MODE == 0) {
@@ -430,6 +390,7 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
         if (MODE == 1) {
           copy_out(C);
         } else {
+          fence_proxy_async();                               // generic reads of the staging planes before the next tile's TMA writes
           __syncwarp();                                      // every lane is done reading the staging planes before the next loads land
           const float inv = inv_amax;
           atomicAdd(p.An + (size_t)(grow / p.npts) * p.H + unit, bias_acc * inv);
@@ -439,9 +400,6 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
         atomicAdd(p.g_bias + unit, bias_acc * inv_amax);
       }
     }
-#ifdef PIGAN_PROBE_TIMING
-    if (blockIdx.x == 0 && e == 0 && lane == 0) printf("TIMING epi C=%d MODE=%d tiles=%d total=%lld wait_tfull=%lld early_release=%lld\n", C, MODE, it, clock64() - te_start, te_tf, te_rel);
-#endif
   }
   tc_fence_before();
   __syncthreads();
@@ -585,21 +543,17 @@ wgrad2_kernel(const __grid_constant__ CUtensorMap tmA,    // ahat planes, box 64
 // =============================================================================================================
 // host side
 // =============================================================================================================
-bool tc2_supported(int H) {
-  static int disabled = -1;
-  if (disabled < 0) { const char* e = getenv("PIGAN_NO_CTA_PAIRS"); disabled = (e && e[0] == '1') ? 1 : 0; }
-  return !disabled && H % 256 == 0;
-}
+bool tc2_supported(const Launcher& L, int H) { return !L.one_cta && H % 256 == 0; }
 
 template <typename T, int C, int MODE>
 static void launch_jet2(Launcher& L, const CUtensorMap& a, const CUtensorMap& b, const CUtensorMap& t,
                         const Jet2Params& p) {
   using Cfg = Jet2Cfg<C, MODE>;
-  static bool attr_set = false;
+  static unsigned long long attr_done = 0;
   auto kern = jet2_layer_kernel<T, C, MODE>;
-  if (!attr_set) { cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::kSmemBytes); attr_set = true; }
+  ensure_smem_attr(L, kern, Cfg::kSmemBytes, attr_done);
   const int tiles = (p.H / 256) * p.n_row_tiles;
-  const int clusters = std::min(tiles, num_sms() / 2);
+  const int clusters = std::min(tiles, L.num_sms / 2);
   kern<<<2 * clusters, k2Threads, Cfg::kSmemBytes, L.stream>>>(a, b, t, p);
   L.check(MODE == 0 ? "jet_layer_fwd" : MODE == 2 ? "jet_layer_fwd_split" : "jet_layer_bwd");
 }
@@ -649,7 +603,7 @@ void tc2_wgrad(Launcher& L, int precision, int C, int H, int R, int R_ld, const 
   Wgrad2Params p{};
   p.H = H; p.C = C; p.R = R; p.gW = gW; p.amax = amax;
   const int n_tiles = (H / 256) * (H / 256);
-  const int n_cl = num_sms() / 2;
+  const int n_cl = L.num_sms / 2;
   // row slices: one work item per CTA (pair) when that fills >= 90 % of the machine, else two; every extra slice costs one
   // more fp32 red.add pass over the H x H gradient (measured on c2 / c3: 1 slice per CTA is 10 % faster than 2)
   const int units = n_cl;
@@ -663,9 +617,9 @@ void tc2_wgrad(Launcher& L, int precision, int C, int H, int R, int R_ld, const 
         plane_map(L, &b, precision, h_prev, H, R_ld, C, 64, 128, 1, CU_TENSOR_MAP_SWIZZLE_128B)))
     return;
   const int smem = kW2Stages * kW2StageBytes + 1024 + 256;
-  static bool attr_set = false;
+  static unsigned long long attr_done = 0;
   const int clusters = std::min(n_tiles * p.n_slices, n_cl);
-  if (!attr_set) { cudaFuncSetAttribute(wgrad2_kernel<__half>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); attr_set = true; }
+  ensure_smem_attr(L, wgrad2_kernel<__half>, smem, attr_done);
   wgrad2_kernel<__half><<<2 * clusters, 192, smem, L.stream>>>(a, b, p);
   L.check("wgrad");
 }

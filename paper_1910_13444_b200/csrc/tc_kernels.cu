@@ -295,7 +295,7 @@ __global__ void __launch_bounds__(256, 1) jet_layer_kernel(const __grid_constant
 constexpr int kWStages = 4;
 struct WgradParams {
   int H, C;
-  int NW;              // output tile width (min(H, 256))
+  int NW;              // output tile width: 256 when it divides H, else 128
   int n_slices;        // row slices
   int slice_rows;      // rows per slice (multiple of 64)
   int R;               // rows of the chunk (multiple of 64)
@@ -457,11 +457,11 @@ template <typename T, int C, int MODE>
 static void launch_jet(Launcher& L, const CUtensorMap& a, const CUtensorMap& b, const CUtensorMap& o, const CUtensorMap& t,
                        const JetParams& p) {
   using Cfg = JetCfg<C>;
-  static bool attr_set = false;
+  static unsigned long long attr_done = 0;
   auto kern = jet_layer_kernel<T, C, MODE>;
-  if (!attr_set) { cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::kSmemBytes); attr_set = true; }
+  ensure_smem_attr(L, kern, Cfg::kSmemBytes, attr_done);
   const int tiles = (p.H / kBM) * p.n_row_tiles;
-  const int grid = std::min(tiles, num_sms());
+  const int grid = std::min(tiles, L.num_sms);
   kern<<<grid, 256, Cfg::kSmemBytes, L.stream>>>(a, b, o, t, p);
   L.check(MODE == 0 ? "jet_layer_fwd" : MODE == 2 ? "jet_layer_fwd_split" : "jet_layer_bwd");
 }
@@ -480,7 +480,7 @@ static void dispatch_jet(Launcher& L, int precision, int C, const CUtensorMap& a
 
 void tc_layer_fwd(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* w16_l, const float* bias, const void* h_in, void* h_out) {
   if (R <= 0) return;
-  if (tc2_supported(H)) { tc2_layer_fwd(L, precision, C, H, R, R_ld, w16_l, bias, h_in, h_out); return; }
+  if (tc2_supported(L, H)) { tc2_layer_fwd(L, precision, C, H, R, R_ld, w16_l, bias, h_in, h_out); return; }
   CUtensorMap a, b, o;
   bool ok = weight_map(L, &a, precision, w16_l, H) && plane_map(L, &b, precision, h_in, H, R_ld, C, kRT, kBK, C, CU_TENSOR_MAP_SWIZZLE_128B) &&
             plane_map(L, &o, precision, h_out, H, R_ld, C, 32, 32, 1, CU_TENSOR_MAP_SWIZZLE_64B);
@@ -493,7 +493,7 @@ void tc_layer_fwd(Launcher& L, int precision, int C, int H, int R, int R_ld, con
 // value-only layer on split activations (2 planes: hi, lo) -> 2 planes; used where the snapshot X_fake is built
 void tc_layer_fwd_split(Launcher& L, int precision, int H, int R, int R_ld, const void* w16_l, const float* bias, const void* h_in, void* h_out) {
   if (R <= 0) return;
-  if (tc2_supported(H)) { tc2_layer_fwd_split(L, precision, H, R, R_ld, w16_l, bias, h_in, h_out); return; }
+  if (tc2_supported(L, H)) { tc2_layer_fwd_split(L, precision, H, R, R_ld, w16_l, bias, h_in, h_out); return; }
   CUtensorMap a, b, o;
   if (!(weight_map(L, &a, precision, w16_l, H) && plane_map(L, &b, precision, h_in, H, R_ld, 2, kRT, kBK, 2, CU_TENSOR_MAP_SWIZZLE_128B) &&
         plane_map(L, &o, precision, h_out, H, R_ld, 2, 32, 32, 1, CU_TENSOR_MAP_SWIZZLE_64B)))
@@ -508,7 +508,7 @@ bool tc_first_layer_fusable(int H, const ChunkGeom& g) { return H % 128 == 0 && 
 void tc_layer_bwd(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* w16T_l, const void* ahat_in, const void* h_prev,
                   void* ahat_out, float* g_bias_prev, const float* amax, const FirstLayerFuse* fl) {
   if (R <= 0) return;
-  if (tc2_supported(H)) { tc2_layer_bwd(L, precision, C, H, R, R_ld, w16T_l, ahat_in, h_prev, ahat_out, g_bias_prev, amax, fl); return; }
+  if (tc2_supported(L, H)) { tc2_layer_bwd(L, precision, C, H, R, R_ld, w16T_l, ahat_in, h_prev, ahat_out, g_bias_prev, amax, fl); return; }
   CUtensorMap a, b, o, t;
   bool ok = weight_map(L, &a, precision, w16T_l, H) && plane_map(L, &b, precision, ahat_in, H, R_ld, C, kRT, kBK, C, CU_TENSOR_MAP_SWIZZLE_128B) &&
             plane_map(L, &o, precision, ahat_out, H, R_ld, C, 32, 32, 1, CU_TENSOR_MAP_SWIZZLE_64B) &&
@@ -526,13 +526,13 @@ void tc_layer_bwd(Launcher& L, int precision, int C, int H, int R, int R_ld, con
 
 void tc_wgrad(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* ahat, const void* h_prev, float* gW, const float* amax) {
   if (R <= 0) return;
-  if (tc2_supported(H)) { tc2_wgrad(L, precision, C, H, R, R_ld, ahat, h_prev, gW, amax); return; }
+  if (tc2_supported(L, H)) { tc2_wgrad(L, precision, C, H, R, R_ld, ahat, h_prev, gW, amax); return; }
   WgradParams p{};
-  p.H = H; p.C = C; p.NW = std::min(H, 256); p.R = R; p.gW = gW; p.amax = amax;
+  p.H = H; p.C = C; p.NW = (H % 256 == 0) ? 256 : 128; p.R = R; p.gW = gW; p.amax = amax;   // NW must divide H (H = 384, 640, ...)
   const int n_tiles = (H / kBM) * (H / p.NW);
   // row slices: one work item per CTA (pair) when that fills >= 90 % of the machine, else two; every extra slice costs one
   // more fp32 red.add pass over the H x H gradient (measured on c2 / c3: 1 slice per CTA is 10 % faster than 2)
-  const int units = num_sms();
+  const int units = L.num_sms;
   int slices = std::max(1, units / n_tiles);
   if (n_tiles * slices * 10 < units * 9) slices = std::max(1, (2 * units) / n_tiles);
   int slice_rows = ((R + slices - 1) / slices + 63) / 64 * 64;
@@ -543,9 +543,9 @@ void tc_wgrad(Launcher& L, int precision, int C, int H, int R, int R_ld, const v
         plane_map(L, &b, precision, h_prev, H, R_ld, C, 64, p.NW, 1, CU_TENSOR_MAP_SWIZZLE_128B)))
     return;
   const int smem = kWStages * (kAStage + 256 * 128) + 1024 + 256;
-  static bool attr_set = false;
-  const int grid = std::min(n_tiles * p.n_slices, num_sms());
-  if (!attr_set) { cudaFuncSetAttribute(wgrad_kernel<__half>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); attr_set = true; }
+  static unsigned long long attr_done = 0;
+  const int grid = std::min(n_tiles * p.n_slices, L.num_sms);
+  ensure_smem_attr(L, wgrad_kernel<__half>, smem, attr_done);
   wgrad_kernel<__half><<<grid, 192, smem, L.stream>>>(a, b, p);
   L.check("wgrad");
 }

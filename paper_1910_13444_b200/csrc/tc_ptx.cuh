@@ -78,9 +78,6 @@ __device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, u
                : "memory");
 }
 __device__ __forceinline__ void tma_store_3d(const CUtensorMap* map, const void* src, int c0, int c1, int c2) {
-#ifdef PIGAN_PROBE_NOSTORE
-  return;
-#endif
   asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.bulk_group [%0, {%2, %3, %4}], [%1];" ::"l"(map), "r"(smem_u32(src)), "r"(c0),
                "r"(c1), "r"(c2)
                : "memory");
@@ -136,7 +133,6 @@ __host__ __device__ constexpr uint32_t umma_idesc(int fmt16, int a_mn, int b_mn,
 }
 
 template <typename T> struct Fmt;
-template <> struct Fmt<__nv_bfloat16> { static constexpr int umma = 1; };
 template <> struct Fmt<__half> { static constexpr int umma = 0; };
 
 __device__ __forceinline__ float fast_tanh(float x) {
@@ -145,16 +141,11 @@ __device__ __forceinline__ float fast_tanh(float x) {
   return y;
 }
 template <typename T> __device__ __forceinline__ uint32_t pack2(float a, float b);
-template <> __device__ __forceinline__ uint32_t pack2<__nv_bfloat16>(float a, float b) {
-  __nv_bfloat162 v = __floats2bfloat162_rn(a, b);
-  return *reinterpret_cast<uint32_t*>(&v);
-}
 template <> __device__ __forceinline__ uint32_t pack2<__half>(float a, float b) {
   __half2 v = __floats2half2_rn(a, b);
   return *reinterpret_cast<uint32_t*>(&v);
 }
 template <typename T> __device__ __forceinline__ float2 unpack2(uint32_t u);
-template <> __device__ __forceinline__ float2 unpack2<__nv_bfloat16>(uint32_t u) { return __bfloat1622float2(*reinterpret_cast<__nv_bfloat162*>(&u)); }
 template <> __device__ __forceinline__ float2 unpack2<__half>(uint32_t u) { return __half22float2(*reinterpret_cast<__half2*>(&u)); }
 
 template <typename T> __device__ __forceinline__ uint4 pack8(const float* v) {
@@ -275,6 +266,7 @@ inline EncodeTiledFn get_encode() {
   return fn;
 }
 
+// precision: both 16-bit modes carry fp16 planes and weight copies (include/pigan.h: PIGAN_BF16 is an alias of PIGAN_FP16)
 inline bool make_map(Launcher& L, CUtensorMap* m, int precision, const void* base, int rank, const cuuint64_t* dims, const cuuint64_t* strides_bytes,
                      const cuuint32_t* box, CUtensorMapSwizzle swz) {
   EncodeTiledFn fn = get_encode();
@@ -301,12 +293,6 @@ inline bool weight_map(Launcher& L, CUtensorMap* m, int precision, const void* b
   cuuint64_t str[1] = {(cuuint64_t)H * 2};
   cuuint32_t box[2] = {64, 128};   // 64 contraction elements (128 B) x 128 units
   return make_map(L, m, precision, base, 2, dims, str, box, CU_TENSOR_MAP_SWIZZLE_128B);
-}
-
-inline int num_sms() {
-  static int n = 0;
-  if (!n) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev); if (n <= 0) n = 148; }
-  return n;
 }
 
 

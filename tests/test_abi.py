@@ -35,11 +35,11 @@ def test_param_count_and_null_handling():
 def test_create_validates_config_before_touching_cuda():
     lib = pkg.load_library()
     ctx = ctypes.c_void_p()
-    bad_shape = pkg._Config(pkg._MlpShape(7, 3, 32), pkg._MlpShape(20, 3, 32), 4, 16, 64, 10, 0, 10.0, 1.0, 0)   # gen.in_dim != 2 + m
+    bad_shape = pkg._Config(pkg._MlpShape(7, 3, 32), pkg._MlpShape(20, 3, 32), 4, 16, 64, 10, 0, 10.0, 1.0, 0, 0, 0)   # gen.in_dim != 2 + m
     assert lib.pigan_create(ctypes.byref(bad_shape), None, ctypes.byref(ctx)) == 2                                   # SHAPE
-    unsup = pkg._Config(pkg._MlpShape(6, 3, 32), pkg._MlpShape(20, 3, 32), 4, 16, 64, 10, 1, 10.0, 1.0, 0)         # bf16 with width 32
+    unsup = pkg._Config(pkg._MlpShape(6, 3, 32), pkg._MlpShape(20, 3, 32), 4, 16, 64, 10, 1, 10.0, 1.0, 0, 0, 0)         # bf16 with width 32
     assert lib.pigan_create(ctypes.byref(unsup), None, ctypes.byref(ctx)) == 5                                       # UNSUPPORTED
-    neg = pkg._Config(pkg._MlpShape(6, 0, 32), pkg._MlpShape(20, 3, 32), 4, 16, 64, 10, 0, 10.0, 1.0, 0)
+    neg = pkg._Config(pkg._MlpShape(6, 0, 32), pkg._MlpShape(20, 3, 32), 4, 16, 64, 10, 0, 10.0, 1.0, 0, 0, 0)
     assert lib.pigan_create(ctypes.byref(neg), None, ctypes.byref(ctx)) == 1
 
 

@@ -146,6 +146,52 @@ def test_c3_reduced_rows_bf16():
     check_step(wl.CONFIGS["c3"].reduced(16, 32), bias_std=0.0)
 
 
+def test_c3_full_size_step_and_graph_replay():
+    """c3 at its BASELINE size (128 samples x 64x64 grid, f = 8 sinusoids, 200 sensors): every gradient tensor and the six
+    losses against the oracle ('c1-c3: full-config oracle vs GPU on every output'), eagerly and through
+    the CUDA-graph replay that bench.py times for c1-c3 (CTA-pair kernels, 256 row tiles per pair and launch)."""
+    cfg = wl.CONFIGS["c3"]
+    check_step(cfg, bias_std=0.0)
+    check_step(cfg, bias_std=0.0, calls=3)                  # call 2 captures, call 3 replays
+
+
+@pytest.mark.parametrize("name,N,G,chunk", [("c4", 8, 64, 8192), ("c5", 4, 64, 4096)])
+def test_c4_c5_dims_many_tiles_per_cta_pair(name, N, G, chunk):
+    """Full network dimensions with N' x 64 x 64 rows: 1024 tiles of 256 units x 64 rows, ~14 per CTA pair, so the
+    persistent loops wrap (phase flips, alternating TMEM placement, deferred MMAs) with n_ut = 2 (c4) and 4 (c5) and the
+    wgrad decodes several row slices -- all gradients against the ORACLE.  Run with the default chunking and with 4 chunks."""
+    cfg = wl.CONFIGS[name].reduced(N, G)
+    ls = 1024.0 if cfg.precision == "fp16" else 1.0
+    check_step(cfg, bias_std=0.0, loss_scale=ls)
+    check_step(cfg, bias_std=0.0, loss_scale=ls, chunk_rows=chunk)
+
+
+def test_width_384_one_cta_kernels_and_one_cta_flag():
+    """Widths that are multiples of 128 but not of 256 run the one-CTA tcgen05 kernels (wgrad tile width must divide H);
+    PIGAN_FLAG_ONE_CTA forces the same kernels on a CTA-pair width."""
+    from paper_1910_13444_b200 import FLAG_ONE_CTA
+    cfg = dataclasses.replace(wl.CONFIGS["c3"], name="w384", H=384, HD=128, N=6, G=16, S=24, f_kind="zero")
+    check_step(cfg)
+    cfg = dataclasses.replace(wl.CONFIGS["c4"], name="c4-onecta", N=4, G=16, S=40, m=64, HD=128, LD=3)
+    check_step(cfg, flags=FLAG_ONE_CTA)
+
+
+@pytest.mark.parametrize("gain", [2.5, 40.0])
+def test_enlarged_weights_are_correct_or_flagged(gain):
+    """Hidden-layer weights scaled over Xavier-at-init: the derivative planes grow with the products of the layer gains and
+    have fp16 range (R2).  Either the step matches the oracle, or the overflow is reported through found_inf --
+    never silently wrong finite values."""
+    cfg = dataclasses.replace(wl.CONFIGS["c4"], name=f"c4-gain{gain}", N=4, G=16, S=40, m=64, HD=128, LD=3)
+    errs, lg, lr, found_inf = step_parity(cfg, weight_gain=gain)
+    if found_inf == 0:
+        bad = {k: v for k, v in errs.items() if not v <= TOL[cfg.precision]}
+        assert not bad, (gain, bad)
+        lrel = np.abs(lg - lr) / np.maximum(np.abs(lr), 1e-12)
+        assert np.all(lrel <= LOSS_TOL), (gain, lg, lr)
+    else:
+        assert found_inf == 1
+
+
 def test_c4_full_dims_reduced_rows_bf16():
     check_step(wl.CONFIGS["c4"].reduced(4, 16), bias_std=0.0)
 
@@ -203,6 +249,10 @@ def test_full_size_jets_sampled_against_oracle(name):
         assert rel_err(gotU[c], refU[c]) <= 2e-2, (name, "u", c, rel_err(gotU[c], refU[c]))
     for c in range(3):
         assert rel_err(gotY[c], refY[c]) <= 2e-2, (name, "Y", c)
+    # r itself at the sampled pairs against the residual of the ORACLE's jets (SURVEY.md 8(d) protocol (ii))
+    r_orc, _ = orc.darcy_residual_ref(refY, refU, inp["f"][ps])
+    got_r = r[ns][:, ps].cpu().numpy()
+    assert rel_err(got_r, r_orc) <= 2e-2, (name, "r", rel_err(got_r, r_orc))
     r_ref, _ = orc.darcy_residual_ref(Y.cpu().numpy(), U.cpu().numpy(), inp["f"])
     assert abs(msq.item() - float(np.mean(r_ref * r_ref))) <= 1e-4 * float(np.mean(r_ref * r_ref))
     pg.close()

@@ -36,3 +36,21 @@ def test_skip_leaves_state_bit_identical():
     rng = np.random.default_rng(0); th, g, m, v = (rng.normal(size=5) for _ in range(4)); v = v * v
     t2, m2, v2 = orc.adam_update_ref(th, g, m, v, 3, LR, B1, B2, EPS, skip=True)
     assert np.array_equal(t2, th) and np.array_equal(m2, m) and np.array_equal(v2, v)
+
+
+def test_three_steps_worked_by_hand():
+    """tests/golden/adam_three_steps.txt: four elements, three steps, exact fractions derived by hand in the file."""
+    import os
+    from fractions import Fraction
+    rows = []
+    with open(os.path.join(os.path.dirname(__file__), "golden", "adam_three_steps.txt")) as fh:
+        for line in fh:
+            if line.strip() and not line.startswith("#"):
+                rows.append([float(Fraction(tok)) for tok in line.split()[1:]])
+    rows = np.array(rows)
+    assert rows.shape == (4, 9)
+    th, m, v = rows[:, 0].copy(), np.zeros(4), np.zeros(4)
+    for t in range(1, 4):
+        th, m, v = orc.adam_update_ref(th, rows[:, t], m, v, t, 1.0, 0.5, 0.5, 1.0)
+        assert np.allclose(th, rows[:, 3 + t], rtol=1e-14, atol=0), (t, th, rows[:, 3 + t])
+    assert np.allclose(m, rows[:, 7], rtol=1e-14) and np.allclose(v, rows[:, 8], rtol=1e-14)
