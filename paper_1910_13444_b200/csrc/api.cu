@@ -17,6 +17,7 @@ namespace {
 struct NetWs {                 // activation workspace of one generator net (planes are [channel][unit][row])
   int Cmax = 0;
   char* h = nullptr;           // L x [Cmax][H][R_ld]      post-activations h^1..h^L
+  char* hs = nullptr;          // sensor rows: n_sens_chunks x L x [2][H][R_ld]  (hi, lo) planes of the snapshot forward, kept for the reverse sweep
   char* ah[2] = {nullptr, nullptr};   // adjoint ping-pong, [Cmax][H][R_ld]
   float* apre = nullptr;       // fp32 mode: [Cmax][H][R_ld] pre-activations / hhat scratch
   float* o = nullptr;          // [Cmax][R_ld] outputs of the chunk
@@ -60,8 +61,12 @@ struct pigan_ctx {
     allocs.push_back(p);
     return reinterpret_cast<T*>(p);
   }
+  int n_sens_chunks = 1;
   size_t plane() const { return (size_t)gen.H * R_ld * elem; }
-  char* h(int n, int l) { return net[n].h + (size_t)(l - 1) * net[n].Cmax * plane(); }              // l = 1..L
+  // activation stash of one chunk: `planes` planes per layer; l = 1..L
+  struct HBuf { char* base; int planes; size_t plane_bytes; char* at(int l) const { return base + (size_t)(l - 1) * planes * plane_bytes; } };
+  HBuf hcol(int n) { return HBuf{net[n].h, net[n].Cmax, plane()}; }
+  HBuf hsens(int n, int chunk) { return HBuf{net[n].hs + (size_t)chunk * gen.L * 2 * plane(), 2, plane()}; }
   void* w16(int n, int l, int transposed) { return (char*)net[n].w16 + ((size_t)(l - 2) * 2 + transposed) * gen.H * gen.H * 2; }
 };
 
@@ -96,8 +101,8 @@ size_t round_up(size_t a, size_t b) { return (a + b - 1) / b * b; }
 
 // ---- one chunk of generator rows, forward ------------------------------------------------------------------------
 template <typename T>
-void gen_forward_chunk(pigan_ctx* c, int n, const float* theta, int C, const float* xy, const ChunkGeom& g, float* o, long long o_stride,
-                       bool split = false) {
+void gen_forward_chunk(pigan_ctx* c, int n, const pigan_ctx::HBuf& hb, const float* theta, int C, const float* xy, const ChunkGeom& g, float* o,
+                       long long o_stride, bool split = false, bool keep_last = true) {
   const NetShape& s = c->gen;
   Launcher& L = c->L;
   const int H = s.H;
@@ -105,51 +110,56 @@ void gen_forward_chunk(pigan_ctx* c, int n, const float* theta, int C, const flo
   // split (16-bit modes, value channel only): activations are carried as two 16-bit planes hi + lo, so that the
   // snapshot X_fake the critic sees is accurate to ~2^-17 (the loss values are compared at 1e-3 relative)
   split = split && C == 1 && c->cfg.precision != PIGAN_FP32;
-  first_layer_fwd<T>(L, C, s, theta, c->net[n].Zp, xy, g, (T*)c->h(n, 1), split);
+  first_layer_fwd<T>(L, C, s, theta, c->net[n].Zp, xy, g, (T*)hb.at(1), split);
+  // the output layer (a4) rides in the epilogue of the last hidden layer where the kernels support it
+  const bool fuse_out = c->cfg.precision != PIGAN_FP32 && s.L >= 2 && tc_out_dot_fusable(L, H);
   for (int l = 2; l <= s.L; ++l) {
     if (c->cfg.precision == PIGAN_FP32) {
       // a_c = W_l h_c^{l-1}: M = H, N = rows, K = H, batched over the C channel planes
-      sgemm(L, false, false, H, g.R, H, theta + s.W_off(l), H, 0, (const float*)c->h(n, l - 1), g.R_ld, pl, c->net[n].apre, g.R_ld, pl, C, false);
-      jet_act_fwd_f32(L, C, H, theta + s.b_off(l), g, c->net[n].apre, (float*)c->h(n, l));
-    } else if (split) {
-      tc_layer_fwd_split(L, c->cfg.precision, H, g.R, g.R_ld, c->w16(n, l, 0), theta + s.b_off(l), c->h(n, l - 1), c->h(n, l));
-    } else {
-      tc_layer_fwd(L, c->cfg.precision, C, H, g.R, g.R_ld, c->w16(n, l, 0), theta + s.b_off(l), c->h(n, l - 1), c->h(n, l));
+      sgemm(L, false, false, H, g.R, H, theta + s.W_off(l), H, 0, (const float*)hb.at(l - 1), g.R_ld, pl, c->net[n].apre, g.R_ld, pl, C, false);
+      jet_act_fwd_f32(L, C, H, theta + s.b_off(l), g, c->net[n].apre, (float*)hb.at(l));
+      continue;
     }
+    OutDot od{theta + s.W_off(s.L + 1), theta + s.b_off(s.L + 1), o, o_stride, g.valid};
+    const OutDot* odp = (fuse_out && l == s.L) ? &od : nullptr;
+    void* h_out = (odp && !keep_last) ? nullptr : hb.at(l);
+    if (odp) cudaMemset2DAsync(o, (size_t)o_stride * 4, 0, (size_t)g.valid * 4, C, L.stream);
+    if (split) tc_layer_fwd_split(L, c->cfg.precision, H, g.R, g.R_ld, c->w16(n, l, 0), theta + s.b_off(l), hb.at(l - 1), h_out, odp);
+    else tc_layer_fwd(L, c->cfg.precision, C, H, g.R, g.R_ld, c->w16(n, l, 0), theta + s.b_off(l), hb.at(l - 1), h_out, odp);
   }
-  out_fwd<T>(L, C, H, theta + s.W_off(s.L + 1), theta + s.b_off(s.L + 1), g, (const T*)c->h(n, s.L), o, o_stride, split);
+  if (!fuse_out) out_fwd<T>(L, C, H, theta + s.W_off(s.L + 1), theta + s.b_off(s.L + 1), g, (const T*)hb.at(s.L), o, o_stride, split);
 }
 
 // ---- one chunk of generator rows, reverse sweep; output adjoints are in net[n].oh [C][R_ld] ------------------------
 template <typename T>
-void gen_backward_chunk(pigan_ctx* c, int n, const float* theta, float* grads, int C, const float* xy, const ChunkGeom& g) {
+void gen_backward_chunk(pigan_ctx* c, int n, const pigan_ctx::HBuf& hb, const float* theta, float* grads, int C, const float* xy, const ChunkGeom& g) {
   const NetShape& s = c->gen;
   Launcher& L = c->L;
   const int H = s.H;
   const long long pl = (long long)H * g.R_ld;
   int cur = 0;
   const float* amax = c->cfg.precision == PIGAN_FP32 ? nullptr : c->amax + n;
-  jet_act_bwd_launch<T>(L, C, H, g, nullptr, theta + s.W_off(s.L + 1), c->net[n].oh, (const T*)c->h(n, s.L),
+  jet_act_bwd_launch<T>(L, C, H, g, nullptr, theta + s.W_off(s.L + 1), c->net[n].oh, (const T*)hb.at(s.L),
                         (T*)c->net[n].ah[cur], grads + s.b_off(s.L),
                         grads + s.W_off(s.L + 1), grads + s.b_off(s.L + 1), amax);
   for (int l = s.L; l >= 2; --l) {
     if (c->cfg.precision == PIGAN_FP32) {
       // W_hat_l += sum_c ahat_c h_c^{l-1 T}: M = H, N = H, K = rows
-      sgemm(L, false, true, H, H, g.R, (const float*)c->net[n].ah[cur], g.R_ld, pl, (const float*)c->h(n, l - 1), g.R_ld, pl, grads + s.W_off(l), H, 0, C, true);
+      sgemm(L, false, true, H, H, g.R, (const float*)c->net[n].ah[cur], g.R_ld, pl, (const float*)hb.at(l - 1), g.R_ld, pl, grads + s.W_off(l), H, 0, C, true);
       // hhat_c^{l-1} = W_l^T ahat_c: M = H (in), N = rows, K = H (out); A stored [K][M]
       sgemm(L, true, false, H, g.R, H, theta + s.W_off(l), H, 0, (const float*)c->net[n].ah[cur], g.R_ld, pl, c->net[n].apre, g.R_ld, pl, C, false);
-      jet_act_bwd_launch<T>(L, C, H, g, c->net[n].apre, nullptr, nullptr, (const T*)c->h(n, l - 1),
+      jet_act_bwd_launch<T>(L, C, H, g, c->net[n].apre, nullptr, nullptr, (const T*)hb.at(l - 1),
                             (T*)c->net[n].ah[cur ^ 1], grads + s.b_off(l - 1), nullptr, nullptr, amax);
     } else {
-      tc_wgrad(L, c->cfg.precision, C, H, g.R, g.R_ld, c->net[n].ah[cur], c->h(n, l - 1), grads + s.W_off(l), amax);
+      tc_wgrad(L, c->cfg.precision, C, H, g.R, g.R_ld, c->net[n].ah[cur], hb.at(l - 1), grads + s.W_off(l), amax);
       if (l == 2 && tc_first_layer_fusable(H, g)) {
         // the adjoint of the first tanh layer is reduced inside the dgrad epilogue (ahat^1 is never written)
         FirstLayerFuse fl{xy, g.row0, g.npts, s.in_dim, grads, c->net[n].An};
-        tc_layer_bwd(L, c->cfg.precision, C, H, g.R, g.R_ld, c->w16(n, l, 1), c->net[n].ah[cur], c->h(n, l - 1),
+        tc_layer_bwd(L, c->cfg.precision, C, H, g.R, g.R_ld, c->w16(n, l, 1), c->net[n].ah[cur], hb.at(l - 1),
                      c->net[n].ah[cur ^ 1], grads + s.b_off(l - 1), amax, &fl);
         return;
       }
-      tc_layer_bwd(L, c->cfg.precision, C, H, g.R, g.R_ld, c->w16(n, l, 1), c->net[n].ah[cur], c->h(n, l - 1),
+      tc_layer_bwd(L, c->cfg.precision, C, H, g.R, g.R_ld, c->w16(n, l, 1), c->net[n].ah[cur], hb.at(l - 1),
                    c->net[n].ah[cur ^ 1], grads + s.b_off(l - 1), amax);
     }
     cur ^= 1;
@@ -181,7 +191,7 @@ pigan_status jet_forward_impl(pigan_ctx* c, const float* theta, const float* xy,
   if (c->cfg.precision != PIGAN_FP32) tc_convert_weights(c->L, c->cfg.precision, c->gen, theta, c->net[n].w16);
   for (long long row0 = 0; row0 < total; row0 += c->R_ld) {
     ChunkGeom g = make_geom(c, row0, total, n_pts);
-    gen_forward_chunk<T>(c, n, theta, C, xy, g, out + row0, total, /*split=*/C == 1);
+    gen_forward_chunk<T>(c, n, c->hcol(n), theta, C, xy, g, out + row0, total, /*split=*/C == 1, /*keep_last=*/false);
   }
   return finish(c);
 }
@@ -205,31 +215,37 @@ pigan_status train_step_impl(pigan_ctx* c, const float* thY, const float* thU, c
     compute_zpart(c, n, th[n], z, N);
     if (cfg.precision != PIGAN_FP32) tc_convert_weights(L, cfg.precision, gs, th[n], c->net[n].w16);
   }
-  // ---- a6: sensor evaluation -> X_fake ----
+  // ---- a6: sensor evaluation -> X_fake; the (hi) activation planes of every sensor chunk stay in net[n].hs for the reverse sweep ----
   const long long srows = (long long)N * S;
-  for (long long row0 = 0; row0 < srows; row0 += c->R_ld) {
+  int sc = 0;
+  for (long long row0 = 0; row0 < srows; row0 += c->R_ld, ++sc) {
     ChunkGeom g = make_geom(c, row0, srows, S);
     for (int n = 0; n < 2; ++n) {
-      gen_forward_chunk<T>(c, n, th[n], 1, xy_s, g, c->net[n].o, c->R_ld, /*split=*/true);
+      gen_forward_chunk<T>(c, n, c->hsens(n, sc), th[n], 1, xy_s, g, c->net[n].o, c->R_ld, /*split=*/true);
       scatter_snapshot(L, c->net[n].o, row0, g.valid, S, d, n * S, c->xfake);
     }
   }
   // ---- a7-a9: critic losses and gradient; dX rows [0, N) = (1/N) grad_X D(X_fake) ----
-  build_snapshots(L, c->xfake, real, eps, N, d, c->cw.X);
-  critic_forward(L, ds, thD, c->cw.X, 3 * N, c->cw.g, c->cw.D);
-  reduce_scores(L, c->cw.D, N, c->cw.acc);
-  fill_seed(L, c->seed, N);
-  const int gstride = 3 * N * HD;
-  critic_backward(L, ds, thD, c->cw.X, c->cw.g, 2 * N, gstride, c->seed, gD, c->dX, c->cw.t0, c->cw.t1);
-  critic_gp(L, ds, thD, c->cw.X + (size_t)2 * N * d, c->cw.g + (size_t)2 * N * HD, N, gstride, cfg.gp_lambda, c->cw, gD, nullptr);
+  if (critic_fused_supported(ds)) {
+    // small critic: one kernel for every per-row sweep + the batched weight-gradient GEMMs (critic_fused.cu)
+    critic_fused(L, ds, thD, c->xfake, real, eps, N, 1, cfg.gp_lambda, c->cw, gD, c->dX, nullptr);
+  } else {
+    build_snapshots(L, c->xfake, real, eps, N, d, c->cw.X);
+    critic_forward(L, ds, thD, c->cw.X, 3 * N, c->cw.g, c->cw.D);
+    reduce_scores(L, c->cw.D, N, c->cw.acc);
+    fill_seed(L, c->seed, N);
+    const int gstride = 3 * N * HD;
+    critic_backward(L, ds, thD, c->cw.X, c->cw.g, 2 * N, gstride, c->seed, gD, c->dX, c->cw.t0, c->cw.t1);
+    critic_gp(L, ds, thD, c->cw.X + (size_t)2 * N * d, c->cw.g + (size_t)2 * N * HD, N, gstride, cfg.gp_lambda, c->cw, gD, nullptr);
+  }
   // ---- O7 + a10 on the sensor rows: dL_G/dX_fake = -(1/N) grad_X D(X_fake), value channel only ----
-  for (long long row0 = 0; row0 < srows; row0 += c->R_ld) {
+  sc = 0;
+  for (long long row0 = 0; row0 < srows; row0 += c->R_ld, ++sc) {
     ChunkGeom g = make_geom(c, row0, srows, S);
     for (int n = 0; n < 2; ++n) {
-      gen_forward_chunk<T>(c, n, th[n], 1, xy_s, g, c->net[n].o, c->R_ld);
       cudaMemsetAsync(c->amax + n, 0, 4, st);
       gather_seed(L, c->dX, row0, g.valid, g.R, S, d, n * S, -loss_scale, c->net[n].oh, c->amax + n);
-      gen_backward_chunk<T>(c, n, th[n], gr[n], 1, xy_s, g);
+      gen_backward_chunk<T>(c, n, c->hsens(n, sc), th[n], gr[n], 1, xy_s, g);
     }
   }
   // ---- a1-a5, a10 on the collocation rows ----
@@ -237,13 +253,13 @@ pigan_status train_step_impl(pigan_ctx* c, const float* thY, const float* thU, c
   const float seed_scale = (float)(2.0 * cfg.pde_weight / (double)crows * loss_scale);
   for (long long row0 = 0; row0 < crows; row0 += c->R_ld) {
     ChunkGeom g = make_geom(c, row0, crows, P);
-    gen_forward_chunk<T>(c, 0, thY, 3, xy_c, g, c->net[0].o, c->R_ld);
-    gen_forward_chunk<T>(c, 1, thU, 5, xy_c, g, c->net[1].o, c->R_ld);
+    gen_forward_chunk<T>(c, 0, c->hcol(0), thY, 3, xy_c, g, c->net[0].o, c->R_ld);
+    gen_forward_chunk<T>(c, 1, c->hcol(1), thU, 5, xy_c, g, c->net[1].o, c->R_ld);
     cudaMemsetAsync(c->amax, 0, 8, st);
     residual(L, c->net[0].o, c->R_ld, c->net[1].o, c->R_ld, f, row0, g.valid, g.R, P, nullptr, c->cw.acc + 3, seed_scale, c->net[0].oh,
              c->net[1].oh, c->R_ld, c->amax, c->amax + 1);
-    gen_backward_chunk<T>(c, 0, thY, gY, 3, xy_c, g);
-    gen_backward_chunk<T>(c, 1, thU, gU, 5, xy_c, g);
+    gen_backward_chunk<T>(c, 0, c->hcol(0), thY, gY, 3, xy_c, g);
+    gen_backward_chunk<T>(c, 1, c->hcol(1), thU, gU, 5, xy_c, g);
   }
   // ---- finalize: z-part of the first layer, unscale, inf/nan flag, loss scalars ----
   for (int n = 0; n < 2; ++n) {
@@ -347,12 +363,14 @@ pigan_status pigan_create(const pigan_config* cfg, void* cuda_stream, pigan_ctx*
   rows = std::min<long long>(rows, (long long)round_up((size_t)max_rows, 256));
   rows = std::max<long long>(rows / 256 * 256, 256);            // workspace_bytes is a hint: never below one 256-row chunk
   c->R_ld = (int)rows;
+  c->n_sens_chunks = (int)(((long long)N * S + c->R_ld - 1) / c->R_ld);
   try {
     for (int n = 0; n < 2; ++n) {
       NetWs& w = c->net[n];
       w.Cmax = n == 0 ? 3 : 5;
       const size_t pl = c->plane();
       w.h = c->alloc<char>((size_t)Lh * w.Cmax * pl);
+      w.hs = c->alloc<char>((size_t)c->n_sens_chunks * Lh * 2 * pl);
       w.ah[0] = c->alloc<char>((size_t)w.Cmax * pl);
       w.ah[1] = c->alloc<char>((size_t)w.Cmax * pl);
       if (f32) w.apre = c->alloc<float>((size_t)w.Cmax * H * c->R_ld);
@@ -376,6 +394,11 @@ pigan_status pigan_create(const pigan_config* cfg, void* cuda_stream, pigan_ctx*
     cw.adjs = c->alloc<float>((size_t)LD * N * HD);
     cw.nu = c->alloc<float>((size_t)N);
     cw.acc = c->alloc<double>(8);
+    if (critic_fused_supported(c->disc)) {
+      cw.cfA = c->alloc<float>((size_t)LD * 4 * N * HD);
+      cw.cfB1 = c->alloc<float>((size_t)4 * N * d);
+      cw.cfBh = c->alloc<float>((size_t)LD * 4 * N * HD);
+    }
     c->xfake = c->alloc<float>((size_t)N * d);
     c->dX = c->alloc<float>((size_t)2 * N * d);
     c->seed = c->alloc<float>((size_t)2 * N);
@@ -457,10 +480,14 @@ pigan_status pigan_gradient_penalty(pigan_ctx* c, const float* disc_params, cons
   cudaStream_t st = c->L.stream;
   cudaMemsetAsync(c->cw.acc, 0, 8 * sizeof(double), st);
   if (d_disc_params) cudaMemsetAsync(d_disc_params, 0, ds.count() * 4, st);
-  build_snapshots(c->L, fake, real, eps, B, d, c->cw.X);
-  float* Xhat = c->cw.X + (size_t)2 * B * d;
-  critic_forward(c->L, ds, disc_params, Xhat, B, c->cw.g, c->cw.D);
-  critic_gp(c->L, ds, disc_params, Xhat, c->cw.g, B, B * HD, c->cfg.gp_lambda, c->cw, d_disc_params, grad_norm);
+  if (critic_fused_supported(ds)) {
+    critic_fused(c->L, ds, disc_params, fake, real, eps, B, 0, c->cfg.gp_lambda, c->cw, d_disc_params, nullptr, grad_norm);
+  } else {
+    build_snapshots(c->L, fake, real, eps, B, d, c->cw.X);
+    float* Xhat = c->cw.X + (size_t)2 * B * d;
+    critic_forward(c->L, ds, disc_params, Xhat, B, c->cw.g, c->cw.D);
+    critic_gp(c->L, ds, disc_params, Xhat, c->cw.g, B, B * HD, c->cfg.gp_lambda, c->cw, d_disc_params, grad_norm);
+  }
   if (gp) write_losses(c->L, c->cw.acc, B, 1, c->cfg.gp_lambda, 0.f, nullptr, gp, nullptr, 0);
   return finish(c);
 }

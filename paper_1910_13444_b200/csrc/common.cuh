@@ -177,7 +177,14 @@ struct CriticWs {
   float* nu = nullptr;      // [B]
   double* acc = nullptr;    // [8] accumulators: 0 sum D fake, 1 sum D real, 2 sum (nu-1)^2, 3 sum r^2
   int maxB = 0;
+  // fused path (critic_fused.cu): per-row factors of the weight gradients, V_hat_l = A_l^T B_l
+  float* cfA = nullptr;     // [LD][4B][HD]
+  float* cfB1 = nullptr;    // [4B][d]
+  float* cfBh = nullptr;    // [LD][4B][HD]
 };
+bool critic_fused_supported(const NetShape& s);
+void critic_fused(Launcher& L, const NetShape& s, const float* theta, const float* fake, const float* real, const float* eps, int B, int plain,
+                  float lambda, CriticWs& w, float* grads, float* dX, float* grad_norm);
 void critic_forward(Launcher& L, const NetShape& s, const float* theta, const float* X, int rows, float* g, float* D);
 // plain backprop of sum_b seed[b] D(X_b) over `rows` rows starting at activations g; accumulates into grads if non-null;
 // writes d/dX into dX if non-null.
@@ -198,10 +205,15 @@ struct TcPlan;   // opaque: tensor maps + 16-bit weight copies for one (net, chu
 bool tc_supported(int H, std::string* why);
 // Converts W_l (l = 2..L) of one net to 16-bit: w16[(l-2)*2+0] = W_l [out][in], w16[(l-2)*2+1] = W_l^T [in][out].
 void tc_convert_weights(Launcher& L, int precision, const NetShape& s, const float* theta, void* w16);
+// Output layer (a4) fused into the epilogue of the LAST hidden layer's forward: o_c[r] += sum_j w_out[j] h^L_c[j][r]
+// (+ b_out on the value channel).  o must be zero on entry; h_out may then be nullptr (forward-only callers).
+struct OutDot { const float* w_out; const float* b_out; float* o; long long o_stride; int valid; };
+bool tc_out_dot_fusable(const Launcher& L, int H);
 // hidden layer l forward: h_in [C][H][R_ld] -> h_out [C][H][R_ld]   (fused tanh-jet epilogue)
 void tc_layer_fwd(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* w16_l, const float* bias,
-                  const void* h_in, void* h_out);
-void tc_layer_fwd_split(Launcher& L, int precision, int H, int R, int R_ld, const void* w16_l, const float* bias, const void* h_in, void* h_out);
+                  const void* h_in, void* h_out, const OutDot* od = nullptr);
+void tc_layer_fwd_split(Launcher& L, int precision, int H, int R, int R_ld, const void* w16_l, const float* bias, const void* h_in, void* h_out,
+                        const OutDot* od = nullptr);
 // dgrad of layer l with the adjoint of layer l-1's tanh fused: ahat_in (layer l) -> ahat_out (layer l-1)
 struct FirstLayerFuse;
 void tc_layer_bwd(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* w16T_l, const void* ahat_in,
@@ -221,8 +233,9 @@ bool tc_first_layer_fusable(int H, const ChunkGeom& g);
 // ---- the same four on CTA pairs (tc2_kernels.cu, cta_group::2), taken when tc2_supported(H) ---------------------
 bool tc2_supported(const Launcher& L, int H);
 void tc2_layer_fwd(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* w16_l, const float* bias,
-                   const void* h_in, void* h_out);
-void tc2_layer_fwd_split(Launcher& L, int precision, int H, int R, int R_ld, const void* w16_l, const float* bias, const void* h_in, void* h_out);
+                   const void* h_in, void* h_out, const OutDot* od);
+void tc2_layer_fwd_split(Launcher& L, int precision, int H, int R, int R_ld, const void* w16_l, const float* bias, const void* h_in, void* h_out,
+                         const OutDot* od);
 void tc2_layer_bwd(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* w16T_l, const void* ahat_in,
                    const void* h_prev, void* ahat_out, float* g_bias_prev, const float* amax, const FirstLayerFuse* fl);
 void tc2_wgrad(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* ahat, const void* h_prev, float* gW, const float* amax);

@@ -51,10 +51,40 @@ struct Jet2Params {
   int npts, in_dim;
   float* gW1;            // W_hat_1 [H][in_dim]: columns 0, 1 += sum_r (ahat x_r + ahat_x), (ahat y_r + ahat_y)
   float* An;             // [N][H] += sum_{r in sample n} ahat
+  // MODE 4, 5 (last hidden layer + output layer a4): o_c[r] += sum_units w_out[unit] h_c[unit][r], reduced over the lanes of a
+  // warp by shuffles and over warps / CTAs / unit tiles by fp32 atomics (o is zeroed by the launcher; b_out enters once).
+  const float* w_out;    // [H]
+  const float* b_out;    // [1]
+  float* o;              // [C][o_stride] fp32 (MODE 5: one plane)
+  long long o_stride;
+  int valid;             // rows of the chunk that exist: rows >= valid are not accumulated
 };
 
 // MODE 0: forward; MODE 1: dgrad + adjoint of the previous tanh; MODE 2: value-only forward on split (hi, lo) planes;
-// MODE 3: MODE 1 with the first-layer backward reduction fused (no adjoint planes written)
+// MODE 3: MODE 1 with the first-layer backward reduction fused (no adjoint planes written);
+// MODE 4 / 5: MODE 0 / 2 for the LAST hidden layer with the output dot (a4) fused into the epilogue; p.out == nullptr then
+//             skips the h^L planes (forward-only callers).
+// sum over the 32 lanes of v[0..7]: every lane ends with the total of v[(lane >> 2) & 7] (3 halving exchanges + 2 butterflies)
+__device__ __forceinline__ float warp_reduce8(const float* v, int lane) {
+  float a[4], b[2];
+  const bool u4 = lane & 16, u3 = lane & 8, u2 = lane & 4;
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    const float send = u4 ? v[k] : v[k + 4], keep = u4 ? v[k + 4] : v[k];
+    a[k] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
+  }
+#pragma unroll
+  for (int k = 0; k < 2; ++k) {
+    const float send = u3 ? a[k] : a[k + 2], keep = u3 ? a[k + 2] : a[k];
+    b[k] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
+  }
+  const float send = u2 ? b[0] : b[1], keep = u2 ? b[1] : b[0];
+  float r = keep + __shfl_xor_sync(0xffffffffu, send, 4);
+  r += __shfl_xor_sync(0xffffffffu, r, 2);
+  r += __shfl_xor_sync(0xffffffffu, r, 1);
+  return r;                                                // row index within the 8: 4 * bit4 + 2 * bit3 + bit2 of the lane
+}
+
 template <typename T, int C, int MODE>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(k2Threads, 1)
 jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H] 16-bit, box 64 x 128, SW128
@@ -81,6 +111,7 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
   const int n_ut = p.H / 256;
   const int n_tiles = n_ut * p.n_row_tiles;
   const int n_kb = p.H / 64;
+  constexpr bool kFwd = MODE == 0 || MODE == 4, kSplit = MODE == 2 || MODE == 5, kOutDot = MODE == 4 || MODE == 5;
 
   if (warp == 0 && lane == 0) {
     prefetch_tmap(&tmA); prefetch_tmap(&tmB);
@@ -232,7 +263,20 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
       const uint32_t tb0 = lane_base + g0_col(it) + hs * (nc0 * 32), tb1 = lane_base + g1_col + hs * 64;
       auto tcol = [&](int c) -> uint32_t { return (C == 5 && c >= 3) ? tb1 + (c - 3) * 32 : tb0 + c * 32; };
       float bias = 0.f, bias_acc = 0.f;
-      if (MODE == 0 || MODE == 2) bias = p.bias[unit];
+      if (kFwd || kSplit) bias = p.bias[unit];
+      float wo = 0.f;
+      if (kOutDot) wo = p.w_out[unit];
+      // MODE 4, 5: lane -> row (4 * bit4 + 2 * bit3 + bit2) of each group of 8 rows; one lane of four adds
+      const int orow = ((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1);
+      auto out_dot = [&](int c, int rc, const float* hv) {  // hv[8]: this unit's h_c at rows rc * 8 .. + 8 (fp32, unrounded)
+        float pv[8];
+#pragma unroll
+        for (int i = 0; i < 8; ++i) pv[i] = wo * hv[i];
+        float tot = warp_reduce8(pv, lane);
+        const int r = row0 + rc * 8 + orow;
+        if (c == 0 && ut == 0 && rank == 0 && q == 0) tot += p.b_out[0];
+        if ((lane & 3) == 0 && r < p.valid) atomicAdd(p.o + (size_t)c * p.o_stride + r, tot);
+      };
       // Staged planes -> global with the epilogue warp's own 16-byte stores (4 lanes cover the 64 contiguous bytes of one
       // unit's 32 rows).  Measured: a TMA store drains shared memory at ~26 B/clk per SM whatever the box shape, and the
       // TMA unit serves loads and stores one after the other, so storing a C = 5 tile through it cost the operand
@@ -303,7 +347,7 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
         release();
       }
 
-      if (MODE == 0) {
+      if (kFwd) {
         // ---- h_c = tanh-jet(a_c) ----
 #pragma unroll
         for (int rc = 0; rc < 4; ++rc) {
@@ -323,31 +367,41 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
             for (int c = 0; c < C; ++c) o[c][i] = h[c];
           }
           const uint32_t off = ((uint32_t)rc ^ swz) << 4;
+          if (!kOutDot || p.out) {
 #pragma unroll
-          for (int c = 0; c < C; ++c) sts128(my_row + c * k2StgPlane + off, pack8<T>(o[c]));
+            for (int c = 0; c < C; ++c) sts128(my_row + c * k2StgPlane + off, pack8<T>(o[c]));
+          }
+          if (kOutDot) {
+#pragma unroll
+            for (int c = 0; c < C; ++c) out_dot(c, rc, o[c]);
+          }
         }
         if (C != 5) release(); else release0();
-        copy_out(C);
-      } else if (MODE == 2) {
+        if (!kOutDot || p.out) copy_out(C);
+      } else if (kSplit) {
         // ---- value-only layer with split activations: a = W (h_hi + h_lo) + b; t = tanh a; t_hi = rn16(t), t_lo = rn16(t - t_hi) ----
 #pragma unroll 1
         for (int rc = 0; rc < 4; ++rc) {
-          float v0[8], v1[8], hi[8], lo[8];
+          float v0[8], v1[8], hi[8], lo[8], tv[8];
           tmem_ld8(tcol(0) + rc * 8, v0);
           tmem_ld8(tcol(1) + rc * 8, v1);
           tmem_ld_wait();
 #pragma unroll
           for (int i = 0; i < 8; ++i) {
             const float tt = tanhf(v0[i] + v1[i] + bias);
+            tv[i] = tt;
             hi[i] = to_f<T>(from_f<T>(tt));
             lo[i] = tt - hi[i];
           }
           const uint32_t off = ((uint32_t)rc ^ swz) << 4;
-          sts128(my_row + off, pack8<T>(hi));
-          sts128(my_row + k2StgPlane + off, pack8<T>(lo));
+          if (!kOutDot || p.out) {
+            sts128(my_row + off, pack8<T>(hi));
+            sts128(my_row + k2StgPlane + off, pack8<T>(lo));
+          }
+          if (kOutDot) out_dot(0, rc, tv);
         }
         release();
-        copy_out(2);
+        if (!kOutDot || p.out) copy_out(2);
       } else {
         // ---- adjoint of the previous layer's tanh: ahat^{l-1} = J^T hhat^{l-1} ----
         mbar_wait(sbar + e, sphase); sphase ^= 1;
@@ -555,7 +609,7 @@ static void launch_jet2(Launcher& L, const CUtensorMap& a, const CUtensorMap& b,
   const int tiles = (p.H / 256) * p.n_row_tiles;
   const int clusters = std::min(tiles, L.num_sms / 2);
   kern<<<2 * clusters, k2Threads, Cfg::kSmemBytes, L.stream>>>(a, b, t, p);
-  L.check(MODE == 0 ? "jet_layer_fwd" : MODE == 2 ? "jet_layer_fwd_split" : "jet_layer_bwd");
+  L.check((MODE == 0 || MODE == 4) ? "jet_layer_fwd" : (MODE == 2 || MODE == 5) ? "jet_layer_fwd_split" : "jet_layer_bwd");
 }
 
 template <int MODE>
@@ -566,20 +620,28 @@ static void dispatch_jet2(Launcher& L, int C, const CUtensorMap& a, const CUtens
   else launch_jet2<__half, 5, MODE>(L, a, b, t, p);
 }
 
-void tc2_layer_fwd(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* w16_l, const float* bias, const void* h_in, void* h_out) {
+static void set_out_dot(Jet2Params& p, const OutDot* od) {
+  p.w_out = od->w_out; p.b_out = od->b_out; p.o = od->o; p.o_stride = od->o_stride; p.valid = od->valid;
+}
+
+void tc2_layer_fwd(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* w16_l, const float* bias, const void* h_in, void* h_out,
+                   const OutDot* od) {
   CUtensorMap a, b;
   bool ok = weight_map(L, &a, precision, w16_l, H) && plane_map(L, &b, precision, h_in, H, R_ld, C, 32, 64, C, CU_TENSOR_MAP_SWIZZLE_64B);
   if (!ok) return;
   Jet2Params p{};
   p.H = H; p.n_row_tiles = R / 64; p.bias = bias; p.out = h_out; p.R_ld = R_ld;
+  if (od) { set_out_dot(p, od); dispatch_jet2<4>(L, C, a, b, b, p); return; }
   dispatch_jet2<0>(L, C, a, b, b, p);
 }
 
-void tc2_layer_fwd_split(Launcher& L, int precision, int H, int R, int R_ld, const void* w16_l, const float* bias, const void* h_in, void* h_out) {
+void tc2_layer_fwd_split(Launcher& L, int precision, int H, int R, int R_ld, const void* w16_l, const float* bias, const void* h_in, void* h_out,
+                         const OutDot* od) {
   CUtensorMap a, b;
   if (!(weight_map(L, &a, precision, w16_l, H) && plane_map(L, &b, precision, h_in, H, R_ld, 2, 32, 64, 2, CU_TENSOR_MAP_SWIZZLE_64B))) return;
   Jet2Params p{};
   p.H = H; p.n_row_tiles = R / 64; p.bias = bias; p.out = h_out; p.R_ld = R_ld;
+  if (od) { set_out_dot(p, od); launch_jet2<__half, 2, 5>(L, a, b, b, p); return; }
   launch_jet2<__half, 2, 2>(L, a, b, b, p);
 }
 

@@ -478,9 +478,12 @@ static void dispatch_jet(Launcher& L, int precision, int C, const CUtensorMap& a
 #undef PIGAN_JET
 }
 
-void tc_layer_fwd(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* w16_l, const float* bias, const void* h_in, void* h_out) {
+bool tc_out_dot_fusable(const Launcher& L, int H) { return tc2_supported(L, H); }   // the one-CTA kernels keep the separate out_fwd pass
+
+void tc_layer_fwd(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* w16_l, const float* bias, const void* h_in, void* h_out,
+                  const OutDot* od) {
   if (R <= 0) return;
-  if (tc2_supported(L, H)) { tc2_layer_fwd(L, precision, C, H, R, R_ld, w16_l, bias, h_in, h_out); return; }
+  if (tc2_supported(L, H)) { tc2_layer_fwd(L, precision, C, H, R, R_ld, w16_l, bias, h_in, h_out, od); return; }
   CUtensorMap a, b, o;
   bool ok = weight_map(L, &a, precision, w16_l, H) && plane_map(L, &b, precision, h_in, H, R_ld, C, kRT, kBK, C, CU_TENSOR_MAP_SWIZZLE_128B) &&
             plane_map(L, &o, precision, h_out, H, R_ld, C, 32, 32, 1, CU_TENSOR_MAP_SWIZZLE_64B);
@@ -491,9 +494,10 @@ void tc_layer_fwd(Launcher& L, int precision, int C, int H, int R, int R_ld, con
 }
 
 // value-only layer on split activations (2 planes: hi, lo) -> 2 planes; used where the snapshot X_fake is built
-void tc_layer_fwd_split(Launcher& L, int precision, int H, int R, int R_ld, const void* w16_l, const float* bias, const void* h_in, void* h_out) {
+void tc_layer_fwd_split(Launcher& L, int precision, int H, int R, int R_ld, const void* w16_l, const float* bias, const void* h_in, void* h_out,
+                        const OutDot* od) {
   if (R <= 0) return;
-  if (tc2_supported(L, H)) { tc2_layer_fwd_split(L, precision, H, R, R_ld, w16_l, bias, h_in, h_out); return; }
+  if (tc2_supported(L, H)) { tc2_layer_fwd_split(L, precision, H, R, R_ld, w16_l, bias, h_in, h_out, od); return; }
   CUtensorMap a, b, o;
   if (!(weight_map(L, &a, precision, w16_l, H) && plane_map(L, &b, precision, h_in, H, R_ld, 2, kRT, kBK, 2, CU_TENSOR_MAP_SWIZZLE_128B) &&
         plane_map(L, &o, precision, h_out, H, R_ld, 2, 32, 32, 1, CU_TENSOR_MAP_SWIZZLE_64B)))
