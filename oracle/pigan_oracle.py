@@ -386,3 +386,182 @@ def adam_update_ref(theta, g, m, v, step, lr, beta1, beta2, adam_eps, skip=False
     vhat = v / (1.0 - beta2 ** step)
     theta = theta - lr * mhat / (np.sqrt(vhat) + adam_eps)
     return theta, m, v
+
+
+# ==============================================================================================================
+# NEXT-1: the paper's own generator -- ONE set of weights, separate log k and u outputs in the final
+# layer, residual connections that skip intermediate layers.  DESIGN.md readings R7 (heads) and R8 (skips):
+#   trunk   a^1 = W_1 [x, y, z] + b_1;  t^l = tanh(a^l);  h^l = t^l + h^{l-2} when l is odd and l >= 3 (a two-layer residual
+#           block, ref. [30]), else h^l = t^l;  a^{l+1} = W_{l+1} h^l + b_{l+1};
+#   heads   [log k, u] = W_{L+1} h^L + b_{L+1} with W_{L+1} of shape [2][H] (row 0: log k, row 1: u).
+# The spatial jet of h^L serves both heads, so the trunk carries 5 channels once; log k uses the first 3 of them.
+# Flat packing: as for the plain MLP, with the last layer W [2][H] then b [2].
+# ==============================================================================================================
+def trunk_param_count(in_dim: int, n_hidden: int, width: int) -> int:
+    return width * in_dim + width + (n_hidden - 1) * (width * width + width) + 2 * width + 2
+
+
+def unpack_trunk_params(theta, in_dim: int, n_hidden: int, width: int):
+    theta = np.asarray(theta, dtype=F64)
+    assert theta.shape == (trunk_param_count(in_dim, n_hidden, width),), theta.shape
+    layers, off, fan_in = [], 0, in_dim
+    for l in range(n_hidden + 1):
+        fan_out = width if l < n_hidden else 2
+        W = theta[off:off + fan_out * fan_in].reshape(fan_out, fan_in); off += fan_out * fan_in
+        b = theta[off:off + fan_out]; off += fan_out
+        layers.append((W, b)); fan_in = fan_out
+    return layers
+
+
+def _skip_source(l: int, skip: bool):
+    """Hidden layer l (1-based) adds h^{l-2} when skips are on and l is odd and >= 3 (reading R8)."""
+    return l - 2 if (skip and l >= 3 and l % 2 == 1) else None
+
+
+def _trunk_forward_one_sample(layers, xy, z_n, C, skip, keep_tape=False):
+    """One latent sample at all points xy [P,2]: returns out [2][C][P] (head 0 = log k, head 1 = u) and the tape."""
+    W1, b1 = layers[0]
+    P, H = xy.shape[0], W1.shape[0]
+    L = len(layers) - 1
+    x, y = xy[:, 0:1], xy[:, 1:2]
+    a = [None] * C
+    a[0] = x * W1[:, 0][None, :] + y * W1[:, 1][None, :] + (W1[:, 2:] @ z_n + b1)[None, :]
+    if C >= 3:
+        a[1] = np.broadcast_to(W1[:, 0], (P, H)).copy(); a[2] = np.broadcast_to(W1[:, 1], (P, H)).copy()
+    if C >= 5:
+        a[3] = np.zeros((P, H), dtype=F64); a[4] = np.zeros((P, H), dtype=F64)
+    hs = [None] * (L + 1)                                   # hs[l] = h^l (list of C arrays), l = 1..L
+    tape = []
+    for l in range(1, L + 1):
+        t = np.tanh(a[0]); s = 1.0 - t * t; q = -2.0 * t * s
+        tj = [None] * C                                     # jet of t^l = tanh(a^l)   (O2)
+        tj[0] = t
+        if C >= 3:
+            tj[1] = s * a[1]; tj[2] = s * a[2]
+        if C >= 5:
+            tj[3] = s * a[3] + q * a[1] * a[1]; tj[4] = s * a[4] + q * a[2] * a[2]
+        src = _skip_source(l, skip)
+        h = [tj[c] + hs[src][c] for c in range(C)] if src is not None else tj
+        hs[l] = h
+        if keep_tape:
+            tape.append((t, a[1:], h))
+        W, b = layers[l]
+        a = [h[c] @ W.T for c in range(C)]
+        a[0] = a[0] + b[None, :]
+    out = np.stack([np.stack([a[c][:, k] for c in range(C)]) for k in range(2)])          # [2][C][P]
+    return (out, tape) if keep_tape else out
+
+
+def trunk_jet_forward_ref(theta, in_dim, n_hidden, width, xy, z, jet_order, skip):
+    """out [2][C][n_samples][n_pts]: head 0 = log k, head 1 = u, with their spatial jets."""
+    layers = unpack_trunk_params(theta, in_dim, n_hidden, width)
+    xy = np.asarray(xy, dtype=F64); z = np.asarray(z, dtype=F64)
+    C = N_CHANNELS[jet_order]
+    out = np.empty((2, C, z.shape[0], xy.shape[0]), dtype=F64)
+    for n in range(z.shape[0]):
+        out[:, :, n, :] = _trunk_forward_one_sample(layers, xy, z[n], C, skip)
+    return out
+
+
+def _trunk_backward_one_sample(layers, xy, z_n, tape, o_hat, C, skip, grads):
+    """Reverse sweep of the trunk for one sample.  o_hat [2][C][P] = adjoints of the two heads' outputs.
+    O4 applies to t^l = tanh(a^l); a skip h^l = t^l + h^{l-2} passes the adjoint of h^l on to h^{l-2} unchanged."""
+    L = len(layers) - 1
+    W_out, _ = layers[L]
+    gWo, gbo = grads[L]
+    t_L, _, h_L = tape[L - 1]
+    for k in range(2):
+        for c in range(C):
+            gWo[k] += o_hat[k][c] @ h_L[c]
+        gbo[k] += o_hat[k][0].sum()
+    h_hat = {L: [o_hat[0][c][:, None] * W_out[0][None, :] + o_hat[1][c][:, None] * W_out[1][None, :] for c in range(C)]}
+    for l in range(L, 0, -1):
+        t, a_der, _ = tape[l - 1]
+        hh = h_hat.pop(l)
+        src = _skip_source(l, skip)
+        if src is not None:                                 # h^l = t^l + h^{l-2}
+            h_hat[src] = [hh[c].copy() for c in range(C)]
+        s = 1.0 - t * t; q = -2.0 * t * s; qp = -2.0 * s * (1.0 - 3.0 * t * t)
+        a_hat = [None] * C
+        val = s * hh[0]
+        if C >= 3:
+            a_x, a_y = a_der[0], a_der[1]
+            val = val + q * (a_x * hh[1] + a_y * hh[2])
+            a_hat[1] = s * hh[1]; a_hat[2] = s * hh[2]
+        if C >= 5:
+            a_xx, a_yy = a_der[2], a_der[3]
+            val = val + q * (a_xx * hh[3] + a_yy * hh[4]) + qp * (a_x * a_x * hh[3] + a_y * a_y * hh[4])
+            a_hat[1] = a_hat[1] + 2.0 * q * a_x * hh[3]
+            a_hat[2] = a_hat[2] + 2.0 * q * a_y * hh[4]
+            a_hat[3] = s * hh[3]; a_hat[4] = s * hh[4]
+        a_hat[0] = val
+        if l >= 2:
+            W, _ = layers[l - 1]                            # W_l (layers[] is 0-based)
+            gW, gb = grads[l - 1]
+            h_prev = tape[l - 2][2]
+            for c in range(C):
+                gW += a_hat[c].T @ h_prev[c]
+            gb += a_hat[0].sum(axis=0)
+            back = [a_hat[c] @ W for c in range(C)]
+            if (l - 1) in h_hat:
+                h_hat[l - 1] = [h_hat[l - 1][c] + back[c] for c in range(C)]
+            else:
+                h_hat[l - 1] = back
+        else:
+            gW1, gb1 = grads[0]
+            col = a_hat[0].sum(axis=0)
+            gW1[:, 0] += (a_hat[0] * xy[:, 0:1]).sum(axis=0)
+            gW1[:, 1] += (a_hat[0] * xy[:, 1:2]).sum(axis=0)
+            if C >= 3:
+                gW1[:, 0] += a_hat[1].sum(axis=0); gW1[:, 1] += a_hat[2].sum(axis=0)
+            gW1[:, 2:] += np.outer(col, z_n)
+            gb1 += col
+
+
+def train_step_grads_trunk_ref(gen_shape, disc_shape, theta_G, theta_D, xy_colloc, f, xy_sensors, z, real_snap, eps,
+                               gp_lambda=10.0, pde_weight=1.0, skip=True):
+    """Oracle of the step with the paper's generator (NEXT-1).  Same losses as train_step_grads_ref; the generator is
+    the shared trunk.  Returns g_G, g_D (flat) and losses = [L_D, mean D(fake), mean D(real), GP, L_G, L_pde]."""
+    lay_G = unpack_trunk_params(theta_G, *gen_shape); lay_D = unpack_params(theta_D, *disc_shape)
+    xy_c = np.asarray(xy_colloc, dtype=F64); xy_s = np.asarray(xy_sensors, dtype=F64)
+    f = np.asarray(f, dtype=F64); z = np.asarray(z, dtype=F64)
+    real = np.asarray(real_snap, dtype=F64); eps = np.asarray(eps, dtype=F64)
+    N, P, S = z.shape[0], xy_c.shape[0], xy_s.shape[0]
+    X_fake = np.empty((N, 2 * S), dtype=F64)
+    sens_tapes = []
+    for n in range(N):
+        o, tp = _trunk_forward_one_sample(lay_G, xy_s, z[n], 1, skip, keep_tape=True)
+        X_fake[n, :S] = o[0][0]; X_fake[n, S:] = o[1][0]
+        sens_tapes.append(tp)
+    gD = _zero_grads(lay_D)
+    g_fake, D_fake = _disc_forward(lay_D, X_fake)
+    g_real, D_real = _disc_forward(lay_D, real)
+    _disc_backward(lay_D, g_fake, np.full(N, 1.0 / N), gD)
+    _disc_backward(lay_D, g_real, np.full(N, -1.0 / N), gD)
+    Xhat = eps[:, None] * real + (1.0 - eps[:, None]) * X_fake
+    gp, _ = _gradient_penalty(lay_D, Xhat, gp_lambda, gD)
+    L_D = float(D_fake.mean() - D_real.mean() + gp)
+    dX = _disc_backward(lay_D, g_fake, np.full(N, -1.0 / N), None)
+    gG = _zero_grads(lay_G)
+    sum_r2 = 0.0
+    for n in range(N):
+        o, tp = _trunk_forward_one_sample(lay_G, xy_c, z[n], 5, skip, keep_tape=True)
+        r, Y_hat, U_hat = _residual_adjoints(o[0][:3], o[1], f, pde_weight, N * P)
+        sum_r2 += float((r * r).sum())
+        zero = np.zeros_like(r)
+        o_hat = [[Y_hat[0], Y_hat[1], Y_hat[2], zero, zero], [U_hat[c] for c in range(5)]]
+        _trunk_backward_one_sample(lay_G, xy_c, z[n], tp, o_hat, 5, skip, gG)
+        _trunk_backward_one_sample(lay_G, xy_s, z[n], sens_tapes[n], [[dX[n, :S]], [dX[n, S:]]], 1, skip, gG)
+    L_pde = sum_r2 / (N * P)
+    L_G = float(-D_fake.mean() + pde_weight * L_pde)
+    losses = np.array([L_D, D_fake.mean(), D_real.mean(), gp, L_G, L_pde], dtype=F64)
+    return pack_grads(gG), pack_grads(gD), losses
+
+
+def trunk_generator_loss_ref(gen_shape, disc_shape, theta_G, theta_D, xy_colloc, f, xy_sensors, z, pde_weight=1.0, skip=True):
+    """L_G of the shared-trunk generator written as its plain definition (finite-difference pins only)."""
+    Jc = trunk_jet_forward_ref(theta_G, *gen_shape, xy_colloc, z, 2, skip)
+    _, mean_sq = darcy_residual_ref(Jc[0][:3], Jc[1], f)
+    Js = trunk_jet_forward_ref(theta_G, *gen_shape, xy_sensors, z, 0, skip)
+    X_fake = np.concatenate([Js[0][0], Js[1][0]], axis=1)
+    return float(-disc_forward_ref(theta_D, *disc_shape, X_fake).mean() + pde_weight * mean_sq)
