@@ -170,12 +170,12 @@ def time_oracle(cfg, steps=1, warmup=0):
 class GpuWorkload:
     """Device-resident synthetic inputs + state of one config."""
 
-    def __init__(self, cfg, device, seed_shift=0):
+    def __init__(self, cfg, device, seed_shift=0, chunk_rows=0):
         import torch
         from paper_1910_13444_b200 import PiGan
         self.cfg, self.device, self.torch = cfg, device, torch
         inp = wl.make_inputs(dataclasses.replace(cfg, index=cfg.index + 10 * seed_shift) if seed_shift else cfg)
-        self.pg = PiGan.from_config(cfg, device=device)
+        self.pg = PiGan.from_config(cfg, device=device, chunk_rows=chunk_rows)
         d = {k: torch.from_numpy(np.ascontiguousarray(v)).to(device) for k, v in inp.items()}
         # "real" snapshots: the frozen teacher pair evaluated at the sensors by the GPU library, outside any timed region
         Ys = self.pg.gen_jet_forward(d["teacher_Y"], d["xy_sensors"], d["z_real"], 0)[0]
@@ -238,9 +238,9 @@ class GpuWorkload:
         return [a.elapsed_time(b) for a, b in ev]
 
 
-def run_config(cfg, device, steps, warmup, rank, world, with_roofline=True, seed_shift=0):
+def run_config(cfg, device, steps, warmup, rank, world, with_roofline=True, seed_shift=0, chunk_rows=0):
     import torch
-    w = GpuWorkload(cfg, device, seed_shift)
+    w = GpuWorkload(cfg, device, seed_shift, chunk_rows)
     peaks = measured_peaks()
     flops = wl.step_flops(cfg)
     res = {}
@@ -357,6 +357,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--samples", type=int, default=None, help="override N (latent samples per step): a smaller job for ncu captures; "
                     "the line then says so in config.workload and is not a benchmark value")
+    ap.add_argument("--chunk-rows", type=int, default=0, help="rows per chunk of the generator passes (0 = library default); sweeps only")
     args = ap.parse_args()
     cfg = wl.CONFIGS[args.config]
     if args.samples:
@@ -389,7 +390,7 @@ def main():
     if world > 1:
         dist.init_process_group("nccl", device_id=device)
         dist.barrier()
-    res = run_config(cfg, device, steps, warmup, rank, world, seed_shift=rank)
+    res = run_config(cfg, device, steps, warmup, rank, world, seed_shift=rank, chunk_rows=args.chunk_rows)
     t_ms = float(np.mean(res["ms_steps"]))
     if world > 1:
         t_ms = max_over_ranks(t_ms, dist, device)           # max over ranks; the replicas exchange nothing else

@@ -12,7 +12,7 @@ namespace pigan {
 
 namespace {
 
-constexpr int kCfThreads = 256;
+constexpr int kCfThreads = 512;       // 16 warps: one CTA per sample, so the loads in flight per SM come from this CTA alone
 constexpr int kCfWarps = kCfThreads / 32;
 constexpr int kCfMaxIn = 512;      // largest layer input (d = 2S or HD) the fused path takes
 constexpr int kCfMaxPer = kCfMaxIn / 32;
@@ -29,28 +29,43 @@ template <int NV>
 __device__ __forceinline__ void matvec_rows(const float* __restrict__ V, const float* __restrict__ bias, int n_out, int n_in,
                                             const float* const* x, float* const* y) {
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  for (int j = warp; j < n_out; j += kCfWarps) {
-    const float* row = V + (size_t)j * n_in;
-    float acc[NV];
+  constexpr int U = 4;                                      // output units per warp iteration: U independent row streams in flight
+  for (int j0 = warp * U; j0 < n_out; j0 += kCfWarps * U) {
+    float acc[U][NV];
 #pragma unroll
-    for (int v = 0; v < NV; ++v) acc[v] = 0.f;
+    for (int u = 0; u < U; ++u)
+#pragma unroll
+      for (int v = 0; v < NV; ++v) acc[u][v] = 0.f;
     for (int i = lane; i < n_in; i += 32) {
-      const float w = __ldg(row + i);
+      float w[U];
 #pragma unroll
-      for (int v = 0; v < NV; ++v) acc[v] = fmaf(w, x[v][i], acc[v]);
+      for (int u = 0; u < U; ++u) w[u] = (j0 + u < n_out) ? __ldg(V + (size_t)(j0 + u) * n_in + i) : 0.f;
+#pragma unroll
+      for (int v = 0; v < NV; ++v) {
+        const float xv = x[v][i];
+#pragma unroll
+        for (int u = 0; u < U; ++u) acc[u][v] = fmaf(w[u], xv, acc[u][v]);
+      }
     }
 #pragma unroll
-    for (int v = 0; v < NV; ++v) acc[v] = wsum(acc[v]);
-    if (lane == 0) {
-      const float b = bias ? bias[j] : 0.f;
+    for (int u = 0; u < U; ++u)
 #pragma unroll
-      for (int v = 0; v < NV; ++v) y[v][j] = acc[v] + b;
+      for (int v = 0; v < NV; ++v) acc[u][v] = wsum(acc[u][v]);
+    if (lane == 0) {
+#pragma unroll
+      for (int u = 0; u < U; ++u) {
+        if (j0 + u < n_out) {
+          const float b = bias ? bias[j0 + u] : 0.f;
+#pragma unroll
+          for (int v = 0; v < NV; ++v) y[v][j0 + u] = acc[u][v] + b;
+        }
+      }
     }
   }
 }
 
-// y_v[i] = sum_j V[j][i] x_v[j] (the transposed product) for NV vectors.  Warp w takes the rows j = w, w + 8, ...; lanes
-// cover i (coalesced); the 8 partial sums per i meet in shared memory.  y must be zero on entry.
+// y_v[i] = sum_j V[j][i] x_v[j] (the transposed product) for NV vectors.  Warp w takes the rows j = w, w + kCfWarps, ...; lanes
+// cover i (coalesced); the per-warp partial sums per i meet in shared memory.  y must be zero on entry.
 template <int NV>
 __device__ __forceinline__ void matvec_cols(const float* __restrict__ V, int n_out, int n_in, const float* const* x, float* const* y) {
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -60,6 +75,7 @@ __device__ __forceinline__ void matvec_cols(const float* __restrict__ V, int n_o
   for (int v = 0; v < NV; ++v)
 #pragma unroll
     for (int k = 0; k < kCfMaxPer; ++k) acc[v][k] = 0.f;
+#pragma unroll 2
   for (int j = warp; j < n_out; j += kCfWarps) {
     const float* row = V + (size_t)j * n_in;
     float xv[NV];
@@ -326,7 +342,7 @@ void critic_fused(Launcher& L, const NetShape& s, const float* theta, const floa
   p.A = w.cfA; p.B1 = w.cfB1; p.Bh = w.cfBh; p.dX = dX; p.nu = w.nu; p.grad_norm = grad_norm; p.acc = w.acc; p.score = w.D;
   const size_t smem = cf_smem_bytes(s);
   static unsigned long long attr_done = 0;
-  ensure_smem_attr(L, critic_fused_kernel, (int)smem, attr_done);
+  ensure_smem_attr(L, critic_fused_kernel, 200 * 1024, attr_done);        // the opt-in is per function: ask for the most any critic needs
   critic_fused_kernel<<<B, kCfThreads, smem, L.stream>>>(p);
   L.check("critic_fused");
   if (!grads) return;

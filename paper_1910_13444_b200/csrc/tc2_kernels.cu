@@ -89,7 +89,7 @@ template <typename T, int C, int MODE>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(k2Threads, 1)
 jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H] 16-bit, box 64 x 128, SW128
                   const __grid_constant__ CUtensorMap tmB,      // input planes, box 32 rows x 64 units x C, SW64
-                  const __grid_constant__ CUtensorMap tmT,      // MODE 1: h_prev planes in (box 32 x 32 x 1, SW64)
+                  const __grid_constant__ CUtensorMap tmT,      // MODE 1, 3: h_prev planes in (box 32 rows x 32 units x C, SW64)
                   Jet2Params p) {
   using Cfg = Jet2Cfg<C, MODE>;
   extern __shared__ uint8_t smem_raw[];
@@ -332,8 +332,10 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
       if ((MODE == 1 || MODE == 3) && elect_one()) {         // the previous layer's output jet h^{l-1} -> staging
         // Generic-proxy accesses of the staging planes by the previous tile were fenced (fence.proxy.async) by every lane
         // inside copy_out (MODE 1) before its trailing __syncwarp; MODE 3 only reads them (see the fence after its loop).
+        // one 3D box (32 rows x 32 units x C channels) lands as C consecutive 2 KB planes: one TMA issue instead of C
+        // (measured: each extra issue stalled the warp ~400 samples behind the producer's loads in the TMA queue)
         mbar_expect_tx(sbar + e, C * k2StgPlane);
-        for (int c = 0; c < C; ++c) tma_load_3d(stg + c * k2StgPlane, &tmT, sbar + e, row0, unit0, c);
+        tma_load_3d(stg, &tmT, sbar + e, row0, unit0, 0);
       }
       mbar_wait(tfull + buf, bphase);
       tc_fence_after();
@@ -649,7 +651,7 @@ void tc2_layer_bwd(Launcher& L, int precision, int C, int H, int R, int R_ld, co
                    void* ahat_out, float* g_bias_prev, const float* amax, const FirstLayerFuse* fl) {
   CUtensorMap a, b, t;
   bool ok = weight_map(L, &a, precision, w16T_l, H) && plane_map(L, &b, precision, ahat_in, H, R_ld, C, 32, 64, C, CU_TENSOR_MAP_SWIZZLE_64B) &&
-            plane_map(L, &t, precision, h_prev, H, R_ld, C, 32, 32, 1, CU_TENSOR_MAP_SWIZZLE_64B);
+            plane_map(L, &t, precision, h_prev, H, R_ld, C, 32, 32, C, CU_TENSOR_MAP_SWIZZLE_64B);
   if (!ok) return;
   Jet2Params p{};
   p.H = H; p.n_row_tiles = R / 64; p.g_bias = g_bias_prev; p.amax = amax; p.out = ahat_out; p.R_ld = R_ld;
