@@ -64,6 +64,15 @@ typedef enum { PIGAN_FP32 = 0, PIGAN_BF16 = 1, PIGAN_FP16 = 2 } pigan_precision;
 
 typedef struct { int in_dim, n_hidden, width; } pigan_mlp_shape;   /* scalar linear output implied (G10) */
 
+/* Which generator the context trains.
+ *   TWO_MLPS    BASELINE.json's variant: two separate plain MLPs G_logk (3 jet channels) and G_u (5)  (reading G4).
+ *   TRUNK       the paper's: ONE set of weights, separate log k and u outputs in the final layer.  The last
+ *               layer is W [2][H] (row 0: log k, row 1: u) then b [2]; the 5-channel jet of the last hidden layer serves
+ *               both heads, so a step costs 5 channel passes instead of 8 (R7).
+ *   TRUNK_SKIP  TRUNK with residual connections that skip intermediate layers: h^l = tanh(a^l) + h^{l-2} for odd
+ *               l >= 3 (two-layer residual blocks of ref. [30]; R8). */
+typedef enum { PIGAN_GEN_TWO_MLPS = 0, PIGAN_GEN_TRUNK = 1, PIGAN_GEN_TRUNK_SKIP = 2 } pigan_gen_variant;
+
 typedef struct {
   pigan_mlp_shape gen;       /* in_dim = 2 + latent_dim; the same shape is used for G_logk and G_u (G4) */
   pigan_mlp_shape disc;      /* in_dim = 2 * n_sensors (G6) */
@@ -77,6 +86,7 @@ typedef struct {
   size_t workspace_bytes;    /* 0 = library default; bounds the row-chunk size of the step (S7 H1) */
   int chunk_rows;            /* 0 = library default (131072); rows per chunk of the generator passes, rounded to 256 */
   unsigned flags;            /* PIGAN_FLAG_* */
+  int gen_variant;           /* pigan_gen_variant; 0 = BASELINE.json's two MLPs */
 } pigan_config;
 
 /* Creates a context: validates cfg, allocates the workspace on the CURRENT CUDA device and binds the context to it
@@ -85,6 +95,7 @@ typedef struct {
 pigan_status pigan_create(const pigan_config* cfg, void* cuda_stream, pigan_ctx** out);
 void         pigan_destroy(pigan_ctx* ctx);                       /* NULL is allowed */
 size_t       pigan_param_count(const pigan_mlp_shape* shape);     /* H*in + H + (L-1)(H*H + H) + H + 1; 0 if shape is NULL/invalid */
+size_t       pigan_trunk_param_count(const pigan_mlp_shape* shape); /* shared trunk: the plain count + H + 1 (second head) */
 const char*  pigan_last_error(const pigan_ctx* ctx);              /* never NULL; "" when no error */
 /* Number of kernels this context has launched since creation (bench.py reports it as gpu_launches). */
 unsigned long long pigan_launch_count(const pigan_ctx* ctx);
@@ -102,6 +113,12 @@ pigan_status pigan_profile_report(pigan_ctx* ctx, char* buf, size_t cap);
  *   out [C][n_samples][n_pts] fp32, overwritten.   Defines: S8c O1, O2. */
 pigan_status pigan_gen_jet_forward(pigan_ctx* ctx, const float* gen_params, const float* xy, int n_pts,
                                    const float* z, int n_samples, int jet_order, float* out);
+
+/* NEXT-1: the shared-trunk generator (context created with gen_variant TRUNK or TRUNK_SKIP).  Same arguments as
+ *   pigan_gen_jet_forward; trunk_params [pigan_trunk_param_count(cfg.gen)]; out [2][C][n_samples][n_pts]: head 0 = log k,
+ *   head 1 = u, each with its C jet channels.   Defines: P:139; R7, R8. */
+pigan_status pigan_trunk_jet_forward(pigan_ctx* ctx, const float* trunk_params, const float* xy, int n_pts,
+                                     const float* z, int n_samples, int jet_order, float* out);
 
 /* a5: Darcy residual r[n][p] = exp(Y)(Y_x u_x + Y_y u_y + u_xx + u_yy) - f[p]  (Eq. 1, with k = exp Y).
  *   logk_jet [>=3][N][P] (only channels 0..2 are read; plane stride N*P), u_jet [5][N][P], f [P].
@@ -133,6 +150,8 @@ pigan_status pigan_gradient_penalty(pigan_ctx* ctx, const float* disc_params, co
  *   behaves exactly as an eager call.  cfg.flags & PIGAN_FLAG_NO_GRAPH disables the replay; cfg.chunk_rows sets the
  *   row-chunk size (default 131072 rows; workspace_bytes of the config bounds it as well).  No environment variable
  *   changes the behaviour of the library. */
+/*   Shared-trunk contexts (gen_variant != 0): logk_params = the trunk's parameters, g_logk = their gradient
+ *   [pigan_trunk_param_count]; u_params and g_u are ignored and may be NULL. */
 pigan_status pigan_train_step_grads(pigan_ctx* ctx, const float* logk_params, const float* u_params,
                                     const float* disc_params, const float* xy_colloc, const float* f,
                                     const float* xy_sensors, const float* z, const float* real_snap,

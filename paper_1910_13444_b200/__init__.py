@@ -19,8 +19,8 @@ FLAG_NO_GRAPH, FLAG_ONE_CTA = 1, 2                     # pigan_config.flags (inc
 PRECISIONS = {"fp32": 0, "bf16": 1, "fp16": 2}
 STATUS = {0: "PIGAN_OK", 1: "PIGAN_ERR_INVALID_ARG", 2: "PIGAN_ERR_SHAPE", 3: "PIGAN_ERR_ALLOC", 4: "PIGAN_ERR_CUDA",
           5: "PIGAN_ERR_UNSUPPORTED"}
-EXPORTED_SYMBOLS = ["pigan_create", "pigan_destroy", "pigan_param_count", "pigan_last_error", "pigan_launch_count",
-                    "pigan_profile_enable", "pigan_profile_report",
+EXPORTED_SYMBOLS = ["pigan_create", "pigan_destroy", "pigan_param_count", "pigan_trunk_param_count", "pigan_last_error", "pigan_launch_count",
+                    "pigan_profile_enable", "pigan_profile_report", "pigan_trunk_jet_forward",
                     "pigan_gen_jet_forward", "pigan_darcy_residual", "pigan_disc_forward", "pigan_gradient_penalty",
                     "pigan_train_step_grads", "pigan_adam_update"]
 
@@ -38,7 +38,7 @@ class _MlpShape(Structure):
 class _Config(Structure):
     _fields_ = [("gen", _MlpShape), ("disc", _MlpShape), ("latent_dim", c_int), ("n_samples", c_int), ("n_colloc", c_int),
                 ("n_sensors", c_int), ("precision", c_int), ("gp_lambda", c_float), ("pde_weight", c_float),
-                ("workspace_bytes", c_size_t), ("chunk_rows", c_int), ("flags", ctypes.c_uint)]
+                ("workspace_bytes", c_size_t), ("chunk_rows", c_int), ("flags", ctypes.c_uint), ("gen_variant", c_int)]
 
 
 _lib = None
@@ -61,6 +61,10 @@ def load_library():
     lib.pigan_destroy.restype = None
     lib.pigan_param_count.argtypes = [POINTER(_MlpShape)]
     lib.pigan_param_count.restype = c_size_t
+    lib.pigan_trunk_param_count.argtypes = [POINTER(_MlpShape)]
+    lib.pigan_trunk_param_count.restype = c_size_t
+    lib.pigan_trunk_jet_forward.argtypes = [c_void_p, c_void_p, c_void_p, c_int, c_void_p, c_int, c_int, c_void_p]
+    lib.pigan_trunk_jet_forward.restype = c_int
     lib.pigan_last_error.argtypes = [c_void_p]
     lib.pigan_last_error.restype = c_char_p
     lib.pigan_launch_count.argtypes = [c_void_p]
@@ -74,8 +78,9 @@ def load_library():
                                       c_float, c_void_p]
     lib.pigan_profile_enable.argtypes = [c_void_p, c_int]
     lib.pigan_profile_report.argtypes = [c_void_p, c_char_p, c_size_t]
-    for name in EXPORTED_SYMBOLS[5:]:
-        getattr(lib, name).restype = c_int
+    for name in EXPORTED_SYMBOLS:
+        if name not in ("pigan_create", "pigan_destroy", "pigan_param_count", "pigan_trunk_param_count", "pigan_last_error", "pigan_launch_count"):
+            getattr(lib, name).restype = c_int
     del fp, ip
     _lib = lib
     return lib
@@ -83,6 +88,13 @@ def load_library():
 
 def param_count(in_dim: int, n_hidden: int, width: int) -> int:
     return int(load_library().pigan_param_count(ctypes.byref(_MlpShape(in_dim, n_hidden, width))))
+
+
+def trunk_param_count(in_dim: int, n_hidden: int, width: int) -> int:
+    return int(load_library().pigan_trunk_param_count(ctypes.byref(_MlpShape(in_dim, n_hidden, width))))
+
+
+GEN_VARIANTS = {"two_mlps": 0, "trunk": 1, "trunk_skip": 2}     # pigan_gen_variant (include/pigan.h)
 
 
 def _ptr(t, name, dtype=None):
@@ -101,7 +113,7 @@ class PiGan:
     """One context = one CUDA stream + the workspaces of one PI-GAN configuration (mirrors pigan_ctx)."""
 
     def __init__(self, *, latent_dim, gen_hidden, gen_width, disc_hidden, disc_width, n_samples, n_colloc, n_sensors,
-                 precision="fp32", gp_lambda=10.0, pde_weight=1.0, workspace_bytes=0, chunk_rows=0, flags=0, stream=None, device=None):
+                 precision="fp32", gp_lambda=10.0, pde_weight=1.0, workspace_bytes=0, chunk_rows=0, flags=0, gen_variant="two_mlps", stream=None, device=None):
         import torch
         self._lib = load_library()
         self._ctx = c_void_p()
@@ -113,14 +125,15 @@ class PiGan:
         self.disc_shape = (2 * n_sensors, disc_hidden, disc_width)
         self.precision = precision
         cfg = _Config(_MlpShape(*self.gen_shape), _MlpShape(*self.disc_shape), latent_dim, n_samples, n_colloc, n_sensors,
-                      PRECISIONS[precision], gp_lambda, pde_weight, workspace_bytes, chunk_rows, flags)
+                      PRECISIONS[precision], gp_lambda, pde_weight, workspace_bytes, chunk_rows, flags, GEN_VARIANTS[gen_variant])
+        self.gen_variant = gen_variant
         self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
         with torch.cuda.device(self.device):
             st = self._lib.pigan_create(ctypes.byref(cfg), c_void_p(self._stream.cuda_stream), ctypes.byref(self._ctx))
         if st != 0:
             self._ctx = c_void_p()
             raise PiganError(st, "pigan_create failed")
-        self.n_gen = param_count(*self.gen_shape)
+        self.n_gen = param_count(*self.gen_shape) if gen_variant == "two_mlps" else trunk_param_count(*self.gen_shape)
         self.n_disc = param_count(*self.disc_shape)
 
     @classmethod
@@ -168,6 +181,16 @@ class PiGan:
                                                     n_samples, jet_order, _ptr(out, "out")))
         return out
 
+    def trunk_jet_forward(self, trunk_params, xy, z, jet_order, out=None):
+        """NEXT-1: out [2][C][N][P], head 0 = log k, head 1 = u (contexts created with gen_variant 'trunk' / 'trunk_skip')."""
+        n_pts, n_samples = xy.shape[0], z.shape[0]
+        C = (1, 3, 5)[jet_order]
+        if out is None:
+            out = self._new(2, C, n_samples, n_pts)
+        self._check(self._lib.pigan_trunk_jet_forward(self._ctx, _ptr(trunk_params, "trunk_params"), _ptr(xy, "xy"), n_pts, _ptr(z, "z"),
+                                                      n_samples, jet_order, _ptr(out, "out")))
+        return out
+
     def darcy_residual(self, logk_jet, u_jet, f, want_r=True, want_mean=True):
         if logk_jet.shape[1:] != u_jet.shape[1:] or logk_jet.shape[0] < 3 or u_jet.shape[0] != 5:
             raise ValueError("logk_jet must be [>=3][N][P] and u_jet [5][N][P]")
@@ -196,7 +219,8 @@ class PiGan:
                          out=None):
         import torch
         if out is None:
-            out = (self._new(self.n_gen), self._new(self.n_gen), self._new(self.n_disc), self._new(6), self._new(1, dtype=torch.int32))
+            out = (self._new(self.n_gen), self._new(self.n_gen) if self.gen_variant == "two_mlps" else None, self._new(self.n_disc), self._new(6),
+                   self._new(1, dtype=torch.int32))
         g_logk, g_u, g_disc, losses, found_inf = out
         if (xy_colloc.shape[0], xy_sensors.shape[0], tuple(z.shape), tuple(real_snap.shape)) != (self.P, self.S, (self.N, self.m), (self.N, 2 * self.S)):
             raise ValueError("input sizes disagree with the configuration of this context")

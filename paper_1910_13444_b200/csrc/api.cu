@@ -8,96 +8,12 @@
 #include <new>
 #include <vector>
 
-#include "common.cuh"
+#include "ctx.cuh"
 
 using namespace pigan;
 
 namespace {
 
-struct NetWs {                 // activation workspace of one generator net (planes are [channel][unit][row])
-  int Cmax = 0;
-  char* h = nullptr;           // L x [Cmax][H][R_ld]      post-activations h^1..h^L
-  char* hs = nullptr;          // sensor rows: n_sens_chunks x L x [2][H][R_ld]  (hi, lo) planes of the snapshot forward, kept for the reverse sweep
-  char* ah[2] = {nullptr, nullptr};   // adjoint ping-pong, [Cmax][H][R_ld]
-  float* apre = nullptr;       // fp32 mode: [Cmax][H][R_ld] pre-activations / hhat scratch
-  float* o = nullptr;          // [Cmax][R_ld] outputs of the chunk
-  float* oh = nullptr;         // [Cmax][R_ld] output adjoints (seeds)
-  float* Zp = nullptr;         // [N][H]  first-layer z-part
-  float* An = nullptr;         // [N][H]  per-sample sums of the first-layer value adjoint
-  void* w16 = nullptr;         // (L-1) x {W_l, W_l^T} 16-bit copies
-};
-
-}  // namespace
-
-struct pigan_ctx {
-  pigan_config cfg{};
-  NetShape gen{}, disc{};
-  Launcher L;
-  std::string err;
-  int elem = 4;                // bytes per activation element
-  int R_ld = 0;                // rows per chunk (leading dimension of every plane)
-  NetWs net[2];                // 0: G_logk (C <= 3), 1: G_u (C <= 5)
-  CriticWs cw;
-  float* xfake = nullptr;      // [N][2S]
-  float* dX = nullptr;         // [2N][2S]
-  float* seed = nullptr;       // [2N]
-  float* amax = nullptr;       // [2] largest output adjoint of the current chunk, per net (block scale of the adjoint planes)
-  std::vector<void*> allocs;
-  // CUDA-graph replay of pigan_train_step_grads: the step is hundreds to thousands of launches, launch-latency bound
-  // for the small configs.  A call whose arguments repeat the previous call's is captured once (on a private stream,
-  // so the caller's stream may be the legacy default stream) and replayed from then on.  PIGAN_FLAG_NO_GRAPH disables it.
-  struct StepGraph {
-    cudaStream_t cap_stream = nullptr;
-    cudaGraphExec_t exec = nullptr;
-    std::vector<unsigned long long> key, last_key;
-    unsigned long long launches = 0;
-    bool disabled = false;
-  } sg;
-
-  template <typename T> T* alloc(size_t n) {
-    void* p = nullptr;
-    if (n == 0) n = 1;
-    if (cudaMalloc(&p, n * sizeof(T)) != cudaSuccess) { cudaGetLastError(); throw std::bad_alloc(); }
-    allocs.push_back(p);
-    return reinterpret_cast<T*>(p);
-  }
-  int n_sens_chunks = 1;
-  size_t plane() const { return (size_t)gen.H * R_ld * elem; }
-  // activation stash of one chunk: `planes` planes per layer; l = 1..L
-  struct HBuf { char* base; int planes; size_t plane_bytes; char* at(int l) const { return base + (size_t)(l - 1) * planes * plane_bytes; } };
-  HBuf hcol(int n) { return HBuf{net[n].h, net[n].Cmax, plane()}; }
-  HBuf hsens(int n, int chunk) { return HBuf{net[n].hs + (size_t)chunk * gen.L * 2 * plane(), 2, plane()}; }
-  void* w16(int n, int l, int transposed) { return (char*)net[n].w16 + ((size_t)(l - 2) * 2 + transposed) * gen.H * gen.H * 2; }
-};
-
-namespace {
-
-// Every entry point runs on the device the context was created on, whatever the caller's current device is.
-struct DeviceGuard {
-  int prev = -1; bool switched = false;
-  explicit DeviceGuard(const pigan_ctx* c) {
-    if (!c) return;
-    if (cudaGetDevice(&prev) == cudaSuccess && prev != c->L.device) switched = cudaSetDevice(c->L.device) == cudaSuccess;
-  }
-  ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
-};
-
-pigan_status fail(pigan_ctx* c, pigan_status s, const std::string& msg) {
-  if (c) c->err = msg;
-  return s;
-}
-
-pigan_status finish(pigan_ctx* c) {
-  if (c->L.err != cudaSuccess) {
-    c->err = std::string("CUDA error at ") + c->L.where + ": " + cudaGetErrorString(c->L.err);
-    c->L.err = cudaSuccess;
-    return PIGAN_ERR_CUDA;
-  }
-  c->err.clear();
-  return PIGAN_OK;
-}
-
-size_t round_up(size_t a, size_t b) { return (a + b - 1) / b * b; }
 
 // ---- one chunk of generator rows, forward ------------------------------------------------------------------------
 template <typename T>
@@ -165,22 +81,6 @@ void gen_backward_chunk(pigan_ctx* c, int n, const pigan_ctx::HBuf& hb, const fl
     cur ^= 1;
   }
   first_layer_bwd<T>(L, C, s, xy, g, (const T*)c->net[n].ah[cur], grads, c->net[n].An, amax);
-}
-
-ChunkGeom make_geom(const pigan_ctx* c, long long row0, long long total, int npts) {
-  ChunkGeom g;
-  g.row0 = row0;
-  g.valid = (int)std::min<long long>(c->R_ld, total - row0);
-  g.R = (int)round_up(g.valid, 64);
-  g.R_ld = c->R_ld;
-  g.npts = npts;
-  return g;
-}
-
-void compute_zpart(pigan_ctx* c, int n, const float* theta, const float* z, int n_samples) {
-  const NetShape& s = c->gen;
-  // Zp[n][j] = sum_k W1[j][2+k] z[n][k]   (a1: once per sample; the bias is added with the xy-part)
-  sgemm(c->L, false, true, n_samples, s.H, s.in_dim - 2, z, s.in_dim - 2, 0, theta + 2, s.in_dim, 0, c->net[n].Zp, s.H, 0, 1, false);
 }
 
 template <typename T>
@@ -284,6 +184,13 @@ size_t pigan_param_count(const pigan_mlp_shape* s) {
   return n.count();
 }
 
+size_t pigan_trunk_param_count(const pigan_mlp_shape* s) {
+  if (!s || !shape_ok(*s)) return 0;
+  NetShape n{s->in_dim, s->n_hidden, s->width};
+  n.heads = 2;
+  return n.count();
+}
+
 const char* pigan_last_error(const pigan_ctx* c) { return c ? c->err.c_str() : "null context"; }
 unsigned long long pigan_launch_count(const pigan_ctx* c) { return c ? c->L.count : 0; }
 
@@ -329,6 +236,7 @@ pigan_status pigan_create(const pigan_config* cfg, void* cuda_stream, pigan_ctx*
   if (!shape_ok(cfg->gen) || !shape_ok(cfg->disc) || cfg->latent_dim < 1 || cfg->n_samples < 1 || cfg->n_colloc < 1 || cfg->n_sensors < 1)
     return PIGAN_ERR_INVALID_ARG;
   if ((int)cfg->precision < 0 || (int)cfg->precision > 2 || !(cfg->gp_lambda >= 0.f) || cfg->chunk_rows < 0) return PIGAN_ERR_INVALID_ARG;
+  if (cfg->gen_variant < 0 || cfg->gen_variant > 2) return PIGAN_ERR_INVALID_ARG;
   if (cfg->gen.in_dim != 2 + cfg->latent_dim || cfg->disc.in_dim != 2 * cfg->n_sensors) return PIGAN_ERR_SHAPE;
   if (cfg->precision != PIGAN_FP32) {
     std::string why;
@@ -340,6 +248,9 @@ pigan_status pigan_create(const pigan_config* cfg, void* cuda_stream, pigan_ctx*
   if (!c) return PIGAN_ERR_ALLOC;
   c->cfg = *cfg;
   c->gen = NetShape{cfg->gen.in_dim, cfg->gen.n_hidden, cfg->gen.width};
+  c->trunk = cfg->gen_variant != PIGAN_GEN_TWO_MLPS;
+  c->skip = cfg->gen_variant == PIGAN_GEN_TRUNK_SKIP;
+  if (c->trunk) c->gen.heads = 2;
   c->disc = NetShape{cfg->disc.in_dim, cfg->disc.n_hidden, cfg->disc.width};
   c->L.stream = (cudaStream_t)cuda_stream;
   cudaGetDevice(&c->L.device);
@@ -352,6 +263,7 @@ pigan_status pigan_create(const pigan_config* cfg, void* cuda_stream, pigan_ctx*
   // bytes per chunk row over both nets: h (L*C) + adjoint ping-pong (2C) planes [+ fp32 scratch]
   size_t per_row = 0;
   for (int C : {3, 5}) per_row += ((size_t)Lh * C + 2 * C) * H * c->elem + (f32 ? (size_t)C * H * 4 : 0) + 2 * C * 4;
+  if (c->skip) per_row += ((size_t)Lh * 5 + 2 * 5) * H * c->elem;           // tanh-jet stash, skip adjoint, raw adjoint planes (net[1])
   const long long max_rows = std::max<long long>((long long)N * cfg->n_colloc, (long long)N * S);
   size_t free_b = 0, total_b = 0;
   cudaMemGetInfo(&free_b, &total_b);
@@ -371,6 +283,12 @@ pigan_status pigan_create(const pigan_config* cfg, void* cuda_stream, pigan_ctx*
       const size_t pl = c->plane();
       w.h = c->alloc<char>((size_t)Lh * w.Cmax * pl);
       w.hs = c->alloc<char>((size_t)c->n_sens_chunks * Lh * 2 * pl);
+      if (c->skip && n == 1) {
+        w.ht = c->alloc<char>((size_t)Lh * w.Cmax * pl);
+        w.hts = c->alloc<char>((size_t)c->n_sens_chunks * Lh * 2 * pl);
+        w.sk = c->alloc<char>((size_t)w.Cmax * pl);
+        w.hhb = c->alloc<char>((size_t)w.Cmax * pl);
+      }
       w.ah[0] = c->alloc<char>((size_t)w.Cmax * pl);
       w.ah[1] = c->alloc<char>((size_t)w.Cmax * pl);
       if (f32) w.apre = c->alloc<float>((size_t)w.Cmax * H * c->R_ld);
@@ -426,6 +344,7 @@ pigan_status pigan_gen_jet_forward(pigan_ctx* c, const float* gen_params, const 
   if (!c) return PIGAN_ERR_INVALID_ARG;
   DeviceGuard dg(c);
   if (jet_order < 0 || jet_order > 2 || n_pts < 0 || n_samples < 0) return fail(c, PIGAN_ERR_INVALID_ARG, "jet_order must be 0..2 and sizes >= 0");
+  if (c->trunk) return fail(c, PIGAN_ERR_UNSUPPORTED, "this context holds the shared-trunk generator: call pigan_trunk_jet_forward");
   if (n_pts == 0 || n_samples == 0) return PIGAN_OK;
   if (!gen_params || !xy || !z || !out) return fail(c, PIGAN_ERR_INVALID_ARG, "null pointer");
   if (n_samples > c->cfg.n_samples) return fail(c, PIGAN_ERR_SHAPE, "n_samples exceeds the n_samples of the config");
@@ -435,6 +354,18 @@ pigan_status pigan_gen_jet_forward(pigan_ctx* c, const float* gen_params, const 
     case PIGAN_BF16: return jet_forward_impl<__half>(c, gen_params, xy, n_pts, z, n_samples, C, out);
     default: return jet_forward_impl<__half>(c, gen_params, xy, n_pts, z, n_samples, C, out);
   }
+}
+
+pigan_status pigan_trunk_jet_forward(pigan_ctx* c, const float* trunk_params, const float* xy, int n_pts, const float* z, int n_samples,
+                                     int jet_order, float* out) {
+  if (!c) return PIGAN_ERR_INVALID_ARG;
+  DeviceGuard dg(c);
+  if (jet_order < 0 || jet_order > 2 || n_pts < 0 || n_samples < 0) return fail(c, PIGAN_ERR_INVALID_ARG, "jet_order must be 0..2 and sizes >= 0");
+  if (!c->trunk) return fail(c, PIGAN_ERR_UNSUPPORTED, "this context holds the two-MLP generator: call pigan_gen_jet_forward");
+  if (n_pts == 0 || n_samples == 0) return PIGAN_OK;
+  if (!trunk_params || !xy || !z || !out) return fail(c, PIGAN_ERR_INVALID_ARG, "null pointer");
+  if (n_samples > c->cfg.n_samples) return fail(c, PIGAN_ERR_SHAPE, "n_samples exceeds the n_samples of the config");
+  return trunk_jet_forward(c, trunk_params, xy, n_pts, z, n_samples, jet_order == 0 ? 1 : jet_order == 1 ? 3 : 5, out);
 }
 
 pigan_status pigan_darcy_residual(pigan_ctx* c, const float* logk_jet, const float* u_jet, const float* f, int n_samples, int n_pts,
@@ -497,10 +428,13 @@ pigan_status pigan_train_step_grads(pigan_ctx* c, const float* logk_params, cons
                                     const float* eps, float loss_scale, float* g_logk, float* g_u, float* g_disc, float* losses, int* found_inf) {
   if (!c) return PIGAN_ERR_INVALID_ARG;
   DeviceGuard dg(c);
-  if (!logk_params || !u_params || !disc_params || !xy_colloc || !f || !xy_sensors || !z || !real_snap || !eps || !g_logk || !g_u || !g_disc)
+  if (!logk_params || !disc_params || !xy_colloc || !f || !xy_sensors || !z || !real_snap || !eps || !g_logk || !g_disc ||
+      (!c->trunk && (!u_params || !g_u)))
     return fail(c, PIGAN_ERR_INVALID_ARG, "null pointer");
   if (!(loss_scale > 0.f) || !std::isfinite(loss_scale)) return fail(c, PIGAN_ERR_INVALID_ARG, "loss_scale must be positive and finite");
   auto run = [&]() -> pigan_status {
+    if (c->trunk)
+      return trunk_train_step(c, logk_params, disc_params, xy_colloc, f, xy_sensors, z, real_snap, eps, loss_scale, g_logk, g_disc, losses, found_inf);
     switch (c->cfg.precision) {
       case PIGAN_FP32: return train_step_impl<float>(c, logk_params, u_params, disc_params, xy_colloc, f, xy_sensors, z, real_snap, eps, loss_scale, g_logk, g_u, g_disc, losses, found_inf);
       default: return train_step_impl<__half>(c, logk_params, u_params, disc_params, xy_colloc, f, xy_sensors, z, real_snap, eps, loss_scale, g_logk, g_u, g_disc, losses, found_inf);

@@ -14,6 +14,7 @@ namespace pigan {
 // ---- flat parameter packing (include/pigan.h): W_l [out][in] then b_l [out], l = 1..L+1 ----------------------
 struct NetShape {
   int in_dim, L, H;
+  int heads = 1;                                                 // outputs of the last layer: 1 (plain MLP) or 2 (shared trunk: log k, u)
   __host__ __device__ size_t first_size() const { return (size_t)H * in_dim + H; }
   __host__ __device__ size_t W_off(int l) const {              // l is 1-based
     if (l == 1) return 0;
@@ -22,9 +23,9 @@ struct NetShape {
   __host__ __device__ size_t b_off(int l) const {
     if (l == 1) return (size_t)H * in_dim;
     if (l <= L) return W_off(l) + (size_t)H * H;
-    return W_off(l) + H;                                       // output layer: w_out [H], then b_out
+    return W_off(l) + (size_t)heads * H;                       // output layer: w_out [heads][H], then b_out [heads]
   }
-  __host__ __device__ size_t count() const { return first_size() + (size_t)(L - 1) * ((size_t)H * H + H) + H + 1; }
+  __host__ __device__ size_t count() const { return first_size() + (size_t)(L - 1) * ((size_t)H * H + H) + (size_t)heads * (H + 1); }
 };
 
 template <typename T> __device__ __forceinline__ float to_f(T v);
@@ -159,6 +160,13 @@ template <typename T>
 void first_layer_bwd(Launcher& L, int C, const NetShape& s, const float* xy, const ChunkGeom& g, const T* ahat,
                      float* gW1 /* flat grads base of this net */, float* An /*[N][H]*/, const float* amax);
 void finalize_first_layer(Launcher& L, const NetShape& s, int N, const float* An, const float* z, float* grads);
+// NEXT-1 (shared trunk, two heads, skip connections): see gen_kernels.cu
+template <typename T>
+void top_act_bwd2(Launcher& L, int C, int H, const ChunkGeom& g, const float* w_out /*[2][H]*/, const float* ohat0, const float* ohat1, const T* h,
+                  const T* tjet, T* ahat, T* sk_out, float* g_bias, float* g_wout /*[2][H]*/, float* g_bout /*[2]*/, const float* amax);
+template <typename T> void plane_add(Launcher& L, int C, int H, const ChunkGeom& g, const T* a, const T* b, T* out);
+template <typename T>
+void skip_adj(Launcher& L, int C, int H, const ChunkGeom& g, const T* hh, const T* sk_in, const T* tjet, T* ahat, T* sk_out, float* g_bias, const float* amax);
 void unscale_and_check(Launcher& L, float* g, size_t n, float inv_scale, int* found_inf);
 void adam(Launcher& L, float* p, const float* g, float* m, float* v, size_t n, float lr, float b1, float b2, float eps,
           float c1, float c2, const int* skip);
@@ -210,8 +218,9 @@ void tc_convert_weights(Launcher& L, int precision, const NetShape& s, const flo
 struct OutDot { const float* w_out; const float* b_out; float* o; long long o_stride; int valid; };
 bool tc_out_dot_fusable(const Launcher& L, int H);
 // hidden layer l forward: h_in [C][H][R_ld] -> h_out [C][H][R_ld]   (fused tanh-jet epilogue)
+// linear: plain GEMM out_c = W in_c (no bias, no tanh) -- the raw adjoint planes hhat = W^T ahat of a skip layer (NEXT-1)
 void tc_layer_fwd(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* w16_l, const float* bias,
-                  const void* h_in, void* h_out, const OutDot* od = nullptr);
+                  const void* h_in, void* h_out, const OutDot* od = nullptr, bool linear = false);
 void tc_layer_fwd_split(Launcher& L, int precision, int H, int R, int R_ld, const void* w16_l, const float* bias, const void* h_in, void* h_out,
                         const OutDot* od = nullptr);
 // dgrad of layer l with the adjoint of layer l-1's tanh fused: ahat_in (layer l) -> ahat_out (layer l-1)
@@ -233,7 +242,7 @@ bool tc_first_layer_fusable(int H, const ChunkGeom& g);
 // ---- the same four on CTA pairs (tc2_kernels.cu, cta_group::2), taken when tc2_supported(H) ---------------------
 bool tc2_supported(const Launcher& L, int H);
 void tc2_layer_fwd(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* w16_l, const float* bias,
-                   const void* h_in, void* h_out, const OutDot* od);
+                   const void* h_in, void* h_out, const OutDot* od, bool linear);
 void tc2_layer_fwd_split(Launcher& L, int precision, int H, int R, int R_ld, const void* w16_l, const float* bias, const void* h_in, void* h_out,
                          const OutDot* od);
 void tc2_layer_bwd(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* w16T_l, const void* ahat_in,

@@ -389,4 +389,173 @@ void first_layer_bwd(Launcher& L, int C, const NetShape& s, const float* xy, con
 template void first_layer_bwd<float>(Launcher&, int, const NetShape&, const float*, const ChunkGeom&, const float*, float*, float*, const float*);
 template void first_layer_bwd<__half>(Launcher&, int, const NetShape&, const float*, const ChunkGeom&, const __half*, float*, float*, const float*);
 
+
+
+// =============================================================================================================
+// NEXT-1: shared-trunk generator with two output heads and skip connections.
+// The trunk reuses the layer kernels; what is new is elementwise and lives here:
+//   top_act_bwd2   adjoint of the last tanh layer seeded by BOTH heads: hhat_c = w_k[j] Yhat_c[r] + w_u[j] uhat_c[r]
+//   plane_add      h^l = t^l + h^{l-2}                                   (skip connection, forward)
+//   skip_adj       hhat_total = hhat + skip adjoint; ahat = J^T hhat_total (O4 on t^l); hands hhat_total on to h^{l-2}
+// =============================================================================================================
+template <typename T, int C>
+__global__ void __launch_bounds__(256) top_act_bwd2_kernel(int H, ChunkGeom g, const float* __restrict__ w_out /*[2][H]*/,
+                                                           const float* __restrict__ ohat0 /*[C0][R_ld]*/, const float* __restrict__ ohat1 /*[C][R_ld]*/,
+                                                           const T* __restrict__ h, const T* __restrict__ tjet, T* __restrict__ ahat,
+                                                           T* __restrict__ sk_out, float* __restrict__ g_bias, float* __restrict__ g_wout /*[2][H]*/,
+                                                           float* __restrict__ g_bout /*[2]*/, const float* __restrict__ amax) {
+  constexpr int C0 = C >= 3 ? 3 : 1;                          // log k carries (value, x, y); its xx, yy adjoints are zero (O3)
+  __shared__ float red[kTopUnits][3];
+  __shared__ float red8[8];
+  const int lane = threadIdx.x & 31;
+  const int jb = blockIdx.y * kTopUnits, je = min(H, jb + kTopUnits);
+  const size_t plane = (size_t)H * g.R_ld;
+  const float sc = adj_scale(amax), inv_sc = adj_inv_scale(amax);
+  if (threadIdx.x < kTopUnits * 3) (&red[0][0])[threadIdx.x] = 0.f;
+  __syncthreads();
+  const int r0 = blockIdx.x * 2048 + threadIdx.x * 8;
+  const bool active = r0 < g.R;
+  float o0[C0][8], o1[C][8];
+#pragma unroll
+  for (int c = 0; c < C; ++c) {
+    if (active) { load8<float>(ohat1 + (size_t)c * g.R_ld + r0, o1[c]); if (c < C0) load8<float>(ohat0 + (size_t)c * g.R_ld + r0, o0[c]); }
+    else {
+#pragma unroll
+      for (int i = 0; i < 8; ++i) { o1[c][i] = 0.f; if (c < C0) o0[c][i] = 0.f; }
+    }
+  }
+  float sb0 = 0.f, sb1 = 0.f;
+#pragma unroll
+  for (int i = 0; i < 8; ++i) { sb0 += o0[0][i]; sb1 += o1[0][i]; }
+  for (int j = jb; j < je; ++j) {
+    float s_bias = 0.f, s_w0 = 0.f, s_w1 = 0.f;
+    if (active) {
+      const float w0 = w_out[j] * sc, w1 = w_out[H + j] * sc;
+      const size_t off = (size_t)j * g.R_ld + r0;
+      float hv[C][8], tv[C][8], o[C][8], hh[C][8];
+#pragma unroll
+      for (int c = 0; c < C; ++c) { load8<T>(h + c * plane + off, hv[c]); load8<T>(tjet + c * plane + off, tv[c]); }
+#pragma unroll
+      for (int i = 0; i < 8; ++i) {
+        float hx[5], hj[5], aa[5];
+#pragma unroll
+        for (int c = 0; c < C; ++c) {
+          hx[c] = w1 * o1[c][i]; s_w1 = fmaf(o1[c][i], hv[c][i], s_w1);
+          if (c < C0) { hx[c] = fmaf(w0, o0[c][i], hx[c]); s_w0 = fmaf(o0[c][i], hv[c][i], s_w0); }
+          hj[c] = tv[c][i]; hh[c][i] = hx[c];
+        }
+        jet_act_bwd<C>(hj, hx, aa);
+        s_bias += aa[0];
+#pragma unroll
+        for (int c = 0; c < C; ++c) o[c][i] = aa[c];
+      }
+#pragma unroll
+      for (int c = 0; c < C; ++c) { store8<T>(ahat + c * plane + off, o[c]); if (sk_out) store8<T>(sk_out + c * plane + off, hh[c]); }
+    }
+    s_bias = warp_sum_f(s_bias); s_w0 = warp_sum_f(s_w0); s_w1 = warp_sum_f(s_w1);
+    if (lane == 0) { atomicAdd(&red[j - jb][0], s_bias); atomicAdd(&red[j - jb][1], s_w0); atomicAdd(&red[j - jb][2], s_w1); }
+  }
+  __syncthreads();
+  if (threadIdx.x < je - jb) {
+    atomicAdd(g_bias + jb + threadIdx.x, red[threadIdx.x][0] * inv_sc);
+    atomicAdd(g_wout + jb + threadIdx.x, red[threadIdx.x][1]);
+    atomicAdd(g_wout + H + jb + threadIdx.x, red[threadIdx.x][2]);
+  }
+  if (blockIdx.y == 0) {
+    float v = block_sum_256(sb0, red8); if (threadIdx.x == 0) atomicAdd(g_bout, v);
+    v = block_sum_256(sb1, red8); if (threadIdx.x == 0) atomicAdd(g_bout + 1, v);
+  }
+}
+
+template <typename T>
+void top_act_bwd2(Launcher& L, int C, int H, const ChunkGeom& g, const float* w_out, const float* ohat0, const float* ohat1, const T* h,
+                  const T* tjet, T* ahat, T* sk_out, float* g_bias, float* g_wout, float* g_bout, const float* amax) {
+  if (g.R <= 0) return;
+  dim3 grid(cdiv(g.R, 2048), cdiv(H, kTopUnits));
+#define PIGAN_TOP2(c) top_act_bwd2_kernel<T, c><<<grid, 256, 0, L.stream>>>(H, g, w_out, ohat0, ohat1, h, tjet, ahat, sk_out, g_bias, g_wout, g_bout, amax)
+  if (C == 1) PIGAN_TOP2(1); else if (C == 3) PIGAN_TOP2(3); else PIGAN_TOP2(5);
+#undef PIGAN_TOP2
+  L.check("jet_act_bwd");
+}
+template void top_act_bwd2<float>(Launcher&, int, int, const ChunkGeom&, const float*, const float*, const float*, const float*, const float*, float*, float*, float*, float*, float*, const float*);
+template void top_act_bwd2<__half>(Launcher&, int, int, const ChunkGeom&, const float*, const float*, const float*, const __half*, const __half*, __half*, __half*, float*, float*, float*, const float*);
+
+// out_c = a_c + b_c on C planes [C][H][R_ld] (rows < R)
+template <typename T>
+__global__ void __launch_bounds__(256) plane_add_kernel(int n_planes_rows /* C*H */, int R, int R_ld, const T* __restrict__ a, const T* __restrict__ b,
+                                                        T* __restrict__ out) {
+  const int r0 = blockIdx.x * 2048 + threadIdx.x * 8;
+  if (r0 >= R) return;
+  for (int pj = blockIdx.y; pj < n_planes_rows; pj += gridDim.y) {
+    const size_t off = (size_t)pj * R_ld + r0;
+    float x[8], y[8];
+    load8<T>(a + off, x); load8<T>(b + off, y);
+#pragma unroll
+    for (int i = 0; i < 8; ++i) x[i] += y[i];
+    store8<T>(out + off, x);
+  }
+}
+template <typename T>
+void plane_add(Launcher& L, int C, int H, const ChunkGeom& g, const T* a, const T* b, T* out) {
+  if (g.R <= 0) return;
+  dim3 grid(cdiv(g.R, 2048), std::min(C * H, 1024));
+  plane_add_kernel<T><<<grid, 256, 0, L.stream>>>(C * H, g.R, g.R_ld, a, b, out);
+  L.check("skip_add");
+}
+template void plane_add<float>(Launcher&, int, int, const ChunkGeom&, const float*, const float*, float*);
+template void plane_add<__half>(Launcher&, int, int, const ChunkGeom&, const __half*, const __half*, __half*);
+
+// skip layers, reverse: total = hh (+ sk_in); sk_out = total (if the layer itself takes a skip); ahat = J^T(tjet) total; b_hat += sum ahat_0
+template <typename T, int C>
+__global__ void __launch_bounds__(256) skip_adj_kernel(int H, ChunkGeom g, const T* __restrict__ hh, const T* __restrict__ sk_in, const T* __restrict__ tjet,
+                                                       T* __restrict__ ahat, T* __restrict__ sk_out, float* __restrict__ g_bias,
+                                                       const float* __restrict__ amax) {
+  __shared__ float red[8];
+  const int j = blockIdx.y;
+  const size_t plane = (size_t)H * g.R_ld;
+  const float inv_sc = adj_inv_scale(amax);
+  float s_bias = 0.f;
+  const int r0 = blockIdx.x * 2048 + threadIdx.x * 8;
+  if (r0 < g.R) {
+    const size_t off = (size_t)j * g.R_ld + r0;
+    float tv[C][8], tot[C][8], o[C][8];
+#pragma unroll
+    for (int c = 0; c < C; ++c) {
+      load8<T>(tjet + c * plane + off, tv[c]);
+      load8<T>(hh + c * plane + off, tot[c]);
+      if (sk_in) {
+        float s[8];
+        load8<T>(sk_in + c * plane + off, s);
+#pragma unroll
+        for (int i = 0; i < 8; ++i) tot[c][i] += s[i];
+      }
+    }
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+      float hx[5], hj[5], aa[5];
+#pragma unroll
+      for (int c = 0; c < C; ++c) { hx[c] = tot[c][i]; hj[c] = tv[c][i]; }
+      jet_act_bwd<C>(hj, hx, aa);
+      s_bias += aa[0];
+#pragma unroll
+      for (int c = 0; c < C; ++c) o[c][i] = aa[c];
+    }
+#pragma unroll
+    for (int c = 0; c < C; ++c) { store8<T>(ahat + c * plane + off, o[c]); if (sk_out) store8<T>(sk_out + c * plane + off, tot[c]); }
+  }
+  const float v = block_sum_256(s_bias, red);
+  if (threadIdx.x == 0) atomicAdd(g_bias + j, v * inv_sc);
+}
+template <typename T>
+void skip_adj(Launcher& L, int C, int H, const ChunkGeom& g, const T* hh, const T* sk_in, const T* tjet, T* ahat, T* sk_out, float* g_bias, const float* amax) {
+  if (g.R <= 0) return;
+  dim3 grid(cdiv(g.R, 2048), H);
+  if (C == 1) skip_adj_kernel<T, 1><<<grid, 256, 0, L.stream>>>(H, g, hh, sk_in, tjet, ahat, sk_out, g_bias, amax);
+  else if (C == 3) skip_adj_kernel<T, 3><<<grid, 256, 0, L.stream>>>(H, g, hh, sk_in, tjet, ahat, sk_out, g_bias, amax);
+  else skip_adj_kernel<T, 5><<<grid, 256, 0, L.stream>>>(H, g, hh, sk_in, tjet, ahat, sk_out, g_bias, amax);
+  L.check("skip_adj");
+}
+template void skip_adj<float>(Launcher&, int, int, const ChunkGeom&, const float*, const float*, const float*, float*, float*, float*, const float*);
+template void skip_adj<__half>(Launcher&, int, int, const ChunkGeom&, const __half*, const __half*, const __half*, __half*, __half*, float*, const float*);
+
 }  // namespace pigan

@@ -58,6 +58,7 @@ struct Jet2Params {
   float* o;              // [C][o_stride] fp32 (MODE 5: one plane)
   long long o_stride;
   int valid;             // rows of the chunk that exist: rows >= valid are not accumulated
+  int linear;            // MODE 0 only: plain GEMM, out_c = W in_c (no bias, no tanh): the raw adjoint planes of a skip layer (NEXT-1)
 };
 
 // MODE 0: forward; MODE 1: dgrad + adjoint of the previous tanh; MODE 2: value-only forward on split (hi, lo) planes;
@@ -263,7 +264,7 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
       const uint32_t tb0 = lane_base + g0_col(it) + hs * (nc0 * 32), tb1 = lane_base + g1_col + hs * 64;
       auto tcol = [&](int c) -> uint32_t { return (C == 5 && c >= 3) ? tb1 + (c - 3) * 32 : tb0 + c * 32; };
       float bias = 0.f, bias_acc = 0.f;
-      if (kFwd || kSplit) bias = p.bias[unit];
+      if ((kFwd || kSplit) && p.bias) bias = p.bias[unit];
       float wo = 0.f;
       if (kOutDot) wo = p.w_out[unit];
       // MODE 4, 5: lane -> row (4 * bit4 + 2 * bit3 + bit2) of each group of 8 rows; one lane of four adds
@@ -364,7 +365,12 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
             for (int c = 0; c < nc0; ++c) a[c] = v[c][i];
             if (C == 5) { a[3] = kxx[rc * 8 + i]; a[4] = kyy[rc * 8 + i]; }
             a[0] += bias;
-            jet_act_fwd<C>(fast_tanh(a[0]), a, h);
+            if (MODE == 0 && p.linear) {
+#pragma unroll
+              for (int c = 0; c < C; ++c) h[c] = a[c];
+            } else {
+              jet_act_fwd<C>(fast_tanh(a[0]), a, h);
+            }
 #pragma unroll
             for (int c = 0; c < C; ++c) o[c][i] = h[c];
           }
@@ -627,12 +633,12 @@ static void set_out_dot(Jet2Params& p, const OutDot* od) {
 }
 
 void tc2_layer_fwd(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* w16_l, const float* bias, const void* h_in, void* h_out,
-                   const OutDot* od) {
+                   const OutDot* od, bool linear) {
   CUtensorMap a, b;
   bool ok = weight_map(L, &a, precision, w16_l, H) && plane_map(L, &b, precision, h_in, H, R_ld, C, 32, 64, C, CU_TENSOR_MAP_SWIZZLE_64B);
   if (!ok) return;
   Jet2Params p{};
-  p.H = H; p.n_row_tiles = R / 64; p.bias = bias; p.out = h_out; p.R_ld = R_ld;
+  p.H = H; p.n_row_tiles = R / 64; p.bias = bias; p.out = h_out; p.R_ld = R_ld; p.linear = linear ? 1 : 0;
   if (od) { set_out_dot(p, od); dispatch_jet2<4>(L, C, a, b, b, p); return; }
   dispatch_jet2<0>(L, C, a, b, b, p);
 }

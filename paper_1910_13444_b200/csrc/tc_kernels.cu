@@ -40,6 +40,7 @@ struct JetParams {
   const float* amax;     // MODE 1, 3: block-scale source of the adjoint planes (common.cuh adj_inv_scale)
   // MODE 3 (MODE 1 + first-layer reduction, O4 'First layer'; see tc2_kernels.cu): ahat^1 is consumed in registers
   const float* xy; long long row0; int npts, in_dim; float* gW1; float* An;
+  int linear;            // MODE 0 only: plain GEMM, out_c = W in_c (no bias, no tanh) -- see tc2_kernels.cu
 };
 
 template <typename T, int C, int MODE>
@@ -150,7 +151,7 @@ __global__ void __launch_bounds__(256, 1) jet_layer_kernel(const __grid_constant
       const int unit0 = ut * kBM + q * 32, unit = unit0 + lane;
       const uint32_t tbase = tmem_base + ((uint32_t)(q * 32) << 16) + buf * Cfg::kCols;
       float bias = 0.f, bias_acc = 0.f;
-      if (MODE == 0 || MODE == 2) bias = p.bias[unit];
+      if ((MODE == 0 || MODE == 2) && p.bias) bias = p.bias[unit];
 
       auto issue_stage_loads = [&](int hf) {                 // MODE 1: the previous layer's output jet h^{l-1} -> staging
         if (elect_one()) {
@@ -182,7 +183,12 @@ __global__ void __launch_bounds__(256, 1) jet_layer_kernel(const __grid_constant
 #pragma unroll
               for (int c = 0; c < C; ++c) a[c] = v[c][i];
               a[0] += bias;
-              jet_act_fwd<C>(fast_tanh(a[0]), a, h);
+              if (p.linear) {
+#pragma unroll
+                for (int c = 0; c < C; ++c) h[c] = a[c];
+              } else {
+                jet_act_fwd<C>(fast_tanh(a[0]), a, h);
+              }
 #pragma unroll
               for (int c = 0; c < C; ++c) o[c][i] = h[c];
             }
@@ -481,15 +487,15 @@ static void dispatch_jet(Launcher& L, int precision, int C, const CUtensorMap& a
 bool tc_out_dot_fusable(const Launcher& L, int H) { return tc2_supported(L, H); }   // the one-CTA kernels keep the separate out_fwd pass
 
 void tc_layer_fwd(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* w16_l, const float* bias, const void* h_in, void* h_out,
-                  const OutDot* od) {
+                  const OutDot* od, bool linear) {
   if (R <= 0) return;
-  if (tc2_supported(L, H)) { tc2_layer_fwd(L, precision, C, H, R, R_ld, w16_l, bias, h_in, h_out, od); return; }
+  if (tc2_supported(L, H)) { tc2_layer_fwd(L, precision, C, H, R, R_ld, w16_l, bias, h_in, h_out, od, linear); return; }
   CUtensorMap a, b, o;
   bool ok = weight_map(L, &a, precision, w16_l, H) && plane_map(L, &b, precision, h_in, H, R_ld, C, kRT, kBK, C, CU_TENSOR_MAP_SWIZZLE_128B) &&
             plane_map(L, &o, precision, h_out, H, R_ld, C, 32, 32, 1, CU_TENSOR_MAP_SWIZZLE_64B);
   if (!ok) return;
   JetParams p{};
-  p.H = H; p.n_row_tiles = R / kRT; p.bias = bias;
+  p.H = H; p.n_row_tiles = R / kRT; p.bias = bias; p.linear = linear ? 1 : 0;
   dispatch_jet<0>(L, precision, C, a, b, o, o, p);
 }
 

@@ -105,3 +105,43 @@ def jets_parity(cfg, jet_order=2, bias_std=0.1, n_samples=None, xy=None, workspa
     got = out.cpu().numpy()
     pg.close()
     return {f"ch{c}": rel_err(got[c], ref[c]) for c in range(ref.shape[0])}, got, ref
+
+
+# ---- NEXT-1: shared-trunk generator ------------------------------------------------------------------------------
+def per_layer_trunk(flat, shape):
+    out = {}
+    for l, (W, b) in enumerate(orc.unpack_trunk_params(np.asarray(flat, dtype=np.float64), *shape), start=1):
+        out[f"W{l}"] = W; out[f"b{l}"] = b
+    return out
+
+
+def trunk_step_parity(cfg, skip, bias_std=0.1, loss_scale=1.0, chunk_rows=0, pde_weight=1.0):
+    """Step with the paper's generator (gen_variant trunk / trunk_skip) against train_step_grads_trunk_ref."""
+    import torch
+    from paper_1910_13444_b200 import PiGan
+    inp = wl.make_inputs(cfg, bias_std=bias_std)
+    J = orc.trunk_jet_forward_ref(inp["teacher_G"], *cfg.gen_shape, inp["xy_sensors"], inp["z_real"], 0, skip)
+    inp["real"] = np.concatenate([J[0][0], J[1][0]], axis=1).astype(np.float32)
+    gG, gD, losses = orc.train_step_grads_trunk_ref(cfg.gen_shape, cfg.disc_shape, inp["theta_G"], inp["theta_D"], inp["xy_colloc"], inp["f"],
+                                                    inp["xy_sensors"], inp["z"], inp["real"], inp["eps"], 10.0, pde_weight, skip=skip)
+    d = to_dev(inp, "cuda:0")
+    pg = PiGan.from_config(cfg, pde_weight=pde_weight, chunk_rows=chunk_rows, gen_variant="trunk_skip" if skip else "trunk")
+    out = pg.train_step_grads(d["theta_G"], None, d["theta_D"], d["xy_colloc"], d["f"], d["xy_sensors"], d["z"], d["real"], d["eps"], loss_scale)
+    torch.cuda.synchronize()
+    errs = {}
+    a = per_layer_trunk(out[0].cpu().numpy(), cfg.gen_shape); b = per_layer_trunk(gG, cfg.gen_shape)
+    for k in a:
+        errs[f"gG.{k}"] = rel_err(a[k], b[k])
+    a = per_layer(out[2].cpu().numpy(), cfg.disc_shape); b = per_layer(gD, cfg.disc_shape)
+    for k in a:
+        errs[f"gD.{k}"] = rel_err(a[k], b[k])
+    lg = out[3].cpu().numpy().astype(np.float64)
+    fi = int(out[4].item())
+    # jets of both heads through the forward-only entry point
+    Jg = pg.trunk_jet_forward(d["theta_G"], d["xy_colloc"], d["z"], 2).cpu().numpy()
+    Jr = orc.trunk_jet_forward_ref(inp["theta_G"], *cfg.gen_shape, inp["xy_colloc"], inp["z"], 2, skip)
+    for k in range(2):
+        for c in range(5):
+            errs[f"jet.head{k}.ch{c}"] = rel_err(Jg[k][c], Jr[k][c])
+    pg.close()
+    return errs, lg, losses, fi

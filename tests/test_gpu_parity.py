@@ -10,7 +10,7 @@ import pytest
 
 import workloads as wl
 from oracle import pigan_oracle as orc
-from parity_util import jets_parity, per_layer, rel_err, step_parity, to_dev
+from parity_util import jets_parity, per_layer, rel_err, step_parity, to_dev, trunk_step_parity
 
 pytestmark = pytest.mark.gpu
 
@@ -330,3 +330,35 @@ def test_graph_replay_matches_eager_and_sees_in_place_updates(name):
         assert rel_err(b.cpu().numpy(), a.cpu().numpy()) <= tol
     assert rel_err(out[0].cpu().numpy(), first[0].cpu().numpy()) > 10 * tol      # and the update did change the result
     pg.close(); pg2.close()
+
+
+# ---- NEXT-1: the paper's generator (shared trunk, two heads, skip connections) ----------------------------
+def check_trunk(cfg, skip, **kw):
+    errs, lg, lr, found_inf = trunk_step_parity(cfg, skip, **kw)
+    bad = {k: v for k, v in errs.items() if not v <= TOL[cfg.precision]}
+    assert not bad, f"{cfg.name} skip={skip}: over tolerance {bad}"
+    assert found_inf == 0
+    lrel = np.abs(lg - lr) / np.maximum(np.abs(lr), 1e-12)
+    assert np.all(lrel <= LOSS_TOL), f"{cfg.name} skip={skip}: losses gpu {lg} ref {lr} rel {lrel}"
+
+
+@pytest.mark.parametrize("skip", [False, True])
+def test_trunk_fp32(skip):
+    cfg = dataclasses.replace(wl.CONFIGS["c1"], name="trunk-fp32", L=5)                  # skips at l = 3 and l = 5 (the top layer)
+    check_trunk(cfg, skip)
+    check_trunk(dataclasses.replace(cfg, name="trunk-fp32-L4", L=4, G=7, N=5, S=3), skip)  # even depth, ragged rows
+
+
+@pytest.mark.parametrize("skip", [False, True])
+def test_trunk_5x128_one_cta_kernels(skip):
+    """The paper's 5 x 128 network (4 hidden layers + the output layer), 16-bit path on the one-CTA tcgen05 kernels."""
+    cfg = dataclasses.replace(wl.CONFIGS["c2"], name="trunk-5x128", N=8, G=16, S=32)
+    check_trunk(cfg, skip)
+
+
+@pytest.mark.parametrize("skip", [False, True])
+def test_trunk_11x512_cta_pair_kernels(skip):
+    """The paper's 11 x 512 network (10 hidden layers + the output layer), CTA-pair kernels, several chunks."""
+    cfg = dataclasses.replace(wl.CONFIGS["c4"], name="trunk-11x512", L=10, m=64, N=4, G=16, S=40, HD=128, LD=3)
+    check_trunk(cfg, skip)
+    check_trunk(cfg, skip, chunk_rows=256)

@@ -86,6 +86,17 @@ def xavier_params(rng, in_dim: int, n_hidden: int, width: int, bias_std: float =
     return np.concatenate(parts)
 
 
+def xavier_trunk_params(rng, in_dim: int, n_hidden: int, width: int, bias_std: float = 0.0) -> np.ndarray:
+    """The paper's shared-trunk generator (NEXT-1): as xavier_params, with a last layer of TWO outputs (log k, u)."""
+    parts, fan_in = [], in_dim
+    for l in range(n_hidden + 1):
+        fan_out = width if l < n_hidden else 2
+        parts.append(rng.normal(0.0, np.sqrt(2.0 / (fan_in + fan_out)), size=fan_out * fan_in))
+        parts.append(rng.normal(0.0, bias_std, size=fan_out) if bias_std > 0 else np.zeros(fan_out))
+        fan_in = fan_out
+    return np.concatenate(parts)
+
+
 def collocation_grid(G: int) -> np.ndarray:
     """Cell-centred G x G grid on the unit square, p = j*G + i -> ((i+1/2)/G, (j+1/2)/G)  (reading G13)."""
     c = (np.arange(G, dtype=np.float64) + 0.5) / G
@@ -127,6 +138,9 @@ def make_inputs(cfg: Config, bias_std: float = 0.0) -> dict:
         "xy_colloc": collocation_grid(cfg.G),
     }
     out["f"] = source_term(cfg, out["xy_colloc"])
+    # NEXT-1: student and teacher of the shared-trunk variant (streams 10, 11)
+    out["theta_G"] = round_to_precision(xavier_trunk_params(_rng(cfg, 10), *gen, bias_std=bias_std), pr)
+    out["teacher_G"] = round_to_precision(xavier_trunk_params(_rng(cfg, 11), *gen, bias_std=bias_std), pr)
     return out
 
 
