@@ -66,9 +66,10 @@ def hbm_class_bytes(cfg) -> dict:
     e = 4 if cfg.precision == "fp32" else 2
     rows, srows, H = cfg.N * cfg.P, cfg.N * cfg.S, cfg.H
     plane = H * e
-    col = (3 + 5) * rows * plane                            # one pass over the C planes of both nets, collocation rows
-    sen = 2 * srows * plane                                 # one pass over the value plane of both nets, sensor rows
-    n_par = 2 * wl.param_count(*cfg.gen_shape) + wl.param_count(*cfg.disc_shape)
+    two = cfg.variant == "two_mlps"
+    col = ((3 + 5) if two else 5) * rows * plane            # one pass over the C planes of the net(s), collocation rows
+    sen = (2 if two else 1) * srows * plane                 # one pass over the value plane of the net(s), sensor rows
+    n_par = (2 if two else 1) * wl.param_count(*cfg.gen_shape) + wl.param_count(*cfg.disc_shape)
     return {"first_layer_fwd": col + sen * (1 + (2 if e == 2 else 1)),   # writes h^1: collocation, sensor pass with stash, snapshot pass (hi, lo)
             "out_fwd": col + sen * (1 + (2 if e == 2 else 1)),           # reads h^L
             "jet_act_bwd": 2 * (col + sen),                               # top layer: reads h^L, writes ahat^L
@@ -175,17 +176,26 @@ class GpuWorkload:
         from paper_1910_13444_b200 import PiGan
         self.cfg, self.device, self.torch = cfg, device, torch
         inp = wl.make_inputs(dataclasses.replace(cfg, index=cfg.index + 10 * seed_shift) if seed_shift else cfg)
-        self.pg = PiGan.from_config(cfg, device=device, chunk_rows=chunk_rows)
+        self.trunk = cfg.variant != "two_mlps"
+        self.pg = PiGan.from_config(cfg, device=device, chunk_rows=chunk_rows, gen_variant=cfg.variant)
         d = {k: torch.from_numpy(np.ascontiguousarray(v)).to(device) for k, v in inp.items()}
-        # "real" snapshots: the frozen teacher pair evaluated at the sensors by the GPU library, outside any timed region
-        Ys = self.pg.gen_jet_forward(d["teacher_Y"], d["xy_sensors"], d["z_real"], 0)[0]
-        Us = self.pg.gen_jet_forward(d["teacher_u"], d["xy_sensors"], d["z_real"], 0)[0]
+        # "real" snapshots: the frozen teacher evaluated at the sensors by the GPU library, outside any timed region
+        if self.trunk:
+            J = self.pg.trunk_jet_forward(d["teacher_G"], d["xy_sensors"], d["z_real"], 0)
+            Ys, Us = J[0][0], J[1][0]
+        else:
+            Ys = self.pg.gen_jet_forward(d["teacher_Y"], d["xy_sensors"], d["z_real"], 0)[0]
+            Us = self.pg.gen_jet_forward(d["teacher_u"], d["xy_sensors"], d["z_real"], 0)[0]
         d["real"] = torch.cat([Ys, Us], dim=1).contiguous()
         self.d = d
-        self.params = [d["theta_Y"].clone(), d["theta_u"].clone(), d["theta_D"].clone()]
+        self.params = [d["theta_G"].clone(), d["theta_D"].clone()] if self.trunk else [d["theta_Y"].clone(), d["theta_u"].clone(), d["theta_D"].clone()]
         self.mom = [(torch.zeros_like(p), torch.zeros_like(p)) for p in self.params]
-        self.out = (torch.empty_like(self.params[0]), torch.empty_like(self.params[1]), torch.empty_like(self.params[2]),
-                    torch.empty(6, device=device), torch.zeros(1, dtype=torch.int32, device=device))
+        if self.trunk:
+            self.out = (torch.empty_like(self.params[0]), None, torch.empty_like(self.params[1]),
+                        torch.empty(6, device=device), torch.zeros(1, dtype=torch.int32, device=device))
+        else:
+            self.out = (torch.empty_like(self.params[0]), torch.empty_like(self.params[1]), torch.empty_like(self.params[2]),
+                        torch.empty(6, device=device), torch.zeros(1, dtype=torch.int32, device=device))
         self.loss_scale = 1024.0 if cfg.precision == "fp16" else 1.0
         self.step_no = 0
         # pinned host copies of the per-step inputs for the end-to-end leg
@@ -196,10 +206,16 @@ class GpuWorkload:
     def step(self):
         d, pg = self.d, self.pg
         self.step_no += 1
-        pg.train_step_grads(self.params[0], self.params[1], self.params[2], d["xy_colloc"], d["f"], d["xy_sensors"], d["z"], d["real"],
-                            d["eps"], self.loss_scale, out=self.out)
-        for k in range(3):
-            pg.adam_update(self.params[k], self.out[k], self.mom[k][0], self.mom[k][1], self.step_no, skip_flag=self.out[4], **ADAM)
+        if self.trunk:
+            pg.train_step_grads(self.params[0], None, self.params[1], d["xy_colloc"], d["f"], d["xy_sensors"], d["z"], d["real"],
+                                d["eps"], self.loss_scale, out=self.out)
+            grads = (self.out[0], self.out[2])
+        else:
+            pg.train_step_grads(self.params[0], self.params[1], self.params[2], d["xy_colloc"], d["f"], d["xy_sensors"], d["z"], d["real"],
+                                d["eps"], self.loss_scale, out=self.out)
+            grads = self.out[:3]
+        for k in range(len(self.params)):
+            pg.adam_update(self.params[k], grads[k], self.mom[k][0], self.mom[k][1], self.step_no, skip_flag=self.out[4], **ADAM)
 
     def step_e2e(self):
         """Same step with the per-step inputs coming from pinned host memory and the losses read back."""
@@ -215,6 +231,10 @@ class GpuWorkload:
         if not hasattr(self, "jet_out"):
             n = self.cfg.N * self.cfg.P
             self.jet_out = (self.torch.empty(5 * n, device=self.device), self.torch.empty(3 * n, device=self.device))
+            self.jet_out2 = self.torch.empty(2, 5, self.cfg.N, self.cfg.P, device=self.device) if self.trunk else None
+        if self.trunk:
+            pg.trunk_jet_forward(self.params[0], d["xy_colloc"], d["z"], 2, out=self.jet_out2)
+            return
         pg.gen_jet_forward(self.params[1], d["xy_colloc"], d["z"], 2, out=self.jet_out[0].view(5, self.cfg.N, self.cfg.P))
         pg.gen_jet_forward(self.params[0], d["xy_colloc"], d["z"], 1, out=self.jet_out[1].view(3, self.cfg.N, self.cfg.P))
 
@@ -232,7 +252,9 @@ class GpuWorkload:
             if self.flush is not None:
                 self.flush.fill_(1)
             a.record()
+            torch.cuda.nvtx.range_push("timed_step")          # lets `ncu --nvtx --nvtx-include "timed_step/"` isolate the timed steps
             fn()
+            torch.cuda.nvtx.range_pop()
             b.record()
         torch.cuda.synchronize(self.device)
         return [a.elapsed_time(b) for a, b in ev]
@@ -275,7 +297,7 @@ def run_config(cfg, device, steps, warmup, rank, world, with_roofline=True, seed
     res["h2d"], res["d2h"] = w.e2e_bytes()
     # jet evaluations/s (north_star's second throughput figure): forward jets of both nets, no residual, no backward
     res["ms_jet"] = w.timed(w.jet_pass, max(2, steps // 2), 1)
-    del w.jet_out
+    del w.jet_out, w.jet_out2
     # roofline of the dominant kernel class (the tcgen05 jet GEMMs: forward, dgrad+adjoint, wgrad)
     if with_roofline:
         tc = {k: v for k, v in prof.items() if k in ("jet_layer_fwd", "jet_layer_bwd", "wgrad")}
@@ -286,7 +308,7 @@ def run_config(cfg, device, steps, warmup, rank, world, with_roofline=True, seed
         res["kernel_launches_per_step"] = {k: v[0] for k, v in per_step.items()}
         if tc_ms > 0:
             # algorithmic flops of the hidden jet layers of the collocation + sensor rows: 3 GEMMs (fwd, dgrad, wgrad) per layer
-            sens_gemm = cfg.N * 3 * cfg.S * 2 * (cfg.L - 1) * 2 * cfg.H * cfg.H
+            sens_gemm = cfg.N * 3 * cfg.S * (2 if cfg.variant == "two_mlps" else 1) * (cfg.L - 1) * 2 * cfg.H * cfg.H
             alg = flops["jet_gemm"] + sens_gemm
             ach = alg / (tc_ms * 1e-3) / 1e12
             peak = peaks["tflops_sustained"]
@@ -308,7 +330,7 @@ def run_config(cfg, device, steps, warmup, rank, world, with_roofline=True, seed
         hb = hbm_class_bytes(cfg)
         t_roof = 0.0
         if cfg.precision != "fp32":
-            sens_gemm = cfg.N * 3 * cfg.S * 2 * (cfg.L - 1) * 2 * cfg.H * cfg.H
+            sens_gemm = cfg.N * 3 * cfg.S * (2 if cfg.variant == "two_mlps" else 1) * (cfg.L - 1) * 2 * cfg.H * cfg.H
             t_roof += (flops["jet_gemm"] + sens_gemm) / (peaks["tflops_sustained"] * 1e12) * 1e3
         hk = {}
         for k, b in hb.items():
@@ -350,7 +372,8 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=None)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", default="c5", choices=list(wl.CONFIGS))
+    ap.add_argument("--config", default="c5", choices=list(wl.CONFIGS) + ["t2"],
+                    help="c1..c5 = BASELINE.json configs; t2 = the paper's Table II generator-worker workload on its own 21x1024 shared-trunk generator (NEXT-1)")
     ap.add_argument("--impl", default="pigan", choices=["pigan", "reference"])
     ap.add_argument("--all-configs", action="store_true", default=True, help="also run the other configs briefly and attach them as per_config (default)")
     ap.add_argument("--headline-only", dest="all_configs", action="store_false", help="time only --config")
@@ -359,7 +382,7 @@ def main():
                     "the line then says so in config.workload and is not a benchmark value")
     ap.add_argument("--chunk-rows", type=int, default=0, help="rows per chunk of the generator passes (0 = library default); sweeps only")
     args = ap.parse_args()
-    cfg = wl.CONFIGS[args.config]
+    cfg = wl.TABLE2 if args.config == "t2" else wl.CONFIGS[args.config]
     if args.samples:
         args.all_configs = False
         cfg = dataclasses.replace(cfg, name=f"{cfg.name}[N={args.samples} profiling subset]", N=args.samples)
@@ -404,6 +427,13 @@ def main():
                 r = run_config(c, device, 5 if c.N * c.P > 1000000 else 20, 3, rank, world)
                 s = summarize(c, r, 1, len(r["ms_steps"]), 3, float(np.mean(r["ms_steps"])))
                 per[name] = {k: s[k] for k in ("value", "ms_per_step", "dtype", "step_tflops", "jet_evals_per_s", "roofline", "step_roofline", "gpu_launches", "e2e", "kernel_ms_per_step")}
+            # NEXT-1: the paper's Table II workload on its own generator (21 x 1024 shared trunk with skips)
+            r = run_config(wl.TABLE2, device, 20, 3, rank, world)
+            s2 = summarize(wl.TABLE2, r, 1, len(r["ms_steps"]), 3, float(np.mean(r["ms_steps"])))
+            per["t2"] = {k: s2[k] for k in ("value", "ms_per_step", "dtype", "step_tflops", "jet_evals_per_s", "roofline", "step_roofline", "gpu_launches", "e2e", "kernel_ms_per_step")}
+            per["t2"]["paper_table2"] = {"flop_per_step_paper": 12.3e12, "flop_per_step_8_channel_model": 6 * (2000 * 8 + 200) * 20 * 2 * 1024 * 1024 * 3,
+                                         "flop_per_step_this_build": wl.step_flops(wl.TABLE2)["total"], "paper_step_s_v100": 12.3e12 / 38.6e12,
+                                         "note": "the shared trunk needs 5 jet channel passes where the paper's TF autodiff graph counts 8; 2025 grid points stand in for the 2000 f sensors"}
             line["per_config"] = per
         if not args.no_cpu_baseline:
             val, sec, cores, sample = time_oracle(cfg)

@@ -565,3 +565,80 @@ def trunk_generator_loss_ref(gen_shape, disc_shape, theta_G, theta_D, xy_colloc,
     Js = trunk_jet_forward_ref(theta_G, *gen_shape, xy_sensors, z, 0, skip)
     X_fake = np.concatenate([Js[0][0], Js[1][0]], axis=1)
     return float(-disc_forward_ref(theta_D, *disc_shape, X_fake).mean() + pde_weight * mean_sq)
+
+
+# ==============================================================================================================
+# NEXT-2: the paper's snapshot -- "f values at random positions scattered in the domain (we call them
+# free sensors) ... concatenate these values and the corresponding spatial coordinates as one fake snapshot";
+# "f sensor locations are chosen randomly for each realization".  DESIGN.md reading R9:
+#   X_fake[n] = [ Y(s_1..S; z_n), u(s_1..S; z_n), f(p_{n,1..F}; z_n), x(p_{n,1..F}), y(p_{n,1..F}) ]      (2S + 3F entries)
+#   f(p; z) = exp(Y) (Y_x u_x + Y_y u_y + u_xx + u_yy) at p: Eq. 1 applied to the generator (the induced network);
+#   L_D as before on these snapshots;  L_G = -mean_n D(X_fake[n]) + w_pde mean_{n,p} f(n,p)^2  (the paper's choice is
+#   w_pde = 0: the physics reaches the generator through the critic, whose real snapshots carry the data's f, here 0).
+# The two-MLP generator of BASELINE.json is kept; the coordinates carry no gradient.
+# ==============================================================================================================
+def free_snapshot_ref(gen_shape, theta_Y, theta_u, xy_free, xy_sensors, z):
+    """X_fake [N][2S + 3F] and the per-sample jets (Yj [3][F], Uj [5][F]) at the free sensors."""
+    xy_free = np.asarray(xy_free, dtype=F64); xy_s = np.asarray(xy_sensors, dtype=F64); z = np.asarray(z, dtype=F64)
+    N, Fp, S = z.shape[0], xy_free.shape[1], xy_s.shape[0]
+    X = np.empty((N, 2 * S + 3 * Fp), dtype=F64)
+    jets = []
+    for n in range(N):
+        Ys = gen_jet_forward_ref(theta_Y, *gen_shape, xy_s, z[n:n + 1], 0)[0, 0]
+        Us = gen_jet_forward_ref(theta_u, *gen_shape, xy_s, z[n:n + 1], 0)[0, 0]
+        Yj = gen_jet_forward_ref(theta_Y, *gen_shape, xy_free[n], z[n:n + 1], 1)[:, 0]
+        Uj = gen_jet_forward_ref(theta_u, *gen_shape, xy_free[n], z[n:n + 1], 2)[:, 0]
+        fv = np.exp(Yj[0]) * (Yj[1] * Uj[1] + Yj[2] * Uj[2] + Uj[3] + Uj[4])
+        X[n] = np.concatenate([Ys, Us, fv, xy_free[n][:, 0], xy_free[n][:, 1]])
+        jets.append((Yj, Uj))
+    return X, jets
+
+
+def free_generator_loss_ref(gen_shape, disc_shape, theta_Y, theta_u, theta_D, xy_free, xy_sensors, z, pde_weight=0.0):
+    """L_G of NEXT-2 written as its plain definition (finite-difference pins only)."""
+    X, _ = free_snapshot_ref(gen_shape, theta_Y, theta_u, xy_free, xy_sensors, z)
+    S, Fp = np.asarray(xy_sensors).shape[0], np.asarray(xy_free).shape[1]
+    fv = X[:, 2 * S:2 * S + Fp]
+    return float(-disc_forward_ref(theta_D, *disc_shape, X).mean() + pde_weight * np.mean(fv * fv))
+
+
+def train_step_grads_free_ref(gen_shape, disc_shape, theta_Y, theta_u, theta_D, xy_free, xy_sensors, z, real_snap, eps,
+                              gp_lambda=10.0, pde_weight=0.0):
+    """Oracle of the step with f at per-sample free sensors fed to the critic.  xy_free [N][F][2]; real_snap [N][2S+3F].
+    Returns g_Y, g_u, g_D (flat) and losses = [L_D, mean D(fake), mean D(real), GP, L_G, mean f^2]."""
+    lay_Y = unpack_params(theta_Y, *gen_shape); lay_u = unpack_params(theta_u, *gen_shape)
+    lay_D = unpack_params(theta_D, *disc_shape)
+    xy_free = np.asarray(xy_free, dtype=F64); xy_s = np.asarray(xy_sensors, dtype=F64); z = np.asarray(z, dtype=F64)
+    real = np.asarray(real_snap, dtype=F64); eps = np.asarray(eps, dtype=F64)
+    N, Fp, S = z.shape[0], xy_free.shape[1], xy_s.shape[0]
+    X_fake, _ = free_snapshot_ref(gen_shape, theta_Y, theta_u, xy_free, xy_s, z)
+    gD = _zero_grads(lay_D)
+    g_fake, D_fake = _disc_forward(lay_D, X_fake)
+    g_real, D_real = _disc_forward(lay_D, real)
+    _disc_backward(lay_D, g_fake, np.full(N, 1.0 / N), gD)
+    _disc_backward(lay_D, g_real, np.full(N, -1.0 / N), gD)
+    Xhat = eps[:, None] * real + (1.0 - eps[:, None]) * X_fake
+    gp, _ = _gradient_penalty(lay_D, Xhat, gp_lambda, gD)
+    L_D = float(D_fake.mean() - D_real.mean() + gp)
+    dX = _disc_backward(lay_D, g_fake, np.full(N, -1.0 / N), None)        # dL_G/dX_fake (critic term)
+    gY = _zero_grads(lay_Y); gu = _zero_grads(lay_u)
+    sum_f2 = 0.0
+    for n in range(N):
+        Yj, tY = _jet_forward_one_sample(lay_Y, xy_free[n], z[n], 3, keep_tape=True)
+        Uj, tU = _jet_forward_one_sample(lay_u, xy_free[n], z[n], 5, keep_tape=True)
+        k = np.exp(Yj[0]); D = Yj[1] * Uj[1] + Yj[2] * Uj[2] + Uj[3] + Uj[4]
+        fv = k * D
+        sum_f2 += float((fv * fv).sum())
+        r_hat = dX[n, 2 * S:2 * S + Fp] + 2.0 * pde_weight * fv / (N * Fp)      # dL_G/df(n,p): through the critic (+ the optional penalty)
+        Y_hat = np.stack([r_hat * k * D, r_hat * k * Uj[1], r_hat * k * Uj[2]])   # O3 with this r_hat
+        U_hat = np.stack([np.zeros_like(fv), r_hat * k * Yj[1], r_hat * k * Yj[2], r_hat * k, r_hat * k])
+        _jet_backward_one_sample(lay_Y, xy_free[n], z[n], tY, Y_hat, 3, gY)
+        _jet_backward_one_sample(lay_u, xy_free[n], z[n], tU, U_hat, 5, gu)
+        _, tYs = _jet_forward_one_sample(lay_Y, xy_s, z[n], 1, keep_tape=True)
+        _, tus = _jet_forward_one_sample(lay_u, xy_s, z[n], 1, keep_tape=True)
+        _jet_backward_one_sample(lay_Y, xy_s, z[n], tYs, dX[n:n + 1, :S], 1, gY)
+        _jet_backward_one_sample(lay_u, xy_s, z[n], tus, dX[n:n + 1, S:2 * S], 1, gu)
+    L_f = sum_f2 / (N * Fp)
+    L_G = float(-D_fake.mean() + pde_weight * L_f)
+    losses = np.array([L_D, D_fake.mean(), D_real.mean(), gp, L_G, L_f], dtype=F64)
+    return pack_grads(gY), pack_grads(gu), pack_grads(gD), losses

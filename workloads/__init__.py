@@ -31,6 +31,7 @@ class Config:
     LD: int               # discriminator hidden layers
     HD: int               # discriminator width
     f_kind: str = "zero"  # "zero" | "sin8"
+    variant: str = "two_mlps"   # generator: "two_mlps" (BASELINE.json) | "trunk" | "trunk_skip" (the paper's, NEXT-1)
 
     @property
     def P(self) -> int: return self.G * self.G
@@ -50,6 +51,13 @@ CONFIGS = {
     "c4": Config("c4", 4, "bf16", 1000, 6, 512, 128, 256, 1000, 6, 512),
     "c5": Config("c5", 5, "fp16", 4000, 6, 1024, 256, 64, 5000, 6, 1024),
 }
+
+
+# The workload of the paper's Table II: 21 x 1024 network (20 hidden layers + the output layer),
+# generator worker with local batch 6 on the top-level subdomain of Dataset 6 (100 log k + 100 u sensors, 2000 f sensors).
+# Stand-ins: a 45 x 45 cell-centred grid (2025 points) for the 2000 free f sensors; latent dimension 1000 (the paper does
+# not give the generator's noise dimension); the critic gets the same 21 x 1024 shape.
+TABLE2 = Config("t2", 6, "fp16", 1000, 20, 1024, 45, 6, 100, 20, 1024, "zero", "trunk_skip")
 
 
 def param_count(in_dim: int, n_hidden: int, width: int) -> int:
@@ -156,11 +164,18 @@ def jet_gemm_flops_per_point(L: int, H: int) -> int:
 
 
 def step_flops(cfg: Config) -> dict:
-    """Algorithmic flops of one train step (forward + dgrad + wgrad = 3x forward)."""
-    jets = 3 * cfg.N * cfg.P * jet_flops_per_point(cfg.L, cfg.H)
-    jet_gemm = 3 * cfg.N * cfg.P * jet_gemm_flops_per_point(cfg.L, cfg.H)
-    zpart = cfg.N * 2 * 2 * cfg.m * cfg.H * 3
-    sensors = cfg.N * 3 * cfg.S * 2 * ((cfg.L - 1) * 2 * cfg.H * cfg.H + 6 * cfg.H)
+    """Algorithmic flops of one train step (forward + dgrad + wgrad = 3x forward).  Two MLPs: 5 + 3 channel passes and two
+    value passes at the sensors; shared trunk (NEXT-1): one 5-channel pass and one value pass."""
+    if cfg.variant == "two_mlps":
+        jets = 3 * cfg.N * cfg.P * jet_flops_per_point(cfg.L, cfg.H)
+        jet_gemm = 3 * cfg.N * cfg.P * jet_gemm_flops_per_point(cfg.L, cfg.H)
+        nets = 2
+    else:
+        jets = 3 * cfg.N * cfg.P * ((cfg.L - 1) * 2 * cfg.H * cfg.H * 5 + 2 * cfg.H * 8 + 2 * cfg.H)
+        jet_gemm = 3 * cfg.N * cfg.P * (cfg.L - 1) * 2 * cfg.H * cfg.H * 5
+        nets = 1
+    zpart = cfg.N * nets * 2 * cfg.m * cfg.H * 3
+    sensors = cfg.N * 3 * cfg.S * nets * ((cfg.L - 1) * 2 * cfg.H * cfg.H + 6 * cfg.H)
     critic = cfg.N * 14 * 2 * (2 * cfg.S * cfg.HD + (cfg.LD - 1) * cfg.HD * cfg.HD + cfg.HD)
     return {"jets": jets, "jet_gemm": jet_gemm, "zpart": zpart, "sensors": sensors, "critic": critic,
             "total": jets + zpart + sensors + critic}
