@@ -87,6 +87,10 @@ typedef struct {
   int chunk_rows;            /* 0 = library default (131072); rows per chunk of the generator passes, rounded to 256 */
   unsigned flags;            /* PIGAN_FLAG_* */
   int gen_variant;           /* pigan_gen_variant; 0 = BASELINE.json's two MLPs */
+  int n_free;                /* NEXT-2: 0 = BASELINE.json's step.  F > 0: every latent sample has its own F free-sensor
+                                points (n_colloc must equal F, xy_colloc is [N][F][2], f is ignored and may be NULL); the critic's
+                                snapshot is [log k(S), u(S), f(F), x(F), y(F)], so disc.in_dim = 2 S + 3 F; L_G = -mean D(fake) +
+                                pde_weight * mean f^2 (the paper's choice is pde_weight = 0); losses[5] = mean f^2.  Two-MLP generator only. */
 } pigan_config;
 
 /* Creates a context: validates cfg, allocates the workspace on the CURRENT CUDA device and binds the context to it

@@ -642,3 +642,71 @@ def train_step_grads_free_ref(gen_shape, disc_shape, theta_Y, theta_u, theta_D, 
     L_G = float(-D_fake.mean() + pde_weight * L_f)
     losses = np.array([L_D, D_fake.mean(), D_real.mean(), gp, L_G, L_f], dtype=F64)
     return pack_grads(gY), pack_grads(gu), pack_grads(gD), losses
+
+
+# ==============================================================================================================
+# NEXT-3 (SURVEY.md 8(f)): hierarchical multi-discriminator loss (P:141-143).  "we partition the whole domain into
+# subdomains and assign one discriminator for each subdomain ... each discriminator will only be in charge of all or part of
+# the sensors within the assigned subdomain ... The loss of the generator is the weighted average of negative critics from
+# all the discriminators ... the weight [is] 1 divided by the product of the number of levels and the number of subdomains
+# in this level."  DESIGN.md reading R10:
+#   critic k sees X[:, idx_k] (idx_k: d_sub columns of the 2S-entry snapshot: the log k and u entries of its sensors);
+#   L_Dk = mean D_k(fake_k) - mean D_k(real_k) + lam mean (||grad D_k(xhat_k)|| - 1)^2 with the shared eps_n, gradient to theta_Dk only;
+#   L_G  = sum_k w_k (-mean_n D_k(X_fake[n][idx_k])) + w_pde mean r^2,   w_k = 1 / (levels * subdomains in k's level).
+# ==============================================================================================================
+def hierarchy_weights(subdomains_per_level):
+    """[n_1, n_2, ...] -> w_k for the critics listed level by level: 1 / (number of levels * n_level)."""
+    n_levels = len(subdomains_per_level)
+    return np.concatenate([np.full(n, 1.0 / (n_levels * n)) for n in subdomains_per_level])
+
+
+def train_step_grads_hier_ref(gen_shape, disc_shape, theta_Y, theta_u, theta_D_list, subsets, weights, xy_colloc, f, xy_sensors, z,
+                              real_snap, eps, gp_lambda=10.0, pde_weight=1.0):
+    """Oracle of the step with K critics.  theta_D_list [K][n_disc]; subsets [K][d_sub] (column indices into the 2S-entry
+    snapshot); weights [K].  Returns g_Y, g_u, g_D [K][n_disc] and losses = [sum_k L_Dk, sum_k w_k mean D_k(fake),
+    sum_k w_k mean D_k(real), sum_k GP_k, L_G, L_pde]."""
+    lay_Y = unpack_params(theta_Y, *gen_shape); lay_u = unpack_params(theta_u, *gen_shape)
+    xy_c = np.asarray(xy_colloc, dtype=F64); xy_s = np.asarray(xy_sensors, dtype=F64)
+    f = np.asarray(f, dtype=F64); z = np.asarray(z, dtype=F64)
+    real = np.asarray(real_snap, dtype=F64); eps = np.asarray(eps, dtype=F64)
+    subsets = np.asarray(subsets, dtype=np.int64); weights = np.asarray(weights, dtype=F64)
+    N, P, S, K = z.shape[0], xy_c.shape[0], xy_s.shape[0], len(theta_D_list)
+    X_fake = np.empty((N, 2 * S), dtype=F64)
+    sens_tapes = []
+    for n in range(N):
+        oY, tY = _jet_forward_one_sample(lay_Y, xy_s, z[n], 1, keep_tape=True)
+        ou, tu = _jet_forward_one_sample(lay_u, xy_s, z[n], 1, keep_tape=True)
+        X_fake[n, :S] = oY[0]; X_fake[n, S:] = ou[0]
+        sens_tapes.append((tY, tu))
+    dX = np.zeros((N, 2 * S), dtype=F64)                    # dL_G/dX_fake, summed over the critics
+    gD_all, sum_LD, wDf, wDr, sum_gp = [], 0.0, 0.0, 0.0, 0.0
+    for k in range(K):
+        lay_D = unpack_params(theta_D_list[k], *disc_shape)
+        idx = subsets[k]
+        Xf, Xr = X_fake[:, idx], real[:, idx]
+        gD = _zero_grads(lay_D)
+        g_fake, D_fake = _disc_forward(lay_D, Xf)
+        g_real, D_real = _disc_forward(lay_D, Xr)
+        _disc_backward(lay_D, g_fake, np.full(N, 1.0 / N), gD)
+        _disc_backward(lay_D, g_real, np.full(N, -1.0 / N), gD)
+        gp, _ = _gradient_penalty(lay_D, eps[:, None] * Xr + (1.0 - eps[:, None]) * Xf, gp_lambda, gD)
+        gD_all.append(pack_grads(gD))
+        sum_LD += float(D_fake.mean() - D_real.mean() + gp); sum_gp += gp
+        wDf += weights[k] * float(D_fake.mean()); wDr += weights[k] * float(D_real.mean())
+        dXk = _disc_backward(lay_D, g_fake, np.full(N, -weights[k] / N), None)     # d(-w_k mean D_k)/dX_fake[:, idx]
+        np.add.at(dX, (slice(None), idx), dXk)
+    gY = _zero_grads(lay_Y); gu = _zero_grads(lay_u)
+    sum_r2 = 0.0
+    for n in range(N):
+        Yj, tY = _jet_forward_one_sample(lay_Y, xy_c, z[n], 3, keep_tape=True)
+        Uj, tU = _jet_forward_one_sample(lay_u, xy_c, z[n], 5, keep_tape=True)
+        r, Y_hat, U_hat = _residual_adjoints(Yj, Uj, f, pde_weight, N * P)
+        sum_r2 += float((r * r).sum())
+        _jet_backward_one_sample(lay_Y, xy_c, z[n], tY, Y_hat, 3, gY)
+        _jet_backward_one_sample(lay_u, xy_c, z[n], tU, U_hat, 5, gu)
+        tYs, tus = sens_tapes[n]
+        _jet_backward_one_sample(lay_Y, xy_s, z[n], tYs, dX[n:n + 1, :S], 1, gY)
+        _jet_backward_one_sample(lay_u, xy_s, z[n], tus, dX[n:n + 1, S:], 1, gu)
+    L_pde = sum_r2 / (N * P)
+    losses = np.array([sum_LD, wDf, wDr, sum_gp, -wDf + pde_weight * L_pde, L_pde], dtype=F64)
+    return pack_grads(gY), pack_grads(gu), np.stack(gD_all), losses

@@ -38,7 +38,7 @@ class _MlpShape(Structure):
 class _Config(Structure):
     _fields_ = [("gen", _MlpShape), ("disc", _MlpShape), ("latent_dim", c_int), ("n_samples", c_int), ("n_colloc", c_int),
                 ("n_sensors", c_int), ("precision", c_int), ("gp_lambda", c_float), ("pde_weight", c_float),
-                ("workspace_bytes", c_size_t), ("chunk_rows", c_int), ("flags", ctypes.c_uint), ("gen_variant", c_int)]
+                ("workspace_bytes", c_size_t), ("chunk_rows", c_int), ("flags", ctypes.c_uint), ("gen_variant", c_int), ("n_free", c_int)]
 
 
 _lib = None
@@ -113,7 +113,7 @@ class PiGan:
     """One context = one CUDA stream + the workspaces of one PI-GAN configuration (mirrors pigan_ctx)."""
 
     def __init__(self, *, latent_dim, gen_hidden, gen_width, disc_hidden, disc_width, n_samples, n_colloc, n_sensors,
-                 precision="fp32", gp_lambda=10.0, pde_weight=1.0, workspace_bytes=0, chunk_rows=0, flags=0, gen_variant="two_mlps", stream=None, device=None):
+                 precision="fp32", gp_lambda=10.0, pde_weight=1.0, workspace_bytes=0, chunk_rows=0, flags=0, gen_variant="two_mlps", n_free=0, stream=None, device=None):
         import torch
         self._lib = load_library()
         self._ctx = c_void_p()
@@ -122,10 +122,11 @@ class PiGan:
         self.device = torch.device(device if device is not None else f"cuda:{torch.cuda.current_device()}")
         self.m, self.N, self.P, self.S = latent_dim, n_samples, n_colloc, n_sensors
         self.gen_shape = (2 + latent_dim, gen_hidden, gen_width)
-        self.disc_shape = (2 * n_sensors, disc_hidden, disc_width)
+        self.disc_shape = (2 * n_sensors + 3 * n_free, disc_hidden, disc_width)
+        self.n_free = n_free
         self.precision = precision
         cfg = _Config(_MlpShape(*self.gen_shape), _MlpShape(*self.disc_shape), latent_dim, n_samples, n_colloc, n_sensors,
-                      PRECISIONS[precision], gp_lambda, pde_weight, workspace_bytes, chunk_rows, flags, GEN_VARIANTS[gen_variant])
+                      PRECISIONS[precision], gp_lambda, pde_weight, workspace_bytes, chunk_rows, flags, GEN_VARIANTS[gen_variant], n_free)
         self.gen_variant = gen_variant
         self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
         with torch.cuda.device(self.device):
@@ -222,7 +223,8 @@ class PiGan:
             out = (self._new(self.n_gen), self._new(self.n_gen) if self.gen_variant == "two_mlps" else None, self._new(self.n_disc), self._new(6),
                    self._new(1, dtype=torch.int32))
         g_logk, g_u, g_disc, losses, found_inf = out
-        if (xy_colloc.shape[0], xy_sensors.shape[0], tuple(z.shape), tuple(real_snap.shape)) != (self.P, self.S, (self.N, self.m), (self.N, 2 * self.S)):
+        n_xy = self.N * self.P if self.n_free else self.P                    # free-sensor mode: xy_colloc is [N][F][2]
+        if (xy_colloc.numel() // 2, xy_sensors.shape[0], tuple(z.shape), tuple(real_snap.shape)) != (n_xy, self.S, (self.N, self.m), (self.N, self.disc_shape[0])):
             raise ValueError("input sizes disagree with the configuration of this context")
         self._check(self._lib.pigan_train_step_grads(
             self._ctx, _ptr(logk_params, "logk_params"), _ptr(u_params, "u_params"), _ptr(disc_params, "disc_params"),

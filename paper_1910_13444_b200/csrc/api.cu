@@ -15,74 +15,6 @@ using namespace pigan;
 namespace {
 
 
-// ---- one chunk of generator rows, forward ------------------------------------------------------------------------
-template <typename T>
-void gen_forward_chunk(pigan_ctx* c, int n, const pigan_ctx::HBuf& hb, const float* theta, int C, const float* xy, const ChunkGeom& g, float* o,
-                       long long o_stride, bool split = false, bool keep_last = true) {
-  const NetShape& s = c->gen;
-  Launcher& L = c->L;
-  const int H = s.H;
-  const long long pl = (long long)H * g.R_ld;
-  // split (16-bit modes, value channel only): activations are carried as two 16-bit planes hi + lo, so that the
-  // snapshot X_fake the critic sees is accurate to ~2^-17 (the loss values are compared at 1e-3 relative)
-  split = split && C == 1 && c->cfg.precision != PIGAN_FP32;
-  first_layer_fwd<T>(L, C, s, theta, c->net[n].Zp, xy, g, (T*)hb.at(1), split);
-  // the output layer (a4) rides in the epilogue of the last hidden layer where the kernels support it
-  const bool fuse_out = c->cfg.precision != PIGAN_FP32 && s.L >= 2 && tc_out_dot_fusable(L, H);
-  for (int l = 2; l <= s.L; ++l) {
-    if (c->cfg.precision == PIGAN_FP32) {
-      // a_c = W_l h_c^{l-1}: M = H, N = rows, K = H, batched over the C channel planes
-      sgemm(L, false, false, H, g.R, H, theta + s.W_off(l), H, 0, (const float*)hb.at(l - 1), g.R_ld, pl, c->net[n].apre, g.R_ld, pl, C, false);
-      jet_act_fwd_f32(L, C, H, theta + s.b_off(l), g, c->net[n].apre, (float*)hb.at(l));
-      continue;
-    }
-    OutDot od{theta + s.W_off(s.L + 1), theta + s.b_off(s.L + 1), o, o_stride, g.valid};
-    const OutDot* odp = (fuse_out && l == s.L) ? &od : nullptr;
-    void* h_out = (odp && !keep_last) ? nullptr : hb.at(l);
-    if (odp) cudaMemset2DAsync(o, (size_t)o_stride * 4, 0, (size_t)g.valid * 4, C, L.stream);
-    if (split) tc_layer_fwd_split(L, c->cfg.precision, H, g.R, g.R_ld, c->w16(n, l, 0), theta + s.b_off(l), hb.at(l - 1), h_out, odp);
-    else tc_layer_fwd(L, c->cfg.precision, C, H, g.R, g.R_ld, c->w16(n, l, 0), theta + s.b_off(l), hb.at(l - 1), h_out, odp);
-  }
-  if (!fuse_out) out_fwd<T>(L, C, H, theta + s.W_off(s.L + 1), theta + s.b_off(s.L + 1), g, (const T*)hb.at(s.L), o, o_stride, split);
-}
-
-// ---- one chunk of generator rows, reverse sweep; output adjoints are in net[n].oh [C][R_ld] ------------------------
-template <typename T>
-void gen_backward_chunk(pigan_ctx* c, int n, const pigan_ctx::HBuf& hb, const float* theta, float* grads, int C, const float* xy, const ChunkGeom& g) {
-  const NetShape& s = c->gen;
-  Launcher& L = c->L;
-  const int H = s.H;
-  const long long pl = (long long)H * g.R_ld;
-  int cur = 0;
-  const float* amax = c->cfg.precision == PIGAN_FP32 ? nullptr : c->amax + n;
-  jet_act_bwd_launch<T>(L, C, H, g, nullptr, theta + s.W_off(s.L + 1), c->net[n].oh, (const T*)hb.at(s.L),
-                        (T*)c->net[n].ah[cur], grads + s.b_off(s.L),
-                        grads + s.W_off(s.L + 1), grads + s.b_off(s.L + 1), amax);
-  for (int l = s.L; l >= 2; --l) {
-    if (c->cfg.precision == PIGAN_FP32) {
-      // W_hat_l += sum_c ahat_c h_c^{l-1 T}: M = H, N = H, K = rows
-      sgemm(L, false, true, H, H, g.R, (const float*)c->net[n].ah[cur], g.R_ld, pl, (const float*)hb.at(l - 1), g.R_ld, pl, grads + s.W_off(l), H, 0, C, true);
-      // hhat_c^{l-1} = W_l^T ahat_c: M = H (in), N = rows, K = H (out); A stored [K][M]
-      sgemm(L, true, false, H, g.R, H, theta + s.W_off(l), H, 0, (const float*)c->net[n].ah[cur], g.R_ld, pl, c->net[n].apre, g.R_ld, pl, C, false);
-      jet_act_bwd_launch<T>(L, C, H, g, c->net[n].apre, nullptr, nullptr, (const T*)hb.at(l - 1),
-                            (T*)c->net[n].ah[cur ^ 1], grads + s.b_off(l - 1), nullptr, nullptr, amax);
-    } else {
-      tc_wgrad(L, c->cfg.precision, C, H, g.R, g.R_ld, c->net[n].ah[cur], hb.at(l - 1), grads + s.W_off(l), amax);
-      if (l == 2 && tc_first_layer_fusable(H, g)) {
-        // the adjoint of the first tanh layer is reduced inside the dgrad epilogue (ahat^1 is never written)
-        FirstLayerFuse fl{xy, g.row0, g.npts, s.in_dim, grads, c->net[n].An};
-        tc_layer_bwd(L, c->cfg.precision, C, H, g.R, g.R_ld, c->w16(n, l, 1), c->net[n].ah[cur], hb.at(l - 1),
-                     c->net[n].ah[cur ^ 1], grads + s.b_off(l - 1), amax, &fl);
-        return;
-      }
-      tc_layer_bwd(L, c->cfg.precision, C, H, g.R, g.R_ld, c->w16(n, l, 1), c->net[n].ah[cur], hb.at(l - 1),
-                   c->net[n].ah[cur ^ 1], grads + s.b_off(l - 1), amax);
-    }
-    cur ^= 1;
-  }
-  first_layer_bwd<T>(L, C, s, xy, g, (const T*)c->net[n].ah[cur], grads, c->net[n].An, amax);
-}
-
 template <typename T>
 pigan_status jet_forward_impl(pigan_ctx* c, const float* theta, const float* xy, int n_pts, const float* z, int n_samples, int C, float* out) {
   const long long total = (long long)n_samples * n_pts;
@@ -237,7 +169,10 @@ pigan_status pigan_create(const pigan_config* cfg, void* cuda_stream, pigan_ctx*
     return PIGAN_ERR_INVALID_ARG;
   if ((int)cfg->precision < 0 || (int)cfg->precision > 2 || !(cfg->gp_lambda >= 0.f) || cfg->chunk_rows < 0) return PIGAN_ERR_INVALID_ARG;
   if (cfg->gen_variant < 0 || cfg->gen_variant > 2) return PIGAN_ERR_INVALID_ARG;
-  if (cfg->gen.in_dim != 2 + cfg->latent_dim || cfg->disc.in_dim != 2 * cfg->n_sensors) return PIGAN_ERR_SHAPE;
+  if (cfg->n_free < 0) return PIGAN_ERR_INVALID_ARG;
+  if (cfg->gen.in_dim != 2 + cfg->latent_dim || cfg->disc.in_dim != 2 * cfg->n_sensors + 3 * cfg->n_free) return PIGAN_ERR_SHAPE;
+  if (cfg->n_free > 0 && cfg->n_colloc != cfg->n_free) return PIGAN_ERR_SHAPE;
+  if (cfg->n_free > 0 && cfg->gen_variant != PIGAN_GEN_TWO_MLPS) return PIGAN_ERR_UNSUPPORTED;
   if (cfg->precision != PIGAN_FP32) {
     std::string why;
     if (!tc_supported(cfg->gen.width, &why)) return PIGAN_ERR_UNSUPPORTED;
@@ -258,7 +193,7 @@ pigan_status pigan_create(const pigan_config* cfg, void* cuda_stream, pigan_ctx*
   c->L.one_cta = (cfg->flags & PIGAN_FLAG_ONE_CTA) != 0;
   c->sg.disabled = (cfg->flags & PIGAN_FLAG_NO_GRAPH) != 0;
   c->elem = cfg->precision == PIGAN_FP32 ? 4 : 2;
-  const int H = c->gen.H, Lh = c->gen.L, N = cfg->n_samples, S = cfg->n_sensors, d = 2 * S, HD = c->disc.H, LD = c->disc.L;
+  const int H = c->gen.H, Lh = c->gen.L, N = cfg->n_samples, S = cfg->n_sensors, d = c->disc.in_dim, HD = c->disc.H, LD = c->disc.L;
   const bool f32 = cfg->precision == PIGAN_FP32;
   // bytes per chunk row over both nets: h (L*C) + adjoint ping-pong (2C) planes [+ fp32 scratch]
   size_t per_row = 0;
@@ -321,6 +256,7 @@ pigan_status pigan_create(const pigan_config* cfg, void* cuda_stream, pigan_ctx*
     c->dX = c->alloc<float>((size_t)2 * N * d);
     c->seed = c->alloc<float>((size_t)2 * N);
     c->amax = c->alloc<float>(2);
+    if (cfg->n_free > 0) c->fbuf = c->alloc<float>((size_t)c->R_ld);
   } catch (const std::bad_alloc&) {
     pigan_destroy(c);
     return PIGAN_ERR_ALLOC;
@@ -428,11 +364,13 @@ pigan_status pigan_train_step_grads(pigan_ctx* c, const float* logk_params, cons
                                     const float* eps, float loss_scale, float* g_logk, float* g_u, float* g_disc, float* losses, int* found_inf) {
   if (!c) return PIGAN_ERR_INVALID_ARG;
   DeviceGuard dg(c);
-  if (!logk_params || !disc_params || !xy_colloc || !f || !xy_sensors || !z || !real_snap || !eps || !g_logk || !g_disc ||
+  if (!logk_params || !disc_params || !xy_colloc || (!f && c->cfg.n_free == 0) || !xy_sensors || !z || !real_snap || !eps || !g_logk || !g_disc ||
       (!c->trunk && (!u_params || !g_u)))
     return fail(c, PIGAN_ERR_INVALID_ARG, "null pointer");
   if (!(loss_scale > 0.f) || !std::isfinite(loss_scale)) return fail(c, PIGAN_ERR_INVALID_ARG, "loss_scale must be positive and finite");
   auto run = [&]() -> pigan_status {
+    if (c->cfg.n_free > 0)
+      return free_train_step(c, logk_params, u_params, disc_params, xy_colloc, xy_sensors, z, real_snap, eps, loss_scale, g_logk, g_u, g_disc, losses, found_inf);
     if (c->trunk)
       return trunk_train_step(c, logk_params, disc_params, xy_colloc, f, xy_sensors, z, real_snap, eps, loss_scale, g_logk, g_disc, losses, found_inf);
     switch (c->cfg.precision) {

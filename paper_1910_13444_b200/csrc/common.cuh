@@ -138,6 +138,7 @@ struct ChunkGeom {          // one chunk of generator rows r = row0 .. row0+vali
   int R;                    // rows computed (valid rounded up to the row tile)
   int R_ld;                 // leading dimension (rows) of every plane
   int npts;                 // points per latent sample
+  int per_sample = 0;       // NEXT-2: every sample has its own points, xy is [n][npts][2] (row r reads xy[r]); else xy is [npts][2] shared
 };
 
 template <typename T>
@@ -147,9 +148,12 @@ void jet_act_fwd_f32(Launcher& L, int C, int H, const float* bias, const ChunkGe
 template <typename T>
 void out_fwd(Launcher& L, int C, int H, const float* w_out, const float* b_out, const ChunkGeom& g, const T* hL,
              float* o, long long o_plane_stride, bool split = false);          // split: C = 1, sums planes (hi, lo)
+// f may be null (target 0); ext_seed (may be null) [R]: an additional adjoint of r per row, already loss-scaled (NEXT-2: -dD/df / N)
 void residual(Launcher& L, const float* Y, long long y_stride, const float* U, long long u_stride, const float* f,
               long long row0, int valid, int R, int npts, float* r_out, double* sum_sq, float seed_scale, float* seedY,
-              float* seedU, int seed_ld, float* amaxY = nullptr, float* amaxU = nullptr);
+              float* seedU, int seed_ld, float* amaxY = nullptr, float* amaxU = nullptr, const float* ext_seed = nullptr);
+// NEXT-2: X[n][col0 + p] = fvals[(n, p)], X[n][col0 + F + p] = x, X[n][col0 + 2F + p] = y for the chunk's rows
+void scatter_free(Launcher& L, const float* fvals, const float* xy_free, long long row0, int valid, int F, int d, int col0, float* X);
 // adjoint of one tanh layer: hh_c = (hhat planes) or (w_out[j] * ohat_c[r]) ; writes ahat planes, accumulates
 // b_hat_l[j] += sum_r ahat_0 (and for the output layer w_hat_out[j], b_hat_out).
 template <typename T>
@@ -235,7 +239,7 @@ void tc_wgrad(Launcher& L, int precision, int C, int H, int R, int R_ld, const v
 // first-layer backward fused into the dgrad of layer 2 (CTA-pair kernels only): the adjoint planes ahat^1 are reduced
 // in the epilogue into W_hat_1[:, 0:2], An and b_hat_1 and never written.  Valid when npts % 64 == 0 and R == valid.
 struct FirstLayerFuse {
-  const float* xy; long long row0; int npts; int in_dim; float* gW1; float* An;
+  const float* xy; long long row0; int npts; int in_dim; float* gW1; float* An; int per_sample = 0;
 };
 bool tc_first_layer_fusable(int H, const ChunkGeom& g);
 

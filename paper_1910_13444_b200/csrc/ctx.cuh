@@ -63,6 +63,7 @@ struct pigan_ctx {
     return reinterpret_cast<T*>(p);
   }
   int n_sens_chunks = 1;
+  float* fbuf = nullptr;       // NEXT-2: [R_ld] f values of a chunk / the critic's adjoint of them
   bool trunk = false, skip = false;   // NEXT-1: shared-trunk generator (workspace of net[1]), with skip connections
   size_t plane() const { return (size_t)gen.H * R_ld * elem; }
   // activation stash of one chunk: `planes` planes per layer; l = 1..L
@@ -119,9 +120,80 @@ inline void compute_zpart(pigan_ctx* c, int n, const float* theta, const float* 
   sgemm(c->L, false, true, n_samples, s.H, s.in_dim - 2, z, s.in_dim - 2, 0, theta + 2, s.in_dim, 0, c->net[n].Zp, s.H, 0, 1, false);
 }
 
+// ---- one chunk of generator rows, forward ------------------------------------------------------------------------
+template <typename T>
+void gen_forward_chunk(pigan_ctx* c, int n, const pigan_ctx::HBuf& hb, const float* theta, int C, const float* xy, const ChunkGeom& g, float* o,
+                       long long o_stride, bool split = false, bool keep_last = true) {
+  const NetShape& s = c->gen;
+  Launcher& L = c->L;
+  const int H = s.H;
+  const long long pl = (long long)H * g.R_ld;
+  // split (16-bit modes, value channel only): activations are carried as two 16-bit planes hi + lo, so that the
+  // snapshot X_fake the critic sees is accurate to ~2^-17 (the loss values are compared at 1e-3 relative)
+  split = split && C == 1 && c->cfg.precision != PIGAN_FP32;
+  first_layer_fwd<T>(L, C, s, theta, c->net[n].Zp, xy, g, (T*)hb.at(1), split);
+  // the output layer (a4) rides in the epilogue of the last hidden layer where the kernels support it
+  const bool fuse_out = c->cfg.precision != PIGAN_FP32 && s.L >= 2 && tc_out_dot_fusable(L, H);
+  for (int l = 2; l <= s.L; ++l) {
+    if (c->cfg.precision == PIGAN_FP32) {
+      // a_c = W_l h_c^{l-1}: M = H, N = rows, K = H, batched over the C channel planes
+      sgemm(L, false, false, H, g.R, H, theta + s.W_off(l), H, 0, (const float*)hb.at(l - 1), g.R_ld, pl, c->net[n].apre, g.R_ld, pl, C, false);
+      jet_act_fwd_f32(L, C, H, theta + s.b_off(l), g, c->net[n].apre, (float*)hb.at(l));
+      continue;
+    }
+    OutDot od{theta + s.W_off(s.L + 1), theta + s.b_off(s.L + 1), o, o_stride, g.valid};
+    const OutDot* odp = (fuse_out && l == s.L) ? &od : nullptr;
+    void* h_out = (odp && !keep_last) ? nullptr : hb.at(l);
+    if (odp) cudaMemset2DAsync(o, (size_t)o_stride * 4, 0, (size_t)g.valid * 4, C, L.stream);
+    if (split) tc_layer_fwd_split(L, c->cfg.precision, H, g.R, g.R_ld, c->w16(n, l, 0), theta + s.b_off(l), hb.at(l - 1), h_out, odp);
+    else tc_layer_fwd(L, c->cfg.precision, C, H, g.R, g.R_ld, c->w16(n, l, 0), theta + s.b_off(l), hb.at(l - 1), h_out, odp);
+  }
+  if (!fuse_out) out_fwd<T>(L, C, H, theta + s.W_off(s.L + 1), theta + s.b_off(s.L + 1), g, (const T*)hb.at(s.L), o, o_stride, split);
+}
+
+// ---- one chunk of generator rows, reverse sweep; output adjoints are in net[n].oh [C][R_ld] ------------------------
+template <typename T>
+void gen_backward_chunk(pigan_ctx* c, int n, const pigan_ctx::HBuf& hb, const float* theta, float* grads, int C, const float* xy, const ChunkGeom& g) {
+  const NetShape& s = c->gen;
+  Launcher& L = c->L;
+  const int H = s.H;
+  const long long pl = (long long)H * g.R_ld;
+  int cur = 0;
+  const float* amax = c->cfg.precision == PIGAN_FP32 ? nullptr : c->amax + n;
+  jet_act_bwd_launch<T>(L, C, H, g, nullptr, theta + s.W_off(s.L + 1), c->net[n].oh, (const T*)hb.at(s.L),
+                        (T*)c->net[n].ah[cur], grads + s.b_off(s.L),
+                        grads + s.W_off(s.L + 1), grads + s.b_off(s.L + 1), amax);
+  for (int l = s.L; l >= 2; --l) {
+    if (c->cfg.precision == PIGAN_FP32) {
+      // W_hat_l += sum_c ahat_c h_c^{l-1 T}: M = H, N = H, K = rows
+      sgemm(L, false, true, H, H, g.R, (const float*)c->net[n].ah[cur], g.R_ld, pl, (const float*)hb.at(l - 1), g.R_ld, pl, grads + s.W_off(l), H, 0, C, true);
+      // hhat_c^{l-1} = W_l^T ahat_c: M = H (in), N = rows, K = H (out); A stored [K][M]
+      sgemm(L, true, false, H, g.R, H, theta + s.W_off(l), H, 0, (const float*)c->net[n].ah[cur], g.R_ld, pl, c->net[n].apre, g.R_ld, pl, C, false);
+      jet_act_bwd_launch<T>(L, C, H, g, c->net[n].apre, nullptr, nullptr, (const T*)hb.at(l - 1),
+                            (T*)c->net[n].ah[cur ^ 1], grads + s.b_off(l - 1), nullptr, nullptr, amax);
+    } else {
+      tc_wgrad(L, c->cfg.precision, C, H, g.R, g.R_ld, c->net[n].ah[cur], hb.at(l - 1), grads + s.W_off(l), amax);
+      if (l == 2 && tc_first_layer_fusable(H, g)) {
+        // the adjoint of the first tanh layer is reduced inside the dgrad epilogue (ahat^1 is never written)
+        FirstLayerFuse fl{xy, g.row0, g.npts, s.in_dim, grads, c->net[n].An, g.per_sample};
+        tc_layer_bwd(L, c->cfg.precision, C, H, g.R, g.R_ld, c->w16(n, l, 1), c->net[n].ah[cur], hb.at(l - 1),
+                     c->net[n].ah[cur ^ 1], grads + s.b_off(l - 1), amax, &fl);
+        return;
+      }
+      tc_layer_bwd(L, c->cfg.precision, C, H, g.R, g.R_ld, c->w16(n, l, 1), c->net[n].ah[cur], hb.at(l - 1),
+                   c->net[n].ah[cur ^ 1], grads + s.b_off(l - 1), amax);
+    }
+    cur ^= 1;
+  }
+  first_layer_bwd<T>(L, C, s, xy, g, (const T*)c->net[n].ah[cur], grads, c->net[n].An, amax);
+}
+
 // NEXT-1 (trunk.cu)
 pigan_status trunk_train_step(pigan_ctx* c, const float* thG, const float* thD, const float* xy_c, const float* f, const float* xy_s, const float* z,
                               const float* real, const float* eps, float loss_scale, float* gG, float* gD, float* losses, int* found_inf);
 pigan_status trunk_jet_forward(pigan_ctx* c, const float* theta, const float* xy, int n_pts, const float* z, int n_samples, int C, float* out);
+// NEXT-2 (free.cu): f at per-sample free sensors fed to the critic
+pigan_status free_train_step(pigan_ctx* c, const float* thY, const float* thU, const float* thD, const float* xy_free, const float* xy_s, const float* z,
+                             const float* real, const float* eps, float loss_scale, float* gY, float* gU, float* gD, float* losses, int* found_inf);
 
 }  // namespace pigan

@@ -72,7 +72,7 @@ __global__ void __launch_bounds__(256) first_layer_fwd_kernel(NetShape s, const 
 #pragma unroll
     for (int i = 0; i < 8; ++i) {
       n[i] = nn;
-      const float2 q = *reinterpret_cast<const float2*>(xy + 2 * p);
+      const float2 q = *reinterpret_cast<const float2*>(xy + 2 * (g.per_sample ? (long long)nn * g.npts + p : (long long)p));
       x[i] = q.x; y[i] = q.y;
       if (r0 + i + 1 < g.valid) { if (++p == g.npts) { p = 0; ++nn; } }
     }
@@ -357,7 +357,7 @@ __global__ void __launch_bounds__(256) first_layer_bwd_kernel(NetShape s, const 
 #pragma unroll
     for (int i = 0; i < 8; ++i) {
       if (r0 + i < g.valid) {
-        const float2 q = *reinterpret_cast<const float2*>(xy + 2 * p);
+        const float2 q = *reinterpret_cast<const float2*>(xy + 2 * (g.per_sample ? (long long)n * g.npts + p : (long long)p));
         sx = fmaf(a0[i], q.x, sx); sy = fmaf(a0[i], q.y, sy);
         if (C >= 3) { sx += ax[i]; sy += ay[i]; }
         if (uniform) sa += a0[i];

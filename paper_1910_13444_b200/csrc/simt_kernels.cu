@@ -168,7 +168,7 @@ __global__ void __launch_bounds__(256) residual_kernel(const float* __restrict__
                                                        const float* __restrict__ f, long long row0, int valid, int R, int npts,
                                                        float* __restrict__ r_out, double* __restrict__ sum_sq, float seed_scale,
                                                        float* __restrict__ seedY, float* __restrict__ seedU, int seed_ld,
-                                                       float* __restrict__ amaxY, float* __restrict__ amaxU) {
+                                                       float* __restrict__ amaxY, float* __restrict__ amaxU, const float* __restrict__ ext_seed) {
   __shared__ double red[8];
   float my = 0.f, mu = 0.f;
   const int r = blockIdx.x * 256 + threadIdx.x;
@@ -181,10 +181,10 @@ __global__ void __launch_bounds__(256) residual_kernel(const float* __restrict__
       const float ux = U[us + r], uy = U[2 * us + r], uxx = U[3 * us + r], uyy = U[4 * us + r];
       const float k = expf(y0);
       const float D = fmaf(yx, ux, fmaf(yy, uy, uxx + uyy));
-      const float res = fmaf(k, D, -f[p]);
+      const float res = fmaf(k, D, f ? -f[p] : 0.f);
       if (r_out) r_out[r] = res;
       sq = (double)res * (double)res;
-      const float rk = seed_scale * res * k;                  // r_hat * k  (loss-scaled in 16-bit modes)
+      const float rk = (seed_scale * res + (ext_seed ? ext_seed[r] : 0.f)) * k;   // r_hat * k  (loss-scaled in 16-bit modes)
       sy[0] = rk * D; sy[1] = rk * ux; sy[2] = rk * uy;
       su[1] = rk * yx; su[2] = rk * yy; su[3] = rk; su[4] = rk;
       my = fmaxf(fabsf(sy[0]), fmaxf(fabsf(sy[1]), fabsf(sy[2])));
@@ -221,10 +221,10 @@ __global__ void __launch_bounds__(256) residual_kernel(const float* __restrict__
 
 void residual(Launcher& L, const float* Y, long long y_stride, const float* U, long long u_stride, const float* f, long long row0,
               int valid, int R, int npts, float* r_out, double* sum_sq, float seed_scale, float* seedY, float* seedU, int seed_ld,
-              float* amaxY, float* amaxU) {
+              float* amaxY, float* amaxU, const float* ext_seed) {
   if (R <= 0) return;
   residual_kernel<<<cdiv(R, 256), 256, 0, L.stream>>>(Y, y_stride, U, u_stride, f, row0, valid, R, npts, r_out, sum_sq, seed_scale,
-                                                      seedY, seedU, seed_ld, amaxY, amaxU);
+                                                      seedY, seedU, seed_ld, amaxY, amaxU, ext_seed);
   L.check("residual");
 }
 
@@ -540,6 +540,19 @@ __global__ void scatter_snapshot_kernel(const float* __restrict__ o, long long r
 void scatter_snapshot(Launcher& L, const float* o, long long row0, int valid, int S, int d, int col0, float* X) {
   if (valid <= 0) return;
   scatter_snapshot_kernel<<<cdiv(valid, 256), 256, 0, L.stream>>>(o, row0, valid, S, d, col0, X);
+  L.check("scatter_snapshot");
+}
+__global__ void scatter_free_kernel(const float* __restrict__ fvals, const float* __restrict__ xy, long long row0, int valid, int F, int d, int col0,
+                                    float* __restrict__ X) {
+  const int r = blockIdx.x * blockDim.x + threadIdx.x;
+  if (r >= valid) return;
+  const long long rg = row0 + r;
+  float* row = X + (rg / F) * d + col0 + (rg % F);
+  row[0] = fvals[r]; row[F] = xy[2 * rg]; row[2 * F] = xy[2 * rg + 1];
+}
+void scatter_free(Launcher& L, const float* fvals, const float* xy_free, long long row0, int valid, int F, int d, int col0, float* X) {
+  if (valid <= 0) return;
+  scatter_free_kernel<<<cdiv(valid, 256), 256, 0, L.stream>>>(fvals, xy_free, row0, valid, F, d, col0, X);
   L.check("scatter_snapshot");
 }
 __global__ void gather_seed_kernel(const float* __restrict__ dX, long long row0, int valid, int R, int S, int d, int col0, float alpha,

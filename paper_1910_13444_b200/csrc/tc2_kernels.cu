@@ -48,7 +48,7 @@ struct Jet2Params {
   // consumed in registers and never written.  Requires npts % 64 == 0 (a row tile lies inside one latent sample).
   const float* xy;       // [npts][2]
   long long row0;        // first global row of the chunk
-  int npts, in_dim;
+  int npts, in_dim, per_sample;
   float* gW1;            // W_hat_1 [H][in_dim]: columns 0, 1 += sum_r (ahat x_r + ahat_x), (ahat y_r + ahat_y)
   float* An;             // [N][H] += sum_{r in sample n} ahat
   // MODE 4, 5 (last hidden layer + output layer a4): o_c[r] += sum_units w_out[unit] h_c[unit][r], reduced over the lanes of a
@@ -415,7 +415,7 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
         mbar_wait(sbar + e, sphase); sphase ^= 1;
         float sx = 0.f, sy = 0.f;                            // MODE 3
         const long long grow = p.row0 + row0;                // MODE 3: global row of this warp's first row
-        const float2* xyp = MODE == 3 ? reinterpret_cast<const float2*>(p.xy) + (int)(grow % p.npts) : nullptr;
+        const float2* xyp = MODE == 3 ? reinterpret_cast<const float2*>(p.xy) + (p.per_sample ? grow : grow % p.npts) : nullptr;
 #pragma unroll
         for (int rc = 0; rc < 4; ++rc) {
           float hh[C][8], hp[C][8], o[C][8];
@@ -662,7 +662,7 @@ void tc2_layer_bwd(Launcher& L, int precision, int C, int H, int R, int R_ld, co
   Jet2Params p{};
   p.H = H; p.n_row_tiles = R / 64; p.g_bias = g_bias_prev; p.amax = amax; p.out = ahat_out; p.R_ld = R_ld;
   if (fl) {
-    p.xy = fl->xy; p.row0 = fl->row0; p.npts = fl->npts; p.in_dim = fl->in_dim; p.gW1 = fl->gW1; p.An = fl->An;
+    p.xy = fl->xy; p.row0 = fl->row0; p.npts = fl->npts; p.in_dim = fl->in_dim; p.gW1 = fl->gW1; p.An = fl->An; p.per_sample = fl->per_sample;
     dispatch_jet2<3>(L, C, a, b, t, p);
     return;
   }

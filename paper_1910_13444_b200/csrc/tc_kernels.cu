@@ -39,7 +39,7 @@ struct JetParams {
   float* g_bias;         // MODE 1: b_hat_{l-1}
   const float* amax;     // MODE 1, 3: block-scale source of the adjoint planes (common.cuh adj_inv_scale)
   // MODE 3 (MODE 1 + first-layer reduction, O4 'First layer'; see tc2_kernels.cu): ahat^1 is consumed in registers
-  const float* xy; long long row0; int npts, in_dim; float* gW1; float* An;
+  const float* xy; long long row0; int npts, in_dim, per_sample; float* gW1; float* An;
   int linear;            // MODE 0 only: plain GEMM, out_c = W in_c (no bias, no tanh) -- see tc2_kernels.cu
 };
 
@@ -234,7 +234,7 @@ __global__ void __launch_bounds__(256, 1) jet_layer_kernel(const __grid_constant
           if (hf == 1) issue_stage_loads(1);
           __syncwarp();
           mbar_wait(sbar + q, sphase); sphase ^= 1;
-          const float2* xyp = MODE == 3 ? reinterpret_cast<const float2*>(p.xy) + (int)((p.row0 + rt * kRT + hf * 32) % p.npts) : nullptr;
+          const float2* xyp = MODE == 3 ? reinterpret_cast<const float2*>(p.xy) + (p.per_sample ? (p.row0 + rt * kRT + hf * 32) : (p.row0 + rt * kRT + hf * 32) % p.npts) : nullptr;
 #pragma unroll 1
           for (int rc = 0; rc < 4; ++rc) {
             float hh[C][8], hp[C][8], o[C][8];
@@ -527,7 +527,7 @@ void tc_layer_bwd(Launcher& L, int precision, int C, int H, int R, int R_ld, con
   JetParams p{};
   p.H = H; p.n_row_tiles = R / kRT; p.g_bias = g_bias_prev; p.amax = amax;
   if (fl) {
-    p.xy = fl->xy; p.row0 = fl->row0; p.npts = fl->npts; p.in_dim = fl->in_dim; p.gW1 = fl->gW1; p.An = fl->An;
+    p.xy = fl->xy; p.row0 = fl->row0; p.npts = fl->npts; p.in_dim = fl->in_dim; p.gW1 = fl->gW1; p.An = fl->An; p.per_sample = fl->per_sample;
     dispatch_jet<3>(L, precision, C, a, b, o, t, p);
     return;
   }

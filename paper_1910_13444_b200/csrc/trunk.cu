@@ -89,7 +89,7 @@ void trunk_backward_chunk(pigan_ctx* c, const pigan_ctx::HBuf& hb, const pigan_c
         sgemm(L, true, false, H, g.R, H, theta + s.W_off(l), H, 0, (const float*)w.ah[cur], g.R_ld, pl, w.apre, g.R_ld, pl, C, false);
         jet_act_bwd_launch<T>(L, C, H, g, w.apre, nullptr, nullptr, (const T*)hb.at(m), (T*)w.ah[cur ^ 1], grads + s.b_off(m), nullptr, nullptr, amax);
       } else if (m == 1 && tc_first_layer_fusable(H, g)) {
-        FirstLayerFuse fl{xy, g.row0, g.npts, s.in_dim, grads, w.An};
+        FirstLayerFuse fl{xy, g.row0, g.npts, s.in_dim, grads, w.An, g.per_sample};
         tc_layer_bwd(L, c->cfg.precision, C, H, g.R, g.R_ld, c->w16(n, l, 1), w.ah[cur], hb.at(m), w.ah[cur ^ 1], grads + s.b_off(m), amax, &fl);
         return;
       } else {

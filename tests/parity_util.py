@@ -145,3 +145,38 @@ def trunk_step_parity(cfg, skip, bias_std=0.1, loss_scale=1.0, chunk_rows=0, pde
             errs[f"jet.head{k}.ch{c}"] = rel_err(Jg[k][c], Jr[k][c])
     pg.close()
     return errs, lg, losses, fi
+
+
+# ---- NEXT-2: f at per-sample free sensors fed to the critic --------------------------------------------------------
+def free_step_parity(cfg, F, bias_std=0.1, loss_scale=1.0, chunk_rows=0, pde_weight=0.0):
+    import dataclasses
+    import torch
+    from paper_1910_13444_b200 import PiGan
+    cfgF = dataclasses.replace(cfg, G=1)                    # the grid is unused: n_colloc = F points per sample
+    inp = wl.make_inputs(cfgF, bias_std=bias_std)
+    S = cfg.S
+    disc_shape = (2 * S + 3 * F, cfg.LD, cfg.HD)
+    inp["theta_D"] = wl.round_to_precision(wl.xavier_params(np.random.default_rng(1000 * cfg.index + 2), *disc_shape, bias_std=bias_std), cfg.precision)
+    xy_free = wl.free_sensor_points(cfg, F); xy_real = wl.free_sensor_points(cfg, F, real=True)
+    # "real" snapshots: the teacher pair at the sensors, f = 0 at that realization's free sensors (the paper's data solve Eq. 1 with f = 0)
+    Xr, _ = orc.free_snapshot_ref(cfg.gen_shape, inp["teacher_Y"], inp["teacher_u"], xy_real, inp["xy_sensors"], inp["z_real"])
+    Xr[:, 2 * S:2 * S + F] = 0.0
+    real = Xr.astype(np.float32)
+    gY, gu, gD, losses = orc.train_step_grads_free_ref(cfg.gen_shape, disc_shape, inp["theta_Y"], inp["theta_u"], inp["theta_D"], xy_free,
+                                                       inp["xy_sensors"], inp["z"], real, inp["eps"], 10.0, pde_weight)
+    dev = "cuda:0"
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+    pg = PiGan(latent_dim=cfg.m, gen_hidden=cfg.L, gen_width=cfg.H, disc_hidden=cfg.LD, disc_width=cfg.HD, n_samples=cfg.N, n_colloc=F,
+               n_sensors=S, precision=cfg.precision, pde_weight=pde_weight, chunk_rows=chunk_rows, n_free=F)
+    out = pg.train_step_grads(t(inp["theta_Y"]), t(inp["theta_u"]), t(inp["theta_D"]), t(xy_free), None, t(inp["xy_sensors"]), t(inp["z"]), t(real),
+                              t(inp["eps"]), loss_scale)
+    torch.cuda.synchronize()
+    errs = {}
+    for name, g_gpu, g_ref, shape in (("gY", out[0], gY, cfg.gen_shape), ("gu", out[1], gu, cfg.gen_shape), ("gD", out[2], gD, disc_shape)):
+        a = per_layer(g_gpu.cpu().numpy(), shape); b = per_layer(g_ref, shape)
+        for k in a:
+            errs[f"{name}.{k}"] = rel_err(a[k], b[k])
+    lg = out[3].cpu().numpy().astype(np.float64)
+    fi = int(out[4].item())
+    pg.close()
+    return errs, lg, losses, fi

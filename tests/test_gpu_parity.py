@@ -10,7 +10,7 @@ import pytest
 
 import workloads as wl
 from oracle import pigan_oracle as orc
-from parity_util import jets_parity, per_layer, rel_err, step_parity, to_dev, trunk_step_parity
+from parity_util import free_step_parity, jets_parity, per_layer, rel_err, step_parity, to_dev, trunk_step_parity
 
 pytestmark = pytest.mark.gpu
 
@@ -362,3 +362,27 @@ def test_trunk_11x512_cta_pair_kernels(skip):
     cfg = dataclasses.replace(wl.CONFIGS["c4"], name="trunk-11x512", L=10, m=64, N=4, G=16, S=40, HD=128, LD=3)
     check_trunk(cfg, skip)
     check_trunk(cfg, skip, chunk_rows=256)
+
+
+# ---- NEXT-2: f at per-realization free sensors (and their coordinates) as critic inputs -----------------
+def check_free(cfg, F, **kw):
+    errs, lg, lr, found_inf = free_step_parity(cfg, F, **kw)
+    bad = {k: v for k, v in errs.items() if not v <= TOL[cfg.precision]}
+    assert not bad, f"{cfg.name} F={F}: over tolerance {bad}"
+    assert found_inf == 0
+    lrel = np.abs(lg - lr) / np.maximum(np.abs(lr), 1e-12)
+    assert np.all(lrel <= LOSS_TOL), f"{cfg.name} F={F}: losses gpu {lg} ref {lr} rel {lrel}"
+
+
+def test_free_sensors_fp32():
+    check_free(wl.CONFIGS["c1"], 24)                                                       # the paper's choice: no penalty, physics through the critic
+    check_free(wl.CONFIGS["c1"], 24, pde_weight=0.7)
+    check_free(dataclasses.replace(wl.CONFIGS["c1"], name="c1-free-ragged", N=5, S=3), 37, chunk_rows=256)   # 185 rows: ragged, one chunk
+
+
+def test_free_sensors_16bit_one_and_many_chunks():
+    cfg = dataclasses.replace(wl.CONFIGS["c2"], name="c2-free", N=8, S=32)
+    check_free(cfg, 64)                                                                    # 512 rows in one chunk (fused first-layer reduction)
+    check_free(cfg, 64, chunk_rows=256, pde_weight=0.5)                                    # two chunks: the forward is recomputed for the reverse sweep
+    cfg = dataclasses.replace(wl.CONFIGS["c4"], name="c4-free", m=64, N=4, S=40, HD=128, LD=3)
+    check_free(cfg, 200)                                                                   # CTA-pair kernels, 800 rows, points per sample not a multiple of 64

@@ -152,6 +152,12 @@ def make_inputs(cfg: Config, bias_std: float = 0.0) -> dict:
     return out
 
 
+def free_sensor_points(cfg: Config, F: int, real: bool = False) -> np.ndarray:
+    """NEXT-2: per-realization free-sensor locations [N][F][2], uniform on the unit square, re-drawn for every sample
+    (P:127); stream 12 for the generated batch, 13 for the real one."""
+    return _rng(cfg, 13 if real else 12).uniform(0.0, 1.0, size=(cfg.N, F, 2)).astype(np.float32)
+
+
 # ---- algorithmic work model (SURVEY.md section 8(d)); used by bench.py for the roofline ---------------------
 def jet_flops_per_point(L: int, H: int) -> int:
     """Forward flops per (sample, point), both nets: sum over C in {5,3} of (L-1) 2H^2 C + 2HC + 4H."""
