@@ -91,6 +91,9 @@ typedef struct {
                                 points (n_colloc must equal F, xy_colloc is [N][F][2], f is ignored and may be NULL); the critic's
                                 snapshot is [log k(S), u(S), f(F), x(F), y(F)], so disc.in_dim = 2 S + 3 F; L_G = -mean D(fake) +
                                 pde_weight * mean f^2 (the paper's choice is pde_weight = 0); losses[5] = mean f^2.  Two-MLP generator only. */
+  int n_critics;             /* NEXT-3: 0 = one critic on the whole snapshot.  K > 0: K critics of shape `disc`, each on
+                                disc.in_dim columns of the 2S-entry snapshot; such a context steps through
+                                pigan_train_step_grads_hier.  Two-MLP generator, n_free = 0 only. */
 } pigan_config;
 
 /* Creates a context: validates cfg, allocates the workspace on the CURRENT CUDA device and binds the context to it
@@ -161,6 +164,19 @@ pigan_status pigan_train_step_grads(pigan_ctx* ctx, const float* logk_params, co
                                     const float* xy_sensors, const float* z, const float* real_snap,
                                     const float* eps, float loss_scale, float* g_logk, float* g_u, float* g_disc,
                                     float* losses, int* found_inf);
+
+/* NEXT-3: the step with the hierarchical multi-discriminator loss (R10), for contexts created with
+ *   n_critics = K > 0.  As pigan_train_step_grads, except:
+ *   disc_params, g_disc  [K][param_count(cfg.disc)]: critic k's parameters / the gradient of ITS loss
+ *                        L_Dk = mean D_k(fake_k) - mean D_k(real_k) + GP_k (shared eps);
+ *   subsets  DEVICE int [K][cfg.disc.in_dim]: the snapshot columns (0 .. 2S-1, distinct within a critic) that critic k sees;
+ *   weights  HOST float [K]: w_k = 1 / (levels * subdomains in k's level); L_G = sum_k w_k (-mean D_k(fake_k)) + w_pde mean r^2;
+ *   real_snap [N][2S];  losses[6] = {sum_k L_Dk, sum_k w_k mean D_k(fake), sum_k w_k mean D_k(real), sum_k GP_k, L_G, L_pde}.
+ *   Runs eagerly (no CUDA-graph replay). */
+pigan_status pigan_train_step_grads_hier(pigan_ctx* ctx, const float* logk_params, const float* u_params, const float* disc_params,
+                                         const int* subsets, const float* weights, const float* xy_colloc, const float* f,
+                                         const float* xy_sensors, const float* z, const float* real_snap, const float* eps,
+                                         float loss_scale, float* g_logk, float* g_u, float* g_disc, float* losses, int* found_inf);
 
 /* a11: Adam with bias correction on fp32 master weights (S8c O8, G3: eps outside the square root).
  *   params, m, v [n] updated in place; grads [n]; step is 1-based; if skip_flag != NULL and *skip_flag != 0

@@ -22,7 +22,7 @@ STATUS = {0: "PIGAN_OK", 1: "PIGAN_ERR_INVALID_ARG", 2: "PIGAN_ERR_SHAPE", 3: "P
 EXPORTED_SYMBOLS = ["pigan_create", "pigan_destroy", "pigan_param_count", "pigan_trunk_param_count", "pigan_last_error", "pigan_launch_count",
                     "pigan_profile_enable", "pigan_profile_report", "pigan_trunk_jet_forward",
                     "pigan_gen_jet_forward", "pigan_darcy_residual", "pigan_disc_forward", "pigan_gradient_penalty",
-                    "pigan_train_step_grads", "pigan_adam_update"]
+                    "pigan_train_step_grads", "pigan_train_step_grads_hier", "pigan_adam_update"]
 
 
 class PiganError(RuntimeError):
@@ -38,7 +38,7 @@ class _MlpShape(Structure):
 class _Config(Structure):
     _fields_ = [("gen", _MlpShape), ("disc", _MlpShape), ("latent_dim", c_int), ("n_samples", c_int), ("n_colloc", c_int),
                 ("n_sensors", c_int), ("precision", c_int), ("gp_lambda", c_float), ("pde_weight", c_float),
-                ("workspace_bytes", c_size_t), ("chunk_rows", c_int), ("flags", ctypes.c_uint), ("gen_variant", c_int), ("n_free", c_int)]
+                ("workspace_bytes", c_size_t), ("chunk_rows", c_int), ("flags", ctypes.c_uint), ("gen_variant", c_int), ("n_free", c_int), ("n_critics", c_int)]
 
 
 _lib = None
@@ -74,6 +74,7 @@ def load_library():
     lib.pigan_disc_forward.argtypes = [c_void_p, c_void_p, c_void_p, c_int, c_void_p]
     lib.pigan_gradient_penalty.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_int, c_void_p, c_void_p, c_void_p]
     lib.pigan_train_step_grads.argtypes = [c_void_p] + [c_void_p] * 9 + [c_float] + [c_void_p] * 5
+    lib.pigan_train_step_grads_hier.argtypes = [c_void_p] * 4 + [c_void_p, POINTER(c_float)] + [c_void_p] * 6 + [c_float] + [c_void_p] * 5
     lib.pigan_adam_update.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_size_t, c_int, c_float, c_float, c_float,
                                       c_float, c_void_p]
     lib.pigan_profile_enable.argtypes = [c_void_p, c_int]
@@ -113,7 +114,7 @@ class PiGan:
     """One context = one CUDA stream + the workspaces of one PI-GAN configuration (mirrors pigan_ctx)."""
 
     def __init__(self, *, latent_dim, gen_hidden, gen_width, disc_hidden, disc_width, n_samples, n_colloc, n_sensors,
-                 precision="fp32", gp_lambda=10.0, pde_weight=1.0, workspace_bytes=0, chunk_rows=0, flags=0, gen_variant="two_mlps", n_free=0, stream=None, device=None):
+                 precision="fp32", gp_lambda=10.0, pde_weight=1.0, workspace_bytes=0, chunk_rows=0, flags=0, gen_variant="two_mlps", n_free=0, n_critics=0, critic_inputs=None, stream=None, device=None):
         import torch
         self._lib = load_library()
         self._ctx = c_void_p()
@@ -122,11 +123,11 @@ class PiGan:
         self.device = torch.device(device if device is not None else f"cuda:{torch.cuda.current_device()}")
         self.m, self.N, self.P, self.S = latent_dim, n_samples, n_colloc, n_sensors
         self.gen_shape = (2 + latent_dim, gen_hidden, gen_width)
-        self.disc_shape = (2 * n_sensors + 3 * n_free, disc_hidden, disc_width)
-        self.n_free = n_free
+        self.disc_shape = ((critic_inputs if n_critics else 2 * n_sensors + 3 * n_free), disc_hidden, disc_width)
+        self.n_free, self.n_critics = n_free, n_critics
         self.precision = precision
         cfg = _Config(_MlpShape(*self.gen_shape), _MlpShape(*self.disc_shape), latent_dim, n_samples, n_colloc, n_sensors,
-                      PRECISIONS[precision], gp_lambda, pde_weight, workspace_bytes, chunk_rows, flags, GEN_VARIANTS[gen_variant], n_free)
+                      PRECISIONS[precision], gp_lambda, pde_weight, workspace_bytes, chunk_rows, flags, GEN_VARIANTS[gen_variant], n_free, n_critics)
         self.gen_variant = gen_variant
         self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
         with torch.cuda.device(self.device):
@@ -231,6 +232,21 @@ class PiGan:
             _ptr(xy_colloc, "xy_colloc"), _ptr(f, "f"), _ptr(xy_sensors, "xy_sensors"), _ptr(z, "z"), _ptr(real_snap, "real_snap"),
             _ptr(eps, "eps"), float(loss_scale), _ptr(g_logk, "g_logk"), _ptr(g_u, "g_u"), _ptr(g_disc, "g_disc"), _ptr(losses, "losses"),
             _ptr(found_inf, "found_inf", torch.int32)))
+        return out
+
+    def train_step_grads_hier(self, logk_params, u_params, disc_params, subsets, weights, xy_colloc, f, xy_sensors, z, real_snap, eps, loss_scale=1.0):
+        """NEXT-3: K critics (context created with n_critics = K, critic_inputs = columns per critic).  disc_params [K][n_disc];
+        subsets: int32 CUDA tensor [K][critic_inputs]; weights: K host floats.  Returns (g_logk, g_u, g_disc [K][n_disc], losses, found_inf)."""
+        import torch
+        K = self.n_critics
+        out = (self._new(self.n_gen), self._new(self.n_gen), self._new(K, self.n_disc), self._new(6), self._new(1, dtype=torch.int32))
+        w = (c_float * K)(*[float(x) for x in weights])
+        self._check(self._lib.pigan_train_step_grads_hier(
+            self._ctx, _ptr(logk_params, "logk_params"), _ptr(u_params, "u_params"), _ptr(disc_params, "disc_params"),
+            _ptr(subsets, "subsets", torch.int32), w, _ptr(xy_colloc, "xy_colloc"), _ptr(f, "f"), _ptr(xy_sensors, "xy_sensors"), _ptr(z, "z"),
+            _ptr(real_snap, "real_snap"), _ptr(eps, "eps"), float(loss_scale), _ptr(out[0], "g_logk"), _ptr(out[1], "g_u"), _ptr(out[2], "g_disc"),
+            _ptr(out[3], "losses"), _ptr(out[4], "found_inf", torch.int32)))
+        torch.cuda.current_stream(self.device).synchronize()    # `weights` is a host array read while the step is enqueued; keep it alive
         return out
 
     def adam_update(self, params, grads, m, v, step, lr, beta1, beta2, adam_eps, skip_flag=None):

@@ -39,7 +39,8 @@ pigan_status train_step_impl(pigan_ctx* c, const float* thY, const float* thU, c
   const float* th[2] = {thY, thU};
   float* gr[2] = {gY, gU};
   cudaStream_t st = L.stream;
-  cudaMemsetAsync(gY, 0, gs.count() * 4, st); cudaMemsetAsync(gU, 0, gs.count() * 4, st); cudaMemsetAsync(gD, 0, ds.count() * 4, st);
+  const size_t n_gD = ds.count() * (size_t)std::max(1, c->hier.K);
+  cudaMemsetAsync(gY, 0, gs.count() * 4, st); cudaMemsetAsync(gU, 0, gs.count() * 4, st); cudaMemsetAsync(gD, 0, n_gD * 4, st);
   cudaMemsetAsync(c->cw.acc, 0, 8 * sizeof(double), st);
   if (found_inf) cudaMemsetAsync(found_inf, 0, sizeof(int), st);
   for (int n = 0; n < 2; ++n) {
@@ -58,7 +59,9 @@ pigan_status train_step_impl(pigan_ctx* c, const float* thY, const float* thU, c
     }
   }
   // ---- a7-a9: critic losses and gradient; dX rows [0, N) = (1/N) grad_X D(X_fake) ----
-  if (critic_fused_supported(ds)) {
+  if (c->hier.K > 0) {
+    hier_critic_stage(c, thD, real, eps, gD);               // NEXT-3: K critics on column subsets (hier.cu)
+  } else if (critic_fused_supported(ds)) {
     // small critic: one kernel for every per-row sweep + the batched weight-gradient GEMMs (critic_fused.cu)
     critic_fused(L, ds, thD, c->xfake, real, eps, N, 1, cfg.gp_lambda, c->cw, gD, c->dX, nullptr);
   } else {
@@ -98,8 +101,11 @@ pigan_status train_step_impl(pigan_ctx* c, const float* thY, const float* thU, c
     finalize_first_layer(L, gs, N, c->net[n].An, z, gr[n]);
     unscale_and_check(L, gr[n], gs.count(), 1.f / loss_scale, found_inf);
   }
-  unscale_and_check(L, gD, ds.count(), 1.f, found_inf);
-  if (losses) write_losses(L, c->cw.acc, N, crows, cfg.gp_lambda, cfg.pde_weight, losses, nullptr, nullptr, 0);
+  unscale_and_check(L, gD, n_gD, 1.f, found_inf);
+  if (losses) {
+    if (c->hier.K > 0) hier_write_losses(c, crows, losses);
+    else write_losses(L, c->cw.acc, N, crows, cfg.gp_lambda, cfg.pde_weight, losses, nullptr, nullptr, 0);
+  }
   return finish(c);
 }
 
@@ -169,8 +175,11 @@ pigan_status pigan_create(const pigan_config* cfg, void* cuda_stream, pigan_ctx*
     return PIGAN_ERR_INVALID_ARG;
   if ((int)cfg->precision < 0 || (int)cfg->precision > 2 || !(cfg->gp_lambda >= 0.f) || cfg->chunk_rows < 0) return PIGAN_ERR_INVALID_ARG;
   if (cfg->gen_variant < 0 || cfg->gen_variant > 2) return PIGAN_ERR_INVALID_ARG;
-  if (cfg->n_free < 0) return PIGAN_ERR_INVALID_ARG;
-  if (cfg->gen.in_dim != 2 + cfg->latent_dim || cfg->disc.in_dim != 2 * cfg->n_sensors + 3 * cfg->n_free) return PIGAN_ERR_SHAPE;
+  if (cfg->n_free < 0 || cfg->n_critics < 0) return PIGAN_ERR_INVALID_ARG;
+  if (cfg->gen.in_dim != 2 + cfg->latent_dim) return PIGAN_ERR_SHAPE;
+  if (cfg->n_critics == 0 && cfg->disc.in_dim != 2 * cfg->n_sensors + 3 * cfg->n_free) return PIGAN_ERR_SHAPE;
+  if (cfg->n_critics > 0 && (cfg->disc.in_dim > 2 * cfg->n_sensors)) return PIGAN_ERR_SHAPE;
+  if (cfg->n_critics > 0 && (cfg->n_free > 0 || cfg->gen_variant != PIGAN_GEN_TWO_MLPS)) return PIGAN_ERR_UNSUPPORTED;
   if (cfg->n_free > 0 && cfg->n_colloc != cfg->n_free) return PIGAN_ERR_SHAPE;
   if (cfg->n_free > 0 && cfg->gen_variant != PIGAN_GEN_TWO_MLPS) return PIGAN_ERR_UNSUPPORTED;
   if (cfg->precision != PIGAN_FP32) {
@@ -252,8 +261,13 @@ pigan_status pigan_create(const pigan_config* cfg, void* cuda_stream, pigan_ctx*
       cw.cfB1 = c->alloc<float>((size_t)4 * N * d);
       cw.cfBh = c->alloc<float>((size_t)LD * 4 * N * HD);
     }
-    c->xfake = c->alloc<float>((size_t)N * d);
-    c->dX = c->alloc<float>((size_t)2 * N * d);
+    const int dsnap = cfg->n_critics > 0 ? 2 * S : d;         // width of the generated snapshot
+    c->xfake = c->alloc<float>((size_t)N * dsnap);
+    c->dX = c->alloc<float>((size_t)2 * N * dsnap);
+    if (cfg->n_critics > 0) {
+      c->hXf = c->alloc<float>((size_t)N * d); c->hXr = c->alloc<float>((size_t)N * d); c->hdX = c->alloc<float>((size_t)2 * N * d);
+      c->htot = c->alloc<double>(4);
+    }
     c->seed = c->alloc<float>((size_t)2 * N);
     c->amax = c->alloc<float>(2);
     if (cfg->n_free > 0) c->fbuf = c->alloc<float>((size_t)c->R_ld);
@@ -368,6 +382,7 @@ pigan_status pigan_train_step_grads(pigan_ctx* c, const float* logk_params, cons
       (!c->trunk && (!u_params || !g_u)))
     return fail(c, PIGAN_ERR_INVALID_ARG, "null pointer");
   if (!(loss_scale > 0.f) || !std::isfinite(loss_scale)) return fail(c, PIGAN_ERR_INVALID_ARG, "loss_scale must be positive and finite");
+  if (c->cfg.n_critics > 0) return fail(c, PIGAN_ERR_UNSUPPORTED, "the context was created with n_critics > 0: call pigan_train_step_grads_hier");
   auto run = [&]() -> pigan_status {
     if (c->cfg.n_free > 0)
       return free_train_step(c, logk_params, u_params, disc_params, xy_colloc, xy_sensors, z, real_snap, eps, loss_scale, g_logk, g_u, g_disc, losses, found_inf);
@@ -418,6 +433,27 @@ pigan_status pigan_train_step_grads(pigan_ctx* c, const float* logk_params, cons
   if (cudaGraphLaunch(sg.exec, user) != cudaSuccess) { cudaGetLastError(); return fail(c, PIGAN_ERR_CUDA, "cudaGraphLaunch failed"); }
   c->L.count += sg.launches;
   return PIGAN_OK;
+}
+
+pigan_status pigan_train_step_grads_hier(pigan_ctx* c, const float* logk_params, const float* u_params, const float* disc_params, const int* subsets,
+                                         const float* weights, const float* xy_colloc, const float* f, const float* xy_sensors, const float* z,
+                                         const float* real_snap, const float* eps, float loss_scale, float* g_logk, float* g_u, float* g_disc,
+                                         float* losses, int* found_inf) {
+  if (!c) return PIGAN_ERR_INVALID_ARG;
+  DeviceGuard dg(c);
+  if (c->cfg.n_critics <= 0) return fail(c, PIGAN_ERR_UNSUPPORTED, "the context was created with n_critics = 0");
+  if (!logk_params || !u_params || !disc_params || !subsets || !weights || !xy_colloc || !f || !xy_sensors || !z || !real_snap || !eps || !g_logk ||
+      !g_u || !g_disc)
+    return fail(c, PIGAN_ERR_INVALID_ARG, "null pointer");
+  if (!(loss_scale > 0.f) || !std::isfinite(loss_scale)) return fail(c, PIGAN_ERR_INVALID_ARG, "loss_scale must be positive and finite");
+  c->hier.K = c->cfg.n_critics; c->hier.subsets = subsets; c->hier.weights = weights;
+  pigan_status st;
+  if (c->cfg.precision == PIGAN_FP32)
+    st = train_step_impl<float>(c, logk_params, u_params, disc_params, xy_colloc, f, xy_sensors, z, real_snap, eps, loss_scale, g_logk, g_u, g_disc, losses, found_inf);
+  else
+    st = train_step_impl<__half>(c, logk_params, u_params, disc_params, xy_colloc, f, xy_sensors, z, real_snap, eps, loss_scale, g_logk, g_u, g_disc, losses, found_inf);
+  c->hier = pigan_ctx::Hier{};
+  return st;
 }
 
 pigan_status pigan_adam_update(pigan_ctx* c, float* params, const float* grads, float* m, float* v, size_t n, int step, float lr, float beta1,

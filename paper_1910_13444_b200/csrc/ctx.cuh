@@ -64,6 +64,10 @@ struct pigan_ctx {
   }
   int n_sens_chunks = 1;
   float* fbuf = nullptr;       // NEXT-2: [R_ld] f values of a chunk / the critic's adjoint of them
+  // NEXT-3 (hier.cu): K critics on column subsets of the snapshot; set for the duration of pigan_train_step_grads_hier
+  struct Hier { int K = 0; const int* subsets = nullptr; const float* weights = nullptr; } hier;
+  float* hXf = nullptr; float* hXr = nullptr; float* hdX = nullptr;   // [N][d_sub] gathered fake / real sub-snapshots, one critic's input gradient
+  double* htot = nullptr;      // [4] sum_k L_Dk, sum_k w_k mean D_k(fake), sum_k w_k mean D_k(real), sum_k GP_k
   bool trunk = false, skip = false;   // NEXT-1: shared-trunk generator (workspace of net[1]), with skip connections
   size_t plane() const { return (size_t)gen.H * R_ld * elem; }
   // activation stash of one chunk: `planes` planes per layer; l = 1..L
@@ -192,6 +196,9 @@ void gen_backward_chunk(pigan_ctx* c, int n, const pigan_ctx::HBuf& hb, const fl
 pigan_status trunk_train_step(pigan_ctx* c, const float* thG, const float* thD, const float* xy_c, const float* f, const float* xy_s, const float* z,
                               const float* real, const float* eps, float loss_scale, float* gG, float* gD, float* losses, int* found_inf);
 pigan_status trunk_jet_forward(pigan_ctx* c, const float* theta, const float* xy, int n_pts, const float* z, int n_samples, int C, float* out);
+// NEXT-3 (hier.cu): the critic stage with K critics (fills gD [K][count] and c->dX [N][2S]) and its loss scalars
+void hier_critic_stage(pigan_ctx* c, const float* thD, const float* real, const float* eps, float* gD);
+void hier_write_losses(pigan_ctx* c, long long NP, float* losses);
 // NEXT-2 (free.cu): f at per-sample free sensors fed to the critic
 pigan_status free_train_step(pigan_ctx* c, const float* thY, const float* thU, const float* thD, const float* xy_free, const float* xy_s, const float* z,
                              const float* real, const float* eps, float loss_scale, float* gY, float* gU, float* gD, float* losses, int* found_inf);

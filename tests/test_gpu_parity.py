@@ -370,7 +370,12 @@ def check_free(cfg, F, **kw):
     bad = {k: v for k, v in errs.items() if not v <= TOL[cfg.precision]}
     assert not bad, f"{cfg.name} F={F}: over tolerance {bad}"
     assert found_inf == 0
-    lrel = np.abs(lg - lr) / np.maximum(np.abs(lr), 1e-12)
+    # The f entries of the snapshot come from the 16-bit jets (each accurate to ~1e-3 of its plane, tolerance 2e-2), so a critic
+    # mean that is small by cancellation cannot be held to 1e-3 of ITSELF: the scores are compared at 1e-3 of the critic's
+    # score scale max(|mean D(fake)|, |mean D(real)|)  (reading R9); GP and mean f^2 stay at 1e-3 relative.
+    scale = np.abs(lr).copy()
+    scale[[0, 1, 2, 4]] = np.maximum(scale[[0, 1, 2, 4]], max(abs(lr[1]), abs(lr[2])))
+    lrel = np.abs(lg - lr) / np.maximum(scale, 1e-12)
     assert np.all(lrel <= LOSS_TOL), f"{cfg.name} F={F}: losses gpu {lg} ref {lr} rel {lrel}"
 
 
@@ -386,3 +391,51 @@ def test_free_sensors_16bit_one_and_many_chunks():
     check_free(cfg, 64, chunk_rows=256, pde_weight=0.5)                                    # two chunks: the forward is recomputed for the reverse sweep
     cfg = dataclasses.replace(wl.CONFIGS["c4"], name="c4-free", m=64, N=4, S=40, HD=128, LD=3)
     check_free(cfg, 200)                                                                   # CTA-pair kernels, 800 rows, points per sample not a multiple of 64
+
+
+# ---- NEXT-3: hierarchical multi-discriminator loss ------------------------------------------------------
+def check_hier(cfg, levels, sensors_per_critic, bias_std=0.1, pde_weight=1.0):
+    """levels = subdomains per level; every critic sees `sensors_per_critic` sensors (log k and u entries), drawn seeded, overlapping."""
+    import torch
+    from paper_1910_13444_b200 import PiGan
+    from parity_util import oracle_real_snapshots
+    K, S = sum(levels), cfg.S
+    rng = np.random.default_rng(1000 * cfg.index + 20)
+    sens = np.stack([np.sort(rng.choice(S, size=sensors_per_critic, replace=False)) for _ in range(K)])
+    subsets = np.concatenate([sens, S + sens], axis=1).astype(np.int32)
+    disc_shape = (2 * sensors_per_critic, cfg.LD, cfg.HD)
+    inp = wl.make_inputs(cfg, bias_std=bias_std)
+    thDs = np.stack([wl.round_to_precision(wl.xavier_params(np.random.default_rng(1000 * cfg.index + 30 + k), *disc_shape, bias_std=bias_std), cfg.precision)
+                     for k in range(K)])
+    w = orc.hierarchy_weights(levels)
+    inp["real"] = oracle_real_snapshots(cfg, inp)
+    gY, gu, gD, losses = orc.train_step_grads_hier_ref(cfg.gen_shape, disc_shape, inp["theta_Y"], inp["theta_u"], thDs, subsets, w, inp["xy_colloc"], inp["f"],
+                                                       inp["xy_sensors"], inp["z"], inp["real"], inp["eps"], 10.0, pde_weight)
+    d = to_dev(inp, "cuda:0")
+    pg = PiGan.from_config(cfg, pde_weight=pde_weight, n_critics=K, critic_inputs=2 * sensors_per_critic)
+    out = pg.train_step_grads_hier(d["theta_Y"], d["theta_u"], torch.from_numpy(thDs).cuda(), torch.from_numpy(subsets).cuda(), w, d["xy_colloc"], d["f"],
+                                   d["xy_sensors"], d["z"], d["real"], d["eps"], 1.0)
+    torch.cuda.synchronize()
+    errs = {}
+    for name, g_gpu, g_ref in (("gY", out[0], gY), ("gu", out[1], gu)):
+        a = per_layer(g_gpu.cpu().numpy(), cfg.gen_shape); b = per_layer(g_ref, cfg.gen_shape)
+        for k in a:
+            errs[f"{name}.{k}"] = rel_err(a[k], b[k])
+    for kk in range(K):
+        a = per_layer(out[2][kk].cpu().numpy(), disc_shape); b = per_layer(gD[kk], disc_shape)
+        for k in a:
+            errs[f"gD{kk}.{k}"] = rel_err(a[k], b[k])
+    bad = {k: v for k, v in errs.items() if not v <= TOL[cfg.precision]}
+    assert not bad, f"{cfg.name}: over tolerance {bad}"
+    lg = out[3].cpu().numpy().astype(np.float64)
+    lrel = np.abs(lg - losses) / np.maximum(np.abs(losses), 1e-12)
+    assert np.all(lrel <= LOSS_TOL) and int(out[4].item()) == 0, (lg, losses)
+    with pytest.raises(Exception):                                                        # such a context does not take the single-critic call
+        pg.train_step_grads(d["theta_Y"], d["theta_u"], d["theta_D"], d["xy_colloc"], d["f"], d["xy_sensors"], d["z"], d["real"], d["eps"], 1.0)
+    pg.close()
+
+
+def test_hierarchical_critics_fp32_and_16bit():
+    check_hier(wl.CONFIGS["c1"], [1, 3], 4)                                                # 4 critics, weights 1/2, 1/6, 1/6, 1/6
+    check_hier(dataclasses.replace(wl.CONFIGS["c2"], name="c2-hier", N=8, G=16, S=32), [1, 2, 4], 12)      # fused small-critic kernel, 7 critics
+    check_hier(dataclasses.replace(wl.CONFIGS["c4"], name="c4-hier", m=64, N=4, G=16, S=40, LD=3), [1, 2], 20)   # HD = 512: layer-by-layer critic path
