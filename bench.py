@@ -28,9 +28,21 @@ import workloads as wl  # noqa: E402
 METRIC = "PI-GAN train-step sample*collocation-points/s"
 UNIT = "sample*collocation-points/s"
 ADAM = dict(lr=1e-4, beta1=0.5, beta2=0.9, adam_eps=1e-8)          # reading G3
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the largest tensor-core kernel (G_u forward, 131072-row chunk),
-# from profiles/r01c_ncu_full_tc_kernels_c5.csv (1.345e9 read + 1.306e9 written); algorithmic bytes of that launch: 2.684e9
-TRAFFIC = {"c5": 2.651e9}
+PROFILE_CSV = os.path.join(ROOT, "profiles", "r02_step_dram_bytes.csv")   # ncu summary of one timed step per config (profiles/r02_summary.md)
+
+
+def ncu_profile(cfg_name):
+    """Per kernel class of `cfg_name`: launches, DRAM bytes and tensor-pipe-active % of ONE timed step, as measured by the ncu
+    pass recorded in profiles/r02_step_dram_bytes.csv (not by this run).  {} when the file has no rows for the config."""
+    out = {}
+    if not os.path.exists(PROFILE_CSV):
+        return out
+    import csv
+    for r in csv.DictReader(open(PROFILE_CSV)):
+        if r["config"] == cfg_name:
+            out[r["kernel_class"]] = {"launches": int(r["launches"]), "dram_bytes": int(r["dram_bytes_read"]) + int(r["dram_bytes_write"]),
+                                      "tensor_pct": float(r["tensor_pipe_active_pct_time_weighted"] or 0.0)}
+    return out
 
 
 # ----------------------------------------------------------------------------------------------------------------
@@ -214,8 +226,21 @@ class GpuWorkload:
             pg.train_step_grads(self.params[0], self.params[1], self.params[2], d["xy_colloc"], d["f"], d["xy_sensors"], d["z"], d["real"],
                                 d["eps"], self.loss_scale, out=self.out)
             grads = self.out[:3]
+        if getattr(self, "dp_dist", None) is not None:
+            self.dp_out.all_reduce_mean(self.dp_dist, self.dp_world)
         for k in range(len(self.params)):
             pg.adam_update(self.params[k], grads[k], self.mom[k][0], self.mom[k][1], self.step_no, skip_flag=self.out[4], **ADAM)
+
+    def enable_dp(self, dist):
+        """NEXT-4: this rank's context holds N / W samples; the three gradient vectors live in ONE flat buffer that is
+        all-reduced (NCCL) right behind the step, then every rank applies the same Adam update."""
+        from paper_1910_13444_b200.dp import FlatGrads
+        self.dp_dist, self.dp_world = dist, dist.get_world_size()
+        self.dp_out = FlatGrads([p.numel() for p in self.params], self.device)
+        if self.trunk:
+            self.out = (self.dp_out.grads[0], None, self.dp_out.grads[1], self.dp_out.losses, self.dp_out.found_inf)
+        else:
+            self.out = (self.dp_out.grads[0], self.dp_out.grads[1], self.dp_out.grads[2], self.dp_out.losses, self.dp_out.found_inf)
 
     def step_e2e(self):
         """Same step with the per-step inputs coming from pinned host memory and the losses read back."""
@@ -241,8 +266,9 @@ class GpuWorkload:
     def e2e_bytes(self):
         return sum(int(v.numel() * 4) for v in self.host.values()), 6 * 4
 
-    def timed(self, fn, steps, warmup):
-        """Per-step CUDA-event timing on the launch stream; L2 is flushed between steps for the small configs."""
+    def timed(self, fn, steps, warmup, tag="timed_step"):
+        """Per-step CUDA-event timing on the launch stream; L2 is flushed between steps for the small configs.  Every timed call
+        sits in an NVTX range `tag` (ncu --nvtx --nvtx-include "timed_step/" profiles exactly the timed train steps)."""
         torch = self.torch
         for _ in range(warmup):
             fn()
@@ -252,7 +278,7 @@ class GpuWorkload:
             if self.flush is not None:
                 self.flush.fill_(1)
             a.record()
-            torch.cuda.nvtx.range_push("timed_step")          # lets `ncu --nvtx --nvtx-include "timed_step/"` isolate the timed steps
+            torch.cuda.nvtx.range_push(tag)
             fn()
             torch.cuda.nvtx.range_pop()
             b.record()
@@ -260,9 +286,11 @@ class GpuWorkload:
         return [a.elapsed_time(b) for a, b in ev]
 
 
-def run_config(cfg, device, steps, warmup, rank, world, with_roofline=True, seed_shift=0, chunk_rows=0):
+def run_config(cfg, device, steps, warmup, rank, world, with_roofline=True, seed_shift=0, chunk_rows=0, dp=None):
     import torch
     w = GpuWorkload(cfg, device, seed_shift, chunk_rows)
+    if dp is not None:
+        w.enable_dp(dp)
     peaks = measured_peaks()
     flops = wl.step_flops(cfg)
     res = {}
@@ -292,11 +320,11 @@ def run_config(cfg, device, steps, warmup, rank, world, with_roofline=True, seed
     res["found_inf"] = int(w.out[4].item())
     res["losses"] = [float(x) for x in w.out[3].cpu()]
     # end-to-end leg: host buffers in, losses out, copies inside the timed region
-    ms_e2e = w.timed(w.step_e2e, max(2, steps // 2), 1)
+    ms_e2e = w.timed(w.step_e2e, max(2, steps // 2), 1, tag="timed_e2e")
     res["ms_e2e"] = ms_e2e
     res["h2d"], res["d2h"] = w.e2e_bytes()
     # jet evaluations/s (north_star's second throughput figure): forward jets of both nets, no residual, no backward
-    res["ms_jet"] = w.timed(w.jet_pass, max(2, steps // 2), 1)
+    res["ms_jet"] = w.timed(w.jet_pass, max(2, steps // 2), 1, tag="timed_jet")
     del w.jet_out, w.jet_out2
     # roofline of the dominant kernel class (the tcgen05 jet GEMMs: forward, dgrad+adjoint, wgrad)
     if with_roofline:
@@ -312,12 +340,41 @@ def run_config(cfg, device, steps, warmup, rank, world, with_roofline=True, seed
             alg = flops["jet_gemm"] + sens_gemm
             ach = alg / (tc_ms * 1e-3) / 1e12
             peak = peaks["tflops_sustained"]
+            # per kernel class: its own roofline = max(flops / sustained tensor rate, algorithmic plane bytes / copy bandwidth).
+            # plane bytes per row and hidden layer (16-bit): forward reads C + writes C planes, dgrad reads 2C (ahat^l, h^{l-1}) + writes C
+            # (nothing for the fused layer-2 dgrad), wgrad reads 2C; C summed over the nets' collocation channels, sensors add 1 (2 split) per net
+            chan = 8 if cfg.variant == "two_mlps" else 5
+            nets = 2 if cfg.variant == "two_mlps" else 1
+            rowsC = cfg.N * cfg.P * chan + cfg.N * cfg.S * nets
+            pb = 2 * cfg.H                                        # bytes of one row of one 16-bit plane
+            Lh = cfg.L - 1
+            cls_bytes = {"jet_layer_fwd": 2 * rowsC * pb * Lh, "jet_layer_bwd": rowsC * pb * (3 * Lh - 1), "wgrad": 2 * rowsC * pb * Lh}
+            prof_ncu = ncu_profile(cfg.name)
+            per_kernel = {}
+            for k, v in tc.items():
+                if v[1] <= 0:
+                    continue
+                t_ms = v[1] / steps
+                t_tensor = alg / 3 / (peak * 1e12) * 1e3
+                t_hbm = cls_bytes[k] / (peaks["hbm_gbs"] * 1e9) * 1e3
+                pct = [d["tensor_pct"] for kk, d in prof_ncu.items() if kk.startswith(k + "(C=5") or kk == k]
+                per_kernel[k] = {"tflops": round(alg / 3 / (t_ms * 1e-3) / 1e12, 1), "gbs_algorithmic": round(cls_bytes[k] / (t_ms * 1e-3) / 1e9, 1),
+                                 "bound": "tensor" if t_tensor >= t_hbm else "hbm", "frac": round(max(t_tensor, t_hbm) / t_ms, 4),
+                                 "tensor_pipe_active_pct_ncu": pct[0] if pct else None}
+            dom = max(tc, key=lambda k: tc[k][1])
+            dom_ncu = next((d for kk, d in prof_ncu.items() if kk.startswith(dom + "(C=5") or kk == dom), None)
+            whole = prof_ncu.get("WHOLE_STEP")
             res["roofline"] = {"bound": "tensor", "achieved": round(ach, 2), "peak": peak, "unit": "TFLOP/s", "frac": round(ach / peak, 4),
-                               "traffic": TRAFFIC.get(cfg.name), "kernel": "jet_layer_fwd + jet_layer_bwd + wgrad (tcgen05)", "peak_source": peaks["source"] + " sustained bf16",
+                               "traffic": (dom_ncu["dram_bytes"] / dom_ncu["launches"]) if dom_ncu else None,
+                               "traffic_kernel": f"{dom} (C=5), DRAM read+write bytes per launch" if dom_ncu else None,
+                               "traffic_whole_step": whole["dram_bytes"] if whole else None,
+                               "traffic_source": "profiles/r02_step_dram_bytes.csv (ncu pass of profiles/r02_summary.md, not this run)" if prof_ncu else None,
+                               "kernel": "jet_layer_fwd + jet_layer_bwd + wgrad (tcgen05)", "peak_source": peaks["source"] + " sustained bf16",
                                "frac_of_burst": round(ach / peaks["tflops_burst"], 4), "frac_of_nominal_2250": round(ach / 2250.0, 4),
                                "share_of_step": round(tc_ms / total_ms, 4) if total_ms > 0 else None,
-                               "profile_pass": "in the timed region" if in_region else "separate eager pass after the timed region (the timed region replays a CUDA graph)",
-                               "per_kernel_tflops": {k: round(alg / 3 / (v[1] / steps * 1e-3) / 1e12, 1) for k, v in tc.items() if v[1] > 0}}
+                               "profile_pass": ("in the timed region: one CUDA event is recorded after every launch inside the timed steps, so `value` carries that "
+                                                "(~1 %) overhead") if in_region else "separate eager pass after the timed region (the timed region replays a CUDA graph)",
+                               "per_kernel": per_kernel}
         else:
             # fp32 mode (c1): plain FP32 FMA path; report against the fp32 ALU peak (148 SMs x 128 lanes x 2 flop x clock)
             mhz = res["clocks"]["sm_mhz"] or 1965.0
@@ -380,6 +437,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--samples", type=int, default=None, help="override N (latent samples per step): a smaller job for ncu captures; "
                     "the line then says so in config.workload and is not a benchmark value")
+    ap.add_argument("--dp", action="store_true", help="NEXT-4: with --gpus N > 1, shard the N latent samples of the step over the ranks and all-reduce "
+                    "the gradients (strong scaling) instead of running N independent replicas")
     ap.add_argument("--chunk-rows", type=int, default=0, help="rows per chunk of the generator passes (0 = library default); sweeps only")
     args = ap.parse_args()
     cfg = wl.TABLE2 if args.config == "t2" else wl.CONFIGS[args.config]
@@ -413,12 +472,21 @@ def main():
     if world > 1:
         dist.init_process_group("nccl", device_id=device)
         dist.barrier()
-    res = run_config(cfg, device, steps, warmup, rank, world, seed_shift=rank, chunk_rows=args.chunk_rows)
+    units_global = cfg.N * cfg.P
+    if args.dp and world > 1:
+        if cfg.N % world:
+            raise SystemExit(f"--dp needs N = {cfg.N} divisible by the world size {world}")
+        cfg = dataclasses.replace(cfg, N=cfg.N // world)      # this rank's shard; inputs are drawn per rank (seed_shift)
+    res = run_config(cfg, device, steps, warmup, rank, world, seed_shift=rank, chunk_rows=args.chunk_rows, dp=dist if (args.dp and world > 1) else None)
     t_ms = float(np.mean(res["ms_steps"]))
     if world > 1:
         t_ms = max_over_ranks(t_ms, dist, device)           # max over ranks; the replicas exchange nothing else
     if rank == 0:
         line = summarize(cfg, res, world, steps, warmup, t_ms)
+        if args.dp and world > 1:
+            line["scaling"] = "strong"
+            line["config"]["parallelism"] = f"data-parallel x{world}: {cfg.N} of {cfg.N * world} samples per rank, one fp32 all-reduce of the gradients per step"
+            line["config"]["rows_per_step"] = units_global
         if args.all_configs:
             per = {}
             for name, c in wl.CONFIGS.items():

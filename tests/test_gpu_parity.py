@@ -439,3 +439,39 @@ def test_hierarchical_critics_fp32_and_16bit():
     check_hier(wl.CONFIGS["c1"], [1, 3], 4)                                                # 4 critics, weights 1/2, 1/6, 1/6, 1/6
     check_hier(dataclasses.replace(wl.CONFIGS["c2"], name="c2-hier", N=8, G=16, S=32), [1, 2, 4], 12)      # fused small-critic kernel, 7 critics
     check_hier(dataclasses.replace(wl.CONFIGS["c4"], name="c4-hier", m=64, N=4, G=16, S=40, LD=3), [1, 2], 20)   # HD = 512: layer-by-layer critic path
+
+
+# ---- NEXT-4: data-parallel step / minimal loop (single rank on the GPU; the 2-rank host logic is tested on CPU ranks) ----
+@pytest.mark.parametrize("schedule", ["parallel", "sequential"])
+def test_data_parallel_trainer_drives_the_library_through_one_flat_gradient_buffer(schedule):
+    import torch
+    from paper_1910_13444_b200 import PiGan
+    from paper_1910_13444_b200.dp import DataParallelTrainer, pigan_step_fns
+    from parity_util import oracle_real_snapshots
+    cfg = wl.CONFIGS["c1"]
+    inp = wl.make_inputs(cfg, bias_std=0.1)
+    inp["real"] = oracle_real_snapshots(cfg, inp)
+    d = to_dev(inp, "cuda:0")
+    pg = PiGan.from_config(cfg)
+    adam = dict(lr=1e-2, beta1=0.5, beta2=0.9, adam_eps=1e-8)
+    step_fn, adam_fn = pigan_step_fns(pg, d["xy_colloc"], d["f"], d["xy_sensors"], 1.0, adam)
+    params = [d[k].clone() for k in ("theta_Y", "theta_u", "theta_D")]
+    tr = DataParallelTrainer(step_fn, adam_fn, params, schedule=schedule)
+    losses = tr.train_step(d["z"], d["real"], d["eps"]).cpu().numpy()
+    torch.cuda.synchronize()
+    # the same iteration by the oracle
+    th = [inp[k].astype(np.float64) for k in ("theta_Y", "theta_u", "theta_D")]
+    args = (inp["xy_colloc"], inp["f"], inp["xy_sensors"], inp["z"], inp["real"], inp["eps"], 10.0, 1.0)
+    gY, gu, gD, lref = orc.train_step_grads_ref(cfg.gen_shape, cfg.disc_shape, *th, *args)
+    z0 = lambda g: (np.zeros_like(g), np.zeros_like(g))
+    newD = orc.adam_update_ref(th[2], gD, *z0(gD), 1, 1e-2, 0.5, 0.9, 1e-8)[0]
+    if schedule == "sequential":
+        gY, gu, _, lref = orc.train_step_grads_ref(cfg.gen_shape, cfg.disc_shape, th[0], th[1], newD, *args)
+    newY = orc.adam_update_ref(th[0], gY, *z0(gY), 1, 1e-2, 0.5, 0.9, 1e-8)[0]
+    newU = orc.adam_update_ref(th[1], gu, *z0(gu), 1, 1e-2, 0.5, 0.9, 1e-8)[0]
+    assert rel_err(tr.out.grads[0].cpu().numpy(), gY) <= 1e-4 and rel_err(tr.out.grads[1].cpu().numpy(), gu) <= 1e-4
+    for got, ref in zip(tr.params, (newY, newU, newD)):
+        # Adam's first step moves every weight by ~lr: compare the UPDATE, whose sign pattern is the gradient's
+        assert np.abs(got.cpu().numpy() - ref).max() <= 2e-3 * 1e-2 + 1e-7
+    assert np.allclose(losses, lref, rtol=1e-3, atol=1e-6)
+    pg.close()
