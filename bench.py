@@ -402,6 +402,59 @@ def run_config(cfg, device, steps, warmup, rank, world, with_roofline=True, seed
     return res
 
 
+def run_next_rows(device, steps=10, warmup=3):
+    """NEXT-2 and NEXT-3 timed on c2's networks: the step with f at per-sample free sensors fed to the critic,
+    and the step with a two-level hierarchy of 20 critics.  Device-resident inputs, CUDA events, eager launches."""
+    import torch
+    from paper_1910_13444_b200 import PiGan
+    cfg = wl.CONFIGS["c2"]
+    out = {}
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(device)
+
+    def timed(fn):
+        for _ in range(warmup):
+            fn()
+        torch.cuda.synchronize(device)
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        for a, b in ev:
+            a.record(); fn(); b.record()
+        torch.cuda.synchronize(device)
+        return float(np.mean([a.elapsed_time(b) for a, b in ev]))
+
+    inp = wl.make_inputs(cfg)
+    # NEXT-2: F = 2000 free sensors per sample (the paper's count for the top-level subdomain, P:232), critic input 2S + 3F
+    F = 2000
+    d_in = 2 * cfg.S + 3 * F
+    thD = wl.round_to_precision(wl.xavier_params(np.random.default_rng(2002), d_in, cfg.LD, cfg.HD), cfg.precision)
+    xy_free = wl.free_sensor_points(cfg, F)
+    real = np.random.default_rng(2003).normal(size=(cfg.N, d_in)).astype(np.float32)
+    real[:, 2 * cfg.S:2 * cfg.S + F] = 0.0
+    pg = PiGan(latent_dim=cfg.m, gen_hidden=cfg.L, gen_width=cfg.H, disc_hidden=cfg.LD, disc_width=cfg.HD, n_samples=cfg.N, n_colloc=F,
+               n_sensors=cfg.S, precision=cfg.precision, pde_weight=0.0, n_free=F, device=device)
+    a = [t(inp["theta_Y"]), t(inp["theta_u"]), t(thD), t(xy_free), t(inp["xy_sensors"]), t(inp["z"]), t(real), t(inp["eps"])]
+    o = pg.train_step_grads(a[0], a[1], a[2], a[3], None, a[4], a[5], a[6], a[7], 1.0)
+    ms = timed(lambda: pg.train_step_grads(a[0], a[1], a[2], a[3], None, a[4], a[5], a[6], a[7], 1.0, out=o))
+    out["next2_free_sensors"] = {"workload": f"c2 networks, {cfg.N} samples x {F} free sensors each, critic input {d_in}", "ms_per_step": ms,
+                                 "value": cfg.N * F / (ms * 1e-3), "unit": "sample*free-sensor-points/s", "found_inf": int(o[4].item())}
+    pg.close()
+    # NEXT-3: levels of 1 and 19 subdomains (P:141), 10 sensors per critic
+    levels, per = [1, 19], 10
+    K = sum(levels)
+    rng = np.random.default_rng(2004)
+    sens = np.stack([np.sort(rng.choice(cfg.S, size=per, replace=False)) for _ in range(K)])
+    subsets = np.concatenate([sens, cfg.S + sens], axis=1).astype(np.int32)
+    thDs = np.stack([wl.round_to_precision(wl.xavier_params(np.random.default_rng(2100 + k), 2 * per, cfg.LD, cfg.HD), cfg.precision) for k in range(K)])
+    w = np.concatenate([np.full(n, 1.0 / (len(levels) * n)) for n in levels])
+    real = np.random.default_rng(2005).normal(size=(cfg.N, 2 * cfg.S)).astype(np.float32)
+    pg = PiGan.from_config(cfg, n_critics=K, critic_inputs=2 * per, device=device)
+    a = [t(inp["theta_Y"]), t(inp["theta_u"]), t(thDs), t(subsets), t(inp["xy_colloc"]), t(inp["f"]), t(inp["xy_sensors"]), t(inp["z"]), t(real), t(inp["eps"])]
+    ms = timed(lambda: pg.train_step_grads_hier(a[0], a[1], a[2], a[3], w, a[4], a[5], a[6], a[7], a[8], a[9], 1.0))
+    out["next3_hierarchical_critics"] = {"workload": f"c2, {K} critics in levels {levels}, {per} sensors each", "ms_per_step": ms,
+                                         "value": cfg.N * cfg.P / (ms * 1e-3), "unit": UNIT}
+    pg.close()
+    return out
+
+
 def summarize(cfg, res, n_gpus, steps, warmup, t_max_ms):
     units = cfg.N * cfg.P
     value = whole_job_value(units, n_gpus, t_max_ms)
@@ -502,6 +555,7 @@ def main():
             per["t2"]["paper_table2"] = {"flop_per_step_paper": 12.3e12, "flop_per_step_8_channel_model": 6 * (2000 * 8 + 200) * 20 * 2 * 1024 * 1024 * 3,
                                          "flop_per_step_this_build": wl.step_flops(wl.TABLE2)["total"], "paper_step_s_v100": 12.3e12 / 38.6e12,
                                          "note": "the shared trunk needs 5 jet channel passes where the paper's TF autodiff graph counts 8; 2025 grid points stand in for the 2000 f sensors"}
+            per.update(run_next_rows(device))
             line["per_config"] = per
         if not args.no_cpu_baseline:
             val, sec, cores, sample = time_oracle(cfg)

@@ -164,6 +164,12 @@ template <typename T>
 void first_layer_bwd(Launcher& L, int C, const NetShape& s, const float* xy, const ChunkGeom& g, const T* ahat,
                      float* gW1 /* flat grads base of this net */, float* An /*[N][H]*/, const float* amax);
 void finalize_first_layer(Launcher& L, const NetShape& s, int N, const float* An, const float* z, float* grads);
+// fp32 mode, H = 32 / 64 (gen_fused_f32.cu): the whole generator pass of a chunk in one kernel (a warp per row)
+bool gen_fused_f32_supported(const NetShape& s);
+void gen_fused_f32_fwd(Launcher& L, int C, const NetShape& s, const float* theta, const float* Zp, const float* xy, const ChunkGeom& g, float* o,
+                       long long o_stride);
+void gen_fused_f32_bwd(Launcher& L, int C, const NetShape& s, const float* theta, const float* Zp, const float* xy, const ChunkGeom& g,
+                       const float* ohat /*[C][R_ld]*/, float* grads, float* An);
 // NEXT-1 (shared trunk, two heads, skip connections): see gen_kernels.cu
 template <typename T>
 void top_act_bwd2(Launcher& L, int C, int H, const ChunkGeom& g, const float* w_out /*[2][H]*/, const float* ohat0, const float* ohat1, const T* h,

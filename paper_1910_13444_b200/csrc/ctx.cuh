@@ -135,6 +135,10 @@ void gen_forward_chunk(pigan_ctx* c, int n, const pigan_ctx::HBuf& hb, const flo
   // split (16-bit modes, value channel only): activations are carried as two 16-bit planes hi + lo, so that the
   // snapshot X_fake the critic sees is accurate to ~2^-17 (the loss values are compared at 1e-3 relative)
   split = split && C == 1 && c->cfg.precision != PIGAN_FP32;
+  if (c->cfg.precision == PIGAN_FP32 && gen_fused_f32_supported(s)) {     // narrow fp32 nets: one kernel, no activation planes
+    gen_fused_f32_fwd(L, C, s, theta, c->net[n].Zp, xy, g, o, o_stride);
+    return;
+  }
   first_layer_fwd<T>(L, C, s, theta, c->net[n].Zp, xy, g, (T*)hb.at(1), split);
   // the output layer (a4) rides in the epilogue of the last hidden layer where the kernels support it
   const bool fuse_out = c->cfg.precision != PIGAN_FP32 && s.L >= 2 && tc_out_dot_fusable(L, H);
@@ -164,6 +168,10 @@ void gen_backward_chunk(pigan_ctx* c, int n, const pigan_ctx::HBuf& hb, const fl
   const long long pl = (long long)H * g.R_ld;
   int cur = 0;
   const float* amax = c->cfg.precision == PIGAN_FP32 ? nullptr : c->amax + n;
+  if (c->cfg.precision == PIGAN_FP32 && gen_fused_f32_supported(s)) {     // recomputes the forward of every row (gen_fused_f32.cu)
+    gen_fused_f32_bwd(L, C, s, theta, c->net[n].Zp, xy, g, c->net[n].oh, grads, c->net[n].An);
+    return;
+  }
   jet_act_bwd_launch<T>(L, C, H, g, nullptr, theta + s.W_off(s.L + 1), c->net[n].oh, (const T*)hb.at(s.L),
                         (T*)c->net[n].ah[cur], grads + s.b_off(s.L),
                         grads + s.W_off(s.L + 1), grads + s.b_off(s.L + 1), amax);

@@ -47,6 +47,13 @@ def test_c1_jets(order):
     assert max(errs.values()) <= 1e-4, errs
 
 
+def test_fp32_width_64_four_layers():
+    """fp32 narrow-generator kernel with two units per lane (H = 64) and three hidden-to-hidden layers; width 96 takes the
+    layer-by-layer SGEMM path."""
+    check_step(dataclasses.replace(wl.CONFIGS["c1"], name="c1-H64", H=64, L=4, HD=64, G=9, N=6, S=7))
+    check_step(dataclasses.replace(wl.CONFIGS["c1"], name="c1-H96", H=96, L=3, HD=48, G=6, N=4, S=5))
+
+
 def test_single_hidden_layer_network():
     cfg = dataclasses.replace(wl.CONFIGS["c1"], name="c1-L1", L=1, LD=1)               # degenerate depth
     check_step(cfg)
