@@ -249,6 +249,7 @@ class GpuWorkload:
             d[k].copy_(self.host[k], non_blocking=True)
         self.step()
         self.host_out.copy_(self.out[3], non_blocking=True)
+        self.torch.cuda.current_stream(self.device).synchronize()   # the host holds this step's losses before the next step is issued
 
     def jet_pass(self):
         """The jet evaluation alone (a1-a4 forward): G_u at order 2 and G_logk at order 1 on every (sample, point)."""

@@ -50,3 +50,20 @@ def test_no_cpu_fallback():
         pytest.skip("a GPU is present")
     with pytest.raises(pkg.PiganError):
         pkg.PiGan(latent_dim=4, gen_hidden=3, gen_width=32, disc_hidden=3, disc_width=32, n_samples=16, n_colloc=64, n_sensors=10)
+
+
+def test_create_validates_the_next_row_fields():
+    """gen_variant / n_free / n_critics are checked before any CUDA call."""
+    lib = pkg.load_library()
+    ctx = ctypes.c_void_p()
+    mk = lambda disc_in, variant, n_free, n_critics, n_colloc=64: pkg._Config(pkg._MlpShape(6, 3, 32), pkg._MlpShape(disc_in, 3, 32), 4, 16, n_colloc, 10, 0,
+                                                                             10.0, 1.0, 0, 0, 0, variant, n_free, n_critics)
+    assert lib.pigan_create(ctypes.byref(mk(20, 3, 0, 0)), None, ctypes.byref(ctx)) == 1          # unknown gen_variant
+    assert lib.pigan_create(ctypes.byref(mk(20, 0, -1, 0)), None, ctypes.byref(ctx)) == 1         # negative n_free
+    assert lib.pigan_create(ctypes.byref(mk(20, 0, 8, 0, n_colloc=8)), None, ctypes.byref(ctx)) == 2     # free sensors: disc.in_dim must be 2S + 3F
+    assert lib.pigan_create(ctypes.byref(mk(44, 0, 8, 0, n_colloc=64)), None, ctypes.byref(ctx)) == 2    # ... and n_colloc = F
+    assert lib.pigan_create(ctypes.byref(mk(44, 1, 8, 0, n_colloc=8)), None, ctypes.byref(ctx)) == 5     # free sensors with the shared trunk: unsupported
+    assert lib.pigan_create(ctypes.byref(mk(24, 0, 0, 3)), None, ctypes.byref(ctx)) == 2          # a critic cannot see more than the 2S columns
+    assert lib.pigan_create(ctypes.byref(mk(8, 2, 0, 3)), None, ctypes.byref(ctx)) == 5           # hierarchical critics with the trunk: unsupported
+    assert not ctx.value
+    assert pkg.trunk_param_count(6, 3, 32) == pkg.param_count(6, 3, 32) + 33
