@@ -617,7 +617,7 @@ static void launch_jet2(Launcher& L, const CUtensorMap& a, const CUtensorMap& b,
   const int tiles = (p.H / 256) * p.n_row_tiles;
   const int clusters = std::min(tiles, L.num_sms / 2);
   kern<<<2 * clusters, k2Threads, Cfg::kSmemBytes, L.stream>>>(a, b, t, p);
-  L.check((MODE == 0 || MODE == 4) ? "jet_layer_fwd" : (MODE == 2 || MODE == 5) ? "jet_layer_fwd_split" : "jet_layer_bwd");
+  L.check(((MODE == 0 && !p.linear) || MODE == 4) ? "jet_layer_fwd" : (MODE == 2 || MODE == 5) ? "jet_layer_fwd_split" : "jet_layer_bwd");   // linear = a dgrad GEMM
 }
 
 template <int MODE>

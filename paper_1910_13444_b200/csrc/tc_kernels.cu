@@ -469,7 +469,7 @@ static void launch_jet(Launcher& L, const CUtensorMap& a, const CUtensorMap& b, 
   const int tiles = (p.H / kBM) * p.n_row_tiles;
   const int grid = std::min(tiles, L.num_sms);
   kern<<<grid, 256, Cfg::kSmemBytes, L.stream>>>(a, b, o, t, p);
-  L.check(MODE == 0 ? "jet_layer_fwd" : MODE == 2 ? "jet_layer_fwd_split" : "jet_layer_bwd");
+  L.check((MODE == 0 && !p.linear) ? "jet_layer_fwd" : MODE == 2 ? "jet_layer_fwd_split" : "jet_layer_bwd");   // linear = a dgrad GEMM
 }
 
 template <int MODE>
