@@ -52,6 +52,7 @@ pigan_status train_step_impl(pigan_ctx* c, const float* thY, const float* thU, c
   const long long srows = (long long)N * S;
   int sc = 0;
   for (long long row0 = 0; row0 < srows; row0 += c->R_ld, ++sc) {
+    NvtxRange nr("pigan:sensor_forward");
     ChunkGeom g = make_geom(c, row0, srows, S);
     for (int n = 0; n < 2; ++n) {
       gen_forward_chunk<T>(c, n, c->hsens(n, sc), th[n], 1, xy_s, g, c->net[n].o, c->R_ld, /*split=*/true);
@@ -59,6 +60,7 @@ pigan_status train_step_impl(pigan_ctx* c, const float* thY, const float* thU, c
     }
   }
   // ---- a7-a9: critic losses and gradient; dX rows [0, N) = (1/N) grad_X D(X_fake) ----
+  nvtxRangePushA("pigan:critic");
   if (c->hier.K > 0) {
     hier_critic_stage(c, thD, real, eps, gD);               // NEXT-3: K critics on column subsets (hier.cu)
   } else if (critic_fused_supported(ds)) {
@@ -73,9 +75,11 @@ pigan_status train_step_impl(pigan_ctx* c, const float* thY, const float* thU, c
     critic_backward(L, ds, thD, c->cw.X, c->cw.g, 2 * N, gstride, c->seed, gD, c->dX, c->cw.t0, c->cw.t1);
     critic_gp(L, ds, thD, c->cw.X + (size_t)2 * N * d, c->cw.g + (size_t)2 * N * HD, N, gstride, cfg.gp_lambda, c->cw, gD, nullptr);
   }
+  nvtxRangePop();
   // ---- O7 + a10 on the sensor rows: dL_G/dX_fake = -(1/N) grad_X D(X_fake), value channel only ----
   sc = 0;
   for (long long row0 = 0; row0 < srows; row0 += c->R_ld, ++sc) {
+    NvtxRange nr("pigan:sensor_backward");
     ChunkGeom g = make_geom(c, row0, srows, S);
     for (int n = 0; n < 2; ++n) {
       cudaMemsetAsync(c->amax + n, 0, 4, st);
@@ -87,6 +91,7 @@ pigan_status train_step_impl(pigan_ctx* c, const float* thY, const float* thU, c
   const long long crows = (long long)N * P;
   const float seed_scale = (float)(2.0 * cfg.pde_weight / (double)crows * loss_scale);
   for (long long row0 = 0; row0 < crows; row0 += c->R_ld) {
+    NvtxRange nr("pigan:collocation_chunk");
     ChunkGeom g = make_geom(c, row0, crows, P);
     gen_forward_chunk<T>(c, 0, c->hcol(0), thY, 3, xy_c, g, c->net[0].o, c->R_ld);
     gen_forward_chunk<T>(c, 1, c->hcol(1), thU, 5, xy_c, g, c->net[1].o, c->R_ld);

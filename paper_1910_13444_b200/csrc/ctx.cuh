@@ -6,6 +6,8 @@
 #include <string>
 #include <vector>
 
+#include <nvtx3/nvToolsExt.h>
+
 #include "common.cuh"
 
 namespace pigan {
@@ -105,6 +107,12 @@ inline pigan_status finish(pigan_ctx* c) {
   c->err.clear();
   return PIGAN_OK;
 }
+
+// NVTX range per phase of a step (tracing): visible in nsys / ncu --nvtx; a no-op without a tool attached
+struct NvtxRange {
+  explicit NvtxRange(const char* name) { nvtxRangePushA(name); }
+  ~NvtxRange() { nvtxRangePop(); }
+};
 
 inline size_t round_up(size_t a, size_t b) { return (a + b - 1) / b * b; }
 

@@ -5,8 +5,8 @@
 // memory (W^T for the forward product, W for the transposed one, both read conflict-free), a layer's matrix-vector products
 // broadcast the previous layer's activations lane by lane with warp shuffles, and the reductions over units (output dot)
 // are warp-shuffle sums.  The reverse kernel recomputes the forward of its row (no activation planes exist in this path),
-// keeps the per-layer jets in a per-warp shared-memory stash, accumulates the weight gradients of the CTA in shared memory
-// and flushes them with one fp32 atomic per entry and CTA.
+// keeps the per-layer jets and adjoints in per-warp shared-memory stashes; the CTA then accumulates the weight gradients of its
+// 8 rows cooperatively in registers and flushes them with one fp32 atomic per entry and CTA.
 #include "common.cuh"
 
 namespace pigan {
@@ -30,9 +30,9 @@ __host__ __device__ inline GfSmem gf_layout(int L, int H, int C, bool bwd) {
   const int hl = (L - 1) * H * H;
   m.WT = 0;
   m.W = m.WT + hl;
-  m.gW = m.W + (bwd ? hl : 0);
-  m.gb = m.gW + (bwd ? hl : 0);
-  m.stash = m.gb + (bwd ? L * H : 0);
+  m.gW = m.W + (bwd ? hl : 0);                               // reverse kernel: the adjoint stash [warp][l][c][unit]
+  m.gb = m.gW;
+  m.stash = m.gW + (bwd ? kGfWarps * L * C * H : 0);         // the jet stash
   m.total = m.stash + (bwd ? kGfWarps * L * C * H : 0);
   return m;
 }
@@ -47,7 +47,7 @@ __device__ __forceinline__ void gf_layer_matvec(const float* __restrict__ WT, co
     for (int u = 0; u < UPL; ++u) a[c][u] = (c == 0) ? bias[lane + 32 * u] : 0.f;
 #pragma unroll
   for (int ku = 0; ku < UPL; ++ku) {
-#pragma unroll 4
+#pragma unroll 16
     for (int kl = 0; kl < 32; ++kl) {
       float w[UPL];
 #pragma unroll
@@ -134,12 +134,20 @@ __global__ void __launch_bounds__(kGfThreads) gen_fused_fwd_kernel(NetShape s, c
   }
 }
 
+// Reverse sweep.  The CTA works on batches of 8 rows (one per warp).  Each warp recomputes the forward of its row (jets of every
+// layer -> shared-memory stash), runs the reverse sweep and leaves the pre-activation adjoints ahat^l in a second stash; after a
+// barrier the 256 threads of the CTA accumulate the batch's outer products  W_hat_l[j][k] += sum_{rows, c} ahat_c[j] h^{l-1}_c[k]
+// into REGISTERS (thread t owns entries t, t + 256, ... of every layer) -- no shared-memory atomics -- and flush them with one
+// global fp32 atomic per entry at the end of the kernel.
+constexpr int kGfMaxOwn = 48;      // (L - 1) H^2 / 256 entries per thread: H = 64, L = 4
+
 template <int UPL, int C>
-__global__ void __launch_bounds__(kGfThreads) gen_fused_bwd_kernel(NetShape s, const float* __restrict__ theta, const float* __restrict__ Zp,
-                                                                   const float* __restrict__ xy, ChunkGeom g, const float* __restrict__ ohat,
-                                                                   float* __restrict__ grads, float* __restrict__ An) {
+__global__ void __launch_bounds__(kGfThreads, 1) gen_fused_bwd_kernel(NetShape s, const float* __restrict__ theta, const float* __restrict__ Zp,
+                                                                      const float* __restrict__ xy, ChunkGeom g, const float* __restrict__ ohat,
+                                                                      float* __restrict__ grads, float* __restrict__ An) {
   extern __shared__ float sm[];
-  const int H = s.H, L = s.L, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  constexpr int H = 32 * UPL;
+  const int L = s.L, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const GfSmem m = gf_layout(L, H, C, true);
   for (int l = 2; l <= L; ++l) {
     const float* W = theta + s.W_off(l);
@@ -147,101 +155,119 @@ __global__ void __launch_bounds__(kGfThreads) gen_fused_bwd_kernel(NetShape s, c
     float* w = sm + m.W + (l - 2) * H * H;
     for (int i = threadIdx.x; i < H * H; i += kGfThreads) { const float v = W[i]; w[i] = v; wt[(i % H) * H + i / H] = v; }
   }
-  for (int i = threadIdx.x; i < (L - 1) * H * H + L * H; i += kGfThreads) sm[m.gW + i] = 0.f;     // gW (transposed: [k][j]) and gb are contiguous
   __syncthreads();
-  float* stash = sm + m.stash + warp * (L * C * H);           // [l][c][unit] jets of this warp's row
+  float* stash_h = sm + m.stash;                              // [warp][l][c][unit] jets h^l of the batch's rows
+  float* stash_a = sm + m.gW;                                 // [warp][l][c][unit] adjoints ahat^l
+  float* my_h = stash_h + warp * (L * C * H);
+  float* my_a = stash_a + warp * (L * C * H);
+  const int n_own = (L - 1) * H * H / kGfThreads;             // weight-gradient entries this thread accumulates
+  float gw[kGfMaxOwn];
+#pragma unroll
+  for (int e = 0; e < kGfMaxOwn; ++e) gw[e] = 0.f;
+  float gbias = 0.f;                                          // thread t < L * H owns b_hat_{t / H + 1}[t % H]
   float wo[UPL], g_wo[UPL], g_wx[UPL], g_wy[UPL];
 #pragma unroll
   for (int u = 0; u < UPL; ++u) { wo[u] = theta[s.W_off(L + 1) + lane + 32 * u]; g_wo[u] = 0.f; g_wx[u] = 0.f; g_wy[u] = 0.f; }
   float g_bo = 0.f;
-  for (int r = blockIdx.x * kGfWarps + warp; r < g.valid; r += gridDim.x * kGfWarps) {
-    int n; float x, y;
-    gf_row_geom(g, r, xy, n, x, y);
-    float h[C][UPL], a[C][UPL];
-    // ---- forward of this row, jets of every layer kept in the stash ----
-    gf_first<UPL, C>(s, theta, Zp, n, x, y, lane, h);
-    for (int l = 1;; ++l) {
+  const int n_batches = (g.valid + kGfWarps - 1) / kGfWarps;
+  for (int b = blockIdx.x; b < n_batches; b += gridDim.x) {
+    const int r = b * kGfWarps + warp;
+    if (r < g.valid) {
+      int n; float x, y;
+      gf_row_geom(g, r, xy, n, x, y);
+      float h[C][UPL], a[C][UPL];
+      // ---- forward of this row, jets of every layer kept in the stash ----
+      gf_first<UPL, C>(s, theta, Zp, n, x, y, lane, h);
+      for (int l = 1;; ++l) {
+#pragma unroll
+        for (int c = 0; c < C; ++c)
+#pragma unroll
+          for (int u = 0; u < UPL; ++u) my_h[((l - 1) * C + c) * H + lane + 32 * u] = h[c][u];
+        if (l == L) break;
+        gf_layer_matvec<UPL, C>(sm + m.WT + (l - 1) * H * H, theta + s.b_off(l + 1), H, lane, h, a);
+        gf_act<UPL, C>(a, h);
+      }
+      // ---- reverse: output layer ----
+      float oh[C], hh[C][UPL];
+#pragma unroll
+      for (int c = 0; c < C; ++c) oh[c] = ohat[(size_t)c * g.R_ld + r];
+      g_bo += oh[0];
 #pragma unroll
       for (int c = 0; c < C; ++c)
 #pragma unroll
-        for (int u = 0; u < UPL; ++u) stash[((l - 1) * C + c) * H + lane + 32 * u] = h[c][u];
-      if (l == L) break;
-      gf_layer_matvec<UPL, C>(sm + m.WT + (l - 1) * H * H, theta + s.b_off(l + 1), H, lane, h, a);
-      gf_act<UPL, C>(a, h);
-    }
-    __syncwarp();                                             // the stash is read across lanes below
-    // ---- reverse: output layer ----
-    float oh[C], hh[C][UPL];
-#pragma unroll
-    for (int c = 0; c < C; ++c) oh[c] = ohat[(size_t)c * g.R_ld + r];
-    g_bo += oh[0];
-#pragma unroll
-    for (int c = 0; c < C; ++c)
-#pragma unroll
-      for (int u = 0; u < UPL; ++u) { hh[c][u] = wo[u] * oh[c]; g_wo[u] = fmaf(oh[c], h[c][u], g_wo[u]); }
-    // ---- reverse: tanh layers L .. 1 ----
-    for (int l = L; l >= 1; --l) {
-      float aa[C][UPL];
-#pragma unroll
-      for (int u = 0; u < UPL; ++u) {
-        float hj[5], hx[5], av[5];
-#pragma unroll
-        for (int c = 0; c < C; ++c) { hj[c] = stash[((l - 1) * C + c) * H + lane + 32 * u]; hx[c] = hh[c][u]; }
-        jet_act_bwd<C>(hj, hx, av);
-#pragma unroll
-        for (int c = 0; c < C; ++c) aa[c][u] = av[c];
-        atomicAdd(sm + m.gb + (l - 1) * H + lane + 32 * u, av[0]);
-      }
-      if (l == 1) {
+        for (int u = 0; u < UPL; ++u) { hh[c][u] = wo[u] * oh[c]; g_wo[u] = fmaf(oh[c], h[c][u], g_wo[u]); }
+      // ---- reverse: tanh layers L .. 1 ----
+      for (int l = L; l >= 1; --l) {
+        float aa[C][UPL];
 #pragma unroll
         for (int u = 0; u < UPL; ++u) {
-          g_wx[u] += aa[0][u] * x + (C >= 3 ? aa[1][u] : 0.f);
-          g_wy[u] += aa[0][u] * y + (C >= 3 ? aa[2][u] : 0.f);
-          atomicAdd(An + (size_t)n * H + lane + 32 * u, aa[0][u]);
+          float hj[5], hx[5], av[5];
+#pragma unroll
+          for (int c = 0; c < C; ++c) { hj[c] = my_h[((l - 1) * C + c) * H + lane + 32 * u]; hx[c] = hh[c][u]; }
+          jet_act_bwd<C>(hj, hx, av);
+#pragma unroll
+          for (int c = 0; c < C; ++c) { aa[c][u] = av[c]; my_a[((l - 1) * C + c) * H + lane + 32 * u] = av[c]; }
         }
-        break;
-      }
-      // W_hat_l[j][k] += sum_c aa_c[j] h^{l-1}_c[k]  (kept transposed in smem: [k][j], lanes j contiguous)
-      // hhat^{l-1}_c[k] = sum_j W_l[j][k] aa_c[j]
-      float* gWl = sm + m.gW + (l - 2) * H * H;
-      const float* Wl = sm + m.W + (l - 2) * H * H;
-      const float* hp = stash + (l - 2) * C * H;
+        if (l == 1) {
 #pragma unroll
-      for (int c = 0; c < C; ++c)
-#pragma unroll
-        for (int u = 0; u < UPL; ++u) hh[c][u] = 0.f;
-      for (int k = 0; k < H; ++k) {
-        float acc[UPL];
-#pragma unroll
-        for (int u = 0; u < UPL; ++u) acc[u] = 0.f;
-#pragma unroll
-        for (int c = 0; c < C; ++c) {
-          const float hv = hp[c * H + k];                      // broadcast read of this warp's stash
-#pragma unroll
-          for (int u = 0; u < UPL; ++u) acc[u] = fmaf(aa[c][u], hv, acc[u]);
+          for (int u = 0; u < UPL; ++u) {
+            g_wx[u] += aa[0][u] * x + (C >= 3 ? aa[1][u] : 0.f);
+            g_wy[u] += aa[0][u] * y + (C >= 3 ? aa[2][u] : 0.f);
+            atomicAdd(An + (size_t)n * H + lane + 32 * u, aa[0][u]);
+          }
+          break;
         }
+        // hhat^{l-1}_c[k] = sum_j W_l[j][k] ahat_c[j]: lane k accumulates, ahat_c[j] arrives by shuffle, W_l[j][k] from smem
+        const float* Wl = sm + m.W + (l - 2) * H * H;
 #pragma unroll
-        for (int u = 0; u < UPL; ++u) atomicAdd(gWl + k * H + lane + 32 * u, acc[u]);
-      }
+        for (int c = 0; c < C; ++c)
 #pragma unroll
-      for (int ju = 0; ju < UPL; ++ju) {
-#pragma unroll 4
-        for (int jl = 0; jl < 32; ++jl) {
-          float w[UPL];
+          for (int u = 0; u < UPL; ++u) hh[c][u] = 0.f;
 #pragma unroll
-          for (int u = 0; u < UPL; ++u) w[u] = Wl[(ju * 32 + jl) * H + lane + 32 * u];
+        for (int ju = 0; ju < UPL; ++ju) {
+#pragma unroll 16
+          for (int jl = 0; jl < 32; ++jl) {
+            float w[UPL];
 #pragma unroll
-          for (int c = 0; c < C; ++c) {
-            const float av = __shfl_sync(0xffffffffu, aa[c][ju], jl);
+            for (int u = 0; u < UPL; ++u) w[u] = Wl[(ju * 32 + jl) * H + lane + 32 * u];
 #pragma unroll
-            for (int u = 0; u < UPL; ++u) hh[c][u] = fmaf(w[u], av, hh[c][u]);
+            for (int c = 0; c < C; ++c) {
+              const float av = __shfl_sync(0xffffffffu, aa[c][ju], jl);
+#pragma unroll
+              for (int u = 0; u < UPL; ++u) hh[c][u] = fmaf(w[u], av, hh[c][u]);
+            }
           }
         }
       }
+    } else {
+      for (int i = lane; i < L * C * H; i += 32) { my_a[i] = 0.f; my_h[i] = 0.f; }   // a missing row adds nothing below
     }
-    __syncwarp();
+    __syncthreads();
+    // ---- the batch's weight and bias gradients, cooperatively: thread t owns entries e = t + 256 q of [l][j][k] ----
+    for (int q = 0; q < n_own; ++q) {
+      const int e = threadIdx.x + q * kGfThreads;
+      const int l2 = e / (H * H), jk = e - l2 * (H * H), jj = jk / H, kk = jk - jj * H;    // layer l = l2 + 2
+      float acc = 0.f;
+#pragma unroll
+      for (int w = 0; w < kGfWarps; ++w) {
+        const float* ap = stash_a + w * (L * C * H) + (l2 + 1) * C * H + jj;            // ahat^{l}_c[jj]
+        const float* hp = stash_h + w * (L * C * H) + l2 * C * H + kk;                  // h^{l-1}_c[kk]
+#pragma unroll
+        for (int c = 0; c < C; ++c) acc = fmaf(ap[c * H], hp[c * H], acc);
+      }
+#pragma unroll
+      for (int qq = 0; qq < kGfMaxOwn; ++qq) if (qq == q) gw[qq] += acc;
+    }
+    if (threadIdx.x < L * H) {
+      const int l0 = threadIdx.x / H, jj = threadIdx.x - l0 * H;
+      float acc = 0.f;
+#pragma unroll
+      for (int w = 0; w < kGfWarps; ++w) acc += stash_a[w * (L * C * H) + l0 * C * H + jj];
+      gbias += acc;
+    }
+    __syncthreads();
   }
-  // ---- flush: per-lane register sums, then the CTA's shared-memory sums ----
+  // ---- flush ----
 #pragma unroll
   for (int u = 0; u < UPL; ++u) {
     const int j = lane + 32 * u;
@@ -250,19 +276,22 @@ __global__ void __launch_bounds__(kGfThreads) gen_fused_bwd_kernel(NetShape s, c
     atomicAdd(grads + (size_t)j * s.in_dim + 1, g_wy[u]);
   }
   if (lane == 0) atomicAdd(grads + s.b_off(L + 1), g_bo);     // every lane carries the same sum of ohat_0: one of them adds it
-  __syncthreads();
-  for (int l = 2; l <= L; ++l) {
-    const float* gWl = sm + m.gW + (l - 2) * H * H;
-    float* dst = grads + s.W_off(l);
-    for (int i = threadIdx.x; i < H * H; i += kGfThreads) atomicAdd(dst + i, gWl[(i % H) * H + i / H]);
+  for (int q = 0; q < n_own; ++q) {
+    const int e = threadIdx.x + q * kGfThreads;
+    const int l2 = e / (H * H), jk = e - l2 * (H * H);
+    float v = 0.f;
+#pragma unroll
+    for (int qq = 0; qq < kGfMaxOwn; ++qq) if (qq == q) v = gw[qq];
+    atomicAdd(grads + s.W_off(l2 + 2) + jk, v);
   }
-  for (int i = threadIdx.x; i < L * H; i += kGfThreads) atomicAdd(grads + s.b_off(i / H + 1) + i % H, sm[m.gb + i]);
+  if (threadIdx.x < L * H) atomicAdd(grads + s.b_off(threadIdx.x / H + 1) + threadIdx.x % H, gbias);
 }
 
 }  // namespace
 
 bool gen_fused_f32_supported(const NetShape& s) {
   if (!(s.H == 32 || s.H == 64) || s.L < 1 || s.heads != 1) return false;
+  if ((s.L - 1) * s.H * s.H / kGfThreads > kGfMaxOwn || s.L * s.H > kGfThreads) return false;
   return (size_t)gf_layout(s.L, s.H, 5, true).total * 4 <= 200 * 1024;
 }
 
