@@ -329,7 +329,7 @@ def run_config(cfg, device, steps, warmup, rank, world, with_roofline=True, seed
     del w.jet_out, w.jet_out2
     # roofline of the dominant kernel class (the tcgen05 jet GEMMs: forward, dgrad+adjoint, wgrad)
     if with_roofline:
-        tc = {k: v for k, v in prof.items() if k in ("jet_layer_fwd", "jet_layer_bwd", "wgrad")}
+        tc = {k: v for k, v in prof.items() if k in ("jet_layer_fwd", "jet_layer_bwd", "wgrad", "jet_layer_bwd_wgrad")}
         per_step = {k: [v[0] / steps, v[1] / steps] for k, v in prof.items()}
         tc_ms = sum(v[1] for v in tc.values()) / steps
         total_ms = sum(v[1] for v in prof.values()) / steps
@@ -349,17 +349,21 @@ def run_config(cfg, device, steps, warmup, rank, world, with_roofline=True, seed
             rowsC = cfg.N * cfg.P * chan + cfg.N * cfg.S * nets
             pb = 2 * cfg.H                                        # bytes of one row of one 16-bit plane
             Lh = cfg.L - 1
-            cls_bytes = {"jet_layer_fwd": 2 * rowsC * pb * Lh, "jet_layer_bwd": rowsC * pb * (3 * Lh - 1), "wgrad": 2 * rowsC * pb * Lh}
+            # width 256: dgrad and wgrad of a layer are ONE kernel (jet_layer_bwd_wgrad): two of the three GEMMs, planes read once
+            cls_bytes = {"jet_layer_fwd": 2 * rowsC * pb * Lh, "jet_layer_bwd": rowsC * pb * (3 * Lh - 1), "wgrad": 2 * rowsC * pb * Lh,
+                         "jet_layer_bwd_wgrad": rowsC * pb * (3 * Lh - 1)}
+            cls_gemms = {"jet_layer_fwd": 1, "jet_layer_bwd": 1, "wgrad": 1, "jet_layer_bwd_wgrad": 2}
             prof_ncu = ncu_profile(cfg.name)
             per_kernel = {}
             for k, v in tc.items():
                 if v[1] <= 0:
                     continue
                 t_ms = v[1] / steps
-                t_tensor = alg / 3 / (peak * 1e12) * 1e3
+                alg_k = alg * cls_gemms[k] / 3
+                t_tensor = alg_k / (peak * 1e12) * 1e3
                 t_hbm = cls_bytes[k] / (peaks["hbm_gbs"] * 1e9) * 1e3
                 pct = [d["tensor_pct"] for kk, d in prof_ncu.items() if kk.startswith(k + "(C=5") or kk == k]
-                per_kernel[k] = {"tflops": round(alg / 3 / (t_ms * 1e-3) / 1e12, 1), "gbs_algorithmic": round(cls_bytes[k] / (t_ms * 1e-3) / 1e9, 1),
+                per_kernel[k] = {"tflops": round(alg_k / (t_ms * 1e-3) / 1e12, 1), "gbs_algorithmic": round(cls_bytes[k] / (t_ms * 1e-3) / 1e9, 1),
                                  "bound": "tensor" if t_tensor >= t_hbm else "hbm", "frac": round(max(t_tensor, t_hbm) / t_ms, 4),
                                  "tensor_pipe_active_pct_ncu": pct[0] if pct else None}
             dom = max(tc, key=lambda k: tc[k][1])

@@ -229,8 +229,9 @@ struct OutDot { const float* w_out; const float* b_out; float* o; long long o_st
 bool tc_out_dot_fusable(const Launcher& L, int H);
 // hidden layer l forward: h_in [C][H][R_ld] -> h_out [C][H][R_ld]   (fused tanh-jet epilogue)
 // linear: plain GEMM out_c = W in_c (no bias, no tanh) -- the raw adjoint planes hhat = W^T ahat of a skip layer (NEXT-1)
+// reverse: sweep the row tiles last-to-first (CTA-pair kernels; alternating it layer by layer keeps a layer's first reads in L2)
 void tc_layer_fwd(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* w16_l, const float* bias,
-                  const void* h_in, void* h_out, const OutDot* od = nullptr, bool linear = false);
+                  const void* h_in, void* h_out, const OutDot* od = nullptr, bool linear = false, bool reverse = false);
 void tc_layer_fwd_split(Launcher& L, int precision, int H, int R, int R_ld, const void* w16_l, const float* bias, const void* h_in, void* h_out,
                         const OutDot* od = nullptr);
 // dgrad of layer l with the adjoint of layer l-1's tanh fused: ahat_in (layer l) -> ahat_out (layer l-1)
@@ -252,11 +253,18 @@ bool tc_first_layer_fusable(int H, const ChunkGeom& g);
 // ---- the same four on CTA pairs (tc2_kernels.cu, cta_group::2), taken when tc2_supported(H) ---------------------
 bool tc2_supported(const Launcher& L, int H);
 void tc2_layer_fwd(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* w16_l, const float* bias,
-                   const void* h_in, void* h_out, const OutDot* od, bool linear);
+                   const void* h_in, void* h_out, const OutDot* od, bool linear, bool reverse);
 void tc2_layer_fwd_split(Launcher& L, int precision, int H, int R, int R_ld, const void* w16_l, const float* bias, const void* h_in, void* h_out,
                          const OutDot* od);
 void tc2_layer_bwd(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* w16T_l, const void* ahat_in,
                    const void* h_prev, void* ahat_out, float* g_bias_prev, const float* amax, const FirstLayerFuse* fl);
 void tc2_wgrad(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* ahat, const void* h_prev, float* gW, const float* amax);
+
+// ---- width 256: wgrad and dgrad (+ adjoint epilogue) of one layer in ONE kernel (tc2_fused_bwd.cu) --------------------
+// gW (W_hat_l) += sum_c ahat_c h_prev_c^T and ahat_out = J^T (W_l^T ahat_in), b_hat_{l-1} += ...; the planes ahat_in and h_prev
+// cross HBM once instead of twice.  fl != nullptr: layer 2 with the first-layer reduction (no ahat_out).
+bool tc2_fused_bwd_supported(const Launcher& L, int H, int C);
+void tc2_fused_bwd(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* w16T_l, const void* ahat_in, const void* h_prev,
+                   void* ahat_out, float* gW, float* g_bias_prev, const float* amax, const FirstLayerFuse* fl);
 
 }  // namespace pigan

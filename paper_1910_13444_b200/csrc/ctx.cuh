@@ -162,7 +162,7 @@ void gen_forward_chunk(pigan_ctx* c, int n, const pigan_ctx::HBuf& hb, const flo
     void* h_out = (odp && !keep_last) ? nullptr : hb.at(l);
     if (odp) cudaMemset2DAsync(o, (size_t)o_stride * 4, 0, (size_t)g.valid * 4, C, L.stream);
     if (split) tc_layer_fwd_split(L, c->cfg.precision, H, g.R, g.R_ld, c->w16(n, l, 0), theta + s.b_off(l), hb.at(l - 1), h_out, odp);
-    else tc_layer_fwd(L, c->cfg.precision, C, H, g.R, g.R_ld, c->w16(n, l, 0), theta + s.b_off(l), hb.at(l - 1), h_out, odp);
+    else tc_layer_fwd(L, c->cfg.precision, C, H, g.R, g.R_ld, c->w16(n, l, 0), theta + s.b_off(l), hb.at(l - 1), h_out, odp, false, /*reverse=*/(l & 1) != 0);
   }
   if (!fuse_out) out_fwd<T>(L, C, H, theta + s.W_off(s.L + 1), theta + s.b_off(s.L + 1), g, (const T*)hb.at(s.L), o, o_stride, split);
 }
@@ -191,6 +191,16 @@ void gen_backward_chunk(pigan_ctx* c, int n, const pigan_ctx::HBuf& hb, const fl
       sgemm(L, true, false, H, g.R, H, theta + s.W_off(l), H, 0, (const float*)c->net[n].ah[cur], g.R_ld, pl, c->net[n].apre, g.R_ld, pl, C, false);
       jet_act_bwd_launch<T>(L, C, H, g, c->net[n].apre, nullptr, nullptr, (const T*)hb.at(l - 1),
                             (T*)c->net[n].ah[cur ^ 1], grads + s.b_off(l - 1), nullptr, nullptr, amax);
+    } else if (tc2_fused_bwd_supported(L, H, C)) {
+      // width 256: wgrad and dgrad of the layer in one kernel (ahat^l and h^{l-1} are read from HBM once)
+      if (l == 2 && tc_first_layer_fusable(H, g)) {
+        FirstLayerFuse fl{xy, g.row0, g.npts, s.in_dim, grads, c->net[n].An, g.per_sample};
+        tc2_fused_bwd(L, c->cfg.precision, C, H, g.R, g.R_ld, c->w16(n, l, 1), c->net[n].ah[cur], hb.at(l - 1), nullptr, grads + s.W_off(l),
+                      grads + s.b_off(l - 1), amax, &fl);
+        return;
+      }
+      tc2_fused_bwd(L, c->cfg.precision, C, H, g.R, g.R_ld, c->w16(n, l, 1), c->net[n].ah[cur], hb.at(l - 1), c->net[n].ah[cur ^ 1],
+                    grads + s.W_off(l), grads + s.b_off(l - 1), amax, nullptr);
     } else {
       tc_wgrad(L, c->cfg.precision, C, H, g.R, g.R_ld, c->net[n].ah[cur], hb.at(l - 1), grads + s.W_off(l), amax);
       if (l == 2 && tc_first_layer_fusable(H, g)) {

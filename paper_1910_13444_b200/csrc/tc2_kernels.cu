@@ -58,6 +58,8 @@ struct Jet2Params {
   float* o;              // [C][o_stride] fp32 (MODE 5: one plane)
   long long o_stride;
   int valid;             // rows of the chunk that exist: rows >= valid are not accumulated
+  int reverse;           // sweep the row tiles from the last to the first: consecutive layers alternate direction, so a layer starts on
+                         // the rows its predecessor wrote last, which are still in the 126 MB L2 (matters where a layer is HBM-bound: H = 256)
   int linear;            // MODE 0 only: plain GEMM, out_c = W in_c (no bias, no tanh): the raw adjoint planes of a skip layer (NEXT-1)
 };
 
@@ -142,7 +144,7 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
     {
       int stage = 0; uint32_t phase = 0;
       for (int t = cluster_id; t < n_tiles; t += n_clusters) {
-        const int ut = t % n_ut, rt = t / n_ut;
+        const int ut = t % n_ut, rt = p.reverse ? p.n_row_tiles - 1 - t / n_ut : t / n_ut;
         for (int kb = 0; kb < n_kb; ++kb) {
           mbar_wait(empty + stage, phase ^ 1);
           uint8_t* sA = stages + stage * Cfg::kStageBytes;
@@ -255,7 +257,7 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
     int it = 0;
     const float inv_amax = (MODE == 1 || MODE == 3) ? adj_inv_scale(p.amax) : 1.f;   // constant over the launch: one global load, not one per tile
     for (int t = cluster_id; t < n_tiles; t += n_clusters, ++it) {
-      const int ut = t % n_ut, rt = t / n_ut;
+      const int ut = t % n_ut, rt = p.reverse ? p.n_row_tiles - 1 - t / n_ut : t / n_ut;
       const int buf = it % Cfg::kNumBuf;
       const uint32_t bphase = (it / Cfg::kNumBuf) & 1;
       const int unit0 = ut * 256 + (int)rank * 128 + q * 32, unit = unit0 + lane;
@@ -633,12 +635,12 @@ static void set_out_dot(Jet2Params& p, const OutDot* od) {
 }
 
 void tc2_layer_fwd(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* w16_l, const float* bias, const void* h_in, void* h_out,
-                   const OutDot* od, bool linear) {
+                   const OutDot* od, bool linear, bool reverse) {
   CUtensorMap a, b;
   bool ok = weight_map(L, &a, precision, w16_l, H) && plane_map(L, &b, precision, h_in, H, R_ld, C, 32, 64, C, CU_TENSOR_MAP_SWIZZLE_64B);
   if (!ok) return;
   Jet2Params p{};
-  p.H = H; p.n_row_tiles = R / 64; p.bias = bias; p.out = h_out; p.R_ld = R_ld; p.linear = linear ? 1 : 0;
+  p.H = H; p.n_row_tiles = R / 64; p.bias = bias; p.out = h_out; p.R_ld = R_ld; p.linear = linear ? 1 : 0; p.reverse = reverse ? 1 : 0;
   if (od) { set_out_dot(p, od); dispatch_jet2<4>(L, C, a, b, b, p); return; }
   dispatch_jet2<0>(L, C, a, b, b, p);
 }

@@ -487,9 +487,9 @@ static void dispatch_jet(Launcher& L, int precision, int C, const CUtensorMap& a
 bool tc_out_dot_fusable(const Launcher& L, int H) { return tc2_supported(L, H); }   // the one-CTA kernels keep the separate out_fwd pass
 
 void tc_layer_fwd(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* w16_l, const float* bias, const void* h_in, void* h_out,
-                  const OutDot* od, bool linear) {
+                  const OutDot* od, bool linear, bool reverse) {
   if (R <= 0) return;
-  if (tc2_supported(L, H)) { tc2_layer_fwd(L, precision, C, H, R, R_ld, w16_l, bias, h_in, h_out, od, linear); return; }
+  if (tc2_supported(L, H)) { tc2_layer_fwd(L, precision, C, H, R, R_ld, w16_l, bias, h_in, h_out, od, linear, reverse); return; }
   CUtensorMap a, b, o;
   bool ok = weight_map(L, &a, precision, w16_l, H) && plane_map(L, &b, precision, h_in, H, R_ld, C, kRT, kBK, C, CU_TENSOR_MAP_SWIZZLE_128B) &&
             plane_map(L, &o, precision, h_out, H, R_ld, C, 32, 32, 1, CU_TENSOR_MAP_SWIZZLE_64B);
