@@ -260,9 +260,13 @@ void tc2_layer_bwd(Launcher& L, int precision, int C, int H, int R, int R_ld, co
                    const void* h_prev, void* ahat_out, float* g_bias_prev, const float* amax, const FirstLayerFuse* fl);
 void tc2_wgrad(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* ahat, const void* h_prev, float* gW, const float* amax);
 
-// ---- width 256: wgrad and dgrad (+ adjoint epilogue) of one layer in ONE kernel (tc2_fused_bwd.cu) --------------------
+// ---- widths 128 / 256: wgrad and dgrad (+ adjoint epilogue) of one layer in ONE kernel ---------------------------------
+// (tc_fused_bwd.cu: width 128 on one CTA; tc2_fused_bwd.cu: width 256 on CTA pairs)
 // gW (W_hat_l) += sum_c ahat_c h_prev_c^T and ahat_out = J^T (W_l^T ahat_in), b_hat_{l-1} += ...; the planes ahat_in and h_prev
 // cross HBM once instead of twice.  fl != nullptr: layer 2 with the first-layer reduction (no ahat_out).
+bool tc_fused_bwd_supported(const Launcher& L, int H, int C);
+void tc_fused_bwd(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* w16T_l, const void* ahat_in, const void* h_prev,
+                  void* ahat_out, float* gW, float* g_bias_prev, const float* amax, const FirstLayerFuse* fl);
 bool tc2_fused_bwd_supported(const Launcher& L, int H, int C);
 void tc2_fused_bwd(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* w16T_l, const void* ahat_in, const void* h_prev,
                    void* ahat_out, float* gW, float* g_bias_prev, const float* amax, const FirstLayerFuse* fl);

@@ -191,15 +191,15 @@ void gen_backward_chunk(pigan_ctx* c, int n, const pigan_ctx::HBuf& hb, const fl
       sgemm(L, true, false, H, g.R, H, theta + s.W_off(l), H, 0, (const float*)c->net[n].ah[cur], g.R_ld, pl, c->net[n].apre, g.R_ld, pl, C, false);
       jet_act_bwd_launch<T>(L, C, H, g, c->net[n].apre, nullptr, nullptr, (const T*)hb.at(l - 1),
                             (T*)c->net[n].ah[cur ^ 1], grads + s.b_off(l - 1), nullptr, nullptr, amax);
-    } else if (tc2_fused_bwd_supported(L, H, C)) {
-      // width 256: wgrad and dgrad of the layer in one kernel (ahat^l and h^{l-1} are read from HBM once)
+    } else if (tc_fused_bwd_supported(L, H, C)) {
+      // widths 128 / 256: wgrad and dgrad of the layer in one kernel (ahat^l and h^{l-1} are read from HBM once)
       if (l == 2 && tc_first_layer_fusable(H, g)) {
         FirstLayerFuse fl{xy, g.row0, g.npts, s.in_dim, grads, c->net[n].An, g.per_sample};
-        tc2_fused_bwd(L, c->cfg.precision, C, H, g.R, g.R_ld, c->w16(n, l, 1), c->net[n].ah[cur], hb.at(l - 1), nullptr, grads + s.W_off(l),
+        tc_fused_bwd(L, c->cfg.precision, C, H, g.R, g.R_ld, c->w16(n, l, 1), c->net[n].ah[cur], hb.at(l - 1), nullptr, grads + s.W_off(l),
                       grads + s.b_off(l - 1), amax, &fl);
         return;
       }
-      tc2_fused_bwd(L, c->cfg.precision, C, H, g.R, g.R_ld, c->w16(n, l, 1), c->net[n].ah[cur], hb.at(l - 1), c->net[n].ah[cur ^ 1],
+      tc_fused_bwd(L, c->cfg.precision, C, H, g.R, g.R_ld, c->w16(n, l, 1), c->net[n].ah[cur], hb.at(l - 1), c->net[n].ah[cur ^ 1],
                     grads + s.W_off(l), grads + s.b_off(l - 1), amax, nullptr);
     } else {
       tc_wgrad(L, c->cfg.precision, C, H, g.R, g.R_ld, c->net[n].ah[cur], hb.at(l - 1), grads + s.W_off(l), amax);

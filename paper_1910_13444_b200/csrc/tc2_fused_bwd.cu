@@ -21,13 +21,10 @@
 //   the output jet (jet_act_bwd), writes ahat^{l-1} in place into the H box and copies it out with 16-byte global stores
 //   (MODE 1), or reduces the first-layer gradients and writes nothing (MODE 3).  b_hat_{l-1} is kept in registers over
 //   all tiles.
-#include "tc_ptx.cuh"
+#include "fused_bwd.cuh"
 
 namespace pigan {
 
-constexpr int kFRows = 32;                   // rows of a tile
-constexpr int kFEpiWarps = 8;
-constexpr int kFThreads = (4 + kFEpiWarps) * 32;
 constexpr int kFWBytes = 4 * 128 * 64 * 2;   // resident W^T half: 4 k-blocks of 128 units x 64 contraction elements
 constexpr uint32_t kFD1Col = 256;            // D2 = columns [0, 256), D1 = [256, 256 + 32 C)
 
@@ -38,18 +35,6 @@ template <int C> struct FusedCfg {
   static constexpr int kNM = C == 5 ? 1 : 2;                   // M1 boxes (C = 5: 64 KB of W^T + 4 boxes of 40 KB fill the 227 KB)
   static constexpr int kSmem = kFWBytes + (kNH + kNA + kNM) * kSlot + 1024 /*align*/ + 256 /*barriers*/;
   static_assert(kSmem <= 232448, "shared memory budget");
-};
-
-struct FusedParams {
-  int n_tiles;           // R / 32
-  float* gW;             // W_hat_l [256][256] fp32, += (scaled back by the block scale of the adjoint planes)
-  float* g_bias;         // b_hat_{l-1} [256]
-  void* out;             // MODE 1: ahat^{l-1} planes [C][256][R_ld]
-  int R_ld;
-  const float* amax;     // block-scale source of the adjoint planes
-  // MODE 3 (layer 2: the adjoint of the FIRST tanh layer is reduced here and never written; npts % 32 == 0)
-  const float* xy; long long row0; int npts, in_dim, per_sample;
-  float* gW1; float* An;
 };
 
 // [61,64) layout 6 = SWIZZLE_32B (MN-major atoms of 16 elements x 8 contraction rows = 256 B)
@@ -225,7 +210,6 @@ fused_bwd256_kernel(const __grid_constant__ CUtensorMap tmW,     // W_l^T [256 i
     const int e = warp - 4, q = e & 3, hs = e >> 2;
     const int ul = q * 32 + lane;                            // unit within this CTA's 128
     const int unit = (int)rank * 128 + ul;
-    const uint32_t swz = (uint32_t)((lane >> 1) & 3);        // 64B swizzle: 16-byte chunk ^= (unit >> 1) & 3
     const uint32_t lane_base = tmem_base + ((uint32_t)(q * 32) << 16);
     const uint32_t tD1 = lane_base + kFD1Col + hs * (16 * C);
     const float inv_amax = adj_inv_scale(p.amax);
@@ -233,7 +217,6 @@ fused_bwd256_kernel(const __grid_constant__ CUtensorMap tmW,     // W_l^T [256 i
     int it = 0;
     for (int t = cluster_id; t < p.n_tiles; t += n_clusters, ++it) {
       const int sh = it % Cfg::kNH;
-      uint8_t* my_row = sH + sh * Cfg::kSlot + ul * 64;
       const int row0 = t * kFRows + hs * 16;
       mbar_wait(tfull, (uint32_t)(it & 1));
       tc_fence_after();
@@ -246,63 +229,7 @@ fused_bwd256_kernel(const __grid_constant__ CUtensorMap tmW,     // W_l^T [256 i
       if (lane == 0) mbar_arrive_cluster(mapa_u32(tempty, 0));
       // MMA2 of this tile reads the H box this warp is about to overwrite in place
       mbar_wait(m2done + sh, (uint32_t)(it / Cfg::kNH) & 1);
-      float bias_acc = 0.f;
-      const long long grow = p.row0 + row0;                  // MODE 3: global row of this warp's first row
-      const float2* xyp = MODE == 3 ? reinterpret_cast<const float2*>(p.xy) + (p.per_sample ? grow : grow % p.npts) : nullptr;
-#pragma unroll
-      for (int hf = 0; hf < 2; ++hf) {
-        const uint32_t off = (((uint32_t)(hs * 2 + hf)) ^ swz) << 4;
-        float hp[C][8], o[C][8];
-#pragma unroll
-        for (int c = 0; c < C; ++c) unpack8<T>(lds128(my_row + c * 8192 + off), hp[c]);
-#pragma unroll
-        for (int i = 0; i < 8; ++i) {
-          float hx[5], hj[5], aa[5];
-#pragma unroll
-          for (int c = 0; c < C; ++c) { hx[c] = hh[c][hf * 8 + i]; hj[c] = hp[c][i]; }
-          jet_act_bwd<C>(hj, hx, aa);
-          bias_acc += aa[0];
-          if (MODE == 3) {
-            const float2 pt = __ldg(xyp + hf * 8 + i);       // same address in every lane: one broadcast load
-            sx = fmaf(aa[0], pt.x, sx); sy = fmaf(aa[0], pt.y, sy);
-            if (C >= 3) { sx += aa[1]; sy += aa[2]; }
-          }
-#pragma unroll
-          for (int c = 0; c < C; ++c) o[c][i] = aa[c];
-        }
-        if (MODE == 1) {
-#pragma unroll
-          for (int c = 0; c < C; ++c) sts128(my_row + c * 8192 + off, pack8<T>(o[c]));
-        }
-      }
-      bias_tot += bias_acc;
-      if (MODE == 1) {
-        // staged planes -> global: two lanes cover the 32 contiguous bytes (one sector) of one unit's 16 rows.  Every lane
-        // pulls its share into registers, orders its generic-proxy accesses before the next TMA write of this box
-        // (fence.proxy.async), and only then issues the global stores.
-        __syncwarp();
-        T* gout = reinterpret_cast<T*>(p.out);
-        const int half = lane & 1, uu = lane >> 1;
-        uint4 v[C][2];
-#pragma unroll
-        for (int c = 0; c < C; ++c)
-#pragma unroll
-          for (int j = 0; j < 2; ++j) {
-            const int u = q * 32 + j * 16 + uu;
-            v[c][j] = lds128(sH + sh * Cfg::kSlot + c * 8192 + u * 64 + ((((uint32_t)(hs * 2 + half)) ^ (uint32_t)((u >> 1) & 3)) << 4));
-          }
-        fence_proxy_async();
-#pragma unroll
-        for (int c = 0; c < C; ++c)
-#pragma unroll
-          for (int j = 0; j < 2; ++j) {
-            const int u = (int)rank * 128 + q * 32 + j * 16 + uu;
-            *reinterpret_cast<uint4*>(gout + ((size_t)c * 256 + u) * p.R_ld + row0 + half * 8) = v[c][j];
-          }
-      } else {
-        fence_proxy_async();                                 // generic reads of the H box before the next TMA write
-        atomicAdd(p.An + (size_t)(grow / p.npts) * 256 + unit, bias_acc * inv_amax);
-      }
+      fused_epi_tile<T, C, MODE>(p, hh, sH + sh * Cfg::kSlot, q, hs, lane, (int)rank * 128, row0, inv_amax, bias_tot, sx, sy);
       __syncwarp();
       if (lane == 0) mbar_arrive(hfree + sh);
     }
@@ -316,18 +243,7 @@ fused_bwd256_kernel(const __grid_constant__ CUtensorMap tmW,     // W_l^T [256 i
       const int last = it - 1;
       mbar_wait(m2done + last % Cfg::kNH, (uint32_t)(last / Cfg::kNH) & 1);
       tc_fence_after();
-      float* dst = p.gW + (size_t)unit * 256 + hs * 128;
-      const uint32_t tD2 = lane_base + hs * 128;
-#pragma unroll 2
-      for (int n = 0; n < 128; n += 8) {
-        float v[8];
-        tmem_ld8(tD2 + n, v);
-        tmem_ld_wait();
-#pragma unroll
-        for (int i = 0; i < 8; ++i) v[i] *= inv_amax;
-        asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(dst + n), "f"(v[0]), "f"(v[1]), "f"(v[2]), "f"(v[3]) : "memory");
-        asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(dst + n + 4), "f"(v[4]), "f"(v[5]), "f"(v[6]), "f"(v[7]) : "memory");
-      }
+      fused_drain(lane_base + hs * 128, p.gW + (size_t)unit * 256 + hs * 128, 128, inv_amax);
     }
   }
   tc_fence_before();
@@ -361,7 +277,7 @@ void tc2_fused_bwd(Launcher& L, int precision, int C, int H, int R, int R_ld, co
             plane_map(L, &m1, precision, ahat_in, H, R_ld, C, 16, 256, C, CU_TENSOR_MAP_SWIZZLE_32B);
   if (!ok) return;
   FusedParams p{};
-  p.n_tiles = R / kFRows; p.gW = gW; p.g_bias = g_bias_prev; p.out = ahat_out; p.R_ld = R_ld; p.amax = amax;
+  p.H = H; p.n_tiles = R / kFRows; p.gW = gW; p.g_bias = g_bias_prev; p.out = ahat_out; p.R_ld = R_ld; p.amax = amax;
   if (fl) {
     p.xy = fl->xy; p.row0 = fl->row0; p.npts = fl->npts; p.in_dim = fl->in_dim; p.gW1 = fl->gW1; p.An = fl->An; p.per_sample = fl->per_sample;
     if (C == 1) launch_fused<1, 3>(L, w, a2, h, m1, p); else if (C == 3) launch_fused<3, 3>(L, w, a2, h, m1, p); else launch_fused<5, 3>(L, w, a2, h, m1, p);
