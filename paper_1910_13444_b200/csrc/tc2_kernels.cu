@@ -92,7 +92,7 @@ template <typename T, int C, int MODE>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(k2Threads, 1)
 jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H] 16-bit, box 64 x 128, SW128
                   const __grid_constant__ CUtensorMap tmB,      // input planes, box 32 rows x 64 units x C, SW64
-                  const __grid_constant__ CUtensorMap tmT,      // MODE 1, 3: h_prev planes in (box 32 rows x 32 units x C, SW64)
+                  const __grid_constant__ CUtensorMap tmT,      // MODE 1, 3: h_prev planes in; MODE 4: h_out planes (box 32 rows x 32 units x C, SW64)
                   Jet2Params p) {
   using Cfg = Jet2Cfg<C, MODE>;
   extern __shared__ uint8_t smem_raw[];
@@ -118,7 +118,7 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
 
   if (warp == 0 && lane == 0) {
     prefetch_tmap(&tmA); prefetch_tmap(&tmB);
-    if (MODE == 1 || MODE == 3) prefetch_tmap(&tmT);
+    if (MODE == 1 || MODE == 3 || MODE == 4) prefetch_tmap(&tmT);
   }
   if (warp == 1 && lane == 0) {
     for (int i = 0; i < Cfg::kNumStages; ++i) { mbar_init(full + i, 1); mbar_init(empty + i, 1); }
@@ -353,6 +353,8 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
       }
 
       if (kFwd) {
+        // MODE 4: the previous tile's TMA store has read the staging planes
+        if (MODE == 4 && p.out) { if (elect_one()) tma_wait_read_all(); __syncwarp(); }
         // ---- h_c = tanh-jet(a_c) ----
 #pragma unroll
         for (int rc = 0; rc < 4; ++rc) {
@@ -387,7 +389,18 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
           }
         }
         if (C != 5) release(); else release0();
-        if (!kOutDot || p.out) copy_out(C);
+        if (MODE == 4 && p.out) {
+          // The output dot's shuffles and atomics make this epilogue the longest of the forward: the tile leaves through ONE
+          // asynchronous TMA store per warp instead of the warp's own 20 LDS + 20 STG (measured on B200, last layer of a
+          // 131072-row chunk: -22 % at H = 256, -21 % at H = 512, -2 % at H = 1024; the plain forward layers gain nothing
+          // from it and lose 3 % at H = 1024, where the TMA unit is the busier side, so they keep their own stores)
+          fence_proxy_async();
+          __syncwarp();
+          if (elect_one()) { tma_store_3d(&tmT, stg, row0, unit0, 0); tma_commit_group(); }
+          __syncwarp();
+        } else if (!kOutDot) {
+          copy_out(C);
+        }
       } else if (kSplit) {
         // ---- value-only layer with split activations: a = W (h_hi + h_lo) + b; t = tanh a; t_hi = rn16(t), t_lo = rn16(t - t_hi) ----
 #pragma unroll 1
@@ -465,6 +478,7 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
       }
     }
   }
+  if (MODE == 4 && warp >= 4) { if (elect_one()) tma_wait_all(); __syncwarp(); }   // the last stores have left shared memory and are complete
   tc_fence_before();
   __syncthreads();
   cluster_sync_all();                                        // neither CTA leaves while the pair still uses its smem / TMEM
@@ -641,7 +655,11 @@ void tc2_layer_fwd(Launcher& L, int precision, int C, int H, int R, int R_ld, co
   if (!ok) return;
   Jet2Params p{};
   p.H = H; p.n_row_tiles = R / 64; p.bias = bias; p.out = h_out; p.R_ld = R_ld; p.linear = linear ? 1 : 0; p.reverse = reverse ? 1 : 0;
-  if (od) { set_out_dot(p, od); dispatch_jet2<4>(L, C, a, b, b, p); return; }
+  if (od) {
+    CUtensorMap o = b;
+    if (h_out && !plane_map(L, &o, precision, h_out, H, R_ld, C, 32, 32, C, CU_TENSOR_MAP_SWIZZLE_64B)) return;
+    set_out_dot(p, od); dispatch_jet2<4>(L, C, a, b, o, p); return;
+  }
   dispatch_jet2<0>(L, C, a, b, b, p);
 }
 
