@@ -30,7 +30,10 @@ template <int C, int MODE> struct Jet2Cfg {
   static constexpr int kNumBuf = C == 5 ? 1 : 2;                       // C = 5: alternating placement, early release
   static constexpr int kTmemCols = C == 5 ? 512 : 2 * kCols <= 128 ? 128 : 2 * kCols <= 256 ? 256 : 512;
   static constexpr int kSlots = C;                                     // staging planes per epilogue warp
-  static constexpr int kStgBytes = k2EpiWarps * kSlots * k2StgPlane;
+  // plain forward at C = 5: the epilogue stages and copies out 16 rows at a time (planes of 32 units x 16 rows), which frees
+  // 40 KB for a fifth operand stage -- the deferred (xx, yy) MMAs hold two stages of the ring at the start of every tile
+  static constexpr bool kHalfStg = MODE == 0 && C == 5;
+  static constexpr int kStgBytes = k2EpiWarps * kSlots * (kHalfStg ? k2StgPlane / 2 : k2StgPlane);
   static constexpr int kBudget = 232448 - 1024 - 512 - kStgBytes;
   static constexpr int kNumStages = kBudget / kStageBytes > 6 ? 6 : kBudget / kStageBytes;
   static constexpr int kSmemBytes = kNumStages * kStageBytes + kStgBytes + 1024 /*align*/ + 512 /*barriers*/;
@@ -249,7 +252,7 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
   } else if (warp >= 4) {
     // ===================== epilogue: warp (q, hs) owns TMEM lanes / units [32q, 32q+32) x rows [32hs, 32hs+32) ==========
     const int e = warp - 4, q = e & 3, hs = e >> 2;
-    uint8_t* stg = staging + e * (Cfg::kSlots * k2StgPlane);
+    uint8_t* stg = staging + e * (Cfg::kSlots * (Cfg::kHalfStg ? k2StgPlane / 2 : k2StgPlane));
     const uint32_t swz = (uint32_t)((lane >> 1) & 3);       // 64B swizzle of a 64-byte row: chunk ^= (row >> 1) & 3
     uint8_t* my_row = stg + lane * 64;
     const uint32_t lane_base = tmem_base + ((uint32_t)(q * 32) << 16);
@@ -352,7 +355,52 @@ jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H
         release();
       }
 
-      if (kFwd) {
+      if (Cfg::kHalfStg) {
+        // ---- h_c = tanh-jet(a_c), 16 rows at a time through staging planes of 32 units x 32 bytes (16-byte chunk ^= (unit >> 2) & 1) ----
+        const uint32_t swz32 = (uint32_t)((lane >> 2) & 1);
+        T* gout = reinterpret_cast<T*>(p.out);
+#pragma unroll
+        for (int hf = 0; hf < 2; ++hf) {
+#pragma unroll
+          for (int r2 = 0; r2 < 2; ++r2) {
+            const int rc = hf * 2 + r2;
+            float v[C][8], o[C][8];
+#pragma unroll
+            for (int c = 0; c < nc0; ++c) tmem_ld8(tcol(c) + rc * 8, v[c]);
+            tmem_ld_wait();
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+              float a[5], h[5];
+#pragma unroll
+              for (int c = 0; c < nc0; ++c) a[c] = v[c][i];
+              a[3] = kxx[rc * 8 + i]; a[4] = kyy[rc * 8 + i];
+              a[0] += bias;
+              if (p.linear) {
+#pragma unroll
+                for (int c = 0; c < C; ++c) h[c] = a[c];
+              } else {
+                jet_act_fwd<C>(fast_tanh(a[0]), a, h);
+              }
+#pragma unroll
+              for (int c = 0; c < C; ++c) o[c][i] = h[c];
+            }
+#pragma unroll
+            for (int c = 0; c < C; ++c) sts128(stg + c * 1024 + lane * 32 + (((uint32_t)r2 ^ swz32) << 4), pack8<T>(o[c]));
+          }
+          if (hf == 1) release0();
+          __syncwarp();
+          const int chw = lane & 1, ulw = lane >> 1;        // two lanes cover the 32 contiguous bytes (one sector) of one unit's 16 rows
+#pragma unroll
+          for (int c = 0; c < C; ++c)
+#pragma unroll
+            for (int j = 0; j < 2; ++j) {
+              const int u = j * 16 + ulw;
+              const uint4 v = lds128(stg + c * 1024 + u * 32 + (((uint32_t)chw ^ (uint32_t)((u >> 2) & 1)) << 4));
+              *reinterpret_cast<uint4*>(gout + ((size_t)c * p.H + unit0 + u) * p.R_ld + row0 + hf * 16 + chw * 8) = v;
+            }
+          __syncwarp();                                      // the staging rows are rewritten by other lanes in the next half
+        }
+      } else if (kFwd) {
         // MODE 4: the previous tile's TMA store has read the staging planes
         if (MODE == 4 && p.out) { if (elect_one()) tma_wait_read_all(); __syncwarp(); }
         // ---- h_c = tanh-jet(a_c) ----
