@@ -260,6 +260,12 @@ void tc2_layer_bwd(Launcher& L, int precision, int C, int H, int R, int R_ld, co
                    const void* h_prev, void* ahat_out, float* g_bias_prev, const float* amax, const FirstLayerFuse* fl);
 void tc2_wgrad(Launcher& L, int precision, int C, int H, int R, int R_ld, const void* ahat, const void* h_prev, float* gW, const float* amax);
 
+// ---- width 128: first layer and every hidden layer of a chunk's forward in ONE kernel (tc_fused_fwd.cu) -----------------
+// h[l - 1] receives the planes of h^l (l = 1 .. L); w16[l - 2] is the 16-bit copy of W_l.  Collocation rows only (C = 3, 5).
+bool tc_fused_fwd_supported(const Launcher& L, const NetShape& s, int C, const ChunkGeom& g);
+void tc_fused_fwd(Launcher& L, int precision, int C, const NetShape& s, const float* theta, const void* const* w16, const float* Zp,
+                  const float* xy, const ChunkGeom& g, void* const* h);
+
 // ---- widths 128 / 256: wgrad and dgrad (+ adjoint epilogue) of one layer in ONE kernel ---------------------------------
 // (tc_fused_bwd.cu: width 128 on one CTA; tc2_fused_bwd.cu: width 256 on CTA pairs)
 // gW (W_hat_l) += sum_c ahat_c h_prev_c^T and ahat_out = J^T (W_l^T ahat_in), b_hat_{l-1} += ...; the planes ahat_in and h_prev

@@ -147,6 +147,15 @@ void gen_forward_chunk(pigan_ctx* c, int n, const pigan_ctx::HBuf& hb, const flo
     gen_fused_f32_fwd(L, C, s, theta, c->net[n].Zp, xy, g, o, o_stride);
     return;
   }
+  if (c->cfg.precision != PIGAN_FP32 && !split && !L.one_cta && tc_fused_fwd_supported(L, s, C, g)) {
+    // width 128: the whole forward of the chunk in one kernel, activations stay on the SM between layers (tc_fused_fwd.cu)
+    const void* wl[8]; void* hp[8];
+    for (int l = 2; l <= s.L; ++l) wl[l - 2] = c->w16(n, l, 0);
+    for (int l = 1; l <= s.L; ++l) hp[l - 1] = hb.at(l);
+    tc_fused_fwd(L, c->cfg.precision, C, s, theta, wl, c->net[n].Zp, xy, g, hp);
+    out_fwd<T>(L, C, H, theta + s.W_off(s.L + 1), theta + s.b_off(s.L + 1), g, (const T*)hb.at(s.L), o, o_stride, false);
+    return;
+  }
   first_layer_fwd<T>(L, C, s, theta, c->net[n].Zp, xy, g, (T*)hb.at(1), split);
   // the output layer (a4) rides in the epilogue of the last hidden layer where the kernels support it
   const bool fuse_out = c->cfg.precision != PIGAN_FP32 && s.L >= 2 && tc_out_dot_fusable(L, H);

@@ -173,6 +173,19 @@ def test_c4_c5_dims_many_tiles_per_cta_pair(name, N, G, chunk):
     check_step(cfg, bias_std=0.0, loss_scale=ls, chunk_rows=chunk)
 
 
+@pytest.mark.parametrize("L", [2, 5])
+def test_width_128_fused_forward_depths_and_layer_by_layer(L):
+    """Width 128 runs the whole forward of the collocation rows in ONE kernel (tc_fused_fwd.cu: weights of L - 1 layers
+    resident, activations handed from layer to layer in shared memory).  c2 covers L = 4; here the shallowest and the deepest
+    network the kernel takes, several tiles per CTA (12 x 32^2 rows = 192 tiles on 148 CTAs) with non-zero biases, and the same
+    network through the layer-by-layer one-CTA kernels (PIGAN_FLAG_ONE_CTA) that the fused kernel replaces."""
+    from paper_1910_13444_b200 import FLAG_ONE_CTA
+    cfg = dataclasses.replace(wl.CONFIGS["c2"], name=f"w128-L{L}", L=L, N=12, G=32, S=40)
+    check_step(cfg)
+    check_step(cfg, chunk_rows=4096)
+    check_step(cfg, flags=FLAG_ONE_CTA)
+
+
 def test_width_384_one_cta_kernels_and_one_cta_flag():
     """Widths that are multiples of 128 but not of 256 run the one-CTA tcgen05 kernels (wgrad tile width must divide H);
     PIGAN_FLAG_ONE_CTA forces the same kernels on a CTA-pair width."""
