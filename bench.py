@@ -82,7 +82,8 @@ def hbm_class_bytes(cfg) -> dict:
     col = ((3 + 5) if two else 5) * rows * plane            # one pass over the C planes of the net(s), collocation rows
     sen = (2 if two else 1) * srows * plane                 # one pass over the value plane of the net(s), sensor rows
     n_par = (2 if two else 1) * wl.param_count(*cfg.gen_shape) + wl.param_count(*cfg.disc_shape)
-    return {"first_layer_fwd": col + sen * (1 + (2 if e == 2 else 1)),   # writes h^1: collocation, sensor pass with stash, snapshot pass (hi, lo)
+    fused_fwd = e == 2 and two and H == 128 and cfg.P % 64 == 0 and 2 <= cfg.L <= 5     # tc_fused_fwd.cu computes the first layer of the collocation rows
+    return {"first_layer_fwd": (0 if fused_fwd else col) + sen * (1 + (2 if e == 2 else 1)),   # writes h^1: collocation, sensor pass with stash, snapshot pass (hi, lo)
             "out_fwd": col + sen * (1 + (2 if e == 2 else 1)),           # reads h^L
             "jet_act_bwd": 2 * (col + sen),                               # top layer: reads h^L, writes ahat^L
             "first_layer_bwd": sen + (0 if (e == 2 and cfg.H % 256 == 0 and cfg.P % 64 == 0) else col),   # collocation part fused into the layer-2 dgrad when it can be
@@ -329,7 +330,7 @@ def run_config(cfg, device, steps, warmup, rank, world, with_roofline=True, seed
     del w.jet_out, w.jet_out2
     # roofline of the dominant kernel class (the tcgen05 jet GEMMs: forward, dgrad+adjoint, wgrad)
     if with_roofline:
-        tc = {k: v for k, v in prof.items() if k in ("jet_layer_fwd", "jet_layer_bwd", "wgrad", "jet_layer_bwd_wgrad")}
+        tc = {k: v for k, v in prof.items() if k in ("jet_layer_fwd", "jet_layer_bwd", "wgrad", "jet_layer_bwd_wgrad", "gen_fwd_fused")}
         per_step = {k: [v[0] / steps, v[1] / steps] for k, v in prof.items()}
         tc_ms = sum(v[1] for v in tc.values()) / steps
         total_ms = sum(v[1] for v in prof.values()) / steps
@@ -350,9 +351,10 @@ def run_config(cfg, device, steps, warmup, rank, world, with_roofline=True, seed
             pb = 2 * cfg.H                                        # bytes of one row of one 16-bit plane
             Lh = cfg.L - 1
             # width 256: dgrad and wgrad of a layer are ONE kernel (jet_layer_bwd_wgrad): two of the three GEMMs, planes read once
+            # width 128: the whole forward of the collocation rows is ONE kernel (gen_fwd_fused): it writes h^1 .. h^L and reads no planes
             cls_bytes = {"jet_layer_fwd": 2 * rowsC * pb * Lh, "jet_layer_bwd": rowsC * pb * (3 * Lh - 1), "wgrad": 2 * rowsC * pb * Lh,
-                         "jet_layer_bwd_wgrad": rowsC * pb * (3 * Lh - 1)}
-            cls_gemms = {"jet_layer_fwd": 1, "jet_layer_bwd": 1, "wgrad": 1, "jet_layer_bwd_wgrad": 2}
+                         "jet_layer_bwd_wgrad": rowsC * pb * (3 * Lh - 1), "gen_fwd_fused": cfg.N * cfg.P * chan * pb * cfg.L}
+            cls_gemms = {"jet_layer_fwd": 1, "jet_layer_bwd": 1, "wgrad": 1, "jet_layer_bwd_wgrad": 2, "gen_fwd_fused": 1}
             prof_ncu = ncu_profile(cfg.name)
             per_kernel = {}
             for k, v in tc.items():
@@ -374,7 +376,7 @@ def run_config(cfg, device, steps, warmup, rank, world, with_roofline=True, seed
                                "traffic_kernel": f"{dom} (C=5), DRAM read+write bytes per launch" if dom_ncu else None,
                                "traffic_whole_step": whole["dram_bytes"] if whole else None,
                                "traffic_source": "profiles/r02_step_dram_bytes.csv (ncu pass of profiles/r02_summary.md, not this run)" if prof_ncu else None,
-                               "kernel": "jet_layer_fwd + jet_layer_bwd + wgrad (tcgen05)", "peak_source": peaks["source"] + " sustained bf16",
+                               "kernel": " + ".join(sorted(tc)) + " (tcgen05)", "peak_source": peaks["source"] + " sustained bf16",
                                "frac_of_burst": round(ach / peaks["tflops_burst"], 4), "frac_of_nominal_2250": round(ach / 2250.0, 4),
                                "share_of_step": round(tc_ms / total_ms, 4) if total_ms > 0 else None,
                                "profile_pass": ("in the timed region: one CUDA event is recorded after every launch inside the timed steps, so `value` carries that "
