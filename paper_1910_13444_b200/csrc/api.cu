@@ -40,31 +40,44 @@ pigan_status train_step_impl(pigan_ctx* c, const float* thY, const float* thU, c
   float* gr[2] = {gY, gU};
   cudaStream_t st = L.stream;
   const size_t n_gD = ds.count() * (size_t)std::max(1, c->hier.K);
+  const long long srows = (long long)N * S, crows = (long long)N * P;
+  // Streams.  The critic stage needs X_fake only and the forward of the collocation rows nothing of the critic's: the critic goes
+  // to a side stream beside the forward of the first collocation chunk.  The two generator nets are independent up to the
+  // residual: at widths <= 256 (c1 - c3: short kernels, launch chains) net 1's kernels go to a second side stream (measured
+  // on B200: c2 step 0.81 -> 0.75 ms, c3 9.3 -> 9.1 ms; at width 512 the two nets' kernels only evict each other's planes from L2).
+  // Per-launch profiling keeps everything on the caller's stream (its events time consecutive launches).
+  const bool fork = c->side != nullptr && !L.profiling;
+  const bool two = fork && c->side2 != nullptr && gs.H <= 256;
+  cudaStream_t sn[2] = {st, two ? c->side2 : st};
+  int evk = 0;
+  auto link = [&](cudaStream_t from, cudaStream_t to) {      // work enqueued on `to` from here on follows what `from` holds now
+    if (from == to) return;
+    cudaEvent_t e = c->ev_pool[evk++ & 7];
+    cudaEventRecord(e, from); cudaStreamWaitEvent(to, e, 0);
+  };
   cudaMemsetAsync(gY, 0, gs.count() * 4, st); cudaMemsetAsync(gU, 0, gs.count() * 4, st); cudaMemsetAsync(gD, 0, n_gD * 4, st);
   cudaMemsetAsync(c->cw.acc, 0, 8 * sizeof(double), st);
   if (found_inf) cudaMemsetAsync(found_inf, 0, sizeof(int), st);
+  link(st, sn[1]);
+  // ---- a1 + a6: z-part, 16-bit weights, sensor evaluation -> X_fake; the (hi) activation planes of every sensor chunk stay in
+  //      net[n].hs for the reverse sweep ----
   for (int n = 0; n < 2; ++n) {
-    cudaMemsetAsync(c->net[n].An, 0, (size_t)N * gs.H * 4, st);
+    L.stream = sn[n];
+    cudaMemsetAsync(c->net[n].An, 0, (size_t)N * gs.H * 4, sn[n]);
     compute_zpart(c, n, th[n], z, N);
     if (cfg.precision != PIGAN_FP32) tc_convert_weights(L, cfg.precision, gs, th[n], c->net[n].w16);
-  }
-  // ---- a6: sensor evaluation -> X_fake; the (hi) activation planes of every sensor chunk stay in net[n].hs for the reverse sweep ----
-  const long long srows = (long long)N * S;
-  int sc = 0;
-  for (long long row0 = 0; row0 < srows; row0 += c->R_ld, ++sc) {
-    NvtxRange nr("pigan:sensor_forward");
-    ChunkGeom g = make_geom(c, row0, srows, S);
-    for (int n = 0; n < 2; ++n) {
+    int sc = 0;
+    for (long long row0 = 0; row0 < srows; row0 += c->R_ld, ++sc) {
+      NvtxRange nr("pigan:sensor_forward");
+      ChunkGeom g = make_geom(c, row0, srows, S);
       gen_forward_chunk<T>(c, n, c->hsens(n, sc), th[n], 1, xy_s, g, c->net[n].o, c->R_ld, /*split=*/true);
       scatter_snapshot(L, c->net[n].o, row0, g.valid, S, d, n * S, c->xfake);
     }
   }
+  L.stream = st;
+  link(sn[1], st);                                           // X_fake is complete
   // ---- a7-a9: critic losses and gradient; dX rows [0, N) = (1/N) grad_X D(X_fake) ----
-  // The critic needs X_fake only, the forward of the collocation rows nothing of the critic's: the critic stage goes to a side
-  // stream and joins before the sensor rows' reverse sweep (one CTA per sample: at c1 / c2 it leaves more than half of the
-  // SMs to the forward kernels; c1 step 0.22 -> 0.19 ms, c2 0.82 -> 0.81 ms).  Per-launch profiling keeps one stream: its events time consecutive launches.
-  const bool fork = c->side != nullptr && !L.profiling;
-  if (fork) { cudaEventRecord(c->ev_fork, st); cudaStreamWaitEvent(c->side, c->ev_fork, 0); L.stream = c->side; }
+  if (fork) { link(st, c->side); L.stream = c->side; }
   nvtxRangePushA("pigan:critic");
   if (c->hier.K > 0) {
     hier_critic_stage(c, thD, real, eps, gD);               // NEXT-3: K critics on column subsets (hier.cu)
@@ -81,47 +94,64 @@ pigan_status train_step_impl(pigan_ctx* c, const float* thY, const float* thU, c
     critic_gp(L, ds, thD, c->cw.X + (size_t)2 * N * d, c->cw.g + (size_t)2 * N * HD, N, gstride, cfg.gp_lambda, c->cw, gD, nullptr);
   }
   nvtxRangePop();
-  const long long crows = (long long)N * P;
-  if (fork) {
-    cudaEventRecord(c->ev_join, c->side);
-    L.stream = st;
+  L.stream = st;
+  const float* thn[2] = {thY, thU};
+  const int Cn[2] = {3, 5};
+  if (fork) {                                                // forward of the first collocation chunk beside the critic
     NvtxRange nr("pigan:collocation_forward_0");
     ChunkGeom g = make_geom(c, 0, crows, P);
-    gen_forward_chunk<T>(c, 0, c->hcol(0), thY, 3, xy_c, g, c->net[0].o, c->R_ld);
-    gen_forward_chunk<T>(c, 1, c->hcol(1), thU, 5, xy_c, g, c->net[1].o, c->R_ld);
-    cudaStreamWaitEvent(st, c->ev_join, 0);
+    for (int n = 0; n < 2; ++n) {
+      L.stream = sn[n];
+      gen_forward_chunk<T>(c, n, c->hcol(n), thn[n], Cn[n], xy_c, g, c->net[n].o, c->R_ld);
+    }
+    L.stream = st;
+    link(c->side, st);                                       // the critic's dX
   }
   // ---- O7 + a10 on the sensor rows: dL_G/dX_fake = -(1/N) grad_X D(X_fake), value channel only ----
-  sc = 0;
-  for (long long row0 = 0; row0 < srows; row0 += c->R_ld, ++sc) {
-    NvtxRange nr("pigan:sensor_backward");
-    ChunkGeom g = make_geom(c, row0, srows, S);
-    for (int n = 0; n < 2; ++n) {
-      cudaMemsetAsync(c->amax + n, 0, 4, st);
+  link(st, sn[1]);
+  for (int n = 0; n < 2; ++n) {
+    L.stream = sn[n];
+    int sc = 0;
+    for (long long row0 = 0; row0 < srows; row0 += c->R_ld, ++sc) {
+      NvtxRange nr("pigan:sensor_backward");
+      ChunkGeom g = make_geom(c, row0, srows, S);
+      cudaMemsetAsync(c->amax + n, 0, 4, sn[n]);
       gather_seed(L, c->dX, row0, g.valid, g.R, S, d, n * S, -loss_scale, c->net[n].oh, c->amax + n);
       gen_backward_chunk<T>(c, n, c->hsens(n, sc), th[n], gr[n], 1, xy_s, g);
     }
   }
+  L.stream = st;
   // ---- a1-a5, a10 on the collocation rows ----
   const float seed_scale = (float)(2.0 * cfg.pde_weight / (double)crows * loss_scale);
   for (long long row0 = 0; row0 < crows; row0 += c->R_ld) {
     NvtxRange nr("pigan:collocation_chunk");
     ChunkGeom g = make_geom(c, row0, crows, P);
     if (!(fork && row0 == 0)) {                              // the first chunk's forward ran beside the critic
-      gen_forward_chunk<T>(c, 0, c->hcol(0), thY, 3, xy_c, g, c->net[0].o, c->R_ld);
-      gen_forward_chunk<T>(c, 1, c->hcol(1), thU, 5, xy_c, g, c->net[1].o, c->R_ld);
+      for (int n = 0; n < 2; ++n) {
+        L.stream = sn[n];
+        gen_forward_chunk<T>(c, n, c->hcol(n), thn[n], Cn[n], xy_c, g, c->net[n].o, c->R_ld);
+      }
+      L.stream = st;
     }
+    link(sn[1], st);                                         // the residual needs both nets' outputs (and amax[1] is net 1's until here)
     cudaMemsetAsync(c->amax, 0, 8, st);
     residual(L, c->net[0].o, c->R_ld, c->net[1].o, c->R_ld, f, row0, g.valid, g.R, P, nullptr, c->cw.acc + 3, seed_scale, c->net[0].oh,
              c->net[1].oh, c->R_ld, c->amax, c->amax + 1);
-    gen_backward_chunk<T>(c, 0, c->hcol(0), thY, gY, 3, xy_c, g);
-    gen_backward_chunk<T>(c, 1, c->hcol(1), thU, gU, 5, xy_c, g);
+    link(st, sn[1]);
+    for (int n = 0; n < 2; ++n) {
+      L.stream = sn[n];
+      gen_backward_chunk<T>(c, n, c->hcol(n), thn[n], gr[n], Cn[n], xy_c, g);
+    }
+    L.stream = st;
   }
   // ---- finalize: z-part of the first layer, unscale, inf/nan flag, loss scalars ----
   for (int n = 0; n < 2; ++n) {
+    L.stream = sn[n];
     finalize_first_layer(L, gs, N, c->net[n].An, z, gr[n]);
     unscale_and_check(L, gr[n], gs.count(), 1.f / loss_scale, found_inf);
   }
+  L.stream = st;
+  link(sn[1], st);
   unscale_and_check(L, gD, n_gD, 1.f, found_inf);
   if (losses) {
     if (c->hier.K > 0) hier_write_losses(c, crows, losses);
@@ -220,11 +250,15 @@ pigan_status pigan_create(const pigan_config* cfg, void* cuda_stream, pigan_ctx*
   c->L.stream = (cudaStream_t)cuda_stream;
   cudaGetDevice(&c->L.device);
   if (cudaDeviceGetAttribute(&c->L.num_sms, cudaDevAttrMultiProcessorCount, c->L.device) != cudaSuccess || c->L.num_sms <= 0) c->L.num_sms = 148;
-  if (cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking) != cudaSuccess || cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
-      cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming) != cudaSuccess) {
-    cudaGetLastError();
-    if (c->side) cudaStreamDestroy(c->side);
-    c->side = nullptr;                                       // no side stream: the critic stage stays on the caller's stream
+  {
+    bool ok = cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking) == cudaSuccess && cudaStreamCreateWithFlags(&c->side2, cudaStreamNonBlocking) == cudaSuccess;
+    for (int i = 0; ok && i < 8; ++i) ok = cudaEventCreateWithFlags(&c->ev_pool[i], cudaEventDisableTiming) == cudaSuccess;
+    if (!ok) {                                               // no side streams: every stage stays on the caller's stream
+      cudaGetLastError();
+      if (c->side) cudaStreamDestroy(c->side);
+      if (c->side2) cudaStreamDestroy(c->side2);
+      c->side = c->side2 = nullptr;
+    }
   }
   c->L.one_cta = (cfg->flags & PIGAN_FLAG_ONE_CTA) != 0;
   c->sg.disabled = (cfg->flags & PIGAN_FLAG_NO_GRAPH) != 0;
@@ -312,8 +346,8 @@ void pigan_destroy(pigan_ctx* c) {
   if (c->sg.exec) cudaGraphExecDestroy(c->sg.exec);
   if (c->sg.cap_stream) cudaStreamDestroy(c->sg.cap_stream);
   if (c->side) cudaStreamDestroy(c->side);
-  if (c->ev_fork) cudaEventDestroy(c->ev_fork);
-  if (c->ev_join) cudaEventDestroy(c->ev_join);
+  if (c->side2) cudaStreamDestroy(c->side2);
+  for (cudaEvent_t e : c->ev_pool) if (e) cudaEventDestroy(e);
   for (void* p : c->allocs) cudaFree(p);
   for (cudaEvent_t e : c->L.events) cudaEventDestroy(e);
   delete c;

@@ -64,9 +64,9 @@ struct pigan_ctx {
     allocs.push_back(p);
     return reinterpret_cast<T*>(p);
   }
-  // the critic stage (a7-a9) depends on the sensor rows only: it runs on a side stream beside the forward of the first collocation chunk
-  cudaStream_t side = nullptr;
-  cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+  // side streams of a step (api.cu): the critic stage beside the first collocation forward; net 1's kernels beside net 0's in one-chunk steps
+  cudaStream_t side = nullptr, side2 = nullptr;
+  cudaEvent_t ev_pool[8] = {};
   int n_sens_chunks = 1;
   float* fbuf = nullptr;       // NEXT-2: [R_ld] f values of a chunk / the critic's adjoint of them
   // NEXT-3 (hier.cu): K critics on column subsets of the snapshot; set for the duration of pigan_train_step_grads_hier
