@@ -94,6 +94,21 @@ pigan_status train_step_impl(pigan_ctx* c, const float* thY, const float* thU, c
     critic_gp(L, ds, thD, c->cw.X + (size_t)2 * N * d, c->cw.g + (size_t)2 * N * HD, N, gstride, cfg.gp_lambda, c->cw, gD, nullptr);
   }
   nvtxRangePop();
+  // ---- O7 + a10 on the sensor rows: dL_G/dX_fake = -(1/N) grad_X D(X_fake), value channel only ----
+  // With their own adjoint set the sensor rows' reverse sweep follows the critic on ITS stream, beside the whole collocation pass.
+  const bool sb = two && c->amax_s != nullptr;
+  auto sensor_backward = [&](int n, bool own) {
+    int sc = 0;
+    for (long long row0 = 0; row0 < srows; row0 += c->R_ld, ++sc) {
+      NvtxRange nr("pigan:sensor_backward");
+      ChunkGeom g = make_geom(c, row0, srows, S);
+      float* am = (own ? c->amax_s : c->amax) + n;
+      cudaMemsetAsync(am, 0, 4, L.stream);
+      gather_seed(L, c->dX, row0, g.valid, g.R, S, d, n * S, -loss_scale, own ? c->net[n].oh_s : c->net[n].oh, am);
+      gen_backward_chunk<T>(c, n, c->hsens(n, sc), th[n], gr[n], 1, xy_s, g, own);
+    }
+  };
+  if (sb) { for (int n = 0; n < 2; ++n) sensor_backward(n, true); }
   L.stream = st;
   const float* thn[2] = {thY, thU};
   const int Cn[2] = {3, 5};
@@ -105,22 +120,13 @@ pigan_status train_step_impl(pigan_ctx* c, const float* thY, const float* thU, c
       gen_forward_chunk<T>(c, n, c->hcol(n), thn[n], Cn[n], xy_c, g, c->net[n].o, c->R_ld);
     }
     L.stream = st;
-    link(c->side, st);                                       // the critic's dX
+    if (!sb) link(c->side, st);                              // the critic's dX
   }
-  // ---- O7 + a10 on the sensor rows: dL_G/dX_fake = -(1/N) grad_X D(X_fake), value channel only ----
-  link(st, sn[1]);
-  for (int n = 0; n < 2; ++n) {
-    L.stream = sn[n];
-    int sc = 0;
-    for (long long row0 = 0; row0 < srows; row0 += c->R_ld, ++sc) {
-      NvtxRange nr("pigan:sensor_backward");
-      ChunkGeom g = make_geom(c, row0, srows, S);
-      cudaMemsetAsync(c->amax + n, 0, 4, sn[n]);
-      gather_seed(L, c->dX, row0, g.valid, g.R, S, d, n * S, -loss_scale, c->net[n].oh, c->amax + n);
-      gen_backward_chunk<T>(c, n, c->hsens(n, sc), th[n], gr[n], 1, xy_s, g);
-    }
+  if (!sb) {
+    link(st, sn[1]);
+    for (int n = 0; n < 2; ++n) { L.stream = sn[n]; sensor_backward(n, false); }
+    L.stream = st;
   }
-  L.stream = st;
   // ---- a1-a5, a10 on the collocation rows ----
   const float seed_scale = (float)(2.0 * cfg.pde_weight / (double)crows * loss_scale);
   for (long long row0 = 0; row0 < crows; row0 += c->R_ld) {
@@ -145,6 +151,7 @@ pigan_status train_step_impl(pigan_ctx* c, const float* thY, const float* thU, c
     L.stream = st;
   }
   // ---- finalize: z-part of the first layer, unscale, inf/nan flag, loss scalars ----
+  if (sb) { link(c->side, st); link(c->side, sn[1]); }       // the sensor rows' gradients and the critic's
   for (int n = 0; n < 2; ++n) {
     L.stream = sn[n];
     finalize_first_layer(L, gs, N, c->net[n].An, z, gr[n]);
@@ -331,6 +338,15 @@ pigan_status pigan_create(const pigan_config* cfg, void* cuda_stream, pigan_ctx*
     }
     c->seed = c->alloc<float>((size_t)2 * N);
     c->amax = c->alloc<float>(2);
+    if (H <= 256 && !c->trunk && cfg->n_free == 0) {          // widths that run the two nets and the critic on three streams (api.cu)
+      c->amax_s = c->alloc<float>(2);
+      for (int n = 0; n < 2; ++n) {
+        NetWs& w = c->net[n];
+        w.ah_s[0] = c->alloc<char>(c->plane()); w.ah_s[1] = c->alloc<char>(c->plane());
+        w.oh_s = c->alloc<float>((size_t)c->R_ld);
+        if (f32) w.apre_s = c->alloc<float>((size_t)H * c->R_ld);
+      }
+    }
     if (cfg->n_free > 0) c->fbuf = c->alloc<float>((size_t)c->R_ld);
   } catch (const std::bad_alloc&) {
     pigan_destroy(c);

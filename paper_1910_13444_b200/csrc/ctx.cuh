@@ -23,6 +23,10 @@ struct NetWs {                 // activation workspace of one generator net (pla
   float* Zp = nullptr;         // [N][H]  first-layer z-part
   float* An = nullptr;         // [N][H]  per-sample sums of the first-layer value adjoint
   void* w16 = nullptr;         // (L-1) x {W_l, W_l^T} 16-bit copies
+  // second adjoint set for the SENSOR rows (value channel only), so that their reverse sweep can run beside the collocation pass
+  char* ah_s[2] = {nullptr, nullptr};   // [1][H][R_ld]
+  float* oh_s = nullptr;       // [R_ld]
+  float* apre_s = nullptr;     // fp32 mode: [1][H][R_ld]
   // NEXT-1, skip connections only (trunk.cu): the tanh jets t^l of the layers that take a skip are kept beside h^l = t^l + h^{l-2}
   char* ht = nullptr;          // L x [Cmax][H][R_ld]
   char* hts = nullptr;         // sensor rows: n_sens_chunks x L x [2][H][R_ld]
@@ -45,6 +49,7 @@ struct pigan_ctx {
   float* dX = nullptr;         // [2N][2S]
   float* seed = nullptr;       // [2N]
   float* amax = nullptr;       // [2] largest output adjoint of the current chunk, per net (block scale of the adjoint planes)
+  float* amax_s = nullptr;     // [2] the same for the sensor rows' own adjoint set (null: the sensor rows share net[n].ah / oh)
   std::vector<void*> allocs;
   // CUDA-graph replay of pigan_train_step_grads: the step is hundreds to thousands of launches, launch-latency bound
   // for the small configs.  A call whose arguments repeat the previous call's is captured once (on a private stream,
@@ -180,54 +185,58 @@ void gen_forward_chunk(pigan_ctx* c, int n, const pigan_ctx::HBuf& hb, const flo
 }
 
 // ---- one chunk of generator rows, reverse sweep; output adjoints are in net[n].oh [C][R_ld] ------------------------
+// sens: the adjoint planes, output adjoints and block scale of the sensor rows' own set (pigan_ctx::amax_s != nullptr)
 template <typename T>
-void gen_backward_chunk(pigan_ctx* c, int n, const pigan_ctx::HBuf& hb, const float* theta, float* grads, int C, const float* xy, const ChunkGeom& g) {
+void gen_backward_chunk(pigan_ctx* c, int n, const pigan_ctx::HBuf& hb, const float* theta, float* grads, int C, const float* xy, const ChunkGeom& g,
+                        bool sens = false) {
   const NetShape& s = c->gen;
   Launcher& L = c->L;
   const int H = s.H;
   const long long pl = (long long)H * g.R_ld;
   int cur = 0;
-  const float* amax = c->cfg.precision == PIGAN_FP32 ? nullptr : c->amax + n;
+  struct { float* oh; char* ah[2]; float* apre; } w = {c->net[n].oh, {c->net[n].ah[0], c->net[n].ah[1]}, c->net[n].apre};
+  if (sens) { w.oh = c->net[n].oh_s; w.ah[0] = c->net[n].ah_s[0]; w.ah[1] = c->net[n].ah_s[1]; w.apre = c->net[n].apre_s; }
+  const float* amax = c->cfg.precision == PIGAN_FP32 ? nullptr : (sens ? c->amax_s : c->amax) + n;
   if (c->cfg.precision == PIGAN_FP32 && gen_fused_f32_supported(s)) {     // recomputes the forward of every row (gen_fused_f32.cu)
-    gen_fused_f32_bwd(L, C, s, theta, c->net[n].Zp, xy, g, c->net[n].oh, grads, c->net[n].An);
+    gen_fused_f32_bwd(L, C, s, theta, c->net[n].Zp, xy, g, w.oh, grads, c->net[n].An);
     return;
   }
-  jet_act_bwd_launch<T>(L, C, H, g, nullptr, theta + s.W_off(s.L + 1), c->net[n].oh, (const T*)hb.at(s.L),
-                        (T*)c->net[n].ah[cur], grads + s.b_off(s.L),
+  jet_act_bwd_launch<T>(L, C, H, g, nullptr, theta + s.W_off(s.L + 1), w.oh, (const T*)hb.at(s.L),
+                        (T*)w.ah[cur], grads + s.b_off(s.L),
                         grads + s.W_off(s.L + 1), grads + s.b_off(s.L + 1), amax);
   for (int l = s.L; l >= 2; --l) {
     if (c->cfg.precision == PIGAN_FP32) {
       // W_hat_l += sum_c ahat_c h_c^{l-1 T}: M = H, N = H, K = rows
-      sgemm(L, false, true, H, H, g.R, (const float*)c->net[n].ah[cur], g.R_ld, pl, (const float*)hb.at(l - 1), g.R_ld, pl, grads + s.W_off(l), H, 0, C, true);
+      sgemm(L, false, true, H, H, g.R, (const float*)w.ah[cur], g.R_ld, pl, (const float*)hb.at(l - 1), g.R_ld, pl, grads + s.W_off(l), H, 0, C, true);
       // hhat_c^{l-1} = W_l^T ahat_c: M = H (in), N = rows, K = H (out); A stored [K][M]
-      sgemm(L, true, false, H, g.R, H, theta + s.W_off(l), H, 0, (const float*)c->net[n].ah[cur], g.R_ld, pl, c->net[n].apre, g.R_ld, pl, C, false);
-      jet_act_bwd_launch<T>(L, C, H, g, c->net[n].apre, nullptr, nullptr, (const T*)hb.at(l - 1),
-                            (T*)c->net[n].ah[cur ^ 1], grads + s.b_off(l - 1), nullptr, nullptr, amax);
+      sgemm(L, true, false, H, g.R, H, theta + s.W_off(l), H, 0, (const float*)w.ah[cur], g.R_ld, pl, w.apre, g.R_ld, pl, C, false);
+      jet_act_bwd_launch<T>(L, C, H, g, w.apre, nullptr, nullptr, (const T*)hb.at(l - 1),
+                            (T*)w.ah[cur ^ 1], grads + s.b_off(l - 1), nullptr, nullptr, amax);
     } else if (tc_fused_bwd_supported(L, H, C)) {
       // widths 128 / 256: wgrad and dgrad of the layer in one kernel (ahat^l and h^{l-1} are read from HBM once)
       if (l == 2 && tc_first_layer_fusable(H, g)) {
         FirstLayerFuse fl{xy, g.row0, g.npts, s.in_dim, grads, c->net[n].An, g.per_sample};
-        tc_fused_bwd(L, c->cfg.precision, C, H, g.R, g.R_ld, c->w16(n, l, 1), c->net[n].ah[cur], hb.at(l - 1), nullptr, grads + s.W_off(l),
+        tc_fused_bwd(L, c->cfg.precision, C, H, g.R, g.R_ld, c->w16(n, l, 1), w.ah[cur], hb.at(l - 1), nullptr, grads + s.W_off(l),
                       grads + s.b_off(l - 1), amax, &fl);
         return;
       }
-      tc_fused_bwd(L, c->cfg.precision, C, H, g.R, g.R_ld, c->w16(n, l, 1), c->net[n].ah[cur], hb.at(l - 1), c->net[n].ah[cur ^ 1],
+      tc_fused_bwd(L, c->cfg.precision, C, H, g.R, g.R_ld, c->w16(n, l, 1), w.ah[cur], hb.at(l - 1), w.ah[cur ^ 1],
                     grads + s.W_off(l), grads + s.b_off(l - 1), amax, nullptr);
     } else {
-      tc_wgrad(L, c->cfg.precision, C, H, g.R, g.R_ld, c->net[n].ah[cur], hb.at(l - 1), grads + s.W_off(l), amax);
+      tc_wgrad(L, c->cfg.precision, C, H, g.R, g.R_ld, w.ah[cur], hb.at(l - 1), grads + s.W_off(l), amax);
       if (l == 2 && tc_first_layer_fusable(H, g)) {
         // the adjoint of the first tanh layer is reduced inside the dgrad epilogue (ahat^1 is never written)
         FirstLayerFuse fl{xy, g.row0, g.npts, s.in_dim, grads, c->net[n].An, g.per_sample};
-        tc_layer_bwd(L, c->cfg.precision, C, H, g.R, g.R_ld, c->w16(n, l, 1), c->net[n].ah[cur], hb.at(l - 1),
-                     c->net[n].ah[cur ^ 1], grads + s.b_off(l - 1), amax, &fl);
+        tc_layer_bwd(L, c->cfg.precision, C, H, g.R, g.R_ld, c->w16(n, l, 1), w.ah[cur], hb.at(l - 1),
+                     w.ah[cur ^ 1], grads + s.b_off(l - 1), amax, &fl);
         return;
       }
-      tc_layer_bwd(L, c->cfg.precision, C, H, g.R, g.R_ld, c->w16(n, l, 1), c->net[n].ah[cur], hb.at(l - 1),
-                   c->net[n].ah[cur ^ 1], grads + s.b_off(l - 1), amax);
+      tc_layer_bwd(L, c->cfg.precision, C, H, g.R, g.R_ld, c->w16(n, l, 1), w.ah[cur], hb.at(l - 1),
+                   w.ah[cur ^ 1], grads + s.b_off(l - 1), amax);
     }
     cur ^= 1;
   }
-  first_layer_bwd<T>(L, C, s, xy, g, (const T*)c->net[n].ah[cur], grads, c->net[n].An, amax);
+  first_layer_bwd<T>(L, C, s, xy, g, (const T*)w.ah[cur], grads, c->net[n].An, amax);
 }
 
 // NEXT-1 (trunk.cu)
