@@ -84,7 +84,7 @@ def hbm_class_bytes(cfg) -> dict:
     n_par = (2 if two else 1) * wl.param_count(*cfg.gen_shape) + wl.param_count(*cfg.disc_shape)
     fused_fwd = e == 2 and two and H == 128 and cfg.P % 64 == 0 and 2 <= cfg.L <= 5     # tc_fused_fwd.cu computes the first layer of the collocation rows
     return {"first_layer_fwd": (0 if fused_fwd else col) + sen * (1 + (2 if e == 2 else 1)),   # writes h^1: collocation, sensor pass with stash, snapshot pass (hi, lo)
-            "out_fwd": col + sen * (1 + (2 if e == 2 else 1)),           # reads h^L
+            "out_fwd": (0 if fused_fwd else col) + sen * (1 + (2 if e == 2 else 1)),           # reads h^L (the fused forward reduces the output dot itself)
             "jet_act_bwd": 2 * (col + sen),                               # top layer: reads h^L, writes ahat^L
             "first_layer_bwd": sen + (0 if (e == 2 and cfg.H % 256 == 0 and cfg.P % 64 == 0) else col),   # collocation part fused into the layer-2 dgrad when it can be
             "adam": 28 * n_par, "residual": 16 * 4 * rows}

@@ -263,8 +263,9 @@ void tc2_wgrad(Launcher& L, int precision, int C, int H, int R, int R_ld, const 
 // ---- width 128: first layer and every hidden layer of a chunk's forward in ONE kernel (tc_fused_fwd.cu) -----------------
 // h[l - 1] receives the planes of h^l (l = 1 .. L); w16[l - 2] is the 16-bit copy of W_l.  Collocation rows only (C = 3, 5).
 bool tc_fused_fwd_supported(const Launcher& L, const NetShape& s, int C, const ChunkGeom& g);
+// od (may be null): the output layer rides in the last layer's epilogue (od->o zeroed by the caller; every row of the chunk is valid)
 void tc_fused_fwd(Launcher& L, int precision, int C, const NetShape& s, const float* theta, const void* const* w16, const float* Zp,
-                  const float* xy, const ChunkGeom& g, void* const* h);
+                  const float* xy, const ChunkGeom& g, void* const* h, const OutDot* od);
 
 // ---- widths 128 / 256: wgrad and dgrad (+ adjoint epilogue) of one layer in ONE kernel ---------------------------------
 // (tc_fused_bwd.cu: width 128 on one CTA; tc2_fused_bwd.cu: width 256 on CTA pairs)

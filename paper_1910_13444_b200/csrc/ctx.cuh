@@ -160,8 +160,9 @@ void gen_forward_chunk(pigan_ctx* c, int n, const pigan_ctx::HBuf& hb, const flo
     const void* wl[8]; void* hp[8];
     for (int l = 2; l <= s.L; ++l) wl[l - 2] = c->w16(n, l, 0);
     for (int l = 1; l <= s.L; ++l) hp[l - 1] = hb.at(l);
-    tc_fused_fwd(L, c->cfg.precision, C, s, theta, wl, c->net[n].Zp, xy, g, hp);
-    out_fwd<T>(L, C, H, theta + s.W_off(s.L + 1), theta + s.b_off(s.L + 1), g, (const T*)hb.at(s.L), o, o_stride, false);
+    OutDot od{theta + s.W_off(s.L + 1), theta + s.b_off(s.L + 1), o, o_stride, g.valid};
+    cudaMemset2DAsync(o, (size_t)o_stride * 4, 0, (size_t)g.valid * 4, C, L.stream);
+    tc_fused_fwd(L, c->cfg.precision, C, s, theta, wl, c->net[n].Zp, xy, g, hp, &od);
     return;
   }
   first_layer_fwd<T>(L, C, s, theta, c->net[n].Zp, xy, g, (T*)hb.at(1), split);

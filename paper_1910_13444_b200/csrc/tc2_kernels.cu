@@ -70,27 +70,6 @@ struct Jet2Params {
 // MODE 3: MODE 1 with the first-layer backward reduction fused (no adjoint planes written);
 // MODE 4 / 5: MODE 0 / 2 for the LAST hidden layer with the output dot (a4) fused into the epilogue; p.out == nullptr then
 //             skips the h^L planes (forward-only callers).
-// sum over the 32 lanes of v[0..7]: every lane ends with the total of v[(lane >> 2) & 7] (3 halving exchanges + 2 butterflies)
-__device__ __forceinline__ float warp_reduce8(const float* v, int lane) {
-  float a[4], b[2];
-  const bool u4 = lane & 16, u3 = lane & 8, u2 = lane & 4;
-#pragma unroll
-  for (int k = 0; k < 4; ++k) {
-    const float send = u4 ? v[k] : v[k + 4], keep = u4 ? v[k + 4] : v[k];
-    a[k] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
-  }
-#pragma unroll
-  for (int k = 0; k < 2; ++k) {
-    const float send = u3 ? a[k] : a[k + 2], keep = u3 ? a[k + 2] : a[k];
-    b[k] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
-  }
-  const float send = u2 ? b[0] : b[1], keep = u2 ? b[1] : b[0];
-  float r = keep + __shfl_xor_sync(0xffffffffu, send, 4);
-  r += __shfl_xor_sync(0xffffffffu, r, 2);
-  r += __shfl_xor_sync(0xffffffffu, r, 1);
-  return r;                                                // row index within the 8: 4 * bit4 + 2 * bit3 + bit2 of the lane
-}
-
 template <typename T, int C, int MODE>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(k2Threads, 1)
 jet2_layer_kernel(const __grid_constant__ CUtensorMap tmA,      // weights [H][H] 16-bit, box 64 x 128, SW128

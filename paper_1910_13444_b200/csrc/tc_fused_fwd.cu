@@ -39,6 +39,9 @@ struct FusedFwdParams {
   const float* xy;                           // [npts][2], or [rows][2] when per_sample
   long long row0;                            // first global row of the chunk (multiple of 64)
   int npts, per_sample;
+  // output layer (a4) in the epilogue of the last hidden layer: o_c[r] += sum_units w_out[unit] h^L_c[unit][r] (+ b_out on the value
+  // channel); o is zeroed by the launcher; o == nullptr: no output dot
+  const float* w_out; const float* b_out; float* o; long long o_stride;
 };
 
 template <typename T, int C>
@@ -132,6 +135,7 @@ __global__ void __launch_bounds__(kFFThreads, 1) fused_fwd128_kernel(const __gri
     const uint32_t sw = (uint32_t)(u & 7);
     const uint32_t tbase = tmem_base + ((uint32_t)(q * 32) << 16) + hs * kFFRows;
     const float wx = p.theta[(size_t)u * p.in_dim], wy = p.theta[(size_t)u * p.in_dim + 1], b1 = p.theta[p.b_off[1] + u];
+    const float wo = p.o ? p.w_out[u] : 0.f, bo = p.o ? p.b_out[0] : 0.f;
     uint32_t ver = 0, tf = 0;
     for (int it = 0; it < n_my; ++it) {
       const int t = (int)blockIdx.x + it * (int)gridDim.x;
@@ -195,6 +199,20 @@ __global__ void __launch_bounds__(kFFThreads, 1) fused_fwd128_kernel(const __gri
           const uint32_t off = (((uint32_t)(hs * kFFGroups + rc)) ^ sw) << 4;
 #pragma unroll
           for (int c = 0; c < C; ++c) sts128(my_row + c * 8192 + off, pack8<T>(o[c]));
+          if (l == p.L && p.o) {
+            // a4: the unrounded fp32 h^L_c times w_out[unit], summed over the warp's 32 units by a transposing shuffle reduction
+            // (lane -> row 4 bit4 + 2 bit3 + bit2 of the group of 8), over the four unit quarters by fp32 atomics
+            const int r = t * 64 + hs * kFFRows + rc * 8 + ((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1);
+#pragma unroll
+            for (int c = 0; c < C; ++c) {
+              float pv[8];
+#pragma unroll
+              for (int i = 0; i < 8; ++i) pv[i] = wo * o[c][i];
+              float tot = warp_reduce8(pv, lane);
+              if (c == 0 && q == 0) tot += bo;
+              if ((lane & 3) == 0) atomicAdd(p.o + (size_t)c * p.o_stride + r, tot);
+            }
+          }
         }
         fence_proxy_async();
         tc_fence_before();                                   // this warp's TMEM reads are done before the next layer's MMAs overwrite them
@@ -228,7 +246,7 @@ static void launch_fused_fwd(Launcher& L, const FusedFwdMaps& maps, const FusedF
 }
 
 void tc_fused_fwd(Launcher& L, int precision, int C, const NetShape& s, const float* theta, const void* const* w16 /*[L - 1]: W_2 .. W_L*/,
-                  const float* Zp, const float* xy, const ChunkGeom& g, void* const* h /*[L]: planes of h^1 .. h^L*/) {
+                  const float* Zp, const float* xy, const ChunkGeom& g, void* const* h /*[L]: planes of h^1 .. h^L*/, const OutDot* od) {
   FusedFwdMaps maps{};
   FusedFwdParams p{};
   for (int l = 2; l <= s.L; ++l)
@@ -239,6 +257,7 @@ void tc_fused_fwd(Launcher& L, int precision, int C, const NetShape& s, const fl
   }
   p.L = s.L; p.n_tiles = g.R / 64; p.in_dim = s.in_dim; p.theta = theta; p.Zp = Zp; p.xy = xy; p.row0 = g.row0; p.npts = g.npts;
   p.per_sample = g.per_sample;
+  if (od) { p.w_out = od->w_out; p.b_out = od->b_out; p.o = od->o; p.o_stride = od->o_stride; }
   if (C == 3) launch_fused_fwd<3>(L, maps, p); else launch_fused_fwd<5>(L, maps, p);
 }
 

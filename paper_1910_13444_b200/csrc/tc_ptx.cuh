@@ -172,6 +172,28 @@ template <typename T> __device__ __forceinline__ void unpack8(uint4 u, float* v)
 // ---- CTA pairs (cta_group::2): the two CTAs of a cluster issue ONE tcgen05.mma of M = 256; each holds 128 rows of A,
 // half of the N columns of B and 128 TMEM lanes of D.  Only the leader (cluster rank 0) issues MMAs; TMA loads of both
 // CTAs complete on the leader's mbarrier; commits are multicast to the same barrier offset in both CTAs.
+// sum over the 32 lanes of v[0..7]: every lane ends with the total of v[(lane >> 2) & 7] (3 halving exchanges + 2 butterflies)
+__device__ __forceinline__ float warp_reduce8(const float* v, int lane) {
+  float a[4], b[2];
+  const bool u4 = lane & 16, u3 = lane & 8, u2 = lane & 4;
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    const float send = u4 ? v[k] : v[k + 4], keep = u4 ? v[k + 4] : v[k];
+    a[k] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
+  }
+#pragma unroll
+  for (int k = 0; k < 2; ++k) {
+    const float send = u3 ? a[k] : a[k + 2], keep = u3 ? a[k + 2] : a[k];
+    b[k] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
+  }
+  const float send = u2 ? b[0] : b[1], keep = u2 ? b[1] : b[0];
+  float r = keep + __shfl_xor_sync(0xffffffffu, send, 4);
+  r += __shfl_xor_sync(0xffffffffu, r, 2);
+  r += __shfl_xor_sync(0xffffffffu, r, 1);
+  return r;                                                // row index within the 8: 4 * bit4 + 2 * bit3 + bit2 of the lane
+}
+
+
 __device__ __forceinline__ uint32_t cluster_ctarank() {
   uint32_t r;
   asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
