@@ -108,7 +108,12 @@ pigan_status train_step_impl(pigan_ctx* c, const float* thY, const float* thU, c
       gen_backward_chunk<T>(c, n, c->hsens(n, sc), th[n], gr[n], 1, xy_s, g, own);
     }
   };
-  if (sb) { for (int n = 0; n < 2; ++n) sensor_backward(n, true); }
+  if (sb) {                                                  // net 0 behind the critic on its stream, net 1 beside it on a stream of its own
+    link(c->side, c->side3);
+    sensor_backward(0, true);
+    L.stream = c->side3;
+    sensor_backward(1, true);
+  }
   L.stream = st;
   const float* thn[2] = {thY, thU};
   const int Cn[2] = {3, 5};
@@ -151,7 +156,7 @@ pigan_status train_step_impl(pigan_ctx* c, const float* thY, const float* thU, c
     L.stream = st;
   }
   // ---- finalize: z-part of the first layer, unscale, inf/nan flag, loss scalars ----
-  if (sb) { link(c->side, st); link(c->side, sn[1]); }       // the sensor rows' gradients and the critic's
+  if (sb) { link(c->side, st); link(c->side3, sn[1]); link(c->side3, st); }       // the critic's gradient and the sensor rows' (net 0: side, net 1: side3)
   for (int n = 0; n < 2; ++n) {
     L.stream = sn[n];
     finalize_first_layer(L, gs, N, c->net[n].An, z, gr[n]);
@@ -258,13 +263,15 @@ pigan_status pigan_create(const pigan_config* cfg, void* cuda_stream, pigan_ctx*
   cudaGetDevice(&c->L.device);
   if (cudaDeviceGetAttribute(&c->L.num_sms, cudaDevAttrMultiProcessorCount, c->L.device) != cudaSuccess || c->L.num_sms <= 0) c->L.num_sms = 148;
   {
-    bool ok = cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking) == cudaSuccess && cudaStreamCreateWithFlags(&c->side2, cudaStreamNonBlocking) == cudaSuccess;
+    bool ok = cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking) == cudaSuccess && cudaStreamCreateWithFlags(&c->side2, cudaStreamNonBlocking) == cudaSuccess &&
+              cudaStreamCreateWithFlags(&c->side3, cudaStreamNonBlocking) == cudaSuccess;
     for (int i = 0; ok && i < 8; ++i) ok = cudaEventCreateWithFlags(&c->ev_pool[i], cudaEventDisableTiming) == cudaSuccess;
     if (!ok) {                                               // no side streams: every stage stays on the caller's stream
       cudaGetLastError();
       if (c->side) cudaStreamDestroy(c->side);
       if (c->side2) cudaStreamDestroy(c->side2);
-      c->side = c->side2 = nullptr;
+      if (c->side3) cudaStreamDestroy(c->side3);
+      c->side = c->side2 = c->side3 = nullptr;
     }
   }
   c->L.one_cta = (cfg->flags & PIGAN_FLAG_ONE_CTA) != 0;
@@ -363,6 +370,7 @@ void pigan_destroy(pigan_ctx* c) {
   if (c->sg.cap_stream) cudaStreamDestroy(c->sg.cap_stream);
   if (c->side) cudaStreamDestroy(c->side);
   if (c->side2) cudaStreamDestroy(c->side2);
+  if (c->side3) cudaStreamDestroy(c->side3);
   for (cudaEvent_t e : c->ev_pool) if (e) cudaEventDestroy(e);
   for (void* p : c->allocs) cudaFree(p);
   for (cudaEvent_t e : c->L.events) cudaEventDestroy(e);

@@ -70,7 +70,7 @@ struct pigan_ctx {
     return reinterpret_cast<T*>(p);
   }
   // side streams of a step (api.cu): the critic stage beside the first collocation forward; net 1's kernels beside net 0's in one-chunk steps
-  cudaStream_t side = nullptr, side2 = nullptr;
+  cudaStream_t side = nullptr, side2 = nullptr, side3 = nullptr;   // side3: net 1's sensor reverse sweep (beside net 0's on `side`)
   cudaEvent_t ev_pool[8] = {};
   int n_sens_chunks = 1;
   float* fbuf = nullptr;       // NEXT-2: [R_ld] f values of a chunk / the critic's adjoint of them
