@@ -186,6 +186,16 @@ def test_width_128_fused_forward_depths_and_layer_by_layer(L):
     check_step(cfg, flags=FLAG_ONE_CTA)
 
 
+def test_multi_stream_step_is_stable_over_contexts_and_replays():
+    """At widths <= 256 a step runs on four event-linked streams (the two nets, the critic + net 0's sensor reverse sweep,
+    net 1's sensor reverse sweep).  A missing dependency would show as an occasional wrong gradient:
+    ten fresh contexts, eager, captured and replayed calls, every tensor against the oracle each time (fp32 and 16-bit)."""
+    small = dataclasses.replace(wl.CONFIGS["c2"], name="c2-streams", N=12, G=32, S=40)
+    for rep in range(10):
+        check_step(small, calls=1 + rep % 4)
+        check_step(wl.CONFIGS["c1"], calls=1 + (rep + 2) % 4)
+
+
 def test_width_384_one_cta_kernels_and_one_cta_flag():
     """Widths that are multiples of 128 but not of 256 run the one-CTA tcgen05 kernels (wgrad tile width must divide H);
     PIGAN_FLAG_ONE_CTA forces the same kernels on a CTA-pair width."""
