@@ -184,6 +184,30 @@ pigan_status pigan_train_step_grads_hier(pigan_ctx* ctx, const float* logk_param
 pigan_status pigan_adam_update(pigan_ctx* ctx, float* params, const float* grads, float* m, float* v, size_t n,
                                int step, float lr, float beta1, float beta2, float adam_eps, const int* skip_flag);
 
+/* a5 WITHOUT A CONTEXT AND WITHOUT ANY ALLOCATION: the Darcy residual of pigan_darcy_residual (Eq. 1) for callers that
+ * cannot allocate device memory.  Who they are: code hosted inside another program (a solver, a simulator, a serving process)
+ * that took nearly all GPU memory for its own pool when it started, so that cudaMalloc fails or is forbidden by the host's
+ * rules; and control / time-stepping loops that must not call cudaMalloc or cudaFree in steady state because those calls can
+ * stall the whole device for an unpredictable time.  pigan_create allocates workspaces, so such callers cannot have a context.
+ * This call makes no cudaMalloc, cudaFree or allocating library call, on its first use or later.  The scratch its reduction needs
+ * (one partial sum of r^2 per 1024 rows, plus a ticket counter) is a fixed array built into the library image.
+ *   logk_jet [>=3][N][P] (channels 0..2 read; plane stride N*P), u_jet [5][N][P], f [P]: DEVICE pointers, fp32, owned by the caller.
+ *   r [N][P] overwritten (may be NULL); mean_sq device scalar = mean r^2, overwritten (may be NULL); N*P = 0 writes mean_sq = 0.
+ *   cuda_stream: a cudaStream_t (NULL = legacy default stream) of the CURRENT device; the call is asynchronous on it.
+ * Limits and sharing:
+ *   - N*P <= PIGAN_STATIC_MAX_ROWS (2^24 rows); more is refused with PIGAN_ERR_UNSUPPORTED and a message naming the limit
+ *     (split the rows over several calls, or use a context).
+ *   - The array (about 128 KiB) sits on every GPU that loads the library's device code, until the process exits.
+ *   - All calls on one GPU share the array and it keeps the previous call's contents; each call zeroes the counter it depends on.
+ *     Calls that can overlap on the same GPU (two streams, two threads) race on it: the caller must order them (one stream does).
+ *   - The first call on each device looks up the array's device address (cudaGetSymbolAddress, with that device current) and
+ *     keeps it; make that first call before starting any stream capture.
+ * Returns a pigan_status; pigan_static_last_error() gives the message of the calling thread's last failed call ("" after success). */
+#define PIGAN_STATIC_MAX_ROWS (1LL << 24)
+pigan_status pigan_darcy_residual_static(const float* logk_jet, const float* u_jet, const float* f, int n_samples, int n_pts,
+                                         float* r, float* mean_sq, void* cuda_stream);
+const char*  pigan_static_last_error(void);
+
 #ifdef __cplusplus
 }
 #endif

@@ -12,7 +12,8 @@ from ctypes import POINTER, Structure, c_char_p, c_float, c_int, c_size_t, c_ulo
 
 from .build import LIB, build, is_stale
 
-__all__ = ["PiGan", "PiganError", "load_library", "param_count", "EXPORTED_SYMBOLS", "PRECISIONS", "FLAG_NO_GRAPH", "FLAG_ONE_CTA"]
+__all__ = ["PiGan", "PiganError", "load_library", "param_count", "EXPORTED_SYMBOLS", "PRECISIONS", "FLAG_NO_GRAPH", "FLAG_ONE_CTA",
+           "darcy_residual_static", "STATIC_MAX_ROWS"]
 
 FLAG_NO_GRAPH, FLAG_ONE_CTA = 1, 2                     # pigan_config.flags (include/pigan.h)
 
@@ -22,7 +23,9 @@ STATUS = {0: "PIGAN_OK", 1: "PIGAN_ERR_INVALID_ARG", 2: "PIGAN_ERR_SHAPE", 3: "P
 EXPORTED_SYMBOLS = ["pigan_create", "pigan_destroy", "pigan_param_count", "pigan_trunk_param_count", "pigan_last_error", "pigan_launch_count",
                     "pigan_profile_enable", "pigan_profile_report", "pigan_trunk_jet_forward",
                     "pigan_gen_jet_forward", "pigan_darcy_residual", "pigan_disc_forward", "pigan_gradient_penalty",
-                    "pigan_train_step_grads", "pigan_train_step_grads_hier", "pigan_adam_update"]
+                    "pigan_train_step_grads", "pigan_train_step_grads_hier", "pigan_adam_update",
+                    "pigan_darcy_residual_static", "pigan_static_last_error"]
+STATIC_MAX_ROWS = 1 << 24                              # PIGAN_STATIC_MAX_ROWS (include/pigan.h)
 
 
 class PiganError(RuntimeError):
@@ -79,8 +82,12 @@ def load_library():
                                       c_float, c_void_p]
     lib.pigan_profile_enable.argtypes = [c_void_p, c_int]
     lib.pigan_profile_report.argtypes = [c_void_p, c_char_p, c_size_t]
+    lib.pigan_darcy_residual_static.argtypes = [c_void_p, c_void_p, c_void_p, c_int, c_int, c_void_p, c_void_p, c_void_p]
+    lib.pigan_static_last_error.argtypes = []
+    lib.pigan_static_last_error.restype = c_char_p
     for name in EXPORTED_SYMBOLS:
-        if name not in ("pigan_create", "pigan_destroy", "pigan_param_count", "pigan_trunk_param_count", "pigan_last_error", "pigan_launch_count"):
+        if name not in ("pigan_create", "pigan_destroy", "pigan_param_count", "pigan_trunk_param_count", "pigan_last_error", "pigan_launch_count",
+                        "pigan_static_last_error"):
             getattr(lib, name).restype = c_int
     del fp, ip
     _lib = lib
@@ -108,6 +115,37 @@ def _ptr(t, name, dtype=None):
     if t.dtype != (dtype or torch.float32):
         raise TypeError(f"{name} must have dtype {dtype or torch.float32}, got {t.dtype}")
     return c_void_p(t.data_ptr())
+
+
+def darcy_residual_static(logk_jet, u_jet, f, r=None, mean_sq=None, stream=None):
+    """The Darcy residual through pigan_darcy_residual_static: no context, and no device allocation inside the library.
+
+    For programs that cannot allocate GPU memory when they call us -- code embedded in a host application that gave all device
+    memory to its own pool at start-up (cudaMalloc fails or is off limits there), or a latency-bound loop that keeps
+    cudaMalloc / cudaFree out of its steady state because they can stall the device.  A PiGan context allocates workspaces when
+    it is created, so it is not an option for them.  Such a caller passes its OWN output tensors: `r` [N][P] and / or `mean_sq` [1]
+    (fp32, CUDA, contiguous) are written in place and returned; at least one must be given, and nothing is allocated here or
+    in the library.  logk_jet [>=3][N][P], u_jet [5][N][P], f [P].
+    Limits: N*P <= STATIC_MAX_ROWS (2^24), else PiganError(PIGAN_ERR_UNSUPPORTED).  The library's built-in scratch array is shared by
+    every call on a GPU: calls that may overlap (different streams / threads) must be ordered by the caller.  The first call on
+    a device also looks up the array's address; make it before any stream capture starts.  Runs on `stream` (default: the
+    current stream) of the tensors' device."""
+    import torch
+    if logk_jet.shape[1:] != u_jet.shape[1:] or logk_jet.shape[0] < 3 or u_jet.shape[0] != 5:
+        raise ValueError("logk_jet must be [>=3][N][P] and u_jet [5][N][P]")
+    if r is None and mean_sq is None:
+        raise ValueError("pass r and / or mean_sq: the caller owns the outputs, nothing is allocated here")
+    lib = load_library()
+    N, P = u_jet.shape[1], u_jet.shape[2]
+    if r is not None and r.numel() != N * P or mean_sq is not None and mean_sq.numel() < 1:
+        raise ValueError("r must hold N*P values and mean_sq one")
+    with torch.cuda.device(u_jet.device):
+        st = stream if stream is not None else torch.cuda.current_stream(u_jet.device)
+        rc = lib.pigan_darcy_residual_static(_ptr(logk_jet, "logk_jet"), _ptr(u_jet, "u_jet"), _ptr(f, "f"), N, P, _ptr(r, "r"),
+                                             _ptr(mean_sq, "mean_sq"), c_void_p(st.cuda_stream))
+    if rc != 0:
+        raise PiganError(rc, lib.pigan_static_last_error().decode())
+    return r, mean_sq
 
 
 class PiGan:
