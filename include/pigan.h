@@ -45,17 +45,17 @@ typedef enum {
   PIGAN_ERR_SHAPE = 2,         /* a size disagrees with the pigan_config the context was created with */
   PIGAN_ERR_ALLOC = 3,         /* workspace allocation failed */
   PIGAN_ERR_CUDA = 4,          /* a CUDA runtime / driver call failed (no device, launch error, ...) */
-  PIGAN_ERR_UNSUPPORTED = 5    /* e.g. 16-bit precision with a width that is not a multiple of 128 */
+  PIGAN_ERR_UNSUPPORTED = 5    /* e.g. 16-bit precision with a width that is not a multiple of 128; PIGAN_BF16 */
 } pigan_status;
 
 /* Arithmetic of the hidden jet layers (S8a a3, a10).  FP32: plain FP32 FMA.  FP16: tcgen05 tensor cores, fp16
  * operands (the paper's arithmetic), fp32 accumulation in TMEM, fp32 epilogue; first layer, output dot, residual,
  * critic, norms, reductions and weight-gradient accumulation stay fp32 (reading G18).
- * PIGAN_BF16 is an ALIAS of PIGAN_FP16: it selects exactly the same fp16-operand path (reading R1: bf16
- * activation planes measure 1-2e-2 against the 2e-2 tolerance, and kind::f16 rejects mixed operands).  Weights that
- * were rounded to bf16 convert to fp16 exactly for |w| >= 2^-14.  Consequence: in both 16-bit modes activation and jet
- * planes have fp16 RANGE (65504); the derivative channels grow with products of layer gains, and a forward overflow
- * surfaces as inf/nan gradients with *found_inf = 1 (never as silently wrong finite values). */
+ * PIGAN_BF16 is NOT IMPLEMENTED: pigan_create returns PIGAN_ERR_UNSUPPORTED for it (reading R1: bf16 activation
+ * planes measure 1-2e-2 against the 2e-2 tolerance, so the library's one 16-bit arithmetic is the paper's FP16; the
+ * enum value is kept so that the numbering of pigan_precision is stable).  Consequence of FP16: activation and jet planes
+ * have fp16 RANGE (65504); the derivative channels grow with products of layer gains, and a forward overflow surfaces
+ * as inf/nan gradients with *found_inf = 1 (never as silently wrong finite values). */
 typedef enum { PIGAN_FP32 = 0, PIGAN_BF16 = 1, PIGAN_FP16 = 2 } pigan_precision;
 
 /* pigan_config.flags (debug / measurement switches; 0 is the product path) */

@@ -245,6 +245,7 @@ pigan_status pigan_create(const pigan_config* cfg, void* cuda_stream, pigan_ctx*
   if (cfg->n_critics > 0 && (cfg->n_free > 0 || cfg->gen_variant != PIGAN_GEN_TWO_MLPS)) return PIGAN_ERR_UNSUPPORTED;
   if (cfg->n_free > 0 && cfg->n_colloc != cfg->n_free) return PIGAN_ERR_SHAPE;
   if (cfg->n_free > 0 && cfg->gen_variant != PIGAN_GEN_TWO_MLPS) return PIGAN_ERR_UNSUPPORTED;
+  if (cfg->precision == PIGAN_BF16) return PIGAN_ERR_UNSUPPORTED;     // no bf16 datapath (pigan.h); never an alias of another arithmetic
   if (cfg->precision != PIGAN_FP32) {
     std::string why;
     if (!tc_supported(cfg->gen.width, &why)) return PIGAN_ERR_UNSUPPORTED;
@@ -389,7 +390,6 @@ pigan_status pigan_gen_jet_forward(pigan_ctx* c, const float* gen_params, const 
   const int C = jet_order == 0 ? 1 : jet_order == 1 ? 3 : 5;
   switch (c->cfg.precision) {
     case PIGAN_FP32: return jet_forward_impl<float>(c, gen_params, xy, n_pts, z, n_samples, C, out);
-    case PIGAN_BF16: return jet_forward_impl<__half>(c, gen_params, xy, n_pts, z, n_samples, C, out);
     default: return jet_forward_impl<__half>(c, gen_params, xy, n_pts, z, n_samples, C, out);
   }
 }

@@ -446,7 +446,7 @@ __global__ void __launch_bounds__(256) convert_weights_kernel(NetShape s, const 
 void tc_convert_weights(Launcher& L, int precision, const NetShape& s, const float* theta, void* w16) {
   if (s.L < 2) return;
   dim3 grid(s.H / 32, s.H / 32, s.L - 1);
-  (void)precision;   // bf16-representable weights convert to fp16 exactly (|w| >= 2^-14), so both 16-bit modes share the fp16 copies
+  (void)precision;   // PIGAN_FP16 is the only 16-bit mode (pigan_create refuses PIGAN_BF16)
   convert_weights_kernel<__half><<<grid, 256, 0, L.stream>>>(s, theta, (__half*)w16);
   L.check("convert_weights");
 }

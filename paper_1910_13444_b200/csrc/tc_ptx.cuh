@@ -300,7 +300,7 @@ inline EncodeTiledFn get_encode() {
   return fn;
 }
 
-// precision: both 16-bit modes carry fp16 planes and weight copies (include/pigan.h: PIGAN_BF16 is an alias of PIGAN_FP16)
+// precision: the 16-bit mode carries fp16 planes and weight copies (include/pigan.h: PIGAN_BF16 is refused by pigan_create)
 inline bool make_map(Launcher& L, CUtensorMap* m, int precision, const void* base, int rank, const cuuint64_t* dims, const cuuint64_t* strides_bytes,
                      const cuuint32_t* box, CUtensorMapSwizzle swz) {
   EncodeTiledFn fn = get_encode();

@@ -39,6 +39,10 @@ def test_create_validates_config_before_touching_cuda():
     assert lib.pigan_create(ctypes.byref(bad_shape), None, ctypes.byref(ctx)) == 2                                   # SHAPE
     unsup = pkg._Config(pkg._MlpShape(6, 3, 32), pkg._MlpShape(20, 3, 32), 4, 16, 64, 10, 1, 10.0, 1.0, 0, 0, 0)         # bf16 with width 32
     assert lib.pigan_create(ctypes.byref(unsup), None, ctypes.byref(ctx)) == 5                                       # UNSUPPORTED
+    fp16_w32 = pkg._Config(pkg._MlpShape(6, 3, 32), pkg._MlpShape(20, 3, 32), 4, 16, 64, 10, 2, 10.0, 1.0, 0, 0, 0)      # fp16 with width 32
+    assert lib.pigan_create(ctypes.byref(fp16_w32), None, ctypes.byref(ctx)) == 5
+    bf16_w128 = pkg._Config(pkg._MlpShape(6, 3, 128), pkg._MlpShape(20, 3, 32), 4, 16, 64, 10, 1, 10.0, 1.0, 0, 0, 0)    # PIGAN_BF16 at a width fp16 supports:
+    assert lib.pigan_create(ctypes.byref(bf16_w128), None, ctypes.byref(ctx)) == 5                                   # refused, never aliased to fp16
     neg = pkg._Config(pkg._MlpShape(6, 0, 32), pkg._MlpShape(20, 3, 32), 4, 16, 64, 10, 0, 10.0, 1.0, 0, 0, 0)
     assert lib.pigan_create(ctypes.byref(neg), None, ctypes.byref(ctx)) == 1
 
