@@ -68,6 +68,21 @@ def test_generator_gradient_matches_finite_differences_with_overlapping_subdomai
     # each critic's gradient is the pinned single-critic WGAN-GP gradient on its sub-snapshot
     X = np.concatenate([orc.gen_jet_forward_ref(tiny["theta_Y"], *cfg.gen_shape, tiny["xy_sensors"], tiny["z"], 0)[0],
                         orc.gen_jet_forward_ref(tiny["theta_u"], *cfg.gen_shape, tiny["xy_sensors"], tiny["z"], 0)[0]], axis=1)
+    # (the VALUE, critic by critic, with DISTINCT subsets: a wrong real[:, idx] or fake[:, idx] for k > 0 fails here).
+    # g_Dk = d/dtheta [mean D_k(fake_k) - mean D_k(real_k)] + d GP_k/dtheta: the Wasserstein part by central differences of the plain
+    # forward disc_forward_ref in every parameter of critic k, the penalty part from gradient_penalty_ref (pinned on its own by
+    # closed forms and torch fp64 double backward in test_oracle_critic.py) evaluated on critic k's sub-snapshots.
     for k in range(3):
-        _, _, gp_grad = orc.gradient_penalty_ref(thDs[k], *disc_shape, tiny["real"][:, subsets[k]], X[:, subsets[k]], tiny["eps"], 10.0)
-        assert np.abs(gD[k]).max() > 0 and gD[k].shape == gp_grad.shape
+        real_k, fake_k = tiny["real"][:, subsets[k]], X[:, subsets[k]]
+        W = lambda th: orc.disc_forward_ref(th, *disc_shape, fake_k).mean() - orc.disc_forward_ref(th, *disc_shape, real_k).mean()
+        fd = np.empty_like(thDs[k])
+        for i in range(thDs[k].size):
+            e = np.zeros_like(thDs[k]); e[i] = h
+            fd[i] = (W(thDs[k] + e) - W(thDs[k] - e)) / (2 * h)
+        _, _, gp_own = orc.gradient_penalty_ref(thDs[k], *disc_shape, real_k, fake_k, tiny["eps"], 10.0)
+        assert np.abs(gD[k]).max() > 0 and gD[k].shape == fd.shape
+        assert np.abs(fd + gp_own - gD[k]).max() <= 5e-7 * max(1.0, np.abs(gD[k]).max()), (k, np.abs(fd + gp_own - gD[k]).max())
+        # and it is NOT the gradient on another critic's columns (the subsets are distinct, so the pin can tell them apart)
+        other = subsets[(k + 1) % 3]
+        _, _, gp_other = orc.gradient_penalty_ref(thDs[k], *disc_shape, tiny["real"][:, other], X[:, other], tiny["eps"], 10.0)
+        assert np.abs(gp_other - gp_own).max() > 1e-3 * np.abs(gp_own).max()
