@@ -188,7 +188,11 @@ class GpuWorkload:
         import torch
         from paper_1910_13444_b200 import PiGan
         self.cfg, self.device, self.torch = cfg, device, torch
-        inp = wl.make_inputs(dataclasses.replace(cfg, index=cfg.index + 10 * seed_shift) if seed_shift else cfg)
+        inp = wl.make_inputs(cfg)
+        if seed_shift:      # data-parallel ranks are REPLICAS: identical parameters (and teachers), their own latent / real / eps streams
+            own = wl.make_inputs(dataclasses.replace(cfg, index=cfg.index + 10 * seed_shift))
+            for k in ("z", "z_real", "eps"):
+                inp[k] = own[k]
         self.trunk = cfg.variant != "two_mlps"
         self.pg = PiGan.from_config(cfg, device=device, chunk_rows=chunk_rows, gen_variant=cfg.variant)
         d = {k: torch.from_numpy(np.ascontiguousarray(v)).to(device) for k, v in inp.items()}

@@ -74,7 +74,11 @@ class DataParallelTrainer:
         dev = self.params[0].device
         self.out = FlatGrads([p.numel() for p in self.params], dev)
         self.mom = [(torch.zeros_like(p), torch.zeros_like(p)) for p in self.params]
-        self.t = [0] * len(self.params)                       # Adam step counters (a skipped step does not advance its counter's effect)
+        # Adam step counters.  They count ATTEMPTED updates: found_inf lives on the device and reading it back every step would
+        # serialise host and GPU, so a step that pigan_adam_update skips (overflow) still advances t.  Parameters and moments
+        # stay bit-identical on a skipped step; only the bias correction 1 - beta^t runs one step ahead per skipped step,
+        # which vanishes as t grows (with beta2 = 0.9: below 1e-4 after ~90 steps).
+        self.t = [0] * len(self.params)
         self.step_calls = 0
 
     def _grads(self, z, real, eps):
