@@ -169,8 +169,9 @@ pigan_status pigan_train_step_grads(pigan_ctx* ctx, const float* logk_params, co
  *   n_critics = K > 0.  As pigan_train_step_grads, except:
  *   disc_params, g_disc  [K][param_count(cfg.disc)]: critic k's parameters / the gradient of ITS loss
  *                        L_Dk = mean D_k(fake_k) - mean D_k(real_k) + GP_k (shared eps);
- *   subsets  DEVICE int [K][cfg.disc.in_dim]: the snapshot columns (0 .. 2S-1, distinct within a critic) that critic k sees;
- *   weights  HOST float [K]: w_k = 1 / (levels * subdomains in k's level); L_G = sum_k w_k (-mean D_k(fake_k)) + w_pde mean r^2;
+ *   subsets  DEVICE int [K][cfg.disc.in_dim]: the snapshot columns (0 .. 2S-1, distinct within a critic) that critic k sees; they are
+ *            not checked here (a device array): a column out of range or repeated within a critic is undefined behaviour;
+ *   weights  HOST float [K], read during the call only (it may be freed or changed as soon as the call returns): w_k = 1 / (levels * subdomains in k's level); L_G = sum_k w_k (-mean D_k(fake_k)) + w_pde mean r^2;
  *   real_snap [N][2S];  losses[6] = {sum_k L_Dk, sum_k w_k mean D_k(fake), sum_k w_k mean D_k(real), sum_k GP_k, L_G, L_pde}.
  *   Runs eagerly (no CUDA-graph replay). */
 pigan_status pigan_train_step_grads_hier(pigan_ctx* ctx, const float* logk_params, const float* u_params, const float* disc_params,

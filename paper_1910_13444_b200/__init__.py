@@ -277,6 +277,16 @@ class PiGan:
         subsets: int32 CUDA tensor [K][critic_inputs]; weights: K host floats.  Returns (g_logk, g_u, g_disc [K][n_disc], losses, found_inf)."""
         import torch
         K = self.n_critics
+        # the kernels index the snapshot with `subsets` and add into it without atomics: columns out of range or repeated within a
+        # critic are undefined behaviour in the C call.  Checked here once per tensor (and again if it is modified in place).
+        key = (subsets.data_ptr(), subsets._version, tuple(subsets.shape))
+        if getattr(self, "_subsets_checked", None) != key:
+            s = subsets.detach().cpu()
+            if tuple(s.shape) != (K, self.disc_shape[0]) or int(s.min()) < 0 or int(s.max()) >= 2 * self.S:
+                raise ValueError(f"subsets must be [{K}][{self.disc_shape[0]}] with entries in [0, {2 * self.S})")
+            if any(len(set(row.tolist())) != row.numel() for row in s):
+                raise ValueError("the columns of one critic must be distinct")
+            self._subsets_checked = key
         out = (self._new(self.n_gen), self._new(self.n_gen), self._new(K, self.n_disc), self._new(6), self._new(1, dtype=torch.int32))
         w = (c_float * K)(*[float(x) for x in weights])
         self._check(self._lib.pigan_train_step_grads_hier(
@@ -284,8 +294,7 @@ class PiGan:
             _ptr(subsets, "subsets", torch.int32), w, _ptr(xy_colloc, "xy_colloc"), _ptr(f, "f"), _ptr(xy_sensors, "xy_sensors"), _ptr(z, "z"),
             _ptr(real_snap, "real_snap"), _ptr(eps, "eps"), float(loss_scale), _ptr(out[0], "g_logk"), _ptr(out[1], "g_u"), _ptr(out[2], "g_disc"),
             _ptr(out[3], "losses"), _ptr(out[4], "found_inf", torch.int32)))
-        torch.cuda.current_stream(self.device).synchronize()    # `weights` is a host array read while the step is enqueued; keep it alive
-        return out
+        return out            # no synchronise: the library reads the host array `weights` during the call and passes w_k to its kernels by value
 
     def adam_update(self, params, grads, m, v, step, lr, beta1, beta2, adam_eps, skip_flag=None):
         import torch
