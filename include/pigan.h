@@ -151,8 +151,9 @@ pigan_status pigan_gradient_penalty(pigan_ctx* ctx, const float* disc_params, co
  *   loss_scale (host value, > 0) multiplies the adjoints of the 16-bit backward pass; gradients are returned
  *   UNSCALED in fp32 (overwritten).  losses[6] = {L_D, mean D(fake), mean D(real), GP, L_G, L_pde}.
  *   *found_inf (device int, overwritten) = 1 if any gradient is inf/nan, else 0.  losses, found_inf may be NULL.
- *   Execution: asynchronous on the context's stream.  A call whose arguments (all pointers and loss_scale) repeat the
- *   previous call's is captured into a CUDA graph and replayed on later identical calls; the arrays are read when the
+ *   Execution: asynchronous on the context's stream.  The first call with a given argument set (all pointers and loss_scale)
+ *   runs eagerly, the second call with that set is captured into a CUDA graph and later ones replay it; the four most recently
+ *   used argument sets are remembered, so alternating between a few sets of buffers replays as well.  The arrays are read when the
  *   step RUNS, so updating them in place between calls (an optimiser step, new z / eps copied into the same buffers)
  *   behaves exactly as an eager call.  cfg.flags & PIGAN_FLAG_NO_GRAPH disables the replay; cfg.chunk_rows sets the
  *   row-chunk size (default 131072 rows; workspace_bytes of the config bounds it as well).  No environment variable

@@ -284,11 +284,18 @@ pigan_status pigan_create(const pigan_config* cfg, void* cuda_stream, pigan_ctx*
   size_t per_row = 0;
   for (int C : {3, 5}) per_row += ((size_t)Lh * C + 2 * C) * H * c->elem + (f32 ? (size_t)C * H * 4 : 0) + 2 * C * 4;
   if (c->skip) per_row += ((size_t)Lh * 5 + 2 * 5) * H * c->elem;           // tanh-jet stash, skip adjoint, raw adjoint planes (net[1])
+  // the sensor rows' stash hs (both nets: L x (hi, lo) planes per sensor chunk, kept from the snapshot forward to the reverse sweep;
+  // + the tanh-jet stash hts with skips) holds ceil(N S / rows) chunks of `rows` rows: at most (N S + rows) rows' worth
+  const size_t sens_row = (size_t)(2 + (c->skip ? 1 : 0)) * Lh * 2 * H * c->elem;
+  per_row += sens_row;
+  // the sensor rows' own adjoint set at widths <= 256 (value channel: two planes, output adjoint, fp32 scratch), both nets
+  if (H <= 256 && !c->trunk && cfg->n_free == 0) per_row += 2 * ((size_t)2 * H * c->elem + 4 + (f32 ? (size_t)H * 4 : 0));
   const long long max_rows = std::max<long long>((long long)N * cfg->n_colloc, (long long)N * S);
   size_t free_b = 0, total_b = 0;
   cudaMemGetInfo(&free_b, &total_b);
   size_t budget = cfg->workspace_bytes ? cfg->workspace_bytes : std::min<size_t>(free_b / 2, (size_t)48 << 30);
-  long long rows = (long long)(budget / per_row);
+  const size_t sens_fixed = (size_t)N * S * sens_row;
+  long long rows = budget > sens_fixed ? (long long)((budget - sens_fixed) / per_row) : 0;
   long long cap = 131072;                                  // default chunk rows (sweep on B200: larger chunks amortise launch ramps)
   if (cfg->chunk_rows > 0) cap = std::max(256, cfg->chunk_rows);
   if (!cfg->workspace_bytes) rows = std::min(rows, cap);
@@ -367,7 +374,7 @@ pigan_status pigan_create(const pigan_config* cfg, void* cuda_stream, pigan_ctx*
 void pigan_destroy(pigan_ctx* c) {
   if (!c) return;
   DeviceGuard dg(c);
-  if (c->sg.exec) cudaGraphExecDestroy(c->sg.exec);
+  for (auto& e : c->sg.entries) if (e.exec) cudaGraphExecDestroy(e.exec);
   if (c->sg.cap_stream) cudaStreamDestroy(c->sg.cap_stream);
   if (c->side) cudaStreamDestroy(c->side);
   if (c->side2) cudaStreamDestroy(c->side2);
@@ -488,17 +495,29 @@ pigan_status pigan_train_step_grads(pigan_ctx* c, const float* logk_params, cons
   std::vector<unsigned long long> key;
   for (const void* q : ptrs) key.push_back((unsigned long long)(uintptr_t)q);
   key.push_back(ls_bits);
-  if (sg.exec && key == sg.key) {                            // replay
-    if (cudaGraphLaunch(sg.exec, c->L.stream) != cudaSuccess) { cudaGetLastError(); return fail(c, PIGAN_ERR_CUDA, "cudaGraphLaunch failed"); }
-    c->L.count += sg.launches;
+  using Entry = pigan_ctx::StepGraph::Entry;
+  Entry* ent = nullptr;
+  for (Entry& e : sg.entries) if (e.key == key) { ent = &e; break; }
+  ++sg.tick;
+  if (ent && ent->exec) {                                    // replay
+    ent->last_use = sg.tick;
+    if (cudaGraphLaunch(ent->exec, c->L.stream) != cudaSuccess) { cudaGetLastError(); return fail(c, PIGAN_ERR_CUDA, "cudaGraphLaunch failed"); }
+    c->L.count += ent->launches;
     return PIGAN_OK;
   }
-  if (key != sg.last_key) {                                  // first sight of these arguments: run eagerly (also sets kernel attributes)
-    sg.last_key = key;
+  if (!ent) {                                                // first sight of these arguments: run eagerly (also sets kernel attributes)
+    if ((int)sg.entries.size() == pigan_ctx::StepGraph::kMaxGraphs) {      // forget the least recently used argument set
+      size_t lru = 0;
+      for (size_t k = 1; k < sg.entries.size(); ++k) if (sg.entries[k].last_use < sg.entries[lru].last_use) lru = k;
+      if (sg.entries[lru].exec) cudaGraphExecDestroy(sg.entries[lru].exec);
+      sg.entries.erase(sg.entries.begin() + lru);
+    }
+    Entry e; e.key = key; e.last_use = sg.tick;
+    sg.entries.push_back(e);
     return run();
   }
-  // second consecutive call with the same arguments: capture on the private stream, then replay on the caller's
-  if (sg.exec) { cudaGraphExecDestroy(sg.exec); sg.exec = nullptr; sg.key.clear(); }
+  // second call with these arguments: capture on the private stream, then replay on the caller's
+  ent->last_use = sg.tick;
   if (!sg.cap_stream && cudaStreamCreateWithFlags(&sg.cap_stream, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); sg.disabled = true; return run(); }
   cudaStream_t user = c->L.stream;
   const unsigned long long count0 = c->L.count;
@@ -510,16 +529,16 @@ pigan_status pigan_train_step_grads(pigan_ctx* c, const float* logk_params, cons
   const cudaError_t e = cudaStreamEndCapture(sg.cap_stream, &graph);
   const unsigned long long n_launch = c->L.count - count0;
   c->L.count = count0;
-  if (st != PIGAN_OK || e != cudaSuccess || !graph || cudaGraphInstantiate(&sg.exec, graph, 0) != cudaSuccess) {
+  if (st != PIGAN_OK || e != cudaSuccess || !graph || cudaGraphInstantiate(&ent->exec, graph, 0) != cudaSuccess) {
     cudaGetLastError();
     if (graph) cudaGraphDestroy(graph);
-    sg.exec = nullptr; sg.disabled = true;                   // capture is not possible here: stay eager for the life of the context
+    ent->exec = nullptr; sg.disabled = true;                 // capture is not possible here: stay eager for the life of the context
     return run();
   }
   cudaGraphDestroy(graph);
-  sg.key = key; sg.launches = n_launch;
-  if (cudaGraphLaunch(sg.exec, user) != cudaSuccess) { cudaGetLastError(); return fail(c, PIGAN_ERR_CUDA, "cudaGraphLaunch failed"); }
-  c->L.count += sg.launches;
+  ent->launches = n_launch;
+  if (cudaGraphLaunch(ent->exec, user) != cudaSuccess) { cudaGetLastError(); return fail(c, PIGAN_ERR_CUDA, "cudaGraphLaunch failed"); }
+  c->L.count += ent->launches;
   return PIGAN_OK;
 }
 

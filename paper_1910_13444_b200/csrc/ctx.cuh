@@ -52,13 +52,21 @@ struct pigan_ctx {
   float* amax_s = nullptr;     // [2] the same for the sensor rows' own adjoint set (null: the sensor rows share net[n].ah / oh)
   std::vector<void*> allocs;
   // CUDA-graph replay of pigan_train_step_grads: the step is hundreds to thousands of launches, launch-latency bound
-  // for the small configs.  A call whose arguments repeat the previous call's is captured once (on a private stream,
-  // so the caller's stream may be the legacy default stream) and replayed from then on.  PIGAN_FLAG_NO_GRAPH disables it.
+  // for the small configs.  The first call with a given argument set runs eagerly (it also sets kernel attributes); the second
+  // call with that set -- not necessarily the next call -- is captured (on a private stream, so the caller's stream may be the
+  // legacy default stream) and replayed from then on.  Up to kMaxGraphs argument sets are remembered (least recently used is
+  // dropped), so a caller that alternates between a few sets, e.g. the sequential schedule with two output buffers, replays
+  // too.  PIGAN_FLAG_NO_GRAPH disables it.
   struct StepGraph {
+    static constexpr int kMaxGraphs = 4;
+    struct Entry {
+      std::vector<unsigned long long> key;
+      cudaGraphExec_t exec = nullptr;                  // null: seen once, not captured yet
+      unsigned long long launches = 0, last_use = 0;
+    };
     cudaStream_t cap_stream = nullptr;
-    cudaGraphExec_t exec = nullptr;
-    std::vector<unsigned long long> key, last_key;
-    unsigned long long launches = 0;
+    std::vector<Entry> entries;
+    unsigned long long tick = 0;
     bool disabled = false;
   } sg;
 

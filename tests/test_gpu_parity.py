@@ -10,7 +10,7 @@ import pytest
 
 import workloads as wl
 from oracle import pigan_oracle as orc
-from parity_util import free_step_parity, jets_parity, per_layer, rel_err, step_parity, to_dev, trunk_step_parity
+from parity_util import free_step_parity, jets_parity, oracle_step, per_layer, rel_err, step_parity, to_dev, trunk_step_parity
 
 pytestmark = pytest.mark.gpu
 
@@ -163,6 +163,43 @@ def test_c3_full_size_step_and_graph_replay():
     cfg = wl.CONFIGS["c3"]
     check_step(cfg, bias_std=0.0)
     check_step(cfg, bias_std=0.0, calls=3)                  # call 2 captures, call 3 replays
+
+
+def test_alternating_argument_sets_are_captured_and_replayed_separately():
+    """A caller that alternates between argument sets (here: two latent batches with two sets of output buffers, as the sequential
+    schedule with separate buffers does) never repeats the PREVIOUS call's arguments.  The library remembers the last four sets:
+    each is run eagerly once, captured on its second call and replayed afterwards.  Set A is checked against the oracle, set B
+    against an eager (PIGAN_FLAG_NO_GRAPH) context; a fifth and sixth set push the oldest out and everything still holds."""
+    import torch
+    from paper_1910_13444_b200 import FLAG_NO_GRAPH, PiGan
+    cfg = wl.CONFIGS["c1"]
+    inp, (gY, gu, gD, losses) = oracle_step(cfg, 0.1, 1.0, 1.0)
+    d = to_dev(inp, "cuda:0")
+    pg, eager = PiGan.from_config(cfg), PiGan.from_config(cfg, flags=FLAG_NO_GRAPH)
+    zs = [d["z"]] + [torch.randn_like(d["z"], generator=torch.Generator(device="cuda").manual_seed(5 + i)) for i in range(5)]
+    call = lambda ctx, z, out=None: ctx.train_step_grads(d["theta_Y"], d["theta_u"], d["theta_D"], d["xy_colloc"], d["f"], d["xy_sensors"], z,
+                                                         d["real"], d["eps"], 1.0, out=out)
+    want = [call(eager, z) for z in zs]
+    outs = [None] * len(zs)
+    per_call = []
+    for rnd in range(4):                                       # A B A B A B A B: eager, capture, replay, replay for each of the two
+        for i in (0, 1):
+            n0 = pg.launch_count
+            outs[i] = call(pg, zs[i], outs[i])
+            per_call.append(pg.launch_count - n0)
+    for rnd in range(3):                                       # six sets in rotation: more than the cache holds, every call still right
+        for i in range(len(zs)):
+            outs[i] = call(pg, zs[i], outs[i])
+    torch.cuda.synchronize()
+    assert len(set(per_call)) == 1, per_call                   # a replay accounts for the launches of the step it replays
+    for i in range(len(zs)):
+        for k in range(3):
+            assert rel_err(outs[i][k].cpu().numpy(), want[i][k].cpu().numpy()) <= 1e-5, (i, k)
+        assert np.allclose(outs[i][3].cpu().numpy(), want[i][3].cpu().numpy(), rtol=1e-5, atol=1e-7) and int(outs[i][4].item()) == 0
+    for g_gpu, g_ref in ((outs[0][0], gY), (outs[0][1], gu), (outs[0][2], gD)):
+        assert rel_err(g_gpu.cpu().numpy(), g_ref) <= TOL["fp32"]
+    assert np.all(np.abs(outs[0][3].cpu().numpy() - losses) <= LOSS_TOL * np.abs(losses))
+    pg.close(); eager.close()
 
 
 @pytest.mark.parametrize("name,N,G,chunk", [("c4", 8, 64, 8192), ("c5", 4, 64, 4096)])
