@@ -356,16 +356,22 @@ def run_config(cfg, device, steps, warmup, rank, world, with_roofline=True, seed
             Lh = cfg.L - 1
             # width 256: dgrad and wgrad of a layer are ONE kernel (jet_layer_bwd_wgrad): two of the three GEMMs, planes read once
             # width 128: the whole forward of the collocation rows is ONE kernel (gen_fwd_fused): it writes h^1 .. h^L and reads no planes
-            cls_bytes = {"jet_layer_fwd": 2 * rowsC * pb * Lh, "jet_layer_bwd": rowsC * pb * (3 * Lh - 1), "wgrad": 2 * rowsC * pb * Lh,
-                         "jet_layer_bwd_wgrad": rowsC * pb * (3 * Lh - 1), "gen_fwd_fused": cfg.N * cfg.P * chan * pb * cfg.L}
-            cls_gemms = {"jet_layer_fwd": 1, "jet_layer_bwd": 1, "wgrad": 1, "jet_layer_bwd_wgrad": 2, "gen_fwd_fused": 1}
+            # Each class is credited the rows it actually processes: where the fused forward exists it does the collocation rows and
+            # the layer-by-layer forward (jet_layer_fwd) only the sensor rows; every other class sees both.
+            col, sen = flops["jet_gemm"] / 3, sens_gemm / 3      # one GEMM type (fwd, dgrad or wgrad) over the collocation / sensor rows
+            fwd_rows_sens_only = "gen_fwd_fused" in tc
+            rowsS = cfg.N * cfg.S * nets
+            cls_bytes = {"jet_layer_fwd": 2 * (rowsS if fwd_rows_sens_only else rowsC) * pb * Lh, "jet_layer_bwd": rowsC * pb * (3 * Lh - 1),
+                         "wgrad": 2 * rowsC * pb * Lh, "jet_layer_bwd_wgrad": rowsC * pb * (3 * Lh - 1), "gen_fwd_fused": cfg.N * cfg.P * chan * pb * cfg.L}
+            cls_flops = {"jet_layer_fwd": sen if fwd_rows_sens_only else col + sen, "jet_layer_bwd": col + sen, "wgrad": col + sen,
+                         "jet_layer_bwd_wgrad": 2 * (col + sen), "gen_fwd_fused": col}
             prof_ncu = ncu_profile(cfg.name)
             per_kernel = {}
             for k, v in tc.items():
                 if v[1] <= 0:
                     continue
                 t_ms = v[1] / steps
-                alg_k = alg * cls_gemms[k] / 3
+                alg_k = cls_flops[k]
                 t_tensor = alg_k / (peak * 1e12) * 1e3
                 t_hbm = cls_bytes[k] / (peaks["hbm_gbs"] * 1e9) * 1e3
                 pct = [d["tensor_pct"] for kk, d in prof_ncu.items() if kk.startswith(k + "(C=5") or kk == k]
@@ -385,7 +391,8 @@ def run_config(cfg, device, steps, warmup, rank, world, with_roofline=True, seed
                                "share_of_step": round(tc_ms / total_ms, 4) if total_ms > 0 else None,
                                "profile_pass": ("in the timed region: one CUDA event is recorded after every launch inside the timed steps, so `value` carries that "
                                                 "(~1 %) overhead") if in_region else "separate eager pass after the timed region (the timed region replays a CUDA graph)",
-                               "per_kernel": per_kernel}
+                               "per_kernel": per_kernel,
+                               "per_kernel_frac_le_1": all(v["frac"] <= 1.0 for v in per_kernel.values())}
         else:
             # fp32 mode (c1): plain FP32 FMA path; report against the fp32 ALU peak (148 SMs x 128 lanes x 2 flop x clock)
             mhz = res["clocks"]["sm_mhz"] or 1965.0
