@@ -51,10 +51,20 @@ class FlatGrads:
         self.found_inf = torch.zeros(1, dtype=torch.int32, device=device)
 
     def all_reduce_mean(self, dist, world: int):
-        """Sum over ranks, then 1/W: gradients and losses become the global means; flag > 0 iff any rank overflowed."""
+        """Sum over ranks, then 1/W: gradients and losses become the global means; flag > 0 iff any rank overflowed.
+
+        Stream order: the library's step -- eager launches or the replay of its CUDA graph -- is enqueued on
+        the context's stream, which is torch's current stream of the device (PiGan takes it at creation).  torch.distributed's
+        collective waits on an event recorded on torch's current stream before it starts on the backend's own stream, and the
+        synchronous form used here makes the current stream wait for its completion; the library's private capture stream and
+        side streams are joined back into the context's stream before a step call returns.  So the collective reads finished
+        gradients and Adam reads reduced ones, as long as the caller keeps ONE current stream around step, collective and update.
+        The collective is issued whenever a process group exists (also for a single rank: that keeps the one-rank path identical
+        to the many-rank path, and lets a one-GPU box execute it)."""
         self.flag.copy_(self.found_inf.to(torch.float32))
-        if world > 1:
+        if dist is not None:
             dist.all_reduce(self.flat, op=dist.ReduceOp.SUM)
+        if world > 1:
             self.flat.mul_(1.0 / world)
         self.found_inf.copy_((self.flag > 0).to(torch.int32))
 

@@ -148,10 +148,9 @@ def trunk_step_parity(cfg, skip, bias_std=0.1, loss_scale=1.0, chunk_rows=0, pde
 
 
 # ---- NEXT-2: f at per-sample free sensors fed to the critic --------------------------------------------------------
-def free_step_parity(cfg, F, bias_std=0.1, loss_scale=1.0, chunk_rows=0, pde_weight=0.0):
+def free_case(cfg, F, bias_std=0.1):
+    """Seeded inputs of a NEXT-2 case (no arithmetic of the method beyond calling the oracle for the real snapshots)."""
     import dataclasses
-    import torch
-    from paper_1910_13444_b200 import PiGan
     cfgF = dataclasses.replace(cfg, G=1)                    # the grid is unused: n_colloc = F points per sample
     inp = wl.make_inputs(cfgF, bias_std=bias_std)
     S = cfg.S
@@ -161,9 +160,30 @@ def free_step_parity(cfg, F, bias_std=0.1, loss_scale=1.0, chunk_rows=0, pde_wei
     # "real" snapshots: the teacher pair at the sensors, f = 0 at that realization's free sensors (the paper's data solve Eq. 1 with f = 0)
     Xr, _ = orc.free_snapshot_ref(cfg.gen_shape, inp["teacher_Y"], inp["teacher_u"], xy_real, inp["xy_sensors"], inp["z_real"])
     Xr[:, 2 * S:2 * S + F] = 0.0
-    real = Xr.astype(np.float32)
+    return inp, disc_shape, xy_free, Xr.astype(np.float32)
+
+
+def free_score_sensitivity(cfg, F, inp, disc_shape, xy_free):
+    """(B, grad_f, f): by the fp64 oracle, grad_f = d mean D(X_fake) / d f [N][F] and B = max|f| * sum|grad_f|, the first-order bound
+    on the change of mean D(fake) per unit RELATIVE (to max|f|) perturbation of the f entries of the snapshot."""
+    S = cfg.S
+    X, _ = orc.free_snapshot_ref(cfg.gen_shape, inp["theta_Y"], inp["theta_u"], xy_free, inp["xy_sensors"], inp["z"])
+    lay = orc.unpack_params(inp["theta_D"], *disc_shape)
+    g, _ = orc._disc_forward(lay, X)
+    dX = orc._disc_backward(lay, g, np.full(X.shape[0], 1.0 / X.shape[0]), None)
+    f, gf = X[:, 2 * S:2 * S + F], dX[:, 2 * S:2 * S + F]
+    return float(np.abs(f).max() * np.abs(gf).sum()), gf, f
+
+
+def free_step_parity(cfg, F, bias_std=0.1, loss_scale=1.0, chunk_rows=0, pde_weight=0.0):
+    """Returns (errors, losses_gpu, losses_ref, found_inf, B) with B from free_score_sensitivity."""
+    import torch
+    from paper_1910_13444_b200 import PiGan
+    inp, disc_shape, xy_free, real = free_case(cfg, F, bias_std)
+    S = cfg.S
     gY, gu, gD, losses = orc.train_step_grads_free_ref(cfg.gen_shape, disc_shape, inp["theta_Y"], inp["theta_u"], inp["theta_D"], xy_free,
                                                        inp["xy_sensors"], inp["z"], real, inp["eps"], 10.0, pde_weight)
+    B = free_score_sensitivity(cfg, F, inp, disc_shape, xy_free)[0]
     dev = "cuda:0"
     t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
     pg = PiGan(latent_dim=cfg.m, gen_hidden=cfg.L, gen_width=cfg.H, disc_hidden=cfg.LD, disc_width=cfg.HD, n_samples=cfg.N, n_colloc=F,
@@ -179,4 +199,4 @@ def free_step_parity(cfg, F, bias_std=0.1, loss_scale=1.0, chunk_rows=0, pde_wei
     lg = out[3].cpu().numpy().astype(np.float64)
     fi = int(out[4].item())
     pg.close()
-    return errs, lg, losses, fi
+    return errs, lg, losses, fi, B

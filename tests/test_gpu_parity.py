@@ -16,6 +16,12 @@ pytestmark = pytest.mark.gpu
 
 TOL = {"fp32": 1e-4, "fp16": 2e-2}
 LOSS_TOL = 1e-3
+# Tripwires, NOT the contract: north_star's bounds above are what the library promises; these sit a small factor above what
+# the kernels measure today (fp16 tensors <= 2e-3, losses <= 2e-4; fp32 tensors <= 1e-5), so that a kernel
+# change that costs several times in accuracy is seen although it would still pass the contract.
+TRIP = {"fp32": 3e-5, "fp16": 5e-3}
+TRIP_BIAS_FP16 = 1e-2    # bias gradients are sums of FP16 adjoint planes over every row: up to 5e-3 (b2) .. 7e-3 (b1) at c5's 6 x 1024, run to run
+LOSS_TRIP = {"fp32": 1e-4, "fp16": 3e-4}
 
 
 def check_step(cfg, **kw):
@@ -25,6 +31,9 @@ def check_step(cfg, **kw):
     assert found_inf == 0
     lrel = np.abs(lg - lr) / np.maximum(np.abs(lr), 1e-12)
     assert np.all(lrel <= LOSS_TOL), f"{cfg.name}: losses gpu {lg} ref {lr} rel {lrel}"
+    drift = {k: v for k, v in errs.items() if not v <= (TRIP_BIAS_FP16 if cfg.precision == "fp16" and ".b" in k else TRIP[cfg.precision])}
+    assert not drift, f"{cfg.name}: within the contract but above the accuracy tripwire {TRIP[cfg.precision]}: {drift}"
+    assert np.all(lrel <= LOSS_TRIP[cfg.precision]), f"{cfg.name}: losses within the contract but above the tripwire: rel {lrel}"
     return errs
 
 
@@ -96,6 +105,62 @@ def test_critic_entry_points():
     g1, _, _ = pg.gradient_penalty(th, torch.from_numpy(real).cuda(), torch.from_numpy(fake).cuda(), one)
     g2, _, _ = pg.gradient_penalty(th, torch.from_numpy(real).cuda(), torch.from_numpy(real).cuda(), 0 * one)
     assert abs(g1.item() - g2.item()) <= 1e-6 * abs(g2.item())
+    pg.close()
+
+
+@pytest.mark.parametrize("name,N,kind", [("c3", 128, "fused small-critic kernel (H_D = 256)"), ("c4", 24, "layer-by-layer SGEMM critic (H_D = 512, 2000 inputs)")])
+def test_critic_entry_points_16bit_contexts_both_critic_paths(name, N, kind):
+    """pigan_disc_forward and pigan_gradient_penalty called directly on contexts of c3 / c4 dimensions: the critic is fp32 in every
+    mode (reading G18), so the fp32 tolerances apply; B > 3 n_samples rows exercise disc_forward's batching."""
+    import torch
+    from paper_1910_13444_b200 import PiGan
+    cfg = dataclasses.replace(wl.CONFIGS[name], name=f"{name}-critic", N=N, G=16)
+    inp = wl.make_inputs(cfg, bias_std=0.1)
+    rng = np.random.default_rng(3)
+    B = 3 * N + 5
+    snap = rng.normal(size=(B, 2 * cfg.S)).astype(np.float32)
+    real, fake = snap[:N].copy(), snap[N:2 * N].copy()
+    pg = PiGan.from_config(cfg)
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    th = t(inp["theta_D"])
+    score = pg.disc_forward(th, t(snap))
+    assert rel_err(score.cpu().numpy(), orc.disc_forward_ref(inp["theta_D"], *cfg.disc_shape, snap)) <= 1e-5, kind
+    gp, nu, d = pg.gradient_penalty(th, t(real), t(fake), t(inp["eps"]))
+    rgp, rnu, rd = orc.gradient_penalty_ref(inp["theta_D"], *cfg.disc_shape, real, fake, inp["eps"], 10.0)
+    assert abs(gp.item() - rgp) <= 1e-4 * abs(rgp) and rel_err(nu.cpu().numpy(), rnu) <= 1e-5, (kind, gp.item(), rgp)
+    errs = {k: rel_err(a, per_layer(rd, cfg.disc_shape)[k]) for k, a in per_layer(d.cpu().numpy(), cfg.disc_shape).items()}
+    assert max(errs.values()) <= TOL["fp32"], (kind, errs)
+    pg.close()
+
+
+def test_c3_jets_direct_entry_point():
+    """pigan_gen_jet_forward at c3's network (CTA-pair kernels, width 256) on the full 64 x 64 grid for 16 latent samples."""
+    for order in (1, 2):
+        errs, _, _ = jets_parity(wl.CONFIGS["c3"], order, n_samples=16)
+        assert max(errs.values()) <= TRIP["fp16"], (order, errs)
+
+
+def test_adam_at_c5_critic_size():
+    """n = 15 490 049 (c5's critic, not a multiple of 4): the vectorised grid-stride path and its scalar tail against the oracle,
+    two steps, then a skipped one."""
+    import torch
+    from paper_1910_13444_b200 import PiGan
+    pg = PiGan.from_config(wl.CONFIGS["c1"])
+    n = wl.param_count(*wl.CONFIGS["c5"].disc_shape)
+    assert n == 15490049
+    rng = np.random.default_rng(4)
+    th = rng.normal(size=n).astype(np.float32)
+    dth = torch.from_numpy(th.copy()).cuda(); dm = torch.zeros(n, device="cuda"); dv = torch.zeros(n, device="cuda")
+    rth, rm, rv = th.astype(np.float64), np.zeros(n), np.zeros(n)
+    for step in (1, 2):
+        g = rng.normal(size=n).astype(np.float32)
+        pg.adam_update(dth, torch.from_numpy(g).cuda(), dm, dv, step, 1e-2, 0.5, 0.9, 1e-8)
+        rth, rm, rv = orc.adam_update_ref(rth, g, rm, rv, step, 1e-2, 0.5, 0.9, 1e-8)
+    assert rel_err(dth.cpu().numpy(), rth) <= 1e-6 and rel_err(dm.cpu().numpy(), rm) <= 1e-6 and rel_err(dv.cpu().numpy(), rv) <= 1e-6
+    assert np.abs(dth.cpu().numpy()[-3:] - rth[-3:]).max() <= 1e-6 * np.abs(rth).max()      # the tail elements were updated
+    before = dth.clone()
+    pg.adam_update(dth, torch.from_numpy(g).cuda(), dm, dv, 3, 1e-2, 0.5, 0.9, 1e-8, skip_flag=torch.ones(1, dtype=torch.int32, device="cuda"))
+    assert torch.equal(before, dth)
     pg.close()
 
 
@@ -435,18 +500,32 @@ def test_trunk_11x512_cta_pair_kernels(skip):
 
 
 # ---- NEXT-2: f at per-realization free sensors (and their coordinates) as critic inputs -----------------
+FP16_HALF_ULP = 2.0 ** -11          # relative error of ONE rounding to FP16, the paper's activation precision
+
+
 def check_free(cfg, F, **kw):
-    errs, lg, lr, found_inf = free_step_parity(cfg, F, **kw)
+    errs, lg, lr, found_inf, B = free_step_parity(cfg, F, **kw)
     bad = {k: v for k, v in errs.items() if not v <= TOL[cfg.precision]}
     assert not bad, f"{cfg.name} F={F}: over tolerance {bad}"
     assert found_inf == 0
-    # The f entries of the snapshot come from the 16-bit jets (each accurate to ~1e-3 of its plane, tolerance 2e-2), so a critic
-    # mean that is small by cancellation cannot be held to 1e-3 of ITSELF: the scores are compared at 1e-3 of the critic's
-    # score scale max(|mean D(fake)|, |mean D(real)|)  (reading R9); GP and mean f^2 stay at 1e-3 relative.
-    scale = np.abs(lr).copy()
-    scale[[0, 1, 2, 4]] = np.maximum(scale[[0, 1, 2, 4]], max(abs(lr[1]), abs(lr[2])))
-    lrel = np.abs(lg - lr) / np.maximum(scale, 1e-12)
-    assert np.all(lrel <= LOSS_TOL), f"{cfg.name} F={F}: losses gpu {lg} ref {lr} rel {lrel}"
+    lrel = np.abs(lg - lr) / np.maximum(np.abs(lr), 1e-12)
+    if cfg.precision == "fp32":                                # north_star's ruler, literally: every loss within 1e-3 of itself
+        assert np.all(lrel <= LOSS_TOL), f"{cfg.name} F={F}: losses gpu {lg} ref {lr} rel {lrel}"
+        return
+    # 16-bit.  mean D(real), GP and mean f^2 (indices 2, 3, 5): the literal ruler.  L_D, mean D(fake), L_G (0, 1, 4) depend on the f
+    # entries of X_fake, which are built from FP16 jet planes.  B (fp64 oracle) bounds the change of mean D(fake) per unit relative
+    # perturbation of f.  Where ONE FP16 rounding of f in the worst direction stays within 1e-3 of the loss (B 2^-11 <= 1e-3 |loss|),
+    # the loss is held to the literal ruler; where it does not -- the loss is small by cancellation, and FP16 storage alone can already
+    # break 1e-3 of it -- it is held to 1e-3 of the score scale max(|mean D(fake)|, |mean D(real)|) (reading R9;
+    # tests/test_oracle_free.py::test_score_mean_small_by_cancellation_is_ill_conditioned_in_f shows the effect with the oracle alone).
+    assert np.all(lrel[[2, 3, 5]] <= LOSS_TOL), f"{cfg.name} F={F}: mean D(real) / GP / mean f^2 gpu {lg} ref {lr} rel {lrel}"
+    scale = max(abs(lr[1]), abs(lr[2]))
+    for i in (0, 1, 4):
+        literal = B * FP16_HALF_ULP <= LOSS_TOL * abs(lr[i])
+        ruler = abs(lr[i]) if literal else scale
+        assert abs(lg[i] - lr[i]) <= LOSS_TOL * ruler, (f"{cfg.name} F={F}: loss {i} gpu {lg[i]} ref {lr[i]} on the "
+                                                         f"{'literal' if literal else 'score-scale'} ruler (B = {B:.3g}, scale = {scale:.3g})")
+    return B * FP16_HALF_ULP / np.abs(lr[[0, 1, 4]])
 
 
 def test_free_sensors_fp32():
@@ -460,7 +539,8 @@ def test_free_sensors_16bit_one_and_many_chunks():
     check_free(cfg, 64)                                                                    # 512 rows in one chunk (fused first-layer reduction)
     check_free(cfg, 64, chunk_rows=256, pde_weight=0.5)                                    # two chunks: the forward is recomputed for the reverse sweep
     cfg = dataclasses.replace(wl.CONFIGS["c4"], name="c4-free", m=64, N=4, S=40, HD=128, LD=3)
-    check_free(cfg, 200)                                                                   # CTA-pair kernels, 800 rows, points per sample not a multiple of 64
+    cond = check_free(cfg, 200)                                                            # CTA-pair kernels, 800 rows, points per sample not a multiple of 64
+    assert np.all(cond <= LOSS_TOL), cond                                                  # this case is well conditioned: all six losses were on the literal ruler
 
 
 # ---- NEXT-3: hierarchical multi-discriminator loss ------------------------------------------------------
@@ -545,6 +625,57 @@ def test_data_parallel_trainer_drives_the_library_through_one_flat_gradient_buff
         assert np.abs(got.cpu().numpy() - ref).max() <= 2e-3 * 1e-2 + 1e-7
     assert np.allclose(losses, lref, rtol=1e-3, atol=1e-6)
     pg.close()
+
+
+def test_nccl_all_reduce_is_ordered_behind_the_graph_replayed_step():
+    """NEXT-4 on the one GPU a box has: a ONE-rank NCCL process group, so that the collective really is ncclAllReduce on the flat
+    gradient buffer, issued behind a step that runs as a CUDA-graph replay (from the third iteration on) with its side streams.
+    Eight iterations with fresh z / eps copied into the same buffers must give the same parameters as the same loop on a context
+    that never uses graphs and has no process group: a collective that overtook the step, or an update that overtook the
+    collective, would use stale or half-written gradients."""
+    import socket
+
+    import torch
+    import torch.distributed as dist
+    from paper_1910_13444_b200 import FLAG_NO_GRAPH, PiGan
+    from paper_1910_13444_b200.dp import DataParallelTrainer, pigan_step_fns
+    from parity_util import oracle_real_snapshots
+    cfg = wl.CONFIGS["c1"]           # fp32: Adam turns gradient noise into update noise, so the comparison wants the quiet arithmetic;
+    inp = wl.make_inputs(cfg, bias_std=0.1)      # the step still forks its three side streams and replays as a graph at this width
+    inp["real"] = oracle_real_snapshots(cfg, inp)
+    d = to_dev(inp, "cuda:0")
+    adam = dict(lr=1e-3, beta1=0.5, beta2=0.9, adam_eps=1e-8)
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0)); port = sk.getsockname()[1]
+    torch.cuda.set_device(0)
+    dist.init_process_group("nccl", init_method=f"tcp://127.0.0.1:{port}", rank=0, world_size=1)
+    try:
+        runs = []
+        for flags, group in ((0, dist), (FLAG_NO_GRAPH, None)):
+            pg = PiGan.from_config(cfg, flags=flags)
+            step_fn, adam_fn = pigan_step_fns(pg, d["xy_colloc"], d["f"], d["xy_sensors"], 1.0, adam)
+            tr = DataParallelTrainer(step_fn, adam_fn, [d[k].clone() for k in ("theta_Y", "theta_u", "theta_D")], schedule="parallel", dist=group)
+            assert (tr.dist is not None) == (group is not None) and tr.world == 1
+            z, eps = d["z"].clone(), d["eps"].clone()
+            gen = torch.Generator(device="cuda").manual_seed(11)
+            hist = []
+            for it in range(8):
+                z.copy_(torch.randn(z.shape, device="cuda", generator=gen))
+                eps.copy_(torch.rand(eps.shape, device="cuda", generator=gen))
+                hist.append(tr.train_step(z, d["real"], eps).clone())
+            torch.cuda.synchronize()
+            assert int(tr.out.found_inf.item()) == 0
+            runs.append(([p.cpu().numpy() for p in tr.params], torch.stack(hist).cpu().numpy(), [g.cpu().numpy() for g in tr.out.grads]))
+            pg.close()
+        (p_nccl, l_nccl, g_nccl), (p_ref, l_ref, g_ref) = runs
+        for a, b in zip(g_nccl, g_ref):                            # the last iteration's (reduced) gradients
+            assert rel_err(a, b) <= 1e-3, rel_err(a, b)
+        for a, b, p0 in zip(p_nccl, p_ref, (inp["theta_Y"], inp["theta_u"], inp["theta_D"])):
+            moved = np.linalg.norm(b - p0)                         # the UPDATES agree, not just the weights; stale gradients would give O(1) here
+            assert moved > 0 and np.linalg.norm(a - b) <= 5e-2 * moved, (moved, np.linalg.norm(a - b))
+        assert np.allclose(l_nccl, l_ref, rtol=2e-3, atol=1e-5)
+    finally:
+        dist.destroy_process_group()
 
 
 def test_minimal_training_loop_runs_and_learns_on_the_tiny_config():

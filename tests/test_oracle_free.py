@@ -74,3 +74,30 @@ def test_reduces_to_the_base_step_when_the_critic_ignores_f():
     bY, bU, bD, blosses = orc.train_step_grads_ref(gen_shape, base_D, thY, thU, thD, pts, np.zeros(Fp), xy_s, z, real, eps, 10.0, 0.7)
     assert np.allclose(gY, bY, rtol=1e-10, atol=1e-14) and np.allclose(gU, bU, rtol=1e-10, atol=1e-14)
     assert np.allclose(losses[[1, 4, 5]], blosses[[1, 4, 5]], rtol=1e-12)
+
+
+def test_score_mean_small_by_cancellation_is_ill_conditioned_in_f():
+    """DESIGN.md reading R9, shown with the fp64 oracle alone.  In the 16-bit NEXT-2 parity case `c2-free` (tests/test_gpu_parity.py)
+    mean D(fake) is 1.7 % of the critic's score scale.  Perturbing the f entries of X_fake by ONE FP16 half-ulp (2^-11, relative to
+    max|f|; FP16 is the paper's activation precision) in the worst direction moves mean D(fake) by far more than 1e-3 of
+    itself -- and by far less than 1e-3 of the score scale.  So no arithmetic that stores f (let alone the jets it is built from)
+    in FP16 can promise north_star's 1e-3 on this number; the score-scale ruler is the one such a case is held to."""
+    import dataclasses
+
+    import workloads as wl
+    from parity_util import free_case, free_score_sensitivity
+    cfg, F = dataclasses.replace(wl.CONFIGS["c2"], name="c2-free", N=8, S=32), 64
+    inp, disc_shape, xy_free, real = free_case(cfg, F)
+    B, gf, f = free_score_sensitivity(cfg, F, inp, disc_shape, xy_free)
+    S = cfg.S
+    X, _ = orc.free_snapshot_ref(cfg.gen_shape, inp["theta_Y"], inp["theta_u"], xy_free, inp["xy_sensors"], inp["z"])
+    D_fake = orc.disc_forward_ref(inp["theta_D"], *disc_shape, X).mean()
+    D_real = orc.disc_forward_ref(inp["theta_D"], *disc_shape, real).mean()
+    scale = max(abs(D_fake), abs(D_real))
+    assert abs(D_fake) < 0.05 * scale                                        # small by cancellation
+    Xp = X.copy()
+    Xp[:, 2 * S:2 * S + F] += 2.0 ** -11 * np.abs(f).max() * np.sign(gf)     # one FP16 half-ulp of max|f|, worst direction
+    moved = abs(orc.disc_forward_ref(inp["theta_D"], *disc_shape, Xp).mean() - D_fake)
+    assert np.isclose(moved, B * 2.0 ** -11, rtol=0.05)                      # the first-order bound B is what actually happens
+    assert moved > 10 * 1e-3 * abs(D_fake)                                   # > 10x north_star's ruler applied to the loss itself
+    assert moved < 0.6 * 1e-3 * scale                                        # inside 1e-3 of the score scale
