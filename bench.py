@@ -28,21 +28,83 @@ import workloads as wl  # noqa: E402
 METRIC = "PI-GAN train-step sample*collocation-points/s"
 UNIT = "sample*collocation-points/s"
 ADAM = dict(lr=1e-4, beta1=0.5, beta2=0.9, adam_eps=1e-8)          # reading G3
-PROFILE_CSV = os.path.join(ROOT, "profiles", "r02_step_dram_bytes.csv")   # ncu summary of one timed step per config (profiles/r02_summary.md)
+PROFILE_CSVS = [os.path.join(ROOT, "profiles", n) for n in ("r03_step_dram_bytes.csv", "r02_step_dram_bytes.csv")]   # newest first
+NCU_METRICS = ("dram__bytes_read.sum", "dram__bytes_write.sum", "gpu__time_duration.sum", "sm__pipe_tensor_cycles_active.avg.pct_of_peak_sustained_elapsed")
+
+
+def library_srchash():
+    """Content hash of the library's sources (what paper_1910_13444_b200/build.py stamps into libpigan.so.srchash)."""
+    from paper_1910_13444_b200.build import source_hash
+    return source_hash()
 
 
 def ncu_profile(cfg_name):
     """Per kernel class of `cfg_name`: launches, DRAM bytes and tensor-pipe-active % of ONE timed step, as measured by the ncu
-    pass recorded in profiles/r02_step_dram_bytes.csv (not by this run).  {} when the file has no rows for the config."""
-    out = {}
-    if not os.path.exists(PROFILE_CSV):
-        return out
+    pass recorded under profiles/ (not by this run); taken from the newest summary that has rows for the config.  Returns
+    (rows, source file, stale): stale = the summary carries no source hash or was taken on other library sources than the
+    ones in the tree, i.e. a kernel may have changed since."""
     import csv
-    for r in csv.DictReader(open(PROFILE_CSV)):
-        if r["config"] == cfg_name:
-            out[r["kernel_class"]] = {"launches": int(r["launches"]), "dram_bytes": int(r["dram_bytes_read"]) + int(r["dram_bytes_write"]),
-                                      "tensor_pct": float(r["tensor_pipe_active_pct_time_weighted"] or 0.0)}
-    return out
+    for path in PROFILE_CSVS:
+        if not os.path.exists(path):
+            continue
+        out, hashes = {}, set()
+        for r in csv.DictReader(open(path)):
+            if r["config"] == cfg_name:
+                out[r["kernel_class"]] = {"launches": int(r["launches"]), "dram_bytes": int(r["dram_bytes_read"]) + int(r["dram_bytes_write"]),
+                                          "tensor_pct": float(r["tensor_pipe_active_pct_time_weighted"] or 0.0)}
+                hashes.add(r.get("srchash") or "")
+        if out:
+            return out, os.path.relpath(path, ROOT), hashes != {library_srchash()}
+    return {}, None, None
+
+
+def kernel_class(name):
+    """ncu's demangled kernel name -> the class names of pigan_profile_report where a class spans several kernels, else the function name."""
+    import re
+    m = re.match(r"(?:void )?(?:\(anonymous namespace\)::|<unnamed>::|pigan::)*([A-Za-z_0-9]+)(?:<([^>]*)>)?", name)
+    fn, targs = m.group(1), [a.strip() for a in (m.group(2) or "").split(",")]
+    ints = [int(a) for a in targs if re.fullmatch(r"-?\d+", a)]
+    if fn in ("jet2_layer_kernel", "jet_layer_kernel") and len(ints) >= 2:
+        C, mode = ints[0], ints[1]
+        return {0: f"jet_layer_fwd(C={C})", 4: f"jet_layer_fwd(C={C})", 2: f"jet_layer_fwd_split(C={C})", 5: f"jet_layer_fwd_split(C={C})",
+                1: f"jet_layer_bwd(C={C})", 3: f"jet_layer_bwd(C={C})"}.get(mode, fn)
+    if fn in ("wgrad2_kernel", "wgrad_kernel"):
+        return "wgrad"
+    if fn in ("fused_bwd256_kernel", "fused_bwd128_kernel") and ints:
+        return f"jet_layer_bwd_wgrad(C={ints[0]})"
+    if fn == "fused_fwd128_kernel" and ints:
+        return f"gen_fwd_fused(C={ints[0]})"
+    return fn
+
+
+def ncu_summary(path, cfg_name, out=sys.stdout):
+    """Sums a per-launch ncu CSV (--csv --metrics NCU_METRICS, one timed step in the NVTX range) per kernel class and prints the
+    rows of profiles/rNN_step_dram_bytes.csv for `cfg_name`, stamped with the hash of the library sources in the tree."""
+    import csv
+    import io
+    lines = [l for l in open(path) if l.startswith('"')]
+    per = {}                                                   # launch id -> {kernel, metric: value}
+    for r in csv.DictReader(io.StringIO("".join(lines))):
+        d = per.setdefault(r["ID"], {"kernel": r["Kernel Name"]})
+        v = float(r["Metric Value"].replace(",", ""))
+        unit = r["Metric Unit"]
+        if r["Metric Name"].startswith("dram__bytes"):
+            v *= {"byte": 1, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}.get(unit, 1)
+        if r["Metric Name"] == "gpu__time_duration.sum":
+            v *= {"ns": 1e-3, "us": 1, "usecond": 1, "ms": 1e3, "msecond": 1e3, "nsecond": 1e-3, "second": 1e6}.get(unit, 1)     # -> us
+        d[r["Metric Name"]] = v
+    agg = {}
+    for d in per.values():
+        for cls in (kernel_class(d["kernel"]), "WHOLE_STEP"):
+            a = agg.setdefault(cls, [0, 0.0, 0.0, 0.0, 0.0])
+            t = d.get(NCU_METRICS[2], 0.0)
+            a[0] += 1; a[1] += t; a[2] += d.get(NCU_METRICS[0], 0.0); a[3] += d.get(NCU_METRICS[1], 0.0); a[4] += t * d.get(NCU_METRICS[3], 0.0)
+    h = library_srchash()
+    w = csv.writer(out)
+    w.writerow(["config", "kernel_class", "launches", "kernel_time_us_under_ncu", "dram_bytes_read", "dram_bytes_write",
+                "tensor_pipe_active_pct_time_weighted", "srchash"])
+    for cls, a in sorted(agg.items(), key=lambda kv: -kv[1][1]):
+        w.writerow([cfg_name, cls, a[0], round(a[1], 1), int(a[2]), int(a[3]), round(a[4] / a[1], 1) if a[1] > 0 else 0.0, h])
 
 
 # ----------------------------------------------------------------------------------------------------------------
@@ -365,7 +427,7 @@ def run_config(cfg, device, steps, warmup, rank, world, with_roofline=True, seed
                          "wgrad": 2 * rowsC * pb * Lh, "jet_layer_bwd_wgrad": rowsC * pb * (3 * Lh - 1), "gen_fwd_fused": cfg.N * cfg.P * chan * pb * cfg.L}
             cls_flops = {"jet_layer_fwd": sen if fwd_rows_sens_only else col + sen, "jet_layer_bwd": col + sen, "wgrad": col + sen,
                          "jet_layer_bwd_wgrad": 2 * (col + sen), "gen_fwd_fused": col}
-            prof_ncu = ncu_profile(cfg.name)
+            prof_ncu, prof_src, prof_stale = ncu_profile(cfg.name)
             per_kernel = {}
             for k, v in tc.items():
                 if v[1] <= 0:
@@ -385,7 +447,8 @@ def run_config(cfg, device, steps, warmup, rank, world, with_roofline=True, seed
                                "traffic": (dom_ncu["dram_bytes"] / dom_ncu["launches"]) if dom_ncu else None,
                                "traffic_kernel": f"{dom} (C=5), DRAM read+write bytes per launch" if dom_ncu else None,
                                "traffic_whole_step": whole["dram_bytes"] if whole else None,
-                               "traffic_source": "profiles/r02_step_dram_bytes.csv (ncu pass of profiles/r02_summary.md, not this run)" if prof_ncu else None,
+                               "traffic_source": f"{prof_src} (an ncu pass recorded under profiles/, not this run)" if prof_ncu else None,
+                               "traffic_stale": prof_stale,      # true: the library sources changed since that pass (or it carries no source hash)
                                "kernel": " + ".join(sorted(tc)) + " (tcgen05)", "peak_source": peaks["source"] + " sustained bf16",
                                "frac_of_burst": round(ach / peaks["tflops_burst"], 4), "frac_of_nominal_2250": round(ach / 2250.0, 4),
                                "share_of_step": round(tc_ms / total_ms, 4) if total_ms > 0 else None,
@@ -511,7 +574,12 @@ def main():
     ap.add_argument("--dp", action="store_true", help="NEXT-4: with --gpus N > 1, shard the N latent samples of the step over the ranks and all-reduce "
                     "the gradients (strong scaling) instead of running N independent replicas")
     ap.add_argument("--chunk-rows", type=int, default=0, help="rows per chunk of the generator passes (0 = library default); sweeps only")
+    ap.add_argument("--ncu-summary", default=None, metavar="CSV", help="no benchmark: sum the per-launch ncu CSV of one timed step of --config per kernel "
+                    "class and print the rows of profiles/rNN_step_dram_bytes.csv (needs no GPU)")
     args = ap.parse_args()
+    if args.ncu_summary:
+        ncu_summary(args.ncu_summary, args.config)
+        return 0
     cfg = wl.TABLE2 if args.config == "t2" else wl.CONFIGS[args.config]
     if args.samples:
         args.all_configs = False

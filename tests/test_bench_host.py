@@ -69,3 +69,28 @@ def test_reference_arm_under_torchrun_prints_one_line_from_rank0():
     assert d["impl"] == "reference" and d["n_gpus"] == 2 and d["gpu_launches"] == 0
     assert d["cpu_baseline"]["kind"] == "oracle" and d["e2e"]["h2d_bytes_per_step"] == 0
     assert d["value"] > 0 and d["unit"] == "sample*collocation-points/s"
+
+
+def test_ncu_summary_groups_launches_into_the_library_s_kernel_classes():
+    """bench.py --ncu-summary on a committed per-launch ncu CSV: kernel names map to the classes of pigan_profile_report, the
+    whole-step row counts every launch, and every row carries the hash of the library sources in the tree (traffic_stale's key)."""
+    import csv
+    import io
+    import bench
+    assert bench.kernel_class("void jet2_layer_kernel<__half, 5, 1>(CUtensorMap_st, CUtensorMap_st, CUtensorMap_st, Jet2Params)") == "jet_layer_bwd(C=5)"
+    assert bench.kernel_class("void jet2_layer_kernel<__half, 3, 4>(CUtensorMap_st)") == "jet_layer_fwd(C=3)"
+    assert bench.kernel_class("void jet_layer_kernel<__half, 2, 5>(CUtensorMap_st)") == "jet_layer_fwd_split(C=2)"
+    assert bench.kernel_class("void wgrad2_kernel<__half>(CUtensorMap_st, CUtensorMap_st, Wgrad2Params)") == "wgrad"
+    assert bench.kernel_class("void fused_bwd256_kernel<__half, 5, 0>(CUtensorMap_st)") == "jet_layer_bwd_wgrad(C=5)"
+    assert bench.kernel_class("void fused_fwd128_kernel<__half, 3>(FusedFwdMaps, FusedFwdParams)") == "gen_fwd_fused(C=3)"
+    assert bench.kernel_class("void <unnamed>::critic_fused_kernel<4>(int)") == "critic_fused_kernel"
+    assert bench.kernel_class("adam_kernel(float *, const float *)") == "adam_kernel"
+    buf = io.StringIO()
+    bench.ncu_summary(os.path.join(bench.ROOT, "profiles", "r02_launches_c5n2.csv"), "c5", out=buf)
+    rows = {r["kernel_class"]: r for r in csv.DictReader(io.StringIO(buf.getvalue()))}
+    assert int(rows["WHOLE_STEP"]["launches"]) == 188 and int(rows["wgrad"]["launches"]) == 20
+    assert sum(int(r["launches"]) for k, r in rows.items() if k != "WHOLE_STEP") == 188
+    assert abs(float(rows["WHOLE_STEP"]["kernel_time_us_under_ncu"]) - 27903.6) < 1.0
+    assert {r["srchash"] for r in rows.values()} == {bench.library_srchash()}
+    prof, src, stale = bench.ncu_profile("c5")
+    assert prof and src.startswith("profiles/") and stale in (True, False)
